@@ -1,0 +1,101 @@
+"""The five BASELINE.json configs as plain parameter records.
+
+C0 64^2 no wake, bilinear      | C1 256^2 shielded CSR, cubic (the bench workload)
+C2 512^2 S_csr sweep           | C3 256 x 256^2 batched scan | C4 2048^2 streaming stress test
+Readings A12 (noise), A13 (beta for C4 = 5e-4, pad for C2 = 2) are applied here.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field, replace
+from typing import Optional, Sequence
+
+import numpy as np
+
+from .impedance import make_impedance
+from .psi0 import make_psi0
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    N: int
+    q_min: float
+    q_max: float
+    p_min: float
+    p_max: float
+    steps_per_period: int
+    beta: float                      # per synchrotron period (reading A1)
+    interp_order: int                # 2 linear, 3 quadratic, 4 cubic
+    pad: int = 2                     # N_f = pad * N
+    members: int = 1
+    Pi: Optional[float] = None       # shielding parameter; None = no wake (Z = NULL)
+    S_csr: Sequence[float] = field(default_factory=tuple)   # one per member
+    noise: float = 0.0               # amplitude of the U[0,1) noise added to psi0 (A12)
+    seeds: Sequence[int] = field(default_factory=tuple)     # one per member
+    periods: float = 1.0             # nominal run length in synchrotron periods
+    sigma_q: float = 1.0
+    sigma_p: float = 1.0
+
+    @property
+    def dq(self) -> float:
+        return (self.q_max - self.q_min) / (self.N - 1)      # reading A2
+
+    @property
+    def dp(self) -> float:
+        return (self.p_max - self.p_min) / (self.N - 1)
+
+    @property
+    def Nf(self) -> int:
+        return self.pad * self.N
+
+    @property
+    def total_steps(self) -> int:
+        return int(round(self.periods * self.steps_per_period))
+
+    def psi0(self, members: Optional[Sequence[int]] = None) -> np.ndarray:
+        """fp32 [members][N][N] (index m, x, y; p contiguous)."""
+        idx = list(range(self.members) if members is None else members)
+        out = np.empty((len(idx), self.N, self.N), dtype=np.float32)
+        for i, m in enumerate(idx):
+            seed = self.seeds[m] if self.seeds else 0
+            out[i] = make_psi0(self.N, self.q_min, self.q_max, self.p_min, self.p_max,
+                               self.sigma_q, self.sigma_p, self.noise, seed)
+        return out
+
+    def impedance(self, members: Optional[Sequence[int]] = None) -> Optional[np.ndarray]:
+        """complex64 [members][N_f/2+1] or None (no wake)."""
+        if self.Pi is None:
+            return None
+        idx = list(range(self.members) if members is None else members)
+        base = make_impedance(self.N, self.pad, self.dq, 1.0, self.Pi, dtype=np.complex128)
+        out = np.empty((len(idx), self.Nf // 2 + 1), dtype=np.complex64)
+        for i, m in enumerate(idx):
+            out[i] = (base * self.S_csr[m]).astype(np.complex64)
+        return out
+
+    def with_(self, **kw) -> "Workload":
+        return replace(self, **kw)
+
+
+def _c3_s(m: int) -> float:
+    return 0.05 + 0.95 * m / 255.0
+
+
+CONFIGS = {
+    "C0": Workload("C0", 64, -6.0, 6.0, -6.0, 6.0, 500, 1e-3, 2, periods=2.0),
+    "C1": Workload("C1", 256, -6.0, 6.0, -6.0, 6.0, 4000, 5e-4, 4, Pi=1.0, S_csr=(0.5,),
+                   noise=1e-6, seeds=(1,), periods=20.0),
+    "C2": Workload("C2", 512, -6.0, 6.0, -6.0, 6.0, 4000, 5e-4, 4, Pi=1.0, S_csr=(0.2,),
+                   noise=1e-6, seeds=(2,), periods=50.0),
+    "C3": Workload("C3", 256, -6.0, 6.0, -6.0, 6.0, 4000, 5e-4, 4, members=256, Pi=1.0,
+                   S_csr=tuple(_c3_s(m) for m in range(256)), noise=1e-6,
+                   seeds=tuple(1000 + m for m in range(256)), periods=10.0),
+    "C4": Workload("C4", 2048, -8.0, 8.0, -8.0, 8.0, 8000, 5e-4, 4, Pi=0.8, S_csr=(0.8,),
+                   noise=1e-6, seeds=(4,), periods=2.0),
+}
+# C2 is run once per S_csr in {0.2, 0.6, 1.0}
+C2_SWEEP = (0.2, 0.6, 1.0)
+
+
+def get_workload(name: str) -> Workload:
+    return CONFIGS[name]
