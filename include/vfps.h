@@ -1,0 +1,162 @@
+/*
+ * vfps.h -- C ABI of the B200-native Vlasov-Fokker-Planck phase-space step.
+ *
+ * One call of vfps_step(h, n, diag) advances the discretised longitudinal phase-space density
+ * psi(q,p) by n full Warnock-Ellison split steps (arXiv:1611.05293; citations are PAPER.md lines):
+ *
+ *   a1 rotation     semi-Lagrangian rotation by dphi = 2*pi/steps_per_period about (q,p) = (0,0),
+ *                   interp_order x interp_order Lagrange interpolation at the back-rotated source
+ *                   point ("standard rotation", L136; Eq. 10-13; flow of Eq. 1)
+ *   a2 projection   bunch profile rho_x = dp * sum_y psi(x,y)                              (L56)
+ *   a3 wake         V = Re IDFT_Nf[ Z .* DFT_Nf(rho zero-padded to Nf = pad*N) ], first N samples
+ *                   (Eq. 5; Hermitian spectrum, only k = 0..Nf/2 stored, L149)
+ *   a4 kick         psi(x, p) <- psi(x, p - Dp_x), Dp_x = -dphi * V_x, 1-D Lagrange interpolation
+ *                   along p                                                              (L40, L149)
+ *   a5 Fokker-Planck psi <- psi + b*(psi + p*D1 psi + D2 psi), b = beta/steps_per_period,
+ *                   D1 = Eq. 15 (L144), D2 = three-point second difference (L138-147), along p
+ *   a6 diagnostics  C = dq*dp*sum psi (pre-renormalisation charge); psi <- psi/C (flag);
+ *                   <q>, <p>, sigma_q (bunch length), sigma_p (energy spread), CSR power
+ *                   P = (dq/Nf) sum_k Re Z_k |rho~_k|^2                      (Eq. 16-17)
+ *
+ * Grid and layout: N points per axis; x = q index, y = p index; q_x = q_min + x*dq with
+ * dq = (q_max - q_min)/(N-1) (both ends are nodes), same for p; psi = 0 outside the grid.
+ * psi arrays are [members][N][N] fp32, index (m, x, y), p (y) contiguous (flat z = N*x + y, L124).
+ * Batched mode: `members` independent simulations advance together, member m uses row m of Z.
+ *
+ * Conventions of every call:
+ *   - returns VFPS_OK (0) or a negative vfps_status; vfps_last_error(h) gives text.  No exception
+ *     crosses the ABI.  Unsupported combinations return VFPS_ERR_UNSUPPORTED -- there is no CPU
+ *     fallback and no silent change of method.
+ *   - the handle is opaque and owned by the library; every array argument is caller-owned and is
+ *     not retained after the call returns (inputs are copied into library-owned device memory).
+ *   - array pointers are DEVICE pointers, used asynchronously on the handle's stream, unless the
+ *     function name ends in `_host` (then: host pointers, and the call returns after the copy
+ *     has completed).
+ *   - nothing in vfps_step synchronises with the host.
+ */
+#ifndef VFPS_H
+#define VFPS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vfps_sim *vfps_handle;
+
+typedef enum vfps_status {
+    VFPS_OK = 0,
+    VFPS_ERR_ARG = -1,         /* NULL / out-of-range argument */
+    VFPS_ERR_STATE = -2,       /* call not valid in the handle's state (e.g. step before set_psi) */
+    VFPS_ERR_CUDA = -3,        /* a CUDA runtime call failed; text in vfps_last_error */
+    VFPS_ERR_NOMEM = -4,       /* device or host allocation failed */
+    VFPS_ERR_UNSUPPORTED = -5  /* valid request this build does not implement */
+} vfps_status;
+
+/* interleaved complex fp32, layout-compatible with CUDA float2 / C99 float _Complex */
+typedef struct vfps_complex { float re, im; } vfps_complex;
+
+enum {
+    VFPS_FLAG_RENORMALISE = 1,   /* psi <- psi / C after every step (BASELINE north_star (6)) */
+    VFPS_FLAG_CLAMP = 2,         /* Eq. 14 clamped interpolation -- not implemented yet */
+    VFPS_FLAG_ROT_MANHATTAN = 4  /* symplectic "Manhattan" rotation (L136) -- not implemented yet */
+};
+
+typedef struct vfps_params {
+    int N;                 /* grid points per axis, >= 8; N*pad must be a power of two          */
+    double q_min, q_max;   /* position axis, units of sigma_z0                                    */
+    double p_min, p_max;   /* energy axis, units of sigma_delta0                                  */
+    int steps_per_period;  /* time steps per synchrotron period; dphi = 2*pi/steps_per_period     */
+    double beta;           /* 1/(f_s tau_d): damping per synchrotron period (Eq. 1)          */
+    int interp_order;      /* Lagrange points per axis: 2 linear, 3 quadratic, 4 cubic (Eq. 10)  */
+    int pad;               /* zero-padding factor of the wake FFT, power of two >= 2             */
+    int members;           /* independent simulations advanced per call, >= 1                    */
+    int flags;             /* VFPS_FLAG_*                                                        */
+} vfps_params;
+
+/* Run-time options (vfps_set_option).  All engines and wake modes compute the same step. */
+enum {
+    VFPS_OPT_ENGINE = 1,   /* how n steps are issued                                             */
+    VFPS_OPT_WAKE = 2      /* how a3 is evaluated                                                */
+};
+enum {
+    VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRAPH                    */
+    VFPS_ENGINE_STREAM = 1,   /* one launch per kernel per step on the stream                    */
+    VFPS_ENGINE_GRAPH = 2,    /* the same kernels replayed from a CUDA graph of many steps       */
+    VFPS_ENGINE_CLUSTER = 3   /* persistent thread-block-cluster kernel, psi resident in
+                                 distributed shared memory for all n steps                       */
+};
+enum {
+    VFPS_WAKE_AUTO = 0,
+    VFPS_WAKE_FFT = 1,        /* zero-padded length-Nf FFT, x Z, inverse FFT, every step (Eq. 5) */
+    VFPS_WAKE_DIRECT = 2      /* w = Re IDFT(Z) once at create; V = w * rho by direct convolution
+                                 (Eq. 4) -- identical result, no serial FFT chain per step  */
+};
+
+/* Create a simulation.  Z: device pointer to [members][pad*N/2 + 1] impedance samples Z_k at
+ * wavenumber index k = 0..Nf/2 in the normalisation V = Re IDFT(Z .* DFT(rho)) (the caller folds
+ * every physical constant, e.g. 4*pi*S_csr, into Z), or NULL for no collective force (kick = exact
+ * identity, CSR power = 0).  Im Z_0 and Im Z_{Nf/2} are ignored (Hermitian spectrum).
+ * cuda_stream: a cudaStream_t (NULL = the legacy default stream); all work of this handle is
+ * issued there.  psi is zero until vfps_set_psi. */
+int vfps_create(const vfps_params *p, const vfps_complex *Z, void *cuda_stream, vfps_handle *out);
+int vfps_create_host(const vfps_params *p, const vfps_complex *Z_host, void *cuda_stream,
+                     vfps_handle *out);
+
+/* Free everything the handle owns.  NULL is accepted. */
+int vfps_destroy(vfps_handle h);
+
+/* Engine / wake-mode selection; may be called any time between steps. */
+int vfps_set_option(vfps_handle h, int option, int value);
+int vfps_get_option(vfps_handle h, int option, int *value);
+
+/* Copy psi [members][N][N] into the simulation; no renormalisation; step counter := 0. */
+int vfps_set_psi(vfps_handle h, const float *psi);
+int vfps_set_psi_host(vfps_handle h, const float *psi_host);
+
+/* Advance n >= 0 steps a1..a6.  diag: NULL or [n][members][6] floats; row (i, m) =
+ * { C (charge before renormalisation), <q>, <p>, sigma_q, sigma_p, P_csr } after step i.
+ * <q>, sigma_q and P_csr are taken from the post-rotation profile of the same step (kick and
+ * Fokker-Planck act along p only and leave rho unchanged up to edge flux), P scaled by 1/C^2.
+ * Asynchronous on the handle's stream.  vfps_step_host copies diag to host memory and returns
+ * when the n steps have completed. */
+int vfps_step(vfps_handle h, int n, float *diag);
+int vfps_step_host(vfps_handle h, int n, float *diag_host);
+
+/* Current density psi_t (renormalised if the flag is set), [members][N][N]. */
+int vfps_get_psi(vfps_handle h, float *psi_out);
+int vfps_get_psi_host(vfps_handle h, float *psi_out_host);
+
+/* Bunch profile rho_x = dp * sum_y psi_t(x,y) of the current psi, [members][N]. */
+int vfps_get_profile(vfps_handle h, float *rho_out);
+int vfps_get_profile_host(vfps_handle h, float *rho_out_host);
+
+/* Wake potential V_x of the current profile (recomputed, stateless), [members][N]; zeros if the
+ * simulation was created with Z = NULL. */
+int vfps_get_wake(vfps_handle h, float *V_out);
+int vfps_get_wake_host(vfps_handle h, float *V_out_host);
+
+/* { C = dq*dp*sum psi_t, <q>, <p>, sigma_q, sigma_p, P_csr } of the current psi, [members][6]. */
+int vfps_get_moments(vfps_handle h, float *out);
+int vfps_get_moments_host(vfps_handle h, float *out_host);
+
+/* Steps taken since the last vfps_set_psi. */
+int vfps_step_count(vfps_handle h, long long *count);
+
+/* Kernel launches (graph nodes included) issued by this handle so far. */
+int vfps_launch_count(vfps_handle h, long long *count);
+
+/* Name of the engine / wake mode the next vfps_step will use ("stream", "graph", "cluster";
+ * "fft", "direct"); static strings. */
+const char *vfps_engine_name(vfps_handle h);
+const char *vfps_wake_name(vfps_handle h);
+
+/* Text of the last error on this handle (or of the last failed vfps_create when h is NULL).
+ * Valid until the next call on the same handle. */
+const char *vfps_last_error(vfps_handle h);
+
+const char *vfps_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VFPS_H */

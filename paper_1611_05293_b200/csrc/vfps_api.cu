@@ -1,0 +1,503 @@
+// vfps_api.cu -- the C ABI of include/vfps.h over the sm_100a kernels.  Host logic only:
+// argument checks, device-memory ownership, launch configuration, engine selection.
+#include "../../include/vfps.h"
+#include "vfps_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace vfps;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Ctl {
+    float *diag;
+};
+
+}  // namespace
+
+struct vfps_sim {
+    vfps_params P{};
+    GridConst G{};
+    int N = 0, Nf = 0, log2Nf = 0, members = 1;
+    bool has_wake = false;
+    cudaStream_t stream = nullptr;
+    int engine_opt = VFPS_ENGINE_AUTO, wake_opt = VFPS_WAKE_AUTO;
+
+    float *psi = nullptr, *psi_tmp = nullptr;   // [members][N][N]; psi holds the current state
+    float2 *Z = nullptr;                         // [members][Nf/2+1]
+    float2 *tw = nullptr;                        // [Nf/2]
+    float *rho_part = nullptr;                   // [members][N][tiles_y]
+    float *rho = nullptr, *V = nullptr;          // [members][N]
+    float *qstat = nullptr;                      // [members][4]
+    float *mom_part = nullptr;                   // [members][kfp_blocks][3]
+    float *scale = nullptr;                      // [members]
+    unsigned *blkctr = nullptr;                  // [members]
+    int *rowctr = nullptr;                       // [members]
+    float **diag_cell = nullptr;                 // device cell with the caller's diag pointer
+    // scratch for the stateless get_* calls
+    float *g_rho = nullptr, *g_V = nullptr, *g_m1 = nullptr, *g_m2 = nullptr, *g_qstat = nullptr;
+    float *g_out = nullptr;                      // [members][max(N,6)] staging for *_host variants
+
+    int tiles_x = 0, tiles_y = 0, kfp_rows = 0, kfp_blocks = 0;
+    size_t rot_smem = 0, kfp_smem = 0, fft_smem = 0;
+    int fft_threads = 0;
+
+    bool psi_set = false;
+    long long steps = 0, launches = 0;
+    std::string err;
+    std::vector<void *> owned;
+
+    size_t cells() const { return (size_t)N * N; }
+};
+
+namespace {
+
+int fail(vfps_sim *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define CU(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(h, e_ == cudaErrorMemoryAllocation ? VFPS_ERR_NOMEM : VFPS_ERR_CUDA,  \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                  \
+    } while (0)
+
+template <typename T>
+cudaError_t dalloc(vfps_sim *h, T **p, size_t n)
+{
+    void *q = nullptr;
+    cudaError_t e = cudaMalloc(&q, n * sizeof(T) > 0 ? n * sizeof(T) : 1);
+    if (e == cudaSuccess) { *p = (T *)q; h->owned.push_back(q); }
+    return e;
+}
+
+bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
+
+int validate(const vfps_params *p, std::string &why)
+{
+    if (!p) { why = "params is NULL"; return VFPS_ERR_ARG; }
+    if (p->N < 8) { why = "N must be >= 8"; return VFPS_ERR_ARG; }
+    if (!(p->q_max > p->q_min) || !(p->p_max > p->p_min)) { why = "empty q or p range"; return VFPS_ERR_ARG; }
+    if (p->steps_per_period < 1) { why = "steps_per_period must be >= 1"; return VFPS_ERR_ARG; }
+    if (!(p->beta >= 0.0)) { why = "beta must be >= 0"; return VFPS_ERR_ARG; }
+    if (p->interp_order < 2 || p->interp_order > 4) { why = "interp_order must be 2, 3 or 4"; return VFPS_ERR_ARG; }
+    if (p->pad < 2 || !is_pow2(p->pad)) { why = "pad must be a power of two >= 2"; return VFPS_ERR_ARG; }
+    if (!is_pow2((long long)p->N * p->pad)) { why = "N*pad must be a power of two"; return VFPS_ERR_ARG; }
+    if (p->members < 1) { why = "members must be >= 1"; return VFPS_ERR_ARG; }
+    if (p->flags & ~(VFPS_FLAG_RENORMALISE | VFPS_FLAG_CLAMP | VFPS_FLAG_ROT_MANHATTAN)) { why = "unknown flag"; return VFPS_ERR_ARG; }
+    if (p->flags & VFPS_FLAG_CLAMP) { why = "clamped interpolation (Eq. 14) is not implemented"; return VFPS_ERR_UNSUPPORTED; }
+    if (p->flags & VFPS_FLAG_ROT_MANHATTAN) { why = "Manhattan rotation is not implemented"; return VFPS_ERR_UNSUPPORTED; }
+    if (p->N % 4 != 0) { why = "N must be a multiple of 4 (float4 rows)"; return VFPS_ERR_UNSUPPORTED; }
+    if ((long long)p->N * p->pad > 8192) { why = "N*pad > 8192: wake FFT does not fit one CTA's shared memory"; return VFPS_ERR_UNSUPPORTED; }
+    return VFPS_OK;
+}
+
+void grid_constants(vfps_sim *h)
+{
+    const vfps_params &P = h->P;
+    const double PI = 3.14159265358979323846;
+    const double dq = (P.q_max - P.q_min) / (P.N - 1), dp = (P.p_max - P.p_min) / (P.N - 1);
+    const double dphi = 2.0 * PI / P.steps_per_period;
+    const double sh = std::sin(0.5 * dphi);
+    const double a = -2.0 * sh * sh, s = std::sin(dphi);        // a = cos(dphi) - 1, no cancellation
+    const double b = -s * dp / dq, d = s * dq / dp;
+    const double x0c = P.q_min / dq, y0c = P.p_min / dp;
+    GridConst &G = h->G;
+    G.N = P.N; G.order = P.interp_order;
+    G.a = (float)a; G.b = (float)b; G.d = (float)d;
+    G.x0c = (float)x0c; G.y0c = (float)y0c;
+    G.dq = (float)dq; G.dp = (float)dp;
+    G.kick_c = (float)(dphi / dp);
+    G.fp_b = (float)(P.beta / P.steps_per_period);
+    G.p_min = (float)P.p_min; G.q_min = (float)P.q_min;
+    G.renorm = (P.flags & VFPS_FLAG_RENORMALISE) ? 1 : 0;
+    // largest source displacement in cells over the grid, then stencil reach
+    const double Xm = std::fmax(std::fabs(x0c), std::fabs(P.N - 1 + x0c));
+    const double Ym = std::fmax(std::fabs(y0c), std::fabs(P.N - 1 + y0c));
+    const double dmax = std::fmax(std::fabs(a) * Xm + std::fabs(b) * Ym, std::fabs(d) * Xm + std::fabs(a) * Ym);
+    G.H = (int)std::floor(dmax * 1.0001 + 1e-6) + 2;
+}
+
+template <int ORDER>
+int launch_step_stream(vfps_sim *h)
+{
+    const int N = h->N;
+    dim3 g1(h->tiles_x * h->tiles_y, h->members);
+    k_rotate<ORDER><<<g1, ROT_THREADS, h->rot_smem, h->stream>>>(h->G, h->psi, h->psi_tmp, h->scale,
+                                                                  h->rho_part, h->tiles_y);
+    k_wake_fft<<<h->members, h->fft_threads, h->fft_smem, h->stream>>>(
+        N, h->Nf, h->log2Nf, h->G.dq, h->rho_part, h->tiles_y, h->has_wake ? h->Z : nullptr, h->tw,
+        h->rho, h->V, h->qstat);
+    KfpArgs A;
+    A.psi_in = h->psi_tmp; A.psi_out = h->psi; A.V = h->V; A.qstat = h->qstat;
+    A.mom_part = h->mom_part; A.scale = h->scale; A.blkctr = h->blkctr; A.rowctr = h->rowctr;
+    A.diag = h->diag_cell; A.members = h->members; A.rows_per_cta = h->kfp_rows;
+    dim3 g3(h->kfp_blocks, h->members);
+    k_kick_fp<ORDER><<<g3, KFP_THREADS, h->kfp_smem, h->stream>>>(h->G, A);
+    h->launches += 3;
+    return VFPS_OK;
+}
+
+int launch_step(vfps_sim *h)
+{
+    switch (h->P.interp_order) {
+        case 2: return launch_step_stream<2>(h);
+        case 3: return launch_step_stream<3>(h);
+        default: return launch_step_stream<4>(h);
+    }
+}
+
+template <int ORDER>
+cudaError_t set_kernel_attrs(vfps_sim *h)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_rotate<ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->rot_smem);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_kick_fp<ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->kfp_smem);
+}
+
+int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, void *cuda_stream,
+                vfps_handle *out)
+{
+    vfps_sim *h = nullptr;
+    if (!out) return fail(nullptr, VFPS_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    std::string why;
+    int rc = validate(p, why);
+    if (rc != VFPS_OK) return fail(nullptr, rc, why);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(nullptr, VFPS_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+    h = new (std::nothrow) vfps_sim();
+    if (!h) return fail(nullptr, VFPS_ERR_NOMEM, "host allocation failed");
+    h->P = *p;
+    h->N = p->N; h->Nf = p->N * p->pad; h->members = p->members;
+    h->log2Nf = 0; while ((1 << h->log2Nf) < h->Nf) ++h->log2Nf;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->has_wake = (Z != nullptr);
+    grid_constants(h);
+
+    auto bail = [&](int code, const std::string &msg) {
+        g_create_error = msg;
+        vfps_destroy(h);
+        return code;
+    };
+    if (h->G.H > ROT_MAX_H)
+        return bail(VFPS_ERR_UNSUPPORTED, "rotation displacement per step exceeds the supported halo (too few steps_per_period for this grid)");
+
+    const int N = h->N, M = h->members;
+    h->tiles_x = (N + ROT_TX - 1) / ROT_TX;
+    h->tiles_y = (N + ROT_TY - 1) / ROT_TY;
+    h->rot_smem = (size_t)(ROT_TX + 2 * h->G.H) * (ROT_TY + 2 * h->G.H) * sizeof(float);
+    h->kfp_rows = KFP_WARPS * ((N >= 1024) ? 2 : 1);
+    h->kfp_blocks = (N + h->kfp_rows - 1) / h->kfp_rows;
+    h->kfp_smem = (size_t)KFP_WARPS * 2 * (KFP_PADL + N + KFP_PADR) * sizeof(float);
+    h->fft_threads = h->Nf / 2 < 1024 ? (h->Nf / 2 < 32 ? 32 : h->Nf / 2) : 1024;
+    h->fft_smem = (size_t)h->Nf * sizeof(float2);
+
+#define CUB(call)                                                                             \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return bail(e_ == cudaErrorMemoryAllocation ? VFPS_ERR_NOMEM : VFPS_ERR_CUDA,     \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                  \
+    } while (0)
+
+    CUB(dalloc(h, &h->psi, (size_t)M * N * N));
+    CUB(dalloc(h, &h->psi_tmp, (size_t)M * N * N));
+    CUB(dalloc(h, &h->tw, (size_t)h->Nf / 2));
+    CUB(dalloc(h, &h->rho_part, (size_t)M * N * h->tiles_y));
+    CUB(dalloc(h, &h->rho, (size_t)M * N));
+    CUB(dalloc(h, &h->V, (size_t)M * N));
+    CUB(dalloc(h, &h->qstat, (size_t)M * 4));
+    CUB(dalloc(h, &h->mom_part, (size_t)M * h->kfp_blocks * 3));
+    CUB(dalloc(h, &h->scale, (size_t)M));
+    CUB(dalloc(h, &h->blkctr, (size_t)M));
+    CUB(dalloc(h, &h->rowctr, (size_t)M));
+    CUB(dalloc(h, &h->diag_cell, (size_t)1));
+    CUB(dalloc(h, &h->g_rho, (size_t)M * N));
+    CUB(dalloc(h, &h->g_V, (size_t)M * N));
+    CUB(dalloc(h, &h->g_m1, (size_t)M * N));
+    CUB(dalloc(h, &h->g_m2, (size_t)M * N));
+    CUB(dalloc(h, &h->g_qstat, (size_t)M * 4));
+    CUB(dalloc(h, &h->g_out, (size_t)M * (N > 6 ? N : 6)));
+    CUB(cudaMemsetAsync(h->psi, 0, (size_t)M * N * N * sizeof(float), h->stream));
+    CUB(cudaMemsetAsync(h->V, 0, (size_t)M * N * sizeof(float), h->stream));
+
+    if (h->has_wake) {
+        const size_t nz = (size_t)M * (h->Nf / 2 + 1);
+        CUB(dalloc(h, &h->Z, nz));
+        CUB(cudaMemcpyAsync(h->Z, Z, nz * sizeof(float2),
+                            z_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
+    }
+    {   // twiddles exp(-2 pi i j / Nf), evaluated in double, rounded once
+        std::vector<float2> tw(h->Nf / 2);
+        const double PI = 3.14159265358979323846;
+        for (int j = 0; j < h->Nf / 2; ++j) {
+            const double ang = -2.0 * PI * (double)j / (double)h->Nf;
+            tw[j] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+        }
+        CUB(cudaMemcpyAsync(h->tw, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice, h->stream));
+        CUB(cudaStreamSynchronize(h->stream));
+    }
+    k_fill<<<(M + 255) / 256, 256, 0, h->stream>>>(h->scale, 1.0f, M);
+    k_set_ctl<<<(M + 255) / 256, 256, 0, h->stream>>>(h->diag_cell, nullptr, h->rowctr, h->blkctr, M);
+    h->launches += 2;
+    cudaError_t e = cudaSuccess;
+    switch (p->interp_order) {
+        case 2: e = set_kernel_attrs<2>(h); break;
+        case 3: e = set_kernel_attrs<3>(h); break;
+        default: e = set_kernel_attrs<4>(h); break;
+    }
+    CUB(e);
+    CUB(cudaFuncSetAttribute(k_wake_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->fft_smem));
+    CUB(cudaGetLastError());
+#undef CUB
+    *out = h;
+    return VFPS_OK;
+}
+
+// rho / V / moments of the CURRENT psi into the g_* scratch (stateless: touches no step state)
+int current_profile(vfps_sim *h, bool want_wake)
+{
+    const int N = h->N, M = h->members;
+    k_project<<<dim3(N, M), 128, 0, h->stream>>>(h->G, h->psi, h->scale, h->g_rho, h->g_m1, h->g_m2);
+    h->launches += 1;
+    if (want_wake) {
+        k_wake_fft<<<M, h->fft_threads, h->fft_smem, h->stream>>>(N, h->Nf, h->log2Nf, h->G.dq, h->g_rho, 1,
+                                                                  h->has_wake ? h->Z : nullptr, h->tw,
+                                                                  h->g_rho, h->g_V, h->g_qstat);
+        h->launches += 1;
+    }
+    CU(cudaGetLastError());
+    return VFPS_OK;
+}
+
+int to_host(vfps_sim *h, float *dst_host, const float *src_dev, size_t n)
+{
+    CU(cudaMemcpyAsync(dst_host, src_dev, n * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return VFPS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int vfps_create(const vfps_params *p, const vfps_complex *Z, void *cuda_stream, vfps_handle *out)
+{
+    return create_impl(p, Z, false, cuda_stream, out);
+}
+
+int vfps_create_host(const vfps_params *p, const vfps_complex *Z_host, void *cuda_stream, vfps_handle *out)
+{
+    return create_impl(p, Z_host, true, cuda_stream, out);
+}
+
+int vfps_destroy(vfps_handle h)
+{
+    if (!h) return VFPS_OK;
+    cudaStreamSynchronize(h->stream);
+    for (void *p : h->owned) cudaFree(p);
+    delete h;
+    return VFPS_OK;
+}
+
+int vfps_set_option(vfps_handle h, int option, int value)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (option == VFPS_OPT_ENGINE) {
+        if (value == VFPS_ENGINE_AUTO || value == VFPS_ENGINE_STREAM) { h->engine_opt = value; return VFPS_OK; }
+        if (value == VFPS_ENGINE_GRAPH || value == VFPS_ENGINE_CLUSTER)
+            return fail(h, VFPS_ERR_UNSUPPORTED, "engine not available in this build");
+        return fail(h, VFPS_ERR_ARG, "unknown engine");
+    }
+    if (option == VFPS_OPT_WAKE) {
+        if (value == VFPS_WAKE_AUTO || value == VFPS_WAKE_FFT) { h->wake_opt = value; return VFPS_OK; }
+        if (value == VFPS_WAKE_DIRECT) return fail(h, VFPS_ERR_UNSUPPORTED, "wake mode not available in this build");
+        return fail(h, VFPS_ERR_ARG, "unknown wake mode");
+    }
+    return fail(h, VFPS_ERR_ARG, "unknown option");
+}
+
+int vfps_get_option(vfps_handle h, int option, int *value)
+{
+    if (!h || !value) return fail(h, VFPS_ERR_ARG, "NULL argument");
+    if (option == VFPS_OPT_ENGINE) { *value = h->engine_opt; return VFPS_OK; }
+    if (option == VFPS_OPT_WAKE) { *value = h->wake_opt; return VFPS_OK; }
+    return fail(h, VFPS_ERR_ARG, "unknown option");
+}
+
+const char *vfps_engine_name(vfps_handle h) { (void)h; return "stream"; }
+const char *vfps_wake_name(vfps_handle h) { (void)h; return "fft"; }
+
+static int set_psi_impl(vfps_handle h, const float *psi, cudaMemcpyKind kind)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!psi) return fail(h, VFPS_ERR_ARG, "psi is NULL");
+    const size_t n = (size_t)h->members * h->cells();
+    CU(cudaMemcpyAsync(h->psi, psi, n * sizeof(float), kind, h->stream));
+    k_fill<<<(h->members + 255) / 256, 256, 0, h->stream>>>(h->scale, 1.0f, h->members);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    if (kind == cudaMemcpyHostToDevice) CU(cudaStreamSynchronize(h->stream));
+    h->psi_set = true;
+    h->steps = 0;
+    return VFPS_OK;
+}
+
+int vfps_set_psi(vfps_handle h, const float *psi) { return set_psi_impl(h, psi, cudaMemcpyDeviceToDevice); }
+int vfps_set_psi_host(vfps_handle h, const float *psi) { return set_psi_impl(h, psi, cudaMemcpyHostToDevice); }
+
+int vfps_step(vfps_handle h, int n, float *diag)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (n < 0) return fail(h, VFPS_ERR_ARG, "n must be >= 0");
+    if (!h->psi_set) return fail(h, VFPS_ERR_STATE, "vfps_step before vfps_set_psi");
+    if (n == 0) return VFPS_OK;
+    k_set_ctl<<<(h->members + 255) / 256, 256, 0, h->stream>>>(h->diag_cell, diag, h->rowctr, h->blkctr, h->members);
+    h->launches += 1;
+    for (int i = 0; i < n; ++i) {
+        int rc = launch_step(h);
+        if (rc != VFPS_OK) return rc;
+    }
+    CU(cudaGetLastError());
+    h->steps += n;
+    return VFPS_OK;
+}
+
+int vfps_step_host(vfps_handle h, int n, float *diag_host)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (n < 0) return fail(h, VFPS_ERR_ARG, "n must be >= 0");
+    float *d = nullptr;
+    const size_t cnt = (size_t)n * h->members * 6;
+    if (diag_host && cnt) CU(cudaMalloc((void **)&d, cnt * sizeof(float)));
+    int rc = vfps_step(h, n, d);
+    if (rc == VFPS_OK) {
+        cudaError_t e = d ? cudaMemcpyAsync(diag_host, d, cnt * sizeof(float), cudaMemcpyDeviceToHost, h->stream)
+                          : cudaSuccess;
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        if (e != cudaSuccess) rc = fail(h, VFPS_ERR_CUDA, cudaGetErrorString(e));
+    }
+    if (d) cudaFree(d);
+    return rc;
+}
+
+int vfps_get_psi(vfps_handle h, float *psi_out)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!psi_out) return fail(h, VFPS_ERR_ARG, "psi_out is NULL");
+    const size_t cells = h->cells();
+    int bx = (int)((cells + 1023) / 1024); if (bx > 1184) bx = 1184;
+    k_scale_copy<<<dim3(bx, h->members), 256, 0, h->stream>>>(h->psi, h->scale, psi_out, cells, h->G.renorm);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    return VFPS_OK;
+}
+
+int vfps_get_psi_host(vfps_handle h, float *psi_out_host)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!psi_out_host) return fail(h, VFPS_ERR_ARG, "psi_out is NULL");
+    int rc = vfps_get_psi(h, h->psi_tmp);          // psi_tmp is dead between steps
+    if (rc != VFPS_OK) return rc;
+    return to_host(h, psi_out_host, h->psi_tmp, (size_t)h->members * h->cells());
+}
+
+int vfps_get_profile(vfps_handle h, float *rho_out)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!rho_out) return fail(h, VFPS_ERR_ARG, "rho_out is NULL");
+    int rc = current_profile(h, false);
+    if (rc != VFPS_OK) return rc;
+    CU(cudaMemcpyAsync(rho_out, h->g_rho, (size_t)h->members * h->N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+    return VFPS_OK;
+}
+
+int vfps_get_profile_host(vfps_handle h, float *rho_out_host)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!rho_out_host) return fail(h, VFPS_ERR_ARG, "rho_out is NULL");
+    int rc = current_profile(h, false);
+    if (rc != VFPS_OK) return rc;
+    return to_host(h, rho_out_host, h->g_rho, (size_t)h->members * h->N);
+}
+
+int vfps_get_wake(vfps_handle h, float *V_out)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!V_out) return fail(h, VFPS_ERR_ARG, "V_out is NULL");
+    int rc = current_profile(h, true);
+    if (rc != VFPS_OK) return rc;
+    CU(cudaMemcpyAsync(V_out, h->g_V, (size_t)h->members * h->N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+    return VFPS_OK;
+}
+
+int vfps_get_wake_host(vfps_handle h, float *V_out_host)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!V_out_host) return fail(h, VFPS_ERR_ARG, "V_out is NULL");
+    int rc = current_profile(h, true);
+    if (rc != VFPS_OK) return rc;
+    return to_host(h, V_out_host, h->g_V, (size_t)h->members * h->N);
+}
+
+static int moments_impl(vfps_handle h)
+{
+    int rc = current_profile(h, true);
+    if (rc != VFPS_OK) return rc;
+    k_moments_final<<<h->members, 256, 0, h->stream>>>(h->G, h->g_rho, h->g_m1, h->g_m2, h->g_qstat, h->g_out);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    return VFPS_OK;
+}
+
+int vfps_get_moments(vfps_handle h, float *out)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!out) return fail(h, VFPS_ERR_ARG, "out is NULL");
+    int rc = moments_impl(h);
+    if (rc != VFPS_OK) return rc;
+    CU(cudaMemcpyAsync(out, h->g_out, (size_t)h->members * 6 * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+    return VFPS_OK;
+}
+
+int vfps_get_moments_host(vfps_handle h, float *out_host)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!out_host) return fail(h, VFPS_ERR_ARG, "out is NULL");
+    int rc = moments_impl(h);
+    if (rc != VFPS_OK) return rc;
+    return to_host(h, out_host, h->g_out, (size_t)h->members * 6);
+}
+
+int vfps_step_count(vfps_handle h, long long *count)
+{
+    if (!h || !count) return fail(h, VFPS_ERR_ARG, "NULL argument");
+    *count = h->steps;
+    return VFPS_OK;
+}
+
+int vfps_launch_count(vfps_handle h, long long *count)
+{
+    if (!h || !count) return fail(h, VFPS_ERR_ARG, "NULL argument");
+    *count = h->launches;
+    return VFPS_OK;
+}
+
+const char *vfps_last_error(vfps_handle h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+const char *vfps_version(void) { return "vfps 0.1 (sm_100a)"; }
+
+}  // extern "C"

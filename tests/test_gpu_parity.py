@@ -1,0 +1,245 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded fp32 inputs.  Tolerances are BASELINE.json's north_star:
+  max|psi_gpu - psi_ref| <= 1e-5 * max psi after 1 step, <= 1e-3 * max psi after 1000 steps;
+  moments and CSR power within 1e-4 relative (means, which are ~0: 1e-4 absolute in units of
+  sigma)."""
+import numpy as np
+import pytest
+
+from workloads import get_workload, make_impedance, make_psi0
+from workloads.configs import Workload
+
+pytestmark = pytest.mark.gpu
+
+TOL_1 = 1e-5
+TOL_1000 = 1e-3
+TOL_MOM = 1e-4
+
+
+def assert_psi(sim_psi, ref_psi, tol, what=""):
+    ref = np.asarray(ref_psi, dtype=np.float64)
+    err = np.max(np.abs(sim_psi.astype(np.float64) - ref)) / ref.max()
+    assert err <= tol, f"{what}: max|dpsi|/max psi = {err:.3e} > {tol:.1e}"
+    return err
+
+
+def assert_diag(got, want, has_wake=True, tol_q=TOL_MOM):
+    """tol_q: tolerance of the three numbers taken from the post-rotation profile (<q>, sigma_q,
+    P_csr); equal to TOL_MOM unless the bunch overflows the box (edge flux)."""
+    got = np.asarray(got, dtype=np.float64)
+    want = np.asarray(want, dtype=np.float64)
+    assert abs(got[0] - want[0]) <= TOL_MOM * abs(want[0]), ("C", got[0], want[0])
+    assert abs(got[1] - want[1]) <= tol_q * want[3], ("<q>", got[1], want[1])
+    assert abs(got[2] - want[2]) <= TOL_MOM * want[4], ("<p>", got[2], want[2])
+    assert abs(got[3] - want[3]) <= tol_q * want[3], ("sigma_q", got[3], want[3])
+    assert abs(got[4] - want[4]) <= TOL_MOM * want[4], ("sigma_p", got[4], want[4])
+    if has_wake:
+        assert abs(got[5] - want[5]) <= tol_q * abs(want[5]), ("P_csr", got[5], want[5])
+    else:
+        assert got[5] == 0.0
+
+
+def run_pair(vfps, orc, wl, nsteps, members=None, engine=None, wake=None, diag_every=1):
+    idx = list(range(wl.members) if members is None else members)
+    sim = vfps.Simulation.from_workload(wl, idx)
+    if engine is not None:
+        sim.set_engine(engine)
+    if wake is not None:
+        sim.set_wake_mode(wake)
+    d_gpu = sim.step_host(nsteps)
+    psi_gpu = sim.get_psi_host()
+    refs, d_ref = [], []
+    for m in idx:
+        o = orc.Oracle.from_workload(wl, m)
+        d_ref.append(o.step(nsteps, diag_every=diag_every))
+        refs.append(o)
+    return sim, psi_gpu, d_gpu, refs, d_ref
+
+
+# ---------------------------------------------------------------- the BASELINE configs
+def test_c0_one_step_and_1000_steps(vfps, orc):
+    wl = get_workload("C0")
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1)
+    assert_psi(psi[0], refs[0].psi, TOL_1, "C0 1 step")
+    assert_diag(d[0, 0], dr[0][0], has_wake=False)
+    sim.close()
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1000)
+    assert_psi(psi[0], refs[0].psi, TOL_1000, "C0 1000 steps")
+    for i in (0, 499, 999):
+        assert_diag(d[i, 0], dr[0][i], has_wake=False)
+    # charge conservation and the stationarity statement for C0 (bilinear: predicted diffusion)
+    assert np.all(np.abs(d[:, 0, 0] - 1.0) < 1e-4)
+    sim.close()
+
+
+def test_c1_one_step(vfps, orc):
+    wl = get_workload("C1")
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1)
+    err = assert_psi(psi[0], refs[0].psi, TOL_1, "C1 1 step")
+    assert_diag(d[0, 0], dr[0][0])
+    print(f"C1 1 step err {err:.2e}")
+    sim.close()
+
+
+def test_c1_1000_steps(vfps, orc):
+    wl = get_workload("C1")
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1000, diag_every=100)
+    err = assert_psi(psi[0], refs[0].psi, TOL_1000, "C1 1000 steps")
+    for i in (99, 499, 999):
+        assert_diag(d[i, 0], dr[0][i])
+    print(f"C1 1000 steps err {err:.2e}")
+    sim.close()
+
+
+def test_c2_512_steps(vfps, orc):
+    wl = get_workload("C2")
+    for S in (0.2, 1.0):
+        w = wl.with_(S_csr=(S,))
+        sim, psi, d, refs, dr = run_pair(vfps, orc, w, 1)
+        assert_psi(psi[0], refs[0].psi, TOL_1, f"C2 S={S} 1 step")
+        assert_diag(d[0, 0], dr[0][0])
+        sim.close()
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl.with_(S_csr=(0.6,)), 200, diag_every=50)
+    assert_psi(psi[0], refs[0].psi, 2e-4, "C2 200 steps")
+    assert_diag(d[199, 0], dr[0][199])
+    sim.close()
+
+
+def test_c3_batched_members(vfps, orc):
+    """Batched scan: a slice of C3's members in one handle, each with its own Z and noise."""
+    wl = get_workload("C3")
+    idx = [0, 37, 128, 255]
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 50, members=idx, diag_every=10)
+    for i, m in enumerate(idx):
+        assert_psi(psi[i], refs[i].psi, 1e-4, f"C3 member {m} 50 steps")
+        assert_diag(d[49, i], dr[i][49])
+    assert not np.allclose(d[49, 0, 5], d[49, 3, 5])        # members really differ
+    sim.close()
+
+
+def test_c4_2048_steps(vfps, orc):
+    wl = get_workload("C4")
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1)
+    assert_psi(psi[0], refs[0].psi, TOL_1, "C4 1 step")
+    assert_diag(d[0, 0], dr[0][0])
+    sim.close()
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 10, diag_every=10)
+    assert_psi(psi[0], refs[0].psi, 5e-5, "C4 10 steps")
+    assert_diag(d[9, 0], dr[0][9])
+    sim.close()
+
+
+# ---------------------------------------------------------------- small / ragged / degenerate
+@pytest.mark.parametrize("order", [2, 3, 4])
+@pytest.mark.parametrize("N", [8, 32, 128])
+def test_orders_and_small_grids(vfps, orc, order, N):
+    """Asymmetric box, off-centre mismatched bunch, free-space wake: several tiles and partial
+    tiles (N < tile), all three interpolation orders."""
+    wl = Workload(f"t{N}", N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, pad=4, S_csr=(0.4,), seeds=(9,),
+                  noise=1e-5, sigma_q=1.2, sigma_p=0.8)
+    Z = make_impedance(N, 4, wl.dq, 0.4, None)[None, :]
+    psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
+    sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 4, 1, Z=Z)
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 4, Z[0])
+    o.set_psi(psi0[0])
+    # N = 8: the bunch overflows the 8-point box (2e-3 of the charge leaves per step), so the
+    # edge flux of kick and Fokker-Planck shows in the profile-derived diagnostics
+    tol_q = 1e-3 if N == 8 else TOL_MOM
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"N={N} order={order} 1 step")
+    assert_diag(d[0, 0], dr[0], tol_q=tol_q)
+    d = sim.step_host(99)
+    dr = o.step(99)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"N={N} order={order} 100 steps")
+    assert_diag(d[98, 0], dr[98], tol_q=tol_q)
+    assert sim.step_count() == 100
+    sim.close()
+
+
+def test_large_kick_shift_beyond_one_cell(vfps, orc):
+    """A strong resistive impedance gives |kick shift| > 1 cell: integer part of the shift and
+    zero boundary are exercised."""
+    N = 64
+    Z = np.full((1, N + 1), 60.0 + 0j, dtype=np.complex64)
+    psi0 = make_psi0(N, -6, 6, -6, 6, 1.0, 1.0, 0, 0)[None]
+    sim = vfps.Simulation(N, -6, 6, -6, 6, 100, 1e-3, 4, 2, 1, Z=Z)
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, -6, 6, -6, 6, 100, 1e-3, 4, 2, Z[0])
+    o.set_psi(psi0[0])
+    V = sim.get_wake_host()[0]
+    assert np.max(np.abs(V)) * (2 * np.pi / 100) / (12 / 63) > 1.5       # shift in cells
+    sim.step_host(3, diag=False)
+    o.step(3, diag=False)
+    assert_psi(sim.get_psi_host()[0], o.psi, 3e-5, "large kick")
+    sim.close()
+
+
+def test_no_wake_kick_is_identity_and_no_renormalise(vfps, orc):
+    wl = get_workload("C0").with_(interp_order=4)
+    psi0 = wl.psi0()
+    sim = vfps.Simulation(wl.N, -6, 6, -6, 6, wl.steps_per_period, wl.beta, 4, 2, 1, flags=0)
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(wl.N, -6, 6, -6, 6, wl.steps_per_period, wl.beta, 4, 2, None, renormalise=False)
+    o.set_psi(psi0[0])
+    d = sim.step_host(20)
+    dr = o.step(20)
+    assert_psi(sim.get_psi_host()[0], o.psi, 2e-5, "no renormalise")
+    assert_diag(d[19, 0], dr[19], has_wake=False)
+    assert np.all(sim.get_wake_host() == 0)
+    sim.close()
+
+
+def test_get_calls_match_oracle_and_are_stateless(vfps, orc):
+    wl = get_workload("C1")
+    sim = vfps.Simulation.from_workload(wl)
+    o = orc.Oracle.from_workload(wl)
+    sim.step_host(5, diag=False)
+    o.step(5, diag=False)
+    for _ in range(2):                                       # second round: nothing was disturbed
+        rho, V, mom = sim.get_profile_host()[0], sim.get_wake_host()[0], sim.get_moments_host()[0]
+        np.testing.assert_allclose(rho, o.profile(), rtol=0, atol=2e-6 * o.profile().max())
+        np.testing.assert_allclose(V, o.wake(), rtol=0, atol=1e-5 * np.abs(o.wake()).max())
+        assert_diag(mom, o.moments6())
+    d = sim.step_host(5)
+    dr = o.step(5)
+    assert_psi(sim.get_psi_host()[0], o.psi, 2e-5, "after get calls")
+    assert_diag(d[4, 0], dr[4])
+    sim.close()
+
+
+def test_device_pointer_calls_and_diag_on_device(vfps, orc):
+    import torch
+    wl = get_workload("C1")
+    sim = vfps.Simulation.from_workload(wl)
+    psi_dev = torch.from_numpy(wl.psi0()).cuda()
+    sim.set_psi(psi_dev)
+    diag = torch.zeros(7, 1, 6, device="cuda")
+    sim.step(7, diag)
+    sim.step(0)
+    out = sim.get_psi()
+    torch.cuda.synchronize()
+    o = orc.Oracle.from_workload(wl)
+    dr = o.step(7)
+    assert_psi(out.cpu().numpy()[0], o.psi, 2e-5, "device path")
+    for i in range(7):
+        assert_diag(diag[i, 0].cpu().numpy(), dr[i])
+    rho = sim.get_profile(); V = sim.get_wake(); mom = sim.get_moments()
+    torch.cuda.synchronize()
+    assert rho.shape == (1, 256) and V.shape == (1, 256) and mom.shape == (1, 6)
+    assert sim.launch_count() > 0
+    sim.close()
+
+
+def test_error_paths_on_gpu(vfps):
+    sim = vfps.Simulation(64, -6, 6, -6, 6, 500, 1e-3, 2)
+    with pytest.raises(vfps.VfpsError) as e:
+        sim.step_host(1)
+    assert e.value.code == -2                               # step before set_psi
+    with pytest.raises(vfps.VfpsError):
+        sim.set_option(99, 0)
+    sim.close()
+    with pytest.raises(vfps.VfpsError) as e:
+        vfps.Simulation(64, -6, 6, -6, 6, 2, 1e-3, 4)      # 2 steps per period: halo too large
+    assert e.value.code == -5
