@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Vlasov-Fokker-Planck split step on B200 (driver contract).
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload C1]
+
+One bench "step" = one call vfps_step(h, n_inner) = n_inner full split steps a1..a6 (rotation,
+projection, wake, kick, Fokker-Planck, diagnostics + renormalisation) of the named BASELINE
+workload; n_inner defaults to one synchrotron period (steps_per_period), so the default
+K = 20 bench steps of C1 are exactly BASELINE config 1 (256^2, 20 periods, 80 000 split steps).
+
+metric  cell-updates/s = N^2 * members * n_inner * K * n_gpus / (max over ranks of the device
+        time of the K bench steps); `steps_per_s` (split steps/s of one simulation) rides along.
+value   inputs resident in HBM when the timed region starts (CUDA events on the library's stream).
+e2e     the same through the host-pointer entry points of the C ABI: every bench step copies
+        psi from pinned host memory (vfps_set_psi_host), advances n_inner steps with the
+        diagnostics copied back (vfps_step_host) and reads psi back (vfps_get_psi_host).
+N > 1   "replicas only": every rank advances its own copy of the workload
+        (rank-dependent seed), no data-path collective; weak scaling.
+--impl reference   times the CPU oracle (oracle/, the reference arm of this tier) on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "phase-space cell-updates/s"
+UNIT = "cell-updates/s"
+ALG_BYTES_PER_CELL_STEP = 8.0     # one fp32 read + one fp32 write per cell per split step
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--inner", type=int, default=0, help="split steps per bench step (0 = one synchrotron period)")
+    ap.add_argument("--engine", default="auto", choices=["auto", "stream", "graph", "cluster"])
+    ap.add_argument("--wake", default="auto", choices=["auto", "fft", "direct"])
+    ap.add_argument("--members", type=int, default=0, help="batch members (0 = the workload's own count)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU-oracle sample budget")
+    return ap.parse_args()
+
+
+def peaks():
+    """Measured roofline denominators (driver-written MEASURED_PEAKS.json), else the fallback of
+    B200_PROFILING.md."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    REASONS = {
+        0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+        0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+    }
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period_s
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                mask = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2.0)
+        med = int(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------- reference arm
+def time_oracle(wl, seconds: float, max_steps: int):
+    """Advance the CPU oracle (as it stands, OpenMP over its own loops) on member 0 of `wl` for
+    about `seconds`; returns (cell-updates/s, split steps done, seconds, threads)."""
+    import oracle
+    o = oracle.Oracle.from_workload(wl, 0)
+    t0 = time.perf_counter()
+    o.step(2, diag=True)                       # first-touch + a rate estimate
+    dt = (time.perf_counter() - t0) / 2
+    n = int(max(2, min(max_steps, seconds / max(dt, 1e-6))))
+    t0 = time.perf_counter()
+    o.step(n, diag=True)
+    el = time.perf_counter() - t0
+    return wl.N * wl.N * n / el, n, el, oracle.num_threads()
+
+
+def run_reference(args, wl, rank, world):
+    """--impl reference: the oracle on the host cores, rank 0 only (the other ranks exit 0)."""
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    n_inner = args.inner if args.inner > 0 else 25
+    o = oracle.Oracle.from_workload(wl, 0)
+    for _ in range(args.warmup):
+        o.step(n_inner, diag=True)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(n_inner, diag=True)
+    el = time.perf_counter() - t0
+    cells = wl.N * wl.N
+    value = cells * n_inner * args.steps / el
+    sample = (f"member 0 of {wl.name}: {args.steps} bench steps x {n_inner} split steps "
+              f"({wl.N}^2 cells, double precision, direct-convolution wake, diagnostics every step)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "steps_per_s": n_inner * args.steps / el,
+        "config": {"workload": wl.name, "N": wl.N, "members": 1, "split_steps_per_bench_step": n_inner,
+                   "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
+                   "note": "CPU oracle on a bounded sample of the workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------ our arm
+ENGINES = {"auto": 0, "stream": 1, "graph": 2, "cluster": 3}
+WAKES = {"auto": 0, "fft": 1, "direct": 2}
+
+
+def run_ours(args, wl, rank, local_rank, world):
+    import torch
+    import paper_1611_05293_b200 as pkg
+    from paper_1611_05293_b200 import dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the vfps library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:                                   # replicas: independent simulations per rank
+        wl = wl.with_(seeds=dist.replica_seeds(wl.seeds, rank))
+    members = args.members if args.members > 0 else wl.members
+    idx = list(range(members))
+    if members > wl.members:
+        raise SystemExit("--members exceeds the workload's member count")
+    n_inner = args.inner if args.inner > 0 else wl.steps_per_period
+    cells = wl.N * wl.N * members
+
+    psi0 = wl.psi0(idx)
+    Z = wl.impedance(idx)
+    sim = pkg.Simulation(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
+                         wl.interp_order, wl.pad, members, Z=Z)
+    sim.set_engine(ENGINES[args.engine])
+    sim.set_wake_mode(WAKES[args.wake])
+    sim.set_psi_host(psi0)
+    diag = torch.zeros(n_inner, members, 6, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    # ---- device-resident timing: W warm-up + K timed bench steps, L2 flushed between them
+    for _ in range(max(args.warmup, 0)):
+        sim.step(n_inner, diag)
+    torch.cuda.synchronize()
+    dist.barrier()
+    sim.set_option(pkg.OPT_TIMING, 1)
+    sim.reset_kernel_times()
+    l0 = sim.launch_count()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)
+        ev[k][0].record()
+        sim.step(n_inner, diag)
+        ev[k][1].record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    dist.barrier()
+    ms_local = sum(a.elapsed_time(b) for a, b in ev)
+    launches = sim.launch_count() - l0
+    ktimes = sim.kernel_times()
+    sim.set_option(pkg.OPT_TIMING, 0)
+    ms = dist.reduce_max(ms_local, dev)
+    engine, wake = sim.engine_name, sim.wake_name
+    diag_last = diag[-1].cpu().numpy().astype(float)
+    value = cells * n_inner * args.steps * world / (ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (device events bracketing each launch of that kernel)
+    hbm_peak, peak_src = peaks()
+    if not any(c for _, (_, c) in ktimes.items()):
+        # engines that replay a graph cannot bracket single kernels: same kernels, stream engine
+        sim.set_engine(ENGINES["stream"])
+        sim.set_option(pkg.OPT_TIMING, 1)
+        sim.reset_kernel_times()
+        sim.step(min(n_inner, 256), diag[: min(n_inner, 256)])
+        torch.cuda.synchronize()
+        ktimes = sim.kernel_times()
+        sim.set_option(pkg.OPT_TIMING, 0)
+        sim.set_engine(ENGINES[args.engine])
+    tot = sum(t for _, (t, c) in ktimes.items())
+    kname, (kt, kc) = max(ktimes.items(), key=lambda kv: kv[1][0])
+    steps_per_launch = n_inner if kname.startswith("k_cluster") else 1
+    alg_bytes = ALG_BYTES_PER_CELL_STEP * cells * steps_per_launch
+    achieved = alg_bytes / (kt / kc * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": 1e3 * kt / kc,
+                "share_of_step": kt / tot if tot > 0 else None,
+                "kernels_ms": {k: {"ms": t, "launches": c} for k, (t, c) in ktimes.items()}}
+
+    # ---- end to end through the host-pointer entry points (pinned host buffers)
+    e2e = None
+    if not args.no_e2e:
+        pin_in = torch.from_numpy(psi0).pin_memory()
+        k_e2e = max(1, min(args.steps, 5))
+        sim.set_psi_host(pin_in.numpy()); sim.step_host(n_inner); sim.get_psi_host()     # warm-up
+        torch.cuda.synchronize()
+        dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            sim.set_psi_host(pin_in.numpy())
+            d_host = sim.step_host(n_inner)
+            psi_host = sim.get_psi_host()
+        torch.cuda.synchronize()
+        el = dist.reduce_max(time.perf_counter() - t0, dev)
+        e2e = {"value": cells * n_inner * k_e2e * world / el, "unit": UNIT,
+               "h2d_bytes_per_step": int(psi0.nbytes), "d2h_bytes_per_step": int(psi_host.nbytes + d_host.nbytes),
+               "bench_steps": k_e2e, "ms_per_step": 1e3 * el / k_e2e}
+    sim.close()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        v, n, el, thr = time_oracle(wl, args.cpu_seconds, 100000)
+        cpu = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
+               "sample": f"member 0 of {wl.name}, {n} split steps in {el:.1f} s (double precision, OpenMP)"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "steps_per_s": n_inner * args.steps / (ms * 1e-3),
+            "us_per_split_step": 1e3 * ms / (n_inner * args.steps),
+            "config": {"workload": wl.name, "N": wl.N, "members": members, "split_steps_per_bench_step": n_inner,
+                       "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
+                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake,
+                       "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
+                       "l2": "256 MB buffer written between timed bench steps (L2 flush)"},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks,
+            "diag_last": {"C": diag_last[0, 0], "sigma_q": diag_last[0, 3], "sigma_p": diag_last[0, 4],
+                          "P_csr": diag_last[0, 5]},
+        }
+        print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    from workloads import get_workload
+    wl = get_workload(args.workload)
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        run_reference(args, wl, rank, int(os.environ.get("WORLD_SIZE", "1")))
+        return
+    from paper_1611_05293_b200 import dist
+    rank, local_rank, world = dist.init("nccl")
+    try:
+        run_ours(args, wl, rank, local_rank, world)
+    finally:
+        dist.shutdown()
+
+
+if __name__ == "__main__":
+    main()

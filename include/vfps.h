@@ -76,7 +76,17 @@ typedef struct vfps_params {
 /* Run-time options (vfps_set_option).  All engines and wake modes compute the same step. */
 enum {
     VFPS_OPT_ENGINE = 1,   /* how n steps are issued                                             */
-    VFPS_OPT_WAKE = 2      /* how a3 is evaluated                                                */
+    VFPS_OPT_WAKE = 2,     /* how a3 is evaluated                                                */
+    VFPS_OPT_TIMING = 3    /* 0/1: bracket kernel launches with CUDA events (measurement aid; while
+                              on, vfps_step may synchronise the stream to read finished events)  */
+};
+/* kernel ids of vfps_kernel_time / vfps_kernel_name */
+enum {
+    VFPS_KERNEL_ROTATE = 0,   /* a1 + a2 partial sums                                            */
+    VFPS_KERNEL_WAKE = 1,     /* a2 finish + a3 + q-moments + CSR power                          */
+    VFPS_KERNEL_KICK_FP = 2,  /* a4 + a5 + a6                                                    */
+    VFPS_KERNEL_CLUSTER = 3,  /* a1..a6 for all n steps of one vfps_step call (cluster engine)   */
+    VFPS_NUM_KERNELS = 4
 };
 enum {
     VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRAPH                    */
@@ -144,6 +154,15 @@ int vfps_step_count(vfps_handle h, long long *count);
 
 /* Kernel launches (graph nodes included) issued by this handle so far. */
 int vfps_launch_count(vfps_handle h, long long *count);
+
+/* Device time spent in one kernel of the hot path, accumulated while VFPS_OPT_TIMING is 1:
+ * total milliseconds between the CUDA events bracketing each launch, and the number of launches
+ * bracketed (STREAM engine: the first 256 steps of every vfps_step call; CLUSTER engine: every
+ * call; the GRAPH engine replays a captured graph and brackets nothing).  Synchronises the stream.
+ * vfps_kernel_name(k) is NULL for k outside 0..VFPS_NUM_KERNELS-1. */
+int vfps_kernel_time(vfps_handle h, int kernel, double *ms_total, long long *launches);
+int vfps_reset_kernel_times(vfps_handle h);
+const char *vfps_kernel_name(int kernel);
 
 /* Name of the engine / wake mode the next vfps_step will use ("stream", "graph", "cluster";
  * "fft", "direct"); static strings. */

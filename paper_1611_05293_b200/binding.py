@@ -15,7 +15,8 @@ from .build import build, lib_path
 
 ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER = 0, 1, 2, 3
 WAKE_AUTO, WAKE_FFT, WAKE_DIRECT = 0, 1, 2
-OPT_ENGINE, OPT_WAKE = 1, 2
+OPT_ENGINE, OPT_WAKE, OPT_TIMING = 1, 2, 3
+NUM_KERNELS = 4
 FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 
 # every symbol include/vfps.h declares (tests check the library exports each of them)
@@ -25,6 +26,7 @@ EXPORTS = [
     "vfps_get_psi", "vfps_get_psi_host", "vfps_get_profile", "vfps_get_profile_host",
     "vfps_get_wake", "vfps_get_wake_host", "vfps_get_moments", "vfps_get_moments_host",
     "vfps_step_count", "vfps_launch_count", "vfps_engine_name", "vfps_wake_name",
+    "vfps_kernel_time", "vfps_reset_kernel_times", "vfps_kernel_name",
     "vfps_last_error", "vfps_version",
 ]
 
@@ -66,7 +68,10 @@ def load():
     L.vfps_step_host.argtypes = [vp, ip, vp]
     L.vfps_step_count.argtypes = [vp, C.POINTER(C.c_longlong)]
     L.vfps_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
-    strings = ("vfps_engine_name", "vfps_wake_name", "vfps_last_error", "vfps_version")
+    L.vfps_kernel_time.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.vfps_reset_kernel_times.argtypes = [vp]
+    L.vfps_kernel_name.argtypes = [ip]
+    strings = ("vfps_engine_name", "vfps_wake_name", "vfps_last_error", "vfps_version", "vfps_kernel_name")
     for name in EXPORTS:
         getattr(L, name).restype = C.c_char_p if name in strings else C.c_int
     for name in strings[:3]:
@@ -177,6 +182,18 @@ class Simulation:
         v = C.c_longlong()
         self._check(self._L.vfps_step_count(self._h, C.byref(v)))
         return v.value
+
+    def kernel_times(self) -> dict:
+        """{kernel name: (total ms, launches bracketed)} accumulated while OPT_TIMING is on."""
+        out = {}
+        for k in range(NUM_KERNELS):
+            ms, cnt = C.c_double(), C.c_longlong()
+            self._check(self._L.vfps_kernel_time(self._h, k, C.byref(ms), C.byref(cnt)))
+            out[self._L.vfps_kernel_name(k).decode()] = (ms.value, cnt.value)
+        return out
+
+    def reset_kernel_times(self) -> None:
+        self._check(self._L.vfps_reset_kernel_times(self._h))
 
     def launch_count(self) -> int:
         v = C.c_longlong()

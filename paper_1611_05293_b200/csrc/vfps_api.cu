@@ -49,6 +49,17 @@ struct vfps_sim {
     size_t rot_smem = 0, kfp_smem = 0, fft_smem = 0;
     int fft_threads = 0;
 
+    // CUDA-graph engine: GRAPH_STEPS split steps captured once, replayed
+    cudaGraphExec_t graph_exec = nullptr;
+    // per-kernel device timing (VFPS_OPT_TIMING): event pairs around launches, resolved lazily
+    bool timing = false;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> ev_kind;                    // kernel id of pair i (events 2i, 2i+1)
+    double k_ms[VFPS_NUM_KERNELS] = {0, 0, 0, 0};
+    long long k_cnt[VFPS_NUM_KERNELS] = {0, 0, 0, 0};
+    float *diag_scratch = nullptr;               // vfps_step_host staging (grow-only)
+    size_t diag_scratch_n = 0;
+
     bool psi_set = false;
     long long steps = 0, launches = 0;
     std::string err;
@@ -129,33 +140,114 @@ void grid_constants(vfps_sim *h)
     G.H = (int)std::floor(dmax * 1.0001 + 1e-6) + 2;
 }
 
+constexpr int GRAPH_STEPS = 50;          // split steps per captured graph (150 kernel nodes)
+constexpr size_t EV_PAIRS_MAX = 3 * 256;  // timed launches per vfps_step call
+
+// bracket the next launch of kernel `kind` with an event pair (timing mode, stream engine only)
+struct Bracket {
+    vfps_sim *h; cudaEvent_t e1 = nullptr;
+    Bracket(vfps_sim *h_, int kind, bool on) : h(h_)
+    {
+        if (!on || h->ev_kind.size() >= EV_PAIRS_MAX) return;
+        const size_t i = h->ev_kind.size();
+        while (h->ev_pool.size() < 2 * (i + 1)) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return;
+            h->ev_pool.push_back(e);
+        }
+        h->ev_kind.push_back(kind);
+        cudaEventRecord(h->ev_pool[2 * i], h->stream);
+        e1 = h->ev_pool[2 * i + 1];
+    }
+    ~Bracket() { if (e1) cudaEventRecord(e1, h->stream); }
+};
+
+// fold finished event pairs into the per-kernel totals (synchronises the stream)
+void resolve_timing(vfps_sim *h)
+{
+    if (h->ev_kind.empty()) return;
+    cudaStreamSynchronize(h->stream);
+    for (size_t i = 0; i < h->ev_kind.size(); ++i) {
+        float ms = 0.0f;
+        if (cudaEventElapsedTime(&ms, h->ev_pool[2 * i], h->ev_pool[2 * i + 1]) == cudaSuccess) {
+            h->k_ms[h->ev_kind[i]] += ms;
+            h->k_cnt[h->ev_kind[i]] += 1;
+        }
+    }
+    h->ev_kind.clear();
+}
+
 template <int ORDER>
-int launch_step_stream(vfps_sim *h)
+int launch_step_stream(vfps_sim *h, bool timed)
 {
     const int N = h->N;
     dim3 g1(h->tiles_x * h->tiles_y, h->members);
-    k_rotate<ORDER><<<g1, ROT_THREADS, h->rot_smem, h->stream>>>(h->G, h->psi, h->psi_tmp, h->scale,
-                                                                  h->rho_part, h->tiles_y);
-    k_wake_fft<<<h->members, h->fft_threads, h->fft_smem, h->stream>>>(
-        N, h->Nf, h->log2Nf, h->G.dq, h->rho_part, h->tiles_y, h->has_wake ? h->Z : nullptr, h->tw,
-        h->rho, h->V, h->qstat);
+    {
+        Bracket br(h, VFPS_KERNEL_ROTATE, timed);
+        k_rotate<ORDER><<<g1, ROT_THREADS, h->rot_smem, h->stream>>>(h->G, h->psi, h->psi_tmp, h->scale,
+                                                                      h->rho_part, h->tiles_y);
+    }
+    {
+        Bracket br(h, VFPS_KERNEL_WAKE, timed);
+        k_wake_fft<<<h->members, h->fft_threads, h->fft_smem, h->stream>>>(
+            N, h->Nf, h->log2Nf, h->G.dq, h->rho_part, h->tiles_y, h->has_wake ? h->Z : nullptr, h->tw,
+            h->rho, h->V, h->qstat);
+    }
     KfpArgs A;
     A.psi_in = h->psi_tmp; A.psi_out = h->psi; A.V = h->V; A.qstat = h->qstat;
     A.mom_part = h->mom_part; A.scale = h->scale; A.blkctr = h->blkctr; A.rowctr = h->rowctr;
     A.diag = h->diag_cell; A.members = h->members; A.rows_per_cta = h->kfp_rows;
     dim3 g3(h->kfp_blocks, h->members);
-    k_kick_fp<ORDER><<<g3, KFP_THREADS, h->kfp_smem, h->stream>>>(h->G, A);
+    {
+        Bracket br(h, VFPS_KERNEL_KICK_FP, timed);
+        k_kick_fp<ORDER><<<g3, KFP_THREADS, h->kfp_smem, h->stream>>>(h->G, A);
+    }
     h->launches += 3;
     return VFPS_OK;
 }
 
-int launch_step(vfps_sim *h)
+int launch_step(vfps_sim *h, bool timed)
 {
     switch (h->P.interp_order) {
-        case 2: return launch_step_stream<2>(h);
-        case 3: return launch_step_stream<3>(h);
-        default: return launch_step_stream<4>(h);
+        case 2: return launch_step_stream<2>(h, timed);
+        case 3: return launch_step_stream<3>(h, timed);
+        default: return launch_step_stream<4>(h, timed);
     }
+}
+
+// the engine the next vfps_step uses
+int resolved_engine(const vfps_sim *h)
+{
+    if (h->engine_opt == VFPS_ENGINE_STREAM) return VFPS_ENGINE_STREAM;
+    return VFPS_ENGINE_GRAPH;                      // AUTO and GRAPH
+}
+
+// capture GRAPH_STEPS split steps once; every step is the same three launches (the diag row and
+// the caller's diag pointer live in device memory), so the instantiated graph is reusable
+int ensure_graph(vfps_sim *h)
+{
+    if (h->graph_exec) return VFPS_OK;
+    cudaStream_t cap = nullptr;
+    CU(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = h->stream;
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        h->stream = cap;
+        const long long l0 = h->launches;
+        for (int i = 0; i < GRAPH_STEPS; ++i) launch_step(h, false);
+        h->launches = l0;
+        h->stream = user;
+        e = cudaStreamEndCapture(cap, &g);
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&h->graph_exec, g, 0);
+    if (g) cudaGraphDestroy(g);
+    cudaStreamDestroy(cap);
+    if (e != cudaSuccess) {
+        h->graph_exec = nullptr;
+        return fail(h, VFPS_ERR_CUDA, std::string("CUDA graph capture: ") + cudaGetErrorString(e));
+    }
+    return VFPS_OK;
 }
 
 template <int ORDER>
@@ -308,6 +400,9 @@ int vfps_destroy(vfps_handle h)
 {
     if (!h) return VFPS_OK;
     cudaStreamSynchronize(h->stream);
+    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+    for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+    if (h->diag_scratch) cudaFree(h->diag_scratch);
     for (void *p : h->owned) cudaFree(p);
     delete h;
     return VFPS_OK;
@@ -317,10 +412,19 @@ int vfps_set_option(vfps_handle h, int option, int value)
 {
     if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
     if (option == VFPS_OPT_ENGINE) {
-        if (value == VFPS_ENGINE_AUTO || value == VFPS_ENGINE_STREAM) { h->engine_opt = value; return VFPS_OK; }
-        if (value == VFPS_ENGINE_GRAPH || value == VFPS_ENGINE_CLUSTER)
+        if (value == VFPS_ENGINE_AUTO || value == VFPS_ENGINE_STREAM || value == VFPS_ENGINE_GRAPH) {
+            h->engine_opt = value;
+            return VFPS_OK;
+        }
+        if (value == VFPS_ENGINE_CLUSTER)
             return fail(h, VFPS_ERR_UNSUPPORTED, "engine not available in this build");
         return fail(h, VFPS_ERR_ARG, "unknown engine");
+    }
+    if (option == VFPS_OPT_TIMING) {
+        if (value != 0 && value != 1) return fail(h, VFPS_ERR_ARG, "timing must be 0 or 1");
+        if (!value) resolve_timing(h);
+        h->timing = (value == 1);
+        return VFPS_OK;
     }
     if (option == VFPS_OPT_WAKE) {
         if (value == VFPS_WAKE_AUTO || value == VFPS_WAKE_FFT) { h->wake_opt = value; return VFPS_OK; }
@@ -335,10 +439,19 @@ int vfps_get_option(vfps_handle h, int option, int *value)
     if (!h || !value) return fail(h, VFPS_ERR_ARG, "NULL argument");
     if (option == VFPS_OPT_ENGINE) { *value = h->engine_opt; return VFPS_OK; }
     if (option == VFPS_OPT_WAKE) { *value = h->wake_opt; return VFPS_OK; }
+    if (option == VFPS_OPT_TIMING) { *value = h->timing ? 1 : 0; return VFPS_OK; }
     return fail(h, VFPS_ERR_ARG, "unknown option");
 }
 
-const char *vfps_engine_name(vfps_handle h) { (void)h; return "stream"; }
+const char *vfps_engine_name(vfps_handle h)
+{
+    if (!h) return "";
+    switch (resolved_engine(h)) {
+        case VFPS_ENGINE_STREAM: return "stream";
+        case VFPS_ENGINE_GRAPH: return "graph";
+        default: return "cluster";
+    }
+}
 const char *vfps_wake_name(vfps_handle h) { (void)h; return "fft"; }
 
 static int set_psi_impl(vfps_handle h, const float *psi, cudaMemcpyKind kind)
@@ -367,8 +480,20 @@ int vfps_step(vfps_handle h, int n, float *diag)
     if (n == 0) return VFPS_OK;
     k_set_ctl<<<(h->members + 255) / 256, 256, 0, h->stream>>>(h->diag_cell, diag, h->rowctr, h->blkctr, h->members);
     h->launches += 1;
-    for (int i = 0; i < n; ++i) {
-        int rc = launch_step(h);
+    int done = 0;
+    if (resolved_engine(h) == VFPS_ENGINE_GRAPH && n >= GRAPH_STEPS) {
+        int rc = ensure_graph(h);
+        if (rc != VFPS_OK) return rc;
+        for (; done + GRAPH_STEPS <= n; done += GRAPH_STEPS) {
+            CU(cudaGraphLaunch(h->graph_exec, h->stream));
+            h->launches += 3 * GRAPH_STEPS;
+        }
+    }
+    // stream engine, and the remainder of a graph run
+    const bool timed = h->timing && resolved_engine(h) == VFPS_ENGINE_STREAM;
+    if (timed) resolve_timing(h);
+    for (; done < n; ++done) {
+        int rc = launch_step(h, timed);
         if (rc != VFPS_OK) return rc;
     }
     CU(cudaGetLastError());
@@ -382,7 +507,16 @@ int vfps_step_host(vfps_handle h, int n, float *diag_host)
     if (n < 0) return fail(h, VFPS_ERR_ARG, "n must be >= 0");
     float *d = nullptr;
     const size_t cnt = (size_t)n * h->members * 6;
-    if (diag_host && cnt) CU(cudaMalloc((void **)&d, cnt * sizeof(float)));
+    if (diag_host && cnt) {
+        if (cnt > h->diag_scratch_n) {
+            CU(cudaStreamSynchronize(h->stream));
+            if (h->diag_scratch) cudaFree(h->diag_scratch);
+            h->diag_scratch = nullptr; h->diag_scratch_n = 0;
+            CU(cudaMalloc((void **)&h->diag_scratch, cnt * sizeof(float)));
+            h->diag_scratch_n = cnt;
+        }
+        d = h->diag_scratch;
+    }
     int rc = vfps_step(h, n, d);
     if (rc == VFPS_OK) {
         cudaError_t e = d ? cudaMemcpyAsync(diag_host, d, cnt * sizeof(float), cudaMemcpyDeviceToHost, h->stream)
@@ -390,7 +524,6 @@ int vfps_step_host(vfps_handle h, int n, float *diag_host)
         if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
         if (e != cudaSuccess) rc = fail(h, VFPS_ERR_CUDA, cudaGetErrorString(e));
     }
-    if (d) cudaFree(d);
     return rc;
 }
 
@@ -494,6 +627,35 @@ int vfps_launch_count(vfps_handle h, long long *count)
     if (!h || !count) return fail(h, VFPS_ERR_ARG, "NULL argument");
     *count = h->launches;
     return VFPS_OK;
+}
+
+int vfps_kernel_time(vfps_handle h, int kernel, double *ms_total, long long *launches)
+{
+    if (!h || !ms_total || !launches) return fail(h, VFPS_ERR_ARG, "NULL argument");
+    if (kernel < 0 || kernel >= VFPS_NUM_KERNELS) return fail(h, VFPS_ERR_ARG, "unknown kernel id");
+    resolve_timing(h);
+    *ms_total = h->k_ms[kernel];
+    *launches = h->k_cnt[kernel];
+    return VFPS_OK;
+}
+
+int vfps_reset_kernel_times(vfps_handle h)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    resolve_timing(h);
+    for (int k = 0; k < VFPS_NUM_KERNELS; ++k) { h->k_ms[k] = 0.0; h->k_cnt[k] = 0; }
+    return VFPS_OK;
+}
+
+const char *vfps_kernel_name(int kernel)
+{
+    switch (kernel) {
+        case VFPS_KERNEL_ROTATE: return "k_rotate";
+        case VFPS_KERNEL_WAKE: return "k_wake_fft";
+        case VFPS_KERNEL_KICK_FP: return "k_kick_fp";
+        case VFPS_KERNEL_CLUSTER: return "k_cluster_step";
+        default: return nullptr;
+    }
 }
 
 const char *vfps_last_error(vfps_handle h) { return h ? h->err.c_str() : g_create_error.c_str(); }

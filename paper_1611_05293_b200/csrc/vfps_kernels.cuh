@@ -122,14 +122,16 @@ k_rotate(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_
     const float sc = G.renorm ? __ldg(scale + m) : 1.0f;
     const int wy = warp & 3, wx = warp >> 2;
     const int y = ty0 + wy * 32 + lane;
-    const float Y = (float)y + G.y0c;
+    // lanes / rows beyond the grid (partial tiles) compute with the last valid coordinate so that
+    // their taps stay inside the staged tile; their results are never stored
+    const float Y = (float)min(y, N - 1) + G.y0c;
     const float bY = G.b * Y, aY = G.a * Y;
     constexpr int O0 = (ORDER - 1) / 2;       // offset of the first node below m
 
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         const int x = tx0 + wx * 8 + r;
-        const float X = (float)x + G.x0c;
+        const float X = (float)min(x, N - 1) + G.x0c;
         const float dx = fmaf(G.a, X, bY);
         const float dy = fmaf(G.d, X, aY);
         const float fx = floorf(dx), fy = floorf(dy);
@@ -137,8 +139,8 @@ k_rotate(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_
         lagrange<ORDER>(dx - fx, lx);
         lagrange<ORDER>(dy - fy, ly);
         // tile coordinates of the first tap
-        const int ix = (x - tx0) + H + (int)fx - O0;
-        const int iy = (y - ty0) + H + (int)fy - O0;
+        const int ix = (min(x, N - 1) - tx0) + H + (int)fx - O0;
+        const int iy = (min(y, N - 1) - ty0) + H + (int)fy - O0;
         const float *t0 = tile + ix * pitch + iy;
         float acc = 0.0f;
 #pragma unroll

@@ -26,8 +26,14 @@ def assert_psi(sim_psi, ref_psi, tol, what=""):
 def assert_diag(got, want, has_wake=True, tol_q=TOL_MOM):
     """tol_q: tolerance of the three numbers taken from the post-rotation profile (<q>, sigma_q,
     P_csr); equal to TOL_MOM unless the bunch overflows the box (edge flux)."""
-    got = np.asarray(got, dtype=np.float64)
-    want = np.asarray(want, dtype=np.float64)
+    got = np.array(got, dtype=np.float64)
+    want = np.array(want, dtype=np.float64)
+    # a negative variance (quadratic/cubic overshoot on a grid too coarse for the bunch) has no
+    # sigma: the oracle reports NaN, the library 0 -- both mean "undefined"
+    for k in (3, 4):
+        if np.isnan(want[k]):
+            assert got[k] == 0.0, ("undefined sigma", k, got[k])
+            got[k] = want[k] = 1.0
     assert abs(got[0] - want[0]) <= TOL_MOM * abs(want[0]), ("C", got[0], want[0])
     assert abs(got[1] - want[1]) <= tol_q * want[3], ("<q>", got[1], want[1])
     assert abs(got[2] - want[2]) <= TOL_MOM * want[4], ("<p>", got[2], want[2])
