@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--inner", type=int, default=0, help="split steps per bench step (0 = one synchrotron period)")
     ap.add_argument("--engine", default="auto", choices=["auto", "stream", "graph", "cluster"])
     ap.add_argument("--wake", default="auto", choices=["auto", "fft", "direct"])
+    ap.add_argument("--cluster-size", type=int, default=0, help="CTAs per cluster of the cluster engine (0 = auto)")
     ap.add_argument("--members", type=int, default=0, help="batch members (0 = the workload's own count)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -191,6 +192,8 @@ def run_ours(args, wl, rank, local_rank, world):
     Z = wl.impedance(idx)
     sim = pkg.Simulation(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
                          wl.interp_order, wl.pad, members, Z=Z)
+    if args.cluster_size:
+        sim.set_cluster_size(args.cluster_size)
     sim.set_engine(ENGINES[args.engine])
     sim.set_wake_mode(WAKES[args.wake])
     sim.set_psi_host(psi0)
@@ -222,6 +225,7 @@ def run_ours(args, wl, rank, local_rank, world):
     sim.set_option(pkg.OPT_TIMING, 0)
     ms = dist.reduce_max(ms_local, dev)
     engine, wake = sim.engine_name, sim.wake_name
+    cluster_size = sim.cluster_size if engine == "cluster" else None
     diag_last = diag[-1].cpu().numpy().astype(float)
     value = cells * n_inner * args.steps * world / (ms * 1e-3)
 
@@ -285,7 +289,7 @@ def run_ours(args, wl, rank, local_rank, world):
             "us_per_split_step": 1e3 * ms / (n_inner * args.steps),
             "config": {"workload": wl.name, "N": wl.N, "members": members, "split_steps_per_bench_step": n_inner,
                        "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
-                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake,
+                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size,
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                        "l2": "256 MB buffer written between timed bench steps (L2 flush)"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),

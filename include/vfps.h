@@ -77,8 +77,10 @@ typedef struct vfps_params {
 enum {
     VFPS_OPT_ENGINE = 1,   /* how n steps are issued                                             */
     VFPS_OPT_WAKE = 2,     /* how a3 is evaluated                                                */
-    VFPS_OPT_TIMING = 3    /* 0/1: bracket kernel launches with CUDA events (measurement aid; while
+    VFPS_OPT_TIMING = 3,   /* 0/1: bracket kernel launches with CUDA events (measurement aid; while
                               on, vfps_step may synchronise the stream to read finished events)  */
+    VFPS_OPT_CLUSTER_SIZE = 4  /* CTAs per cluster of the CLUSTER engine: 0 = auto, 1, 2, 4, 8, 16;
+                              vfps_get_option returns the size in use (0 = engine unavailable)  */
 };
 /* kernel ids of vfps_kernel_time / vfps_kernel_name */
 enum {
@@ -125,8 +127,9 @@ int vfps_set_psi_host(vfps_handle h, const float *psi_host);
 
 /* Advance n >= 0 steps a1..a6.  diag: NULL or [n][members][6] floats; row (i, m) =
  * { C (charge before renormalisation), <q>, <p>, sigma_q, sigma_p, P_csr } after step i.
- * <q>, sigma_q and P_csr are taken from the post-rotation profile of the same step (kick and
- * Fokker-Planck act along p only and leave rho unchanged up to edge flux), P scaled by 1/C^2.
+ * All moments are those of the end-of-step psi.  P_csr is taken from the post-rotation profile of
+ * the same step, scaled by 1/C^2 (kick and Fokker-Planck act along p only and leave rho unchanged
+ * up to the flux over the p edges of the box).
  * Asynchronous on the handle's stream.  vfps_step_host copies diag to host memory and returns
  * when the n steps have completed. */
 int vfps_step(vfps_handle h, int n, float *diag);

@@ -7,7 +7,7 @@ shared library cannot be built or loaded, importing symbols from it raises.
 from .build import build, lib_path
 from .binding import (
     ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER,
-    WAKE_AUTO, WAKE_FFT, WAKE_DIRECT, OPT_ENGINE, OPT_WAKE, OPT_TIMING,
+    WAKE_AUTO, WAKE_FFT, WAKE_DIRECT, OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE,
     FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN,
     VfpsError, VfpsParams, Simulation, load, version, EXPORTS,
 )
@@ -15,7 +15,7 @@ from .binding import (
 __all__ = [
     "build", "lib_path", "load", "version", "EXPORTS",
     "ENGINE_AUTO", "ENGINE_STREAM", "ENGINE_GRAPH", "ENGINE_CLUSTER",
-    "WAKE_AUTO", "WAKE_FFT", "WAKE_DIRECT", "OPT_ENGINE", "OPT_WAKE", "OPT_TIMING",
+    "WAKE_AUTO", "WAKE_FFT", "WAKE_DIRECT", "OPT_ENGINE", "OPT_WAKE", "OPT_TIMING", "OPT_CLUSTER_SIZE",
     "FLAG_RENORMALISE", "FLAG_CLAMP", "FLAG_ROT_MANHATTAN",
     "VfpsError", "VfpsParams", "Simulation",
 ]

@@ -15,7 +15,7 @@ from .build import build, lib_path
 
 ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER = 0, 1, 2, 3
 WAKE_AUTO, WAKE_FFT, WAKE_DIRECT = 0, 1, 2
-OPT_ENGINE, OPT_WAKE, OPT_TIMING = 1, 2, 3
+OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE = 1, 2, 3, 4
 NUM_KERNELS = 4
 FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 
@@ -169,6 +169,18 @@ class Simulation:
 
     def set_wake_mode(self, mode: int) -> None:
         self.set_option(OPT_WAKE, mode)
+
+    def get_option(self, option: int) -> int:
+        v = C.c_int()
+        self._check(self._L.vfps_get_option(self._h, option, C.byref(v)))
+        return v.value
+
+    def set_cluster_size(self, size: int) -> None:
+        self.set_option(OPT_CLUSTER_SIZE, size)
+
+    @property
+    def cluster_size(self) -> int:
+        return self.get_option(OPT_CLUSTER_SIZE)
 
     @property
     def engine_name(self) -> str:

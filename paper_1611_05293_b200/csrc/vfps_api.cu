@@ -2,6 +2,7 @@
 // argument checks, device-memory ownership, launch configuration, engine selection.
 #include "../../include/vfps.h"
 #include "vfps_kernels.cuh"
+#include "vfps_cluster.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -36,7 +37,7 @@ struct vfps_sim {
     float *rho_part = nullptr;                   // [members][N][tiles_y]
     float *rho = nullptr, *V = nullptr;          // [members][N]
     float *qstat = nullptr;                      // [members][4]
-    float *mom_part = nullptr;                   // [members][kfp_blocks][3]
+    float *mom_part = nullptr;                   // [members][kfp_blocks][5]
     float *scale = nullptr;                      // [members]
     unsigned *blkctr = nullptr;                  // [members]
     int *rowctr = nullptr;                       // [members]
@@ -44,6 +45,12 @@ struct vfps_sim {
     // scratch for the stateless get_* calls
     float *g_rho = nullptr, *g_V = nullptr, *g_m1 = nullptr, *g_m2 = nullptr, *g_qstat = nullptr;
     float *g_out = nullptr;                      // [members][max(N,6)] staging for *_host variants
+
+    float *wfun = nullptr;                       // [members][2N] wake function w = Re IDFT(Z)
+    // cluster engine (0 = not available for this grid)
+    int cl_S = 0, cl_S_opt = 0, cl_max_clusters = 0;
+    size_t cl_smem = 0;
+    std::string cl_why;                          // why the cluster engine is unavailable
 
     int tiles_x = 0, tiles_y = 0, kfp_rows = 0, kfp_blocks = 0;
     size_t rot_smem = 0, kfp_smem = 0, fft_smem = 0;
@@ -177,6 +184,125 @@ void resolve_timing(vfps_sim *h)
     h->ev_kind.clear();
 }
 
+
+// ---------------------------------------------------------------- wake function w = Re IDFT(Z)
+// One thread per (member, lag d = -(N-1)..N-1); double precision, angle reduced in integers.
+// w[d] = (1/Nf) [ Re Z_0 + 2 sum_{k=1}^{Nf/2-1} Re(Z_k e^{2 pi i k d/Nf}) + Re Z_{Nf/2} (-1)^d ]
+// (Hermitian spectrum, L149); stored at index d + N - 1 of a row of 2N floats.
+__global__ void k_wake_function(int N, int Nf, int members, const float2 *__restrict__ Z, float *__restrict__ w)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= members * 2 * N) return;
+    const int m = i / (2 * N), j = i - m * 2 * N;
+    if (j >= 2 * N - 1) { w[i] = 0.0f; return; }
+    const int d = j - (N - 1);
+    const float2 *Zm = Z + (size_t)m * (Nf / 2 + 1);
+    double acc = (double)Zm[0].x;
+    for (int k = 1; k < Nf / 2; ++k) {
+        long long kd = ((long long)k * d) % Nf;
+        double sn, cs;
+        sincospi(2.0 * (double)kd / (double)Nf, &sn, &cs);
+        acc += 2.0 * ((double)Zm[k].x * cs - (double)Zm[k].y * sn);
+    }
+    acc += (double)Zm[Nf / 2].x * ((d & 1) ? -1.0 : 1.0);
+    w[i] = (float)(acc / (double)Nf);
+}
+
+template <int ORDER, int N>
+cudaError_t cluster_launch_t(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *max_clusters)
+{
+    auto kern = k_cluster_step<ORDER, N>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->cl_smem);
+    if (e != cudaSuccess) return e;
+    if (A.S > 8) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(A.S * nclusters));
+    cfg.blockDim = dim3(CL_THREADS);
+    cfg.dynamicSmemBytes = h->cl_smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)A.S;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (query) return cudaOccupancyMaxActiveClusters(max_clusters, kern, &cfg);
+    return cudaLaunchKernelEx(&cfg, kern, h->G, A);
+}
+
+template <int ORDER>
+cudaError_t cluster_launch_o(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *mc)
+{
+    switch (h->N) {
+        case 32: return cluster_launch_t<ORDER, 32>(h, A, nclusters, query, mc);
+        case 64: return cluster_launch_t<ORDER, 64>(h, A, nclusters, query, mc);
+        case 128: return cluster_launch_t<ORDER, 128>(h, A, nclusters, query, mc);
+        case 256: return cluster_launch_t<ORDER, 256>(h, A, nclusters, query, mc);
+        case 512: return cluster_launch_t<ORDER, 512>(h, A, nclusters, query, mc);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *mc)
+{
+    switch (h->P.interp_order) {
+        case 2: return cluster_launch_o<2>(h, A, nclusters, query, mc);
+        case 3: return cluster_launch_o<3>(h, A, nclusters, query, mc);
+        default: return cluster_launch_o<4>(h, A, nclusters, query, mc);
+    }
+}
+
+// Pick the cluster size: the request (cl_S_opt) if feasible; otherwise the largest feasible size
+// for a single simulation (shortest step), the smallest for a batch (most work per barrier).
+void cluster_configure(vfps_sim *h)
+{
+    h->cl_S = 0; h->cl_max_clusters = 0; h->cl_why.clear();
+    const int N = h->N, H = h->G.H;
+    if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
+    if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
+    int dev = 0, smem_max = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    const int cand_single[5] = {16, 8, 4, 2, 1}, cand_batch[5] = {1, 2, 4, 8, 16};
+    const int *cand = (h->members == 1) ? cand_single : cand_batch;
+    for (int c = 0; c < 5; ++c) {
+        const int S = cand[c];
+        if (h->cl_S_opt && S != h->cl_S_opt) continue;
+        if (N / S < (H > 1 ? H : 1) || N % S) continue;
+        const size_t bytes = cluster_smem_floats(N, S, H) * sizeof(float);
+        if (bytes > (size_t)smem_max) continue;
+        h->cl_smem = bytes;
+        ClusterArgs A{};
+        A.S = S; A.R = N / S;
+        int mc = 0;
+        cudaError_t e = cluster_launch(h, A, 1, true, &mc);
+        if (e != cudaSuccess || mc < 1) { cudaGetLastError(); continue; }
+        h->cl_S = S; h->cl_max_clusters = mc;
+        return;
+    }
+    h->cl_why = "no feasible cluster size (shared memory or cluster scheduling)";
+}
+
+int launch_cluster_steps(vfps_sim *h, int n, float *diag)
+{
+    ClusterArgs A{};
+    A.psi = h->psi; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr; A.diag = diag;
+    A.members = h->members; A.nsteps = n; A.S = h->cl_S; A.R = h->N / h->cl_S;
+    const int nclusters = h->members < h->cl_max_clusters ? h->members : h->cl_max_clusters;
+    cudaError_t e;
+    {
+        Bracket br(h, VFPS_KERNEL_CLUSTER, h->timing);
+        e = cluster_launch(h, A, nclusters, false, nullptr);
+    }
+    if (e != cudaSuccess) return fail(h, VFPS_ERR_CUDA, std::string("cluster launch: ") + cudaGetErrorString(e));
+    h->launches += 1;
+    return VFPS_OK;
+}
+
 template <int ORDER>
 int launch_step_stream(vfps_sim *h, bool timed)
 {
@@ -219,7 +345,8 @@ int launch_step(vfps_sim *h, bool timed)
 int resolved_engine(const vfps_sim *h)
 {
     if (h->engine_opt == VFPS_ENGINE_STREAM) return VFPS_ENGINE_STREAM;
-    return VFPS_ENGINE_GRAPH;                      // AUTO and GRAPH
+    if (h->engine_opt == VFPS_ENGINE_GRAPH) return VFPS_ENGINE_GRAPH;
+    return h->cl_S > 0 ? VFPS_ENGINE_CLUSTER : VFPS_ENGINE_GRAPH;      // AUTO, CLUSTER
 }
 
 // capture GRAPH_STEPS split steps once; every step is the same three launches (the diag row and
@@ -312,7 +439,7 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     CUB(dalloc(h, &h->rho, (size_t)M * N));
     CUB(dalloc(h, &h->V, (size_t)M * N));
     CUB(dalloc(h, &h->qstat, (size_t)M * 4));
-    CUB(dalloc(h, &h->mom_part, (size_t)M * h->kfp_blocks * 3));
+    CUB(dalloc(h, &h->mom_part, (size_t)M * h->kfp_blocks * 5));
     CUB(dalloc(h, &h->scale, (size_t)M));
     CUB(dalloc(h, &h->blkctr, (size_t)M));
     CUB(dalloc(h, &h->rowctr, (size_t)M));
@@ -345,6 +472,13 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     k_fill<<<(M + 255) / 256, 256, 0, h->stream>>>(h->scale, 1.0f, M);
     k_set_ctl<<<(M + 255) / 256, 256, 0, h->stream>>>(h->diag_cell, nullptr, h->rowctr, h->blkctr, M);
     h->launches += 2;
+    if (h->has_wake) {
+        CUB(dalloc(h, &h->wfun, (size_t)M * 2 * N));
+        const int nw = M * 2 * N;
+        k_wake_function<<<(nw + 127) / 128, 128, 0, h->stream>>>(N, h->Nf, M, h->Z, h->wfun);
+        h->launches += 1;
+    }
+    cluster_configure(h);
     cudaError_t e = cudaSuccess;
     switch (p->interp_order) {
         case 2: e = set_kernel_attrs<2>(h); break;
@@ -416,9 +550,26 @@ int vfps_set_option(vfps_handle h, int option, int value)
             h->engine_opt = value;
             return VFPS_OK;
         }
-        if (value == VFPS_ENGINE_CLUSTER)
-            return fail(h, VFPS_ERR_UNSUPPORTED, "engine not available in this build");
+        if (value == VFPS_ENGINE_CLUSTER) {
+            if (h->cl_S == 0) return fail(h, VFPS_ERR_UNSUPPORTED, "cluster engine unavailable: " + h->cl_why);
+            h->engine_opt = value;
+            return VFPS_OK;
+        }
         return fail(h, VFPS_ERR_ARG, "unknown engine");
+    }
+    if (option == VFPS_OPT_CLUSTER_SIZE) {
+        if (!(value == 0 || value == 1 || value == 2 || value == 4 || value == 8 || value == 16))
+            return fail(h, VFPS_ERR_ARG, "cluster size must be 0 (auto), 1, 2, 4, 8 or 16");
+        const int old = h->cl_S_opt;
+        h->cl_S_opt = value;
+        cluster_configure(h);
+        if (h->cl_S == 0) {
+            const std::string why = h->cl_why;
+            h->cl_S_opt = old;
+            cluster_configure(h);
+            return fail(h, VFPS_ERR_UNSUPPORTED, "cluster size not feasible for this grid: " + why);
+        }
+        return VFPS_OK;
     }
     if (option == VFPS_OPT_TIMING) {
         if (value != 0 && value != 1) return fail(h, VFPS_ERR_ARG, "timing must be 0 or 1");
@@ -440,6 +591,7 @@ int vfps_get_option(vfps_handle h, int option, int *value)
     if (option == VFPS_OPT_ENGINE) { *value = h->engine_opt; return VFPS_OK; }
     if (option == VFPS_OPT_WAKE) { *value = h->wake_opt; return VFPS_OK; }
     if (option == VFPS_OPT_TIMING) { *value = h->timing ? 1 : 0; return VFPS_OK; }
+    if (option == VFPS_OPT_CLUSTER_SIZE) { *value = h->cl_S; return VFPS_OK; }
     return fail(h, VFPS_ERR_ARG, "unknown option");
 }
 
@@ -452,7 +604,11 @@ const char *vfps_engine_name(vfps_handle h)
         default: return "cluster";
     }
 }
-const char *vfps_wake_name(vfps_handle h) { (void)h; return "fft"; }
+const char *vfps_wake_name(vfps_handle h)
+{
+    if (!h) return "";
+    return resolved_engine(h) == VFPS_ENGINE_CLUSTER ? "direct" : "fft";
+}
 
 static int set_psi_impl(vfps_handle h, const float *psi, cudaMemcpyKind kind)
 {
@@ -478,6 +634,13 @@ int vfps_step(vfps_handle h, int n, float *diag)
     if (n < 0) return fail(h, VFPS_ERR_ARG, "n must be >= 0");
     if (!h->psi_set) return fail(h, VFPS_ERR_STATE, "vfps_step before vfps_set_psi");
     if (n == 0) return VFPS_OK;
+    if (resolved_engine(h) == VFPS_ENGINE_CLUSTER) {
+        if (h->timing) resolve_timing(h);
+        int rc = launch_cluster_steps(h, n, diag);
+        if (rc != VFPS_OK) return rc;
+        h->steps += n;
+        return VFPS_OK;
+    }
     k_set_ctl<<<(h->members + 255) / 256, 256, 0, h->stream>>>(h->diag_cell, diag, h->rowctr, h->blkctr, h->members);
     h->launches += 1;
     int done = 0;

@@ -296,7 +296,7 @@ struct KfpArgs {
     float *psi_out;         // psi''' (un-normalised)
     const float *V;         // [members][N]
     const float *qstat;     // [members][4] from k_wake_fft
-    float *mom_part;        // [members][gridDim.x][3]
+    float *mom_part;        // [members][gridDim.x][5]: sum psi, sum Yc psi, sum Yc^2 psi, sum Xc psi, sum Xc^2 psi
     float *scale;           // [members] out: 1/C
     unsigned *blkctr;       // [members], zero between launches
     int *rowctr;            // [members] diagnostics row of this step
@@ -330,7 +330,7 @@ __global__ void __launch_bounds__(KFP_THREADS)
 k_kick_fp(GridConst G, KfpArgs A)
 {
     extern __shared__ float smem[];
-    __shared__ float red[3][KFP_WARPS];
+    __shared__ float red[5][KFP_WARPS];
     __shared__ bool is_last;
     const int N = G.N, m = blockIdx.y;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -348,7 +348,7 @@ k_kick_fp(GridConst G, KfpArgs A)
     for (int i = lane; i < KFP_PADL; i += 32) { r1[-1 - i] = 0.0f; r2[-1 - i] = 0.0f; }
     for (int i = lane; i < KFP_PADR; i += 32) { r1[N + i] = 0.0f; r2[N + i] = 0.0f; }
 
-    float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f;
+    float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, q1 = 0.0f, q2 = 0.0f;
     const int x_begin = blockIdx.x * A.rows_per_cta;
     const int x_end = min(N, x_begin + A.rows_per_cta);
     for (int x = x_begin + warp; x < x_end; x += KFP_WARPS) {
@@ -364,6 +364,7 @@ k_kick_fp(GridConst G, KfpArgs A)
         __syncwarp();
         for (int y = lane; y < N; y += 32) r2[y] = kicked<ORDER>(r1, N, y, mm, l);
         __syncwarp();
+        float rs = 0.0f;
         for (int y = lane; y < N; y += 32) {
             const float fm1 = r2[y - 1], f0 = r2[y], fp1 = r2[y + 1], fp2 = r2[y + 2];
             const float p = fmaf((float)y, G.dp, G.p_min);
@@ -374,17 +375,22 @@ k_kick_fp(GridConst G, KfpArgs A)
             dst[(size_t)x * N + y] = out;
             const float yy = (float)y - yc;
             const float t = out * yy;
-            s0 += out; s1 += t; s2 = fmaf(t, yy, s2);
+            rs += out; s1 += t; s2 = fmaf(t, yy, s2);
         }
+        // q moments of the end-of-step psi from the row sum (every lane gets the same value)
+        rs = warp_sum(rs);
+        const float xx = (float)x - yc;
+        const float tq = rs * xx;
+        s0 += rs; q1 += tq; q2 = fmaf(tq, xx, q2);
     }
-    s0 = warp_sum(s0); s1 = warp_sum(s1); s2 = warp_sum(s2);
-    if (lane == 0) { red[0][warp] = s0; red[1][warp] = s1; red[2][warp] = s2; }
+    s1 = warp_sum(s1); s2 = warp_sum(s2);
+    if (lane == 0) { red[0][warp] = s0; red[1][warp] = s1; red[2][warp] = s2; red[3][warp] = q1; red[4][warp] = q2; }
     __syncthreads();
-    if (threadIdx.x < 3) {
+    if (threadIdx.x < 5) {
         float t = 0.0f;
 #pragma unroll
         for (int w = 0; w < KFP_WARPS; ++w) t += red[threadIdx.x][w];
-        A.mom_part[((size_t)m * gridDim.x + blockIdx.x) * 3 + threadIdx.x] = t;
+        A.mom_part[((size_t)m * gridDim.x + blockIdx.x) * 5 + threadIdx.x] = t;
     }
     // ---- last CTA of this member finalises the step (deterministic: fixed summation order)
     __threadfence();
@@ -397,16 +403,18 @@ k_kick_fp(GridConst G, KfpArgs A)
     if (!is_last) return;
     __threadfence();
     if (warp == 0) {
-        double t0 = 0, t1 = 0, t2 = 0;
-        const volatile float *mp = A.mom_part + (size_t)m * gridDim.x * 3;
-        for (int i = lane; i < (int)gridDim.x; i += 32) { t0 += mp[3 * i]; t1 += mp[3 * i + 1]; t2 += mp[3 * i + 2]; }
-        t0 = warp_sum(t0); t1 = warp_sum(t1); t2 = warp_sum(t2);
+        double t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
+        const volatile float *mp = A.mom_part + (size_t)m * gridDim.x * 5;
+        for (int i = lane; i < (int)gridDim.x; i += 32) {
+            t0 += mp[5 * i]; t1 += mp[5 * i + 1]; t2 += mp[5 * i + 2]; t3 += mp[5 * i + 3]; t4 += mp[5 * i + 4];
+        }
+        t0 = warp_sum(t0); t1 = warp_sum(t1); t2 = warp_sum(t2); t3 = warp_sum(t3); t4 = warp_sum(t4);
         if (lane == 0) {
             const double C = (double)G.dq * (double)G.dp * t0;
             const double mp_c = t1 / t0;                       // <p> in centred cells
             const double vp = t2 / t0 - mp_c * mp_c;
             const float *qs = A.qstat + (size_t)m * 4;
-            const double r0 = qs[0], mq_c = qs[1] / r0, vq = qs[2] / r0 - mq_c * mq_c;
+            const double mq_c = t3 / t0, vq = t4 / t0 - mq_c * mq_c;
             A.scale[m] = (float)(1.0 / C);
             const int row = A.rowctr[m];
             A.rowctr[m] = row + 1;
