@@ -79,8 +79,12 @@ enum {
     VFPS_OPT_WAKE = 2,     /* how a3 is evaluated                                                */
     VFPS_OPT_TIMING = 3,   /* 0/1: bracket kernel launches with CUDA events (measurement aid; while
                               on, vfps_step may synchronise the stream to read finished events)  */
-    VFPS_OPT_CLUSTER_SIZE = 4  /* CTAs per cluster of the CLUSTER engine: 0 = auto, 1, 2, 4, 8, 16;
+    VFPS_OPT_CLUSTER_SIZE = 4, /* CTAs per cluster of the CLUSTER engine: 0 = auto, 1, 2, 4, 8, 16;
                               vfps_get_option returns the size in use (0 = engine unavailable)  */
+    VFPS_OPT_CLUSTER_KERNEL = 5, /* kernel of the CLUSTER engine: 0 = auto, 1 = scalar fp32
+                              (k_cluster_step), 2 = packed fp32x2, two cells per thread
+                              (k_cluster2_step; N = 128, 256, 512); get returns the one in use  */
+    VFPS_OPT_CLUSTER_THREADS = 6 /* threads per CTA of the packed kernel: 0 = auto, 256, 512     */
 };
 /* kernel ids of vfps_kernel_time / vfps_kernel_name */
 enum {

@@ -15,7 +15,7 @@ from .build import build, lib_path
 
 ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER = 0, 1, 2, 3
 WAKE_AUTO, WAKE_FFT, WAKE_DIRECT = 0, 1, 2
-OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE = 1, 2, 3, 4
+OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL, OPT_CLUSTER_THREADS = 1, 2, 3, 4, 5, 6
 NUM_KERNELS = 4
 FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 
@@ -181,6 +181,20 @@ class Simulation:
     @property
     def cluster_size(self) -> int:
         return self.get_option(OPT_CLUSTER_SIZE)
+
+    def set_cluster_kernel(self, version: int) -> None:
+        self.set_option(OPT_CLUSTER_KERNEL, version)
+
+    @property
+    def cluster_kernel(self) -> int:
+        return self.get_option(OPT_CLUSTER_KERNEL)
+
+    def set_cluster_threads(self, threads: int) -> None:
+        self.set_option(OPT_CLUSTER_THREADS, threads)
+
+    @property
+    def cluster_threads(self) -> int:
+        return self.get_option(OPT_CLUSTER_THREADS)
 
     @property
     def engine_name(self) -> str:

@@ -3,6 +3,7 @@
 #include "../../include/vfps.h"
 #include "vfps_kernels.cuh"
 #include "vfps_cluster.cuh"
+#include "vfps_cluster2.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -49,6 +50,7 @@ struct vfps_sim {
     float *wfun = nullptr;                       // [members][2N] wake function w = Re IDFT(Z)
     // cluster engine (0 = not available for this grid)
     int cl_S = 0, cl_S_opt = 0, cl_max_clusters = 0;
+    int cl_ver = 0, cl_ver_opt = 0, cl_threads = 0, cl_threads_opt = 0;   // kernel in use (1 scalar, 2 packed), request, block size
     size_t cl_smem = 0;
     std::string cl_why;                          // why the cluster engine is unavailable
 
@@ -208,10 +210,10 @@ __global__ void k_wake_function(int N, int Nf, int members, const float2 *__rest
     w[i] = (float)(acc / (double)Nf);
 }
 
-template <int ORDER, int N>
-cudaError_t cluster_launch_t(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *max_clusters)
+template <typename K>
+cudaError_t cluster_launch_k(vfps_sim *h, K kern, int threads, const ClusterArgs &A, int nclusters, bool query,
+                             int *max_clusters)
 {
-    auto kern = k_cluster_step<ORDER, N>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->cl_smem);
     if (e != cudaSuccess) return e;
     if (A.S > 8) {
@@ -220,7 +222,7 @@ cudaError_t cluster_launch_t(vfps_sim *h, const ClusterArgs &A, int nclusters, b
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(A.S * nclusters));
-    cfg.blockDim = dim3(CL_THREADS);
+    cfg.blockDim = dim3((unsigned)threads);
     cfg.dynamicSmemBytes = h->cl_smem;
     cfg.stream = h->stream;
     cudaLaunchAttribute attr[1];
@@ -237,12 +239,23 @@ cudaError_t cluster_launch_t(vfps_sim *h, const ClusterArgs &A, int nclusters, b
 template <int ORDER>
 cudaError_t cluster_launch_o(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *mc)
 {
+    if (h->cl_ver == 2) {
+        // packed kernel: block size chosen in cluster_configure (cl_threads)
+        switch (h->N * 4 + (h->cl_threads == 512 ? 1 : 0)) {
+            case 128 * 4: return cluster_launch_k(h, k_cluster2_step<ORDER, 128, 256>, 256, A, nclusters, query, mc);
+            case 128 * 4 + 1: return cluster_launch_k(h, k_cluster2_step<ORDER, 128, 512>, 512, A, nclusters, query, mc);
+            case 256 * 4: return cluster_launch_k(h, k_cluster2_step<ORDER, 256, 256>, 256, A, nclusters, query, mc);
+            case 256 * 4 + 1: return cluster_launch_k(h, k_cluster2_step<ORDER, 256, 512>, 512, A, nclusters, query, mc);
+            case 512 * 4 + 1: return cluster_launch_k(h, k_cluster2_step<ORDER, 512, 512>, 512, A, nclusters, query, mc);
+            default: return cudaErrorInvalidValue;
+        }
+    }
     switch (h->N) {
-        case 32: return cluster_launch_t<ORDER, 32>(h, A, nclusters, query, mc);
-        case 64: return cluster_launch_t<ORDER, 64>(h, A, nclusters, query, mc);
-        case 128: return cluster_launch_t<ORDER, 128>(h, A, nclusters, query, mc);
-        case 256: return cluster_launch_t<ORDER, 256>(h, A, nclusters, query, mc);
-        case 512: return cluster_launch_t<ORDER, 512>(h, A, nclusters, query, mc);
+        case 32: return cluster_launch_k(h, k_cluster_step<ORDER, 32>, CL_THREADS, A, nclusters, query, mc);
+        case 64: return cluster_launch_k(h, k_cluster_step<ORDER, 64>, CL_THREADS, A, nclusters, query, mc);
+        case 128: return cluster_launch_k(h, k_cluster_step<ORDER, 128>, CL_THREADS, A, nclusters, query, mc);
+        case 256: return cluster_launch_k(h, k_cluster_step<ORDER, 256>, CL_THREADS, A, nclusters, query, mc);
+        case 512: return cluster_launch_k(h, k_cluster_step<ORDER, 512>, CL_THREADS, A, nclusters, query, mc);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -256,11 +269,13 @@ cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, boo
     }
 }
 
-// Pick the cluster size: the request (cl_S_opt) if feasible; otherwise the largest feasible size
-// for a single simulation (shortest step), the smallest for a batch (most work per barrier).
+// Pick the cluster kernel and size.  Kernel: the request (cl_ver_opt) or, on AUTO, the packed
+// kernel (2) where it supports the grid, else the scalar one (1).  Size: the request (cl_S_opt) if
+// feasible; otherwise the largest feasible size for a single simulation (shortest step), the
+// smallest for a batch (most work per barrier).
 void cluster_configure(vfps_sim *h)
 {
-    h->cl_S = 0; h->cl_max_clusters = 0; h->cl_why.clear();
+    h->cl_S = 0; h->cl_max_clusters = 0; h->cl_ver = 0; h->cl_why.clear();
     const int N = h->N, H = h->G.H;
     if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
     if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
@@ -269,21 +284,30 @@ void cluster_configure(vfps_sim *h)
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const int cand_single[5] = {16, 8, 4, 2, 1}, cand_batch[5] = {1, 2, 4, 8, 16};
     const int *cand = (h->members == 1) ? cand_single : cand_batch;
-    for (int c = 0; c < 5; ++c) {
-        const int S = cand[c];
-        if (h->cl_S_opt && S != h->cl_S_opt) continue;
-        if (N / S < (H > 1 ? H : 1) || N % S) continue;
-        const size_t bytes = cluster_smem_floats(N, S, H) * sizeof(float);
-        if (bytes > (size_t)smem_max) continue;
-        h->cl_smem = bytes;
-        ClusterArgs A{};
-        A.S = S; A.R = N / S;
-        int mc = 0;
-        cudaError_t e = cluster_launch(h, A, 1, true, &mc);
-        if (e != cudaSuccess || mc < 1) { cudaGetLastError(); continue; }
-        h->cl_S = S; h->cl_max_clusters = mc;
-        return;
+    for (int ver = 2; ver >= 1; --ver) {
+        if (h->cl_ver_opt && ver != h->cl_ver_opt) continue;
+        if (ver == 2 && !(N == 128 || N == 256 || N == 512)) continue;
+        for (int c = 0; c < 5; ++c) {
+            const int S = cand[c];
+            if (h->cl_S_opt && S != h->cl_S_opt) continue;
+            if (N / S < (H > 1 ? H : 1) || N % S) continue;
+            const int R = N / S;
+            if (ver == 2 && ((R & 3) != 0 || R < 2 * H)) continue;
+            const size_t bytes = (ver == 2 ? cluster2_smem_floats(N, S, H) : cluster_smem_floats(N, S, H)) * sizeof(float);
+            if (bytes > (size_t)smem_max) continue;
+            h->cl_smem = bytes;
+            h->cl_ver = ver;
+            h->cl_threads = (ver == 2) ? ((N == 512 || h->cl_threads_opt == 512) ? 512 : 256) : CL_THREADS;
+            ClusterArgs A{};
+            A.S = S; A.R = R;
+            int mc = 0;
+            cudaError_t e = cluster_launch(h, A, 1, true, &mc);
+            if (e != cudaSuccess || mc < 1) { cudaGetLastError(); continue; }
+            h->cl_S = S; h->cl_max_clusters = mc;
+            return;
+        }
     }
+    h->cl_ver = 0;
     h->cl_why = "no feasible cluster size (shared memory or cluster scheduling)";
 }
 
@@ -571,6 +595,22 @@ int vfps_set_option(vfps_handle h, int option, int value)
         }
         return VFPS_OK;
     }
+    if (option == VFPS_OPT_CLUSTER_KERNEL || option == VFPS_OPT_CLUSTER_THREADS) {
+        const bool is_k = (option == VFPS_OPT_CLUSTER_KERNEL);
+        if (is_k ? !(value >= 0 && value <= 2) : !(value == 0 || value == 256 || value == 512))
+            return fail(h, VFPS_ERR_ARG, is_k ? "cluster kernel must be 0 (auto), 1 or 2" : "cluster threads must be 0 (auto), 256 or 512");
+        int &slot = is_k ? h->cl_ver_opt : h->cl_threads_opt;
+        const int old = slot;
+        slot = value;
+        cluster_configure(h);
+        if (h->cl_S == 0) {
+            const std::string why = h->cl_why;
+            slot = old;
+            cluster_configure(h);
+            return fail(h, VFPS_ERR_UNSUPPORTED, "cluster kernel not available for this grid: " + why);
+        }
+        return VFPS_OK;
+    }
     if (option == VFPS_OPT_TIMING) {
         if (value != 0 && value != 1) return fail(h, VFPS_ERR_ARG, "timing must be 0 or 1");
         if (!value) resolve_timing(h);
@@ -592,6 +632,8 @@ int vfps_get_option(vfps_handle h, int option, int *value)
     if (option == VFPS_OPT_WAKE) { *value = h->wake_opt; return VFPS_OK; }
     if (option == VFPS_OPT_TIMING) { *value = h->timing ? 1 : 0; return VFPS_OK; }
     if (option == VFPS_OPT_CLUSTER_SIZE) { *value = h->cl_S; return VFPS_OK; }
+    if (option == VFPS_OPT_CLUSTER_KERNEL) { *value = h->cl_ver; return VFPS_OK; }
+    if (option == VFPS_OPT_CLUSTER_THREADS) { *value = h->cl_threads; return VFPS_OK; }
     return fail(h, VFPS_ERR_ARG, "unknown option");
 }
 

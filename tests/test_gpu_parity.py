@@ -47,9 +47,11 @@ def assert_diag(got, want, has_wake=True, tol_q=TOL_MOM, tol_p=None):
         assert got[5] == 0.0
 
 
-def run_pair(vfps, orc, wl, nsteps, members=None, engine=None, wake=None, diag_every=1):
+def run_pair(vfps, orc, wl, nsteps, members=None, engine=None, wake=None, diag_every=1, cluster_kernel=None):
     idx = list(range(wl.members) if members is None else members)
     sim = vfps.Simulation.from_workload(wl, idx)
+    if cluster_kernel is not None:
+        sim.set_cluster_kernel(cluster_kernel)
     if engine is not None:
         sim.set_engine(engine)
     if wake is not None:
@@ -255,15 +257,20 @@ def test_error_paths_on_gpu(vfps):
 
 # ---------------------------------------------------------------- engines
 def _engine_id(vfps, name):
-    return {"stream": vfps.ENGINE_STREAM, "graph": vfps.ENGINE_GRAPH, "cluster": vfps.ENGINE_CLUSTER}[name]
+    return {"stream": vfps.ENGINE_STREAM, "graph": vfps.ENGINE_GRAPH, "cluster": vfps.ENGINE_CLUSTER,
+            "cluster1": vfps.ENGINE_CLUSTER}[name]
 
 
-@pytest.mark.parametrize("engine", ["stream", "graph", "cluster"])
+@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster1"])
 def test_c1_every_engine_100_steps(vfps, orc, engine):
-    """The same 100 steps of C1 through each engine (graph: two replays of 50 captured steps)."""
+    """The same 100 steps of C1 through each engine (graph: two replays of 50 captured steps;
+    cluster: the packed kernel, which AUTO picks at 256^2; cluster1: the scalar kernel)."""
     wl = get_workload("C1")
-    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 100, engine=_engine_id(vfps, engine), diag_every=1)
-    assert sim.engine_name == engine
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 100, engine=_engine_id(vfps, engine), diag_every=1,
+                                     cluster_kernel=1 if engine == "cluster1" else None)
+    assert sim.engine_name == engine.rstrip("1")
+    if engine.startswith("cluster"):
+        assert sim.cluster_kernel == (1 if engine == "cluster1" else 2)
     assert_psi(psi[0], refs[0].psi, 1e-4, f"C1 100 steps, {engine}")
     for i in (0, 1, 49, 50, 99):
         assert_diag(d[i, 0], dr[0][i])
@@ -272,22 +279,30 @@ def test_c1_every_engine_100_steps(vfps, orc, engine):
 
 @pytest.mark.parametrize("S", [1, 2, 4, 8, 16])
 @pytest.mark.parametrize("order", [2, 3, 4])
-@pytest.mark.parametrize("N", [32, 64, 128, 256])
-def test_cluster_engine_sizes(vfps, orc, N, order, S):
-    """Persistent cluster engine for every grid size / interpolation order / cluster size that is
-    feasible: asymmetric box, off-centre mismatched bunch, free-space wake (as
-    test_orders_and_small_grids), 1 step and 60 steps, diagnostics of every step."""
+@pytest.mark.parametrize("N,kernel,threads", [(32, 1, 0), (64, 1, 0), (128, 1, 0), (256, 1, 0),
+                                              (128, 2, 256), (128, 2, 512), (256, 2, 256), (256, 2, 512)])
+def test_cluster_engine_sizes(vfps, orc, N, order, S, kernel, threads):
+    """Persistent cluster engine, scalar (1) and packed (2) kernel, for every grid size /
+    interpolation order / cluster size / block size that is feasible: asymmetric box, off-centre
+    mismatched bunch, free-space wake (as test_orders_and_small_grids), 1 step and 60 steps,
+    diagnostics of every step.  300 steps per period moves the corner cells by two cells per step,
+    so floor(dx), floor(dy) change inside a CTA's rows (the packed kernel's scalar paths run) and
+    the wake of the 0.4-strength free-space impedance shifts rows by different integer parts."""
     Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
     psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
     sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, 1, Z=Z)
     try:
+        sim.set_cluster_kernel(kernel)
+        if threads:
+            sim.set_cluster_threads(threads)
         sim.set_cluster_size(S)
     except vfps.VfpsError as e:
         assert e.code == -5
         sim.close()
-        pytest.skip(f"cluster size {S} not feasible for N={N}")
+        pytest.skip(f"kernel {kernel} with cluster size {S} not feasible for N={N}")
     sim.set_engine(vfps.ENGINE_CLUSTER)
     assert sim.engine_name == "cluster" and sim.cluster_size == S and sim.wake_name == "direct"
+    assert sim.cluster_kernel == kernel and (not threads or sim.cluster_threads == threads)
     sim.set_psi_host(psi0)
     o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, Z[0])
     o.set_psi(psi0[0])
@@ -304,22 +319,25 @@ def test_cluster_engine_sizes(vfps, orc, N, order, S):
     sim.close()
 
 
-def test_cluster_engine_c2_512(vfps, orc):
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_cluster_engine_c2_512(vfps, orc, kernel):
     wl = get_workload("C2").with_(S_csr=(0.6,))
-    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 40, engine=vfps.ENGINE_CLUSTER, diag_every=1)
-    assert sim.engine_name == "cluster" and sim.cluster_size == 16
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 40, engine=vfps.ENGINE_CLUSTER, diag_every=1, cluster_kernel=kernel)
+    assert sim.engine_name == "cluster" and sim.cluster_size == 16 and sim.cluster_kernel == kernel
     assert_psi(psi[0], refs[0].psi, 5e-5, "C2 cluster 40 steps")
     for i in (0, 20, 39):
         assert_diag(d[i, 0], dr[0][i])
     sim.close()
 
 
+@pytest.mark.parametrize("kernel", [1, 2])
 @pytest.mark.parametrize("S", [4, 8, 16])
-def test_cluster_engine_batched(vfps, orc, S):
+def test_cluster_engine_batched(vfps, orc, S, kernel):
     """More members than one cluster: every cluster walks through its members one after another."""
     wl = get_workload("C3")
     idx = [0, 37, 128, 255, 3, 64]
     sim = vfps.Simulation.from_workload(wl, idx)
+    sim.set_cluster_kernel(kernel)
     sim.set_cluster_size(S)
     sim.set_engine(vfps.ENGINE_CLUSTER)
     d = sim.step_host(30)
@@ -333,16 +351,19 @@ def test_cluster_engine_batched(vfps, orc, S):
     sim.close()
 
 
-def test_cluster_engine_large_kick_and_switching(vfps, orc):
-    """|kick shift| > 1 cell (generic-shift path of the cluster engine), then continue the same
-    simulation on the stream engine: state hand-over between engines is exact."""
-    N = 64
+@pytest.mark.parametrize("N", [64, 128])
+def test_cluster_engine_large_kick_and_switching(vfps, orc, N):
+    """|kick shift| > 1 cell (generic-shift path of the cluster engine; N = 128 runs the packed
+    kernel), then continue the same simulation on the stream engine: state hand-over between
+    engines is exact."""
     Z = np.full((1, N + 1), 60.0 + 0j, dtype=np.complex64)
     psi0 = make_psi0(N, -6, 6, -6, 6, 1.0, 1.0, 0, 0)[None]
-    sim = vfps.Simulation(N, -6, 6, -6, 6, 100, 1e-3, 4, 2, 1, Z=Z)
+    spp = 100 * N // 64          # the same rotation displacement in cells on both grids
+    sim = vfps.Simulation(N, -6, 6, -6, 6, spp, 1e-3, 4, 2, 1, Z=Z)
     sim.set_engine(vfps.ENGINE_CLUSTER)
+    assert sim.cluster_kernel == (2 if N == 128 else 1)
     sim.set_psi_host(psi0)
-    o = orc.Oracle(N, -6, 6, -6, 6, 100, 1e-3, 4, 2, Z[0])
+    o = orc.Oracle(N, -6, 6, -6, 6, spp, 1e-3, 4, 2, Z[0])
     o.set_psi(psi0[0])
     d = sim.step_host(3)
     dr = o.step(3)
