@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--engine", default="auto", choices=["auto", "stream", "graph", "cluster"])
     ap.add_argument("--wake", default="auto", choices=["auto", "fft", "direct"])
     ap.add_argument("--cluster-size", type=int, default=0, help="CTAs per cluster of the cluster engine (0 = auto)")
+    ap.add_argument("--stream-gen", type=int, default=0, help="streaming kernels: 0 auto, 1 first generation, 2 second")
     ap.add_argument("--cluster-kernel", type=int, default=0, help="cluster engine kernel: 0 auto, 1 scalar, 2 packed fp32x2")
     ap.add_argument("--cluster-threads", type=int, default=0, help="threads per CTA of the packed cluster kernel (0 = auto)")
     ap.add_argument("--members", type=int, default=0, help="batch members (0 = the workload's own count)")
@@ -194,6 +195,8 @@ def run_ours(args, wl, rank, local_rank, world):
     Z = wl.impedance(idx)
     sim = pkg.Simulation(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
                          wl.interp_order, wl.pad, members, Z=Z)
+    if args.stream_gen:
+        sim.set_stream_gen(args.stream_gen)
     if args.cluster_kernel:
         sim.set_cluster_kernel(args.cluster_kernel)
     if args.cluster_threads:
@@ -232,6 +235,7 @@ def run_ours(args, wl, rank, local_rank, world):
     ms = dist.reduce_max(ms_local, dev)
     engine, wake = sim.engine_name, sim.wake_name
     cluster_size = sim.cluster_size if engine == "cluster" else None
+    sim_gen = sim.stream_gen if engine != "cluster" else None
     cluster_kernel = {1: "k_cluster_step (scalar fp32)", 2: "k_cluster2_step (packed fp32x2)"}.get(sim.cluster_kernel) if engine == "cluster" else None
     cluster_threads = sim.cluster_threads if engine == "cluster" else None
     diag_last = diag[-1].cpu().numpy().astype(float)
@@ -297,7 +301,7 @@ def run_ours(args, wl, rank, local_rank, world):
             "us_per_split_step": 1e3 * ms / (n_inner * args.steps),
             "config": {"workload": wl.name, "N": wl.N, "members": members, "split_steps_per_bench_step": n_inner,
                        "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
-                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size,
+                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size, "stream_gen": sim_gen,
                        "cluster_kernel": cluster_kernel, "cluster_threads": cluster_threads,
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                        "l2": "256 MB buffer written between timed bench steps (L2 flush)"},

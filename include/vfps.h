@@ -84,7 +84,10 @@ enum {
     VFPS_OPT_CLUSTER_KERNEL = 5, /* kernel of the CLUSTER engine: 0 = auto, 1 = scalar fp32
                               (k_cluster_step), 2 = packed fp32x2, two cells per thread
                               (k_cluster2_step; N = 128, 256, 512); get returns the one in use  */
-    VFPS_OPT_CLUSTER_THREADS = 6 /* threads per CTA of the packed kernel: 0 = auto, 256, 512     */
+    VFPS_OPT_CLUSTER_THREADS = 6, /* threads per CTA of the packed kernel: 0 = auto, 256, 512    */
+    VFPS_OPT_STREAM_GEN = 7 /* kernels of the STREAM / GRAPH engines: 0 = auto (2), 1 = first
+                              generation (k_rotate, k_wake_fft, k_kick_fp), 2 = second (k_rotate2,
+                              k_wake_direct or k_wake_fft, k_kick_fp2); get returns the one in use */
 };
 /* kernel ids of vfps_kernel_time / vfps_kernel_name */
 enum {
@@ -92,7 +95,10 @@ enum {
     VFPS_KERNEL_WAKE = 1,     /* a2 finish + a3 + q-moments + CSR power                          */
     VFPS_KERNEL_KICK_FP = 2,  /* a4 + a5 + a6                                                    */
     VFPS_KERNEL_CLUSTER = 3,  /* a1..a6 for all n steps of one vfps_step call (cluster engine)   */
-    VFPS_NUM_KERNELS = 4
+    VFPS_KERNEL_ROTATE2 = 4,  /* a1 + a2, second-generation streaming kernel (register window)   */
+    VFPS_KERNEL_WAKE_DIRECT = 5, /* a2 finish + a3 by direct convolution on N/32 CTAs             */
+    VFPS_KERNEL_KICK_FP2 = 6, /* a4 + a5 + a6, second generation (four cells per thread)         */
+    VFPS_NUM_KERNELS = 7
 };
 enum {
     VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRAPH                    */

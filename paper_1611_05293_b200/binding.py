@@ -15,8 +15,8 @@ from .build import build, lib_path
 
 ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER = 0, 1, 2, 3
 WAKE_AUTO, WAKE_FFT, WAKE_DIRECT = 0, 1, 2
-OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL, OPT_CLUSTER_THREADS = 1, 2, 3, 4, 5, 6
-NUM_KERNELS = 4
+OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL, OPT_CLUSTER_THREADS, OPT_STREAM_GEN = 1, 2, 3, 4, 5, 6, 7
+NUM_KERNELS = 7
 FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 
 # every symbol include/vfps.h declares (tests check the library exports each of them)
@@ -181,6 +181,13 @@ class Simulation:
     @property
     def cluster_size(self) -> int:
         return self.get_option(OPT_CLUSTER_SIZE)
+
+    def set_stream_gen(self, gen: int) -> None:
+        self.set_option(OPT_STREAM_GEN, gen)
+
+    @property
+    def stream_gen(self) -> int:
+        return self.get_option(OPT_STREAM_GEN)
 
     def set_cluster_kernel(self, version: int) -> None:
         self.set_option(OPT_CLUSTER_KERNEL, version)

@@ -4,9 +4,11 @@
 #include "vfps_kernels.cuh"
 #include "vfps_cluster.cuh"
 #include "vfps_cluster2.cuh"
+#include "vfps_stream2.cuh"
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -55,17 +57,23 @@ struct vfps_sim {
     std::string cl_why;                          // why the cluster engine is unavailable
 
     int tiles_x = 0, tiles_y = 0, kfp_rows = 0, kfp_blocks = 0;
+    // second-generation streaming kernels (vfps_stream2.cuh)
+    int gen_opt = 0;                             // 0 auto (2), 1, 2
+    int tiles_x2 = 0, tiles_y2 = 0, kfp2_rows = 0, kfp2_blocks = 0, wd_blocks = 0;
+    float *pw_part = nullptr;                    // [members][wd_blocks]
+    unsigned *tilectr = nullptr;                 // [members][tiles_x2], zero between launches
     size_t rot_smem = 0, kfp_smem = 0, fft_smem = 0;
     int fft_threads = 0;
 
     // CUDA-graph engine: GRAPH_STEPS split steps captured once, replayed
     cudaGraphExec_t graph_exec = nullptr;
+    long long graph_launches = 0;                // kernel nodes of the captured graph
     // per-kernel device timing (VFPS_OPT_TIMING): event pairs around launches, resolved lazily
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;
     std::vector<int> ev_kind;                    // kernel id of pair i (events 2i, 2i+1)
-    double k_ms[VFPS_NUM_KERNELS] = {0, 0, 0, 0};
-    long long k_cnt[VFPS_NUM_KERNELS] = {0, 0, 0, 0};
+    double k_ms[VFPS_NUM_KERNELS] = {};
+    long long k_cnt[VFPS_NUM_KERNELS] = {};
     float *diag_scratch = nullptr;               // vfps_step_host staging (grow-only)
     size_t diag_scratch_n = 0;
 
@@ -269,8 +277,8 @@ cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, boo
     }
 }
 
-// Pick the cluster kernel and size.  Kernel: the request (cl_ver_opt) or, on AUTO, the packed
-// kernel (2) where it supports the grid, else the scalar one (1).  Size: the request (cl_S_opt) if
+// Pick the cluster kernel and size.  Kernel: the request (cl_ver_opt) or, on AUTO, the scalar
+// kernel (1).  Size: the request (cl_S_opt) if
 // feasible; otherwise the largest feasible size for a single simulation (shortest step), the
 // smallest for a batch (most work per barrier).
 void cluster_configure(vfps_sim *h)
@@ -284,8 +292,10 @@ void cluster_configure(vfps_sim *h)
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const int cand_single[5] = {16, 8, 4, 2, 1}, cand_batch[5] = {1, 2, 4, 8, 16};
     const int *cand = (h->members == 1) ? cand_single : cand_batch;
-    for (int ver = 2; ver >= 1; --ver) {
-        if (h->cl_ver_opt && ver != h->cl_ver_opt) continue;
+    // AUTO takes the scalar kernel: on B200 the packed one is not faster yet (C1 4.5 vs 3.5 us per
+    // step, C3 79 vs 79 us; profiles/r01_cluster2.md), it is there to be selected and measured
+    for (int ver = 1; ver <= 2; ++ver) {
+        if (ver != (h->cl_ver_opt ? h->cl_ver_opt : 1)) continue;
         if (ver == 2 && !(N == 128 || N == 256 || N == 512)) continue;
         for (int c = 0; c < 5; ++c) {
             const int S = cand[c];
@@ -318,9 +328,29 @@ int launch_cluster_steps(vfps_sim *h, int n, float *diag)
     A.members = h->members; A.nsteps = n; A.S = h->cl_S; A.R = h->N / h->cl_S;
     const int nclusters = h->members < h->cl_max_clusters ? h->members : h->cl_max_clusters;
     cudaError_t e;
+    // debug aid: VFPS_PHASE_DUMP=<file> writes the packed kernel's per-phase clock stamps of the
+    // first 64 steps of every CTA (synchronises; never set in measurements)
+    const char *dump = (h->cl_ver == 2) ? std::getenv("VFPS_PHASE_DUMP") : nullptr;
+    const size_t ndbg = (size_t)A.S * nclusters * 64 * 8;
+    if (dump && cudaMalloc((void **)&A.dbg, ndbg * sizeof(long long)) != cudaSuccess) { A.dbg = nullptr; dump = nullptr; }
+    if (dump) cudaMemsetAsync(A.dbg, 0, ndbg * sizeof(long long), h->stream);
     {
         Bracket br(h, VFPS_KERNEL_CLUSTER, h->timing);
         e = cluster_launch(h, A, nclusters, false, nullptr);
+    }
+    if (dump) {
+        std::vector<long long> t(ndbg);
+        cudaMemcpyAsync(t.data(), A.dbg, ndbg * sizeof(long long), cudaMemcpyDeviceToHost, h->stream);
+        cudaStreamSynchronize(h->stream);
+        cudaFree(A.dbg);
+        if (FILE *f = std::fopen(dump, "w")) {
+            for (size_t i = 0; i < ndbg; i += 8) {
+                std::fprintf(f, "%zu %zu", i / (64 * 8), (i / 8) % 64);
+                for (int k = 0; k < 8; ++k) std::fprintf(f, " %lld", t[i + k]);
+                std::fprintf(f, "\n");
+            }
+            std::fclose(f);
+        }
     }
     if (e != cudaSuccess) return fail(h, VFPS_ERR_CUDA, std::string("cluster launch: ") + cudaGetErrorString(e));
     h->launches += 1;
@@ -356,8 +386,58 @@ int launch_step_stream(vfps_sim *h, bool timed)
     return VFPS_OK;
 }
 
+// which kernels the STREAM / GRAPH engines launch, and how they evaluate the wake
+int resolved_gen(const vfps_sim *h) { return h->gen_opt ? h->gen_opt : 2; }
+bool wake_is_direct(const vfps_sim *h)
+{
+    if (resolved_gen(h) == 1) return false;
+    return h->wake_opt != VFPS_WAKE_FFT;
+}
+
+template <int ORDER>
+int launch_step_stream2(vfps_sim *h, bool timed)
+{
+    const int N = h->N;
+    const bool direct = wake_is_direct(h);
+    {
+        Bracket br(h, VFPS_KERNEL_ROTATE2, timed);
+        k_rotate2<ORDER><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
+            h->G, h->psi, h->psi_tmp, h->scale, h->rho_part, h->tiles_y2, h->rho, h->tilectr);
+    }
+    if (!direct) {
+        Bracket br(h, VFPS_KERNEL_WAKE, timed);
+        k_wake_fft<<<h->members, h->fft_threads, h->fft_smem, h->stream>>>(
+            N, h->Nf, h->log2Nf, h->G.dq, h->rho_part, h->tiles_y2, h->has_wake ? h->Z : nullptr, h->tw,
+            h->rho, h->V, h->qstat);
+        h->launches += 1;
+    } else if (h->has_wake) {      // without an impedance V stays 0 (set at create) and P = 0
+        Bracket br(h, VFPS_KERNEL_WAKE_DIRECT, timed);
+        k_wake_direct<<<dim3(h->wd_blocks, h->members), WD_THREADS, (size_t)(2 * N + WD_ROWS) * sizeof(float), h->stream>>>(
+            N, h->rho, h->wfun, h->V, h->pw_part);
+        h->launches += 1;
+    }
+    Kfp2Args A;
+    A.psi_in = h->psi_tmp; A.psi_out = h->psi; A.V = h->V; A.qstat = h->qstat;
+    A.pw_part = direct ? h->pw_part : nullptr; A.npw = h->wd_blocks;
+    A.mom_part = h->mom_part; A.scale = h->scale; A.blkctr = h->blkctr; A.rowctr = h->rowctr;
+    A.diag = h->diag_cell; A.members = h->members; A.rows_per_cta = h->kfp2_rows;
+    {
+        Bracket br(h, VFPS_KERNEL_KICK_FP2, timed);
+        k_kick_fp2<ORDER><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
+    }
+    h->launches += 2;
+    return VFPS_OK;
+}
+
 int launch_step(vfps_sim *h, bool timed)
 {
+    if (resolved_gen(h) == 2) {
+        switch (h->P.interp_order) {
+            case 2: return launch_step_stream2<2>(h, timed);
+            case 3: return launch_step_stream2<3>(h, timed);
+            default: return launch_step_stream2<4>(h, timed);
+        }
+    }
     switch (h->P.interp_order) {
         case 2: return launch_step_stream<2>(h, timed);
         case 3: return launch_step_stream<3>(h, timed);
@@ -371,6 +451,15 @@ int resolved_engine(const vfps_sim *h)
     if (h->engine_opt == VFPS_ENGINE_STREAM) return VFPS_ENGINE_STREAM;
     if (h->engine_opt == VFPS_ENGINE_GRAPH) return VFPS_ENGINE_GRAPH;
     return h->cl_S > 0 ? VFPS_ENGINE_CLUSTER : VFPS_ENGINE_GRAPH;      // AUTO, CLUSTER
+}
+
+// the captured graph depends on the kernel generation and the wake mode
+void drop_graph(vfps_sim *h)
+{
+    if (!h->graph_exec) return;
+    cudaStreamSynchronize(h->stream);
+    cudaGraphExecDestroy(h->graph_exec);
+    h->graph_exec = nullptr;
 }
 
 // capture GRAPH_STEPS split steps once; every step is the same three launches (the diag row and
@@ -387,6 +476,7 @@ int ensure_graph(vfps_sim *h)
         h->stream = cap;
         const long long l0 = h->launches;
         for (int i = 0; i < GRAPH_STEPS; ++i) launch_step(h, false);
+        h->graph_launches = h->launches - l0;
         h->launches = l0;
         h->stream = user;
         e = cudaStreamEndCapture(cap, &g);
@@ -445,6 +535,11 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     h->kfp_rows = KFP_WARPS * ((N >= 1024) ? 2 : 1);
     h->kfp_blocks = (N + h->kfp_rows - 1) / h->kfp_rows;
     h->kfp_smem = (size_t)KFP_WARPS * 2 * (KFP_PADL + N + KFP_PADR) * sizeof(float);
+    h->tiles_x2 = (N + R2_RT - 1) / R2_RT;
+    h->tiles_y2 = (N + 32 * R2_WARPS - 1) / (32 * R2_WARPS);
+    h->kfp2_rows = 4096 / N > 0 ? (4096 / N < N ? 4096 / N : N) : 1;
+    h->kfp2_blocks = (N + h->kfp2_rows - 1) / h->kfp2_rows;
+    h->wd_blocks = (N + WD_ROWS - 1) / WD_ROWS;
     h->fft_threads = h->Nf / 2 < 1024 ? (h->Nf / 2 < 32 ? 32 : h->Nf / 2) : 1024;
     h->fft_smem = (size_t)h->Nf * sizeof(float2);
 
@@ -459,11 +554,15 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     CUB(dalloc(h, &h->psi, (size_t)M * N * N));
     CUB(dalloc(h, &h->psi_tmp, (size_t)M * N * N));
     CUB(dalloc(h, &h->tw, (size_t)h->Nf / 2));
-    CUB(dalloc(h, &h->rho_part, (size_t)M * N * h->tiles_y));
+    CUB(dalloc(h, &h->rho_part, (size_t)M * N * (h->tiles_y > h->tiles_y2 ? h->tiles_y : h->tiles_y2)));
+    CUB(dalloc(h, &h->pw_part, (size_t)M * h->wd_blocks));
+    CUB(dalloc(h, &h->tilectr, (size_t)M * h->tiles_x2));
+    CUB(cudaMemsetAsync(h->tilectr, 0, (size_t)M * h->tiles_x2 * sizeof(unsigned), h->stream));
+    CUB(cudaMemsetAsync(h->pw_part, 0, (size_t)M * h->wd_blocks * sizeof(float), h->stream));
     CUB(dalloc(h, &h->rho, (size_t)M * N));
     CUB(dalloc(h, &h->V, (size_t)M * N));
     CUB(dalloc(h, &h->qstat, (size_t)M * 4));
-    CUB(dalloc(h, &h->mom_part, (size_t)M * h->kfp_blocks * 5));
+    CUB(dalloc(h, &h->mom_part, (size_t)M * (h->kfp_blocks > h->kfp2_blocks ? h->kfp_blocks : h->kfp2_blocks) * 5));
     CUB(dalloc(h, &h->scale, (size_t)M));
     CUB(dalloc(h, &h->blkctr, (size_t)M));
     CUB(dalloc(h, &h->rowctr, (size_t)M));
@@ -618,9 +717,21 @@ int vfps_set_option(vfps_handle h, int option, int value)
         return VFPS_OK;
     }
     if (option == VFPS_OPT_WAKE) {
-        if (value == VFPS_WAKE_AUTO || value == VFPS_WAKE_FFT) { h->wake_opt = value; return VFPS_OK; }
-        if (value == VFPS_WAKE_DIRECT) return fail(h, VFPS_ERR_UNSUPPORTED, "wake mode not available in this build");
-        return fail(h, VFPS_ERR_ARG, "unknown wake mode");
+        if (!(value == VFPS_WAKE_AUTO || value == VFPS_WAKE_FFT || value == VFPS_WAKE_DIRECT))
+            return fail(h, VFPS_ERR_ARG, "unknown wake mode");
+        if (value == VFPS_WAKE_DIRECT && resolved_gen(h) == 1)
+            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels have no direct-convolution wake");
+        if (value != h->wake_opt) drop_graph(h);
+        h->wake_opt = value;
+        return VFPS_OK;
+    }
+    if (option == VFPS_OPT_STREAM_GEN) {
+        if (value < 0 || value > 2) return fail(h, VFPS_ERR_ARG, "stream generation must be 0 (auto), 1 or 2");
+        if (value == 1 && h->wake_opt == VFPS_WAKE_DIRECT)
+            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels have no direct-convolution wake");
+        if (value != h->gen_opt) drop_graph(h);
+        h->gen_opt = value;
+        return VFPS_OK;
     }
     return fail(h, VFPS_ERR_ARG, "unknown option");
 }
@@ -634,6 +745,7 @@ int vfps_get_option(vfps_handle h, int option, int *value)
     if (option == VFPS_OPT_CLUSTER_SIZE) { *value = h->cl_S; return VFPS_OK; }
     if (option == VFPS_OPT_CLUSTER_KERNEL) { *value = h->cl_ver; return VFPS_OK; }
     if (option == VFPS_OPT_CLUSTER_THREADS) { *value = h->cl_threads; return VFPS_OK; }
+    if (option == VFPS_OPT_STREAM_GEN) { *value = resolved_gen(h); return VFPS_OK; }
     return fail(h, VFPS_ERR_ARG, "unknown option");
 }
 
@@ -649,7 +761,8 @@ const char *vfps_engine_name(vfps_handle h)
 const char *vfps_wake_name(vfps_handle h)
 {
     if (!h) return "";
-    return resolved_engine(h) == VFPS_ENGINE_CLUSTER ? "direct" : "fft";
+    if (resolved_engine(h) == VFPS_ENGINE_CLUSTER) return "direct";
+    return wake_is_direct(h) ? "direct" : "fft";
 }
 
 static int set_psi_impl(vfps_handle h, const float *psi, cudaMemcpyKind kind)
@@ -691,7 +804,7 @@ int vfps_step(vfps_handle h, int n, float *diag)
         if (rc != VFPS_OK) return rc;
         for (; done + GRAPH_STEPS <= n; done += GRAPH_STEPS) {
             CU(cudaGraphLaunch(h->graph_exec, h->stream));
-            h->launches += 3 * GRAPH_STEPS;
+            h->launches += h->graph_launches;
         }
     }
     // stream engine, and the remainder of a graph run
@@ -859,6 +972,9 @@ const char *vfps_kernel_name(int kernel)
         case VFPS_KERNEL_WAKE: return "k_wake_fft";
         case VFPS_KERNEL_KICK_FP: return "k_kick_fp";
         case VFPS_KERNEL_CLUSTER: return "k_cluster_step";
+        case VFPS_KERNEL_ROTATE2: return "k_rotate2";
+        case VFPS_KERNEL_WAKE_DIRECT: return "k_wake_direct";
+        case VFPS_KERNEL_KICK_FP2: return "k_kick_fp2";
         default: return nullptr;
     }
 }

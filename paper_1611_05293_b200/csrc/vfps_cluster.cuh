@@ -45,6 +45,7 @@ struct ClusterArgs {
     int nsteps;
     int S;               // CTAs per cluster
     int R;               // rows per CTA = N / S
+    long long *dbg;      // nullptr, or [CTA][64 steps][8] clock64 stamps of the packed kernel's phases (debug aid)
 };
 
 __host__ __device__ inline size_t cluster_smem_floats(int N, int S, int H)

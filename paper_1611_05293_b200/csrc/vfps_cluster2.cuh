@@ -24,15 +24,37 @@
 
 namespace vfps {
 
+// Column order inside a pair-row.  A pair-row is cut into 16-byte chunks of two columns
+// { (A,B)(y), (A,B)(y+1) }, y even, counted from column -CL_PAD; the even chunks lie in one region
+// and the odd chunks in a second one, NH2 chunks further on.  A thread of the kick pass owns four
+// columns = one even and one odd chunk, so a warp's 128-bit accesses are contiguous in each region
+// (no bank conflict; with the plain column order they are 32 bytes apart = two-way conflicts, which
+// made the kick pass shared-memory bound).  NH2 = 4 mod 8 keeps the 64-bit accesses of the
+// rotation (thread = column) on disjoint banks for even column offsets.
+__host__ __device__ constexpr int cluster2_nh2(int N)
+{
+    int n = (N + 2 * CL_PAD) / 4;
+    while ((n & 7) != 4) ++n;
+    return n;
+}
+// byte offset of column y (-CL_PAD <= y < N + CL_PAD) inside a pair-row
+template <int NH2>
+__device__ __forceinline__ uint32_t col_off(int y)
+{
+    const int yy = y + CL_PAD, cp = yy >> 1;
+    return (uint32_t)((((cp >> 1) + (cp & 1) * NH2) << 4) + ((yy & 1) << 3));
+}
+
 __host__ __device__ inline size_t cluster2_smem_floats(int N, int S, int H)
 {
-    const int R = N / S, Rh = R / 2, pitch = N + 2 * CL_PAD;
+    const int R = N / S, Rh = R / 2, pitch = 4 * cluster2_nh2(N);   // float2 slots per pair-row
     return (size_t)(Rh + 2 * H) * pitch * 2     // bufA
            + (size_t)Rh * pitch * 2             // bufB
            + 2 * (size_t)N                      // wake function
            + (size_t)N                          // rho (all rows)
            + 2 * CL_MAX_S * CL_NPART            // partial sums of all CTAs, two parities
-           + CL_WARPS * 8 + 8;                  // block reduction scratch, mbarriers
+           + CL_WARPS * 8 + 8                   // block reduction scratch, mbarriers
+           + 8 * (size_t)R;                     // kick weights and integer shift of every own row
 }
 
 // ---- packed fp32 (two independent lanes .x / .y per instruction)
@@ -119,9 +141,9 @@ __device__ __forceinline__ void kick_fp_granule2(const float2 (&b)[12], const fl
 }
 
 // any integer shift, one row of the pair (h = 0 / 1), scalar, bounds-checked taps.
-// row: pair-interleaved row, float index 2*y + h = column y.
-template <int ORDER>
-__device__ __forceinline__ void kick_fp_granule_any2(const float *row, int h, const float (&l)[ORDER], int mm, int g,
+// row: shared address of the pair-row.
+template <int ORDER, int NH2>
+__device__ __forceinline__ void kick_fp_granule_any2(uint32_t row, int h, const float (&l)[ORDER], int mm, int g,
                                                      int N, float fp_b, float c2, const float2 (&c1p)[4],
                                                      float (&out)[4])
 {
@@ -134,7 +156,7 @@ __device__ __forceinline__ void kick_fp_granule_any2(const float *row, int h, co
 #pragma unroll
         for (int j = 0; j < ORDER; ++j) {
             const int s = y + mm - O0 + j;
-            const float v = (s >= 0 && s < N) ? row[2 * s + h] : 0.0f;
+            const float v = (s >= 0 && s < N) ? lds(row + col_off<NH2>(s) + h * 4) : 0.0f;
             acc = fmaf(l[j], v, acc);
         }
         k[i] = (y >= 0 && y < N) ? acc : 0.0f;
@@ -149,19 +171,80 @@ __device__ __forceinline__ void kick_fp_granule_any2(const float *row, int h, co
     }
 }
 
+// Everything the kick pass of one pair-row needs besides the weights (addresses are shared-window).
+struct KickRow2 {
+    uint32_t row, orow;          // bufB pair-row, bufA pair-row (start of the row)
+    uint32_t adupA, adupB;       // second slots of rows stored twice
+    uint32_t aup, mup, adn, mdn; // halo slots in the neighbours and their mbarriers
+    bool dupA, dupB, up, dn;
+};
+
+// all NG granules of one pair-row with compile-time shift MM and NW common nodes:
+// bufB -> bufA (+ second slots, + halo pushes); adds the new values to colsum (per column, both
+// rows packed) -- every moment of a6 is formed from colsum and the row sums rs afterwards.
+template <int ORDER, int N, int MM, int NW>
+__device__ __forceinline__ void kick_fp_row2(const KickRow2 &K, const float2 (&W)[ORDER + 1], int lane, float2 fp_b,
+                                             float2 c2, const float2 (&c1p)[N / 128][4], float2 (&colsum)[N / 128][4],
+                                             float2 &rs)
+{
+    constexpr int NG = N / 128, NH2 = cluster2_nh2(N);
+#pragma unroll
+    for (int k = 0; k < NG; ++k) {
+        const int g = 4 * lane + 128 * k;
+        float2 b[12], o[4];
+        // columns g - 4 + 2q, q = 0..5: chunk 2 (lane + 32 k) + q -> even chunks in region 0, odd in 1
+        const uint32_t c0 = (uint32_t)((lane + 32 * k) * 16);
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            const float4 v = lds4(K.row + c0 + (uint32_t)(((q >> 1) + (q & 1) * NH2) * 16));
+            b[2 * q] = make_float2(v.x, v.y);
+            b[2 * q + 1] = make_float2(v.z, v.w);
+        }
+        kick_fp_granule2<ORDER, MM, NW>(b, W, g, N, fp_b, c2, c1p[k], o);
+        // columns g, g+1 = chunk 2 (lane + 32 k) + 2, columns g+2, g+3 = the odd chunk after it
+        const uint32_t e0 = c0 + 16, e1 = c0 + 16 + NH2 * 16;
+        sts4(K.orow + e0, make_float4(o[0].x, o[0].y, o[1].x, o[1].y));
+        sts4(K.orow + e1, make_float4(o[2].x, o[2].y, o[3].x, o[3].y));
+        if (K.dupA) {
+            sts(K.adupA + e0, o[0].x); sts(K.adupA + e0 + 8, o[1].x); sts(K.adupA + e1, o[2].x); sts(K.adupA + e1 + 8, o[3].x);
+        }
+        if (K.dupB) {
+            sts(K.adupB + e0, o[0].y); sts(K.adupB + e0 + 8, o[1].y); sts(K.adupB + e1, o[2].y); sts(K.adupB + e1 + 8, o[3].y);
+        }
+        if (K.up) {
+            st_async(K.aup + e0, o[0].x, K.mup); st_async(K.aup + e0 + 8, o[1].x, K.mup);
+            st_async(K.aup + e1, o[2].x, K.mup); st_async(K.aup + e1 + 8, o[3].x, K.mup);
+        }
+        if (K.dn) {
+            st_async(K.adn + e0, o[0].y, K.mdn); st_async(K.adn + e0 + 8, o[1].y, K.mdn);
+            st_async(K.adn + e1, o[2].y, K.mdn); st_async(K.adn + e1 + 8, o[3].y, K.mdn);
+        }
+        rs = add2(rs, add2(add2(o[0], o[1]), add2(o[2], o[3])));
+#pragma unroll
+        for (int c = 0; c < 4; ++c) colsum[k][c] = add2(colsum[k][c], o[c]);
+    }
+}
+
 // ---------------------------------------------------------------- packed rotation of pair-rows
 // Thread = column y; pair-rows w0..w1-1 of bufA -> bufB, i.e. the cells (x0 + w, y) and
-// (x0 + w + Rh, y).  aA / aB: shared addresses of bufA[pair-row 0][CL_PAD + y - O0] and
-// bufB[pair-row 0][CL_PAD + y] (float2 elements, PITCH of them per pair-row).
-template <int ORDER, int PITCH>
+// (x0 + w + Rh, y).  aA: shared address of bufA's pair-row 0; aB: of this thread's column in
+// bufB's pair-row 0; toff[j]: byte offset of tap column y + iy - O0 + j inside a pair-row.
+template <int ORDER, int NH2>
 struct Rotator2 {
     static constexpr int O0 = (ORDER - 1) / 2;
-    static constexpr int PB = PITCH * 8;          // bytes per pair-row
+    static constexpr int PB = NH2 * 32;           // bytes per pair-row
     static constexpr unsigned FULL = 0xffffffffu;
     float2 win[ORDER][ORDER];
     float a, d, bY, aY, Xoff;     // dx = a*X + bY, dy = d*X + aY, X = x + Xoff
     uint32_t aA, aB;
-    int H, Rh;
+    uint32_t toff[ORDER];
+    int H, Rh, y;
+
+    __device__ __forceinline__ void set_taps(int iy)
+    {
+#pragma unroll
+        for (int j = 0; j < ORDER; ++j) toff[j] = col_off<NH2>(y + iy - O0 + j);
+    }
 
     template <int SUB, bool FULLWIN>
     __device__ __forceinline__ void load(uint32_t base)
@@ -170,10 +253,10 @@ struct Rotator2 {
 #pragma unroll
             for (int i = 0; i < ORDER; ++i)
 #pragma unroll
-                for (int j = 0; j < ORDER; ++j) win[(SUB + i) % ORDER][j] = lds2(base + i * PB + j * 8);
+                for (int j = 0; j < ORDER; ++j) win[(SUB + i) % ORDER][j] = lds2(base + i * PB + toff[j]);
         } else {
 #pragma unroll
-            for (int j = 0; j < ORDER; ++j) win[(SUB + ORDER - 1) % ORDER][j] = lds2(base + (ORDER - 1) * PB + j * 8);
+            for (int j = 0; j < ORDER; ++j) win[(SUB + ORDER - 1) % ORDER][j] = lds2(base + (ORDER - 1) * PB + toff[j]);
         }
     }
     template <int SUB>
@@ -201,16 +284,19 @@ struct Rotator2 {
         float tx, ty;
         floor_frac(fmaf(a, X, bY), ix, tx);
         floor_frac(fmaf(d, X, aY), iy, ty);
-        const uint32_t base = aA + (uint32_t)((w + H + ix - O0) * PB + iy * 8 + h * 4);
+        const uint32_t base = aA + (uint32_t)((w + H + ix - O0) * PB + h * 4);
+        uint32_t to[ORDER];
+#pragma unroll
+        for (int j = 0; j < ORDER; ++j) to[j] = col_off<NH2>(y + iy - O0 + j);
         float lx[ORDER], ly[ORDER];
         lagrange<ORDER>(tx, lx);
         lagrange<ORDER>(ty, ly);
         float acc = 0.0f;
 #pragma unroll
         for (int i = 0; i < ORDER; ++i) {
-            float rsum = ly[0] * lds(base + i * PB);
+            float rsum = ly[0] * lds(base + i * PB + to[0]);
 #pragma unroll
-            for (int j = 1; j < ORDER; ++j) rsum = fmaf(ly[j], lds(base + i * PB + j * 8), rsum);
+            for (int j = 1; j < ORDER; ++j) rsum = fmaf(ly[j], lds(base + i * PB + to[j]), rsum);
             acc = (i == 0) ? lx[0] * rsum : fmaf(lx[i], rsum, acc);
         }
         sts(aB + (uint32_t)(w * PB + h * 4), acc);
@@ -243,7 +329,8 @@ struct Rotator2 {
             if (__all_sync(FULL, (rx0 == rxL) && (ry0 == ryL))) {
                 const int ix = __float_as_int(rx0) - CL_IMAGIC, iy = __float_as_int(ry0) - CL_IMAGIC;
                 const float fx = rx0 - CL_MAGIC, fy = ry0 - CL_MAGIC;
-                uint32_t base = aA + (uint32_t)((w0 + H + ix - O0) * PB + iy * 8);
+                set_taps(iy);
+                uint32_t base = aA + (uint32_t)((w0 + H + ix - O0) * PB);
                 uint32_t ob = aB + (uint32_t)(w0 * PB);
                 float2 X = make_float2(X0, X0 + (float)Rh);
                 int w = w0;
@@ -265,7 +352,8 @@ struct Rotator2 {
             if (__all_sync(FULL, (rxA == rxB) && (ryA == ryB))) {
                 // (lanes may still differ from one another: every lane has its own base address)
                 const int ix = __float_as_int(rxA) - CL_IMAGIC, iy = __float_as_int(ryA) - CL_IMAGIC;
-                const uint32_t base = aA + (uint32_t)((w + H + ix - O0) * PB + iy * 8);
+                set_taps(iy);
+                const uint32_t base = aA + (uint32_t)((w + H + ix - O0) * PB);
                 chunk_rows<0, true>(base, aB + (uint32_t)(w * PB), make_float2(XA, XB), rxA - CL_MAGIC, ryA - CL_MAGIC, false, 1);
             } else {
                 cell_generic(w, 0, x0);
@@ -279,11 +367,12 @@ struct Rotator2 {
 // grid = S * (concurrent clusters), cluster = S CTAs, block = NT.  Protocol between the CTAs:
 // exactly that of k_cluster_step (MB_RHO / MB_HALO / MB_PART, one phase per step).
 template <int ORDER, int N, int NT>
-__global__ void __launch_bounds__(NT, 1)
+__global__ void __launch_bounds__(NT, (NT <= 256) ? 2 : 1)
 k_cluster2_step(GridConst G, ClusterArgs A)
 {
     static_assert(N >= 128 && N % 128 == 0, "N must be a multiple of 128");
-    constexpr int PITCH = N + 2 * CL_PAD;            // float2 elements per pair-row
+    constexpr int NH2 = cluster2_nh2(N);             // 16-byte chunks per region of a pair-row
+    constexpr int PITCH = 4 * NH2;                   // float2 slots per pair-row (two regions)
     constexpr int PB = PITCH * 8;                    // bytes per pair-row
     constexpr int NWARPS = NT / 32;
     constexpr int CW = N / 32;                       // warps across one row in the rotation
@@ -308,7 +397,9 @@ k_cluster2_step(GridConst G, ClusterArgs A)
     float *part = rho + N;                                // 2 * CL_MAX_S * CL_NPART
     float *wred = part + 2 * CL_MAX_S * CL_NPART;         // CL_WARPS * 8
     float *scal = wred + CL_WARPS * 8;                    // [2..7] = three mbarriers
+    float *rowinfo = scal + 8;                            // R x { l_0..l_3 (times 1/C), mm, -, -, - }
     const uint32_t sA = smem_u32(bufA), sB = smem_u32(bufB), sRho = smem_u32(rho), sPart = smem_u32(part);
+    const uint32_t sInfo = smem_u32(rowinfo);
     const uint32_t mbRho = smem_u32(scal + 2), mbHalo = mbRho + 8, mbPart = mbRho + 16;
     const int nbrs = (rank > 0 ? 1 : 0) + (rank < S - 1 ? 1 : 0);
     const uint32_t bytesRho = (uint32_t)(N - R) * 4u, bytesHalo = (uint32_t)(nbrs * H * N) * 4u,
@@ -318,14 +409,15 @@ k_cluster2_step(GridConst G, ClusterArgs A)
     const int cw = warp % CW, rg = warp / CW;
     const int PPG = (Rh + RG - 1) / RG;
     const int wbeg = min(Rh, rg * PPG), wend = min(Rh, wbeg + PPG);
-    Rotator2<ORDER, PITCH> rot;
+    Rotator2<ORDER, NH2> rot;
     {
         constexpr int O0 = (ORDER - 1) / 2;
         const int y = cw * 32 + lane;
         const float Yc = (float)y + G.y0c;
         rot.a = G.a; rot.d = G.d; rot.bY = G.b * Yc; rot.aY = G.a * Yc; rot.Xoff = G.x0c; rot.H = H; rot.Rh = Rh;
-        rot.aA = sA + (uint32_t)((CL_PAD + y - O0) * 8);
-        rot.aB = sB + (uint32_t)((CL_PAD + y) * 8);
+        rot.y = y;
+        rot.aA = sA;
+        rot.aB = sB + col_off<NH2>(y);
         asm volatile("" : "+r"(rot.aA), "+r"(rot.aB));      // opaque: do not re-derive per use
     }
 
@@ -348,15 +440,19 @@ k_cluster2_step(GridConst G, ClusterArgs A)
         float *gpsi = A.psi + (size_t)m * N * N;
         const float *gw = A.wfun ? A.wfun + (size_t)m * 2 * N : nullptr;
         // ---- load: own rows + halo rows straight from HBM into one or two slots of bufA
-        for (int i = tid; i < (R + 2 * H) * PITCH; i += NT) {
-            const int lr = i / PITCH, cc = i - lr * PITCH, c = cc - CL_PAD;
+        // (every pad column, and the unused chunks between the regions, stay zero for good)
+        for (int i = tid; i < (PA + Rh) * PITCH * 2; i += NT) bufA[i] = 0.0f;       // bufA and bufB
+        __syncthreads();
+        for (int i = tid; i < (R + 2 * H) * N; i += NT) {
+            const int lr = i / N, c = i - lr * N;
             const int x = x0 - H + lr;
-            float v = 0.0f;
-            if (x >= 0 && x < N && c >= 0 && c < N) v = gpsi[(size_t)x * N + c];
-            if (lr < PA) bufA[((size_t)lr * PITCH + cc) * 2] = v;
-            if (lr >= Rh) bufA[((size_t)(lr - Rh) * PITCH + cc) * 2 + 1] = v;
+            if (x >= 0 && x < N) {
+                const float v = gpsi[(size_t)x * N + c];
+                const uint32_t o = col_off<NH2>(c);
+                if (lr < PA) sts(sA + (uint32_t)(lr * PB) + o, v);
+                if (lr >= Rh) sts(sA + (uint32_t)((lr - Rh) * PB) + o + 4, v);
+            }
         }
-        for (int i = tid; i < Rh * PITCH * 2; i += NT) bufB[i] = 0.0f;
         for (int i = tid; i < 2 * N; i += NT) wf[i] = (gw && i < 2 * N - 1) ? gw[i] : 0.0f;
         float sc = G.renorm ? A.scale[m] : 1.0f;
         if (tid == 0) { mbar_expect_tx(mbRho, bytesRho); mbar_expect_tx(mbHalo, bytesHalo); mbar_expect_tx(mbPart, bytesPart); }
@@ -370,9 +466,12 @@ k_cluster2_step(GridConst G, ClusterArgs A)
                 mbar_wait(mbHalo, phase ^ 1u);
                 if (tid == 0 && !last) mbar_expect_tx(mbHalo, bytesHalo);
             }
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 0] = clock64();
             // ================= 1. rotation: bufA -> bufB
             if (!last) rot.run(wbeg, wend, x0);
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 1] = clock64();
             __syncthreads();
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 2] = clock64();
             if (step > 0) {
                 // ================= 6. a6 of step t-1: charge, scale, diagnostics
                 mbar_wait(mbPart, phase ^ 1u);
@@ -405,14 +504,19 @@ k_cluster2_step(GridConst G, ClusterArgs A)
                 }
             }
             if (last) break;
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 3] = clock64();
             // ================= 2. projection: rho_x = dp * sc * sum_y bufB(x, y), all-gathered
             for (int w = warp; w < Rh; w += NWARPS) {
-                const uint32_t row = sB + (uint32_t)(w * PB + CL_PAD * 8);
+                // every 16-byte chunk of the pair-row (pads and gaps are zero), in storage order
+                const uint32_t row = sB + (uint32_t)(w * PB);
                 float2 s = f2(0.0f);
 #pragma unroll
-                for (int k = 0; k < N / 64; ++k) {
-                    const float4 v = lds4(row + (uint32_t)((2 * lane + 64 * k) * 8));
-                    s = add2(s, add2(make_float2(v.x, v.y), make_float2(v.z, v.w)));
+                for (int k = 0; k < (2 * NH2 + 31) / 32; ++k) {
+                    const int ch = lane + 32 * k;
+                    if (ch < 2 * NH2) {
+                        const float4 v = lds4(row + (uint32_t)(ch * 16));
+                        s = add2(s, add2(make_float2(v.x, v.y), make_float2(v.z, v.w)));
+                    }
                 }
                 const float sa = warp_sum(s.x) * (G.dp * sc), sb = warp_sum(s.y) * (G.dp * sc);
                 if (lane == 0) { rho[x0 + w] = sa; rho[x0 + w + Rh] = sb; }   // own slots double as staging
@@ -427,41 +531,72 @@ k_cluster2_step(GridConst G, ClusterArgs A)
                     st_async4(mapa(a, dd), lds4(a), mapa(mbRho, dd));
                 }
             }
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 4] = clock64();
             mbar_wait(mbRho, phase);
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 5] = clock64();
             if (tid == 0 && step + 1 < A.nsteps) mbar_expect_tx(mbRho, bytesRho);
-            // ================= 3.+4. wake (own rows), kick + Fokker-Planck: bufB -> bufA
-            // per-warp sums: s0 sum psi, q1/q2 q moments, pw = sum rho V; per-lane column sums
-            float s0 = 0.0f, q1 = 0.0f, q2 = 0.0f, pw = 0.0f;
-            float colsum[NG][4];
+            // ================= 3. wake a3 of the own rows, then the kick weights of every row, once:
+            // TPR threads share one row (x' interleaved), V_x = sum_x' w[x - x'] rho_x' (Eq. 4;
+            // w[d] at wf[d + N - 1]); the group's first lane turns V_x into the integer shift mm and
+            // the Lagrange weights (times 1/C) and leaves them in rowinfo[row].
+            float pw = 0.0f;                                   // sum rho V (group leaders only)
+            {
+                const int TPR = min(32, max(1, NT / R)), sub = tid & (TPR - 1);
+                for (int r = tid / TPR; r < R; r += NT / TPR) {
+                    const int x = x0 + r;
+                    float V = 0.0f;
+                    if (gw != nullptr) {
+                        float v0 = 0.0f, v1 = 0.0f, v2 = 0.0f, v3 = 0.0f;
+                        const float *wx = wf + (x + N - 1);
+                        for (int xp = sub; xp < N; xp += 4 * TPR) {
+                            v0 = fmaf(wx[-xp], rho[xp], v0);
+                            v1 = fmaf(wx[-(xp + TPR)], rho[xp + TPR], v1);
+                            v2 = fmaf(wx[-(xp + 2 * TPR)], rho[xp + 2 * TPR], v2);
+                            v3 = fmaf(wx[-(xp + 3 * TPR)], rho[xp + 3 * TPR], v3);
+                        }
+                        V = (v0 + v1) + (v2 + v3);
+                        for (int o = TPR >> 1; o > 0; o >>= 1) V += __shfl_xor_sync(FULL, V, o);
+                    }
+                    if (sub == 0) {
+                        pw = fmaf(rho[x], V, pw);
+                        int mm;
+                        float t;
+                        floor_frac(G.kick_c * V, mm, t);
+                        float l[ORDER];
+                        lagrange<ORDER>(t, l);
+                        float4 lw = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        lw.x = l[0] * sc; lw.y = l[1] * sc;
+                        if (ORDER > 2) lw.z = l[ORDER > 2 ? 2 : 0] * sc;
+                        if (ORDER > 3) lw.w = l[ORDER > 3 ? 3 : 0] * sc;
+                        *reinterpret_cast<float4 *>(rowinfo + 8 * r) = lw;
+                        *reinterpret_cast<int *>(rowinfo + 8 * r + 4) = mm;
+                    }
+                }
+            }
+            __syncthreads();
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 6] = clock64();
+            // ================= 4. kick + Fokker-Planck: bufB -> bufA
+            // per lane: column sums of the new psi (both rows packed), q-moment sums of its part of
+            // every row
+            float2 q1v = f2(0.0f), q2v = f2(0.0f);
+            float2 colsum[NG][4];
 #pragma unroll
             for (int k = 0; k < NG; ++k)
 #pragma unroll
-                for (int c = 0; c < 4; ++c) colsum[k][c] = 0.0f;
+                for (int c = 0; c < 4; ++c) colsum[k][c] = f2(0.0f);
+            const float2 fb2 = f2(G.fp_b), cc2 = f2(c2);
             for (int w = warp; w < Rh; w += NWARPS) {
                 const int xA = x0 + w, xB = xA + Rh;
-                float VA = 0.0f, VB = 0.0f;
-                if (gw != nullptr) {
-                    // V_x = sum_x' w[x - x'] rho_x'; w[d] at wf[d + N - 1]
-#pragma unroll
-                    for (int k = 0; k < CW; ++k) {
-                        const int xp = lane + 32 * k;
-                        const float rr = rho[xp];
-                        VA = fmaf(wf[xA - xp + N - 1], rr, VA);
-                        VB = fmaf(wf[xB - xp + N - 1], rr, VB);
-                    }
-                    VA = warp_sum(VA); VB = warp_sum(VB);
-                }
-                pw = fmaf(rho[xA], VA, pw);
-                pw = fmaf(rho[xB], VB, pw);
-                int mmA, mmB;
-                float tA, tB;
-                floor_frac(G.kick_c * VA, mmA, tA);
-                floor_frac(G.kick_c * VB, mmB, tB);
                 float lA[ORDER], lB[ORDER];
-                lagrange<ORDER>(tA, lA);
-                lagrange<ORDER>(tB, lB);
+                int mmA, mmB;
+                {
+                    const float4 a4 = lds4(sInfo + (uint32_t)(w * 32)), b4 = lds4(sInfo + (uint32_t)((w + Rh) * 32));
+                    mmA = __float_as_int(lds(sInfo + (uint32_t)(w * 32 + 16)));
+                    mmB = __float_as_int(lds(sInfo + (uint32_t)((w + Rh) * 32 + 16)));
+                    const float la[4] = {a4.x, a4.y, a4.z, a4.w}, lb[4] = {b4.x, b4.y, b4.z, b4.w};
 #pragma unroll
-                for (int j = 0; j < ORDER; ++j) { lA[j] *= sc; lB[j] *= sc; }
+                    for (int j = 0; j < ORDER; ++j) { lA[j] = la[j]; lB[j] = lb[j]; }
+                }
                 const int mlo = min(mmA, mmB), dm = max(mmA, mmB) - mlo;
                 // common-node weights of both rows (see kick_fp_granule2)
                 float2 W[ORDER + 1];
@@ -469,94 +604,75 @@ k_cluster2_step(GridConst G, ClusterArgs A)
                     const bool sa = (mmA != mlo), sb = (mmB != mlo);   // row shifted one node up
 #pragma unroll
                     for (int j = 0; j <= ORDER; ++j) {
-                        const float wa = sa ? (j > 0 ? lA[j > 0 ? j - 1 : 0] : 0.0f) : (j < ORDER ? lA[j < ORDER ? j : 0] : 0.0f);
-                        const float wb = sb ? (j > 0 ? lB[j > 0 ? j - 1 : 0] : 0.0f) : (j < ORDER ? lB[j < ORDER ? j : 0] : 0.0f);
-                        W[j] = make_float2(wa, wb);
+                        const float a0 = (j < ORDER) ? lA[j < ORDER ? j : 0] : 0.0f, a1 = (j > 0) ? lA[j > 0 ? j - 1 : 0] : 0.0f;
+                        const float b0 = (j < ORDER) ? lB[j < ORDER ? j : 0] : 0.0f, b1 = (j > 0) ? lB[j > 0 ? j - 1 : 0] : 0.0f;
+                        W[j] = make_float2(sa ? a1 : a0, sb ? b1 : b0);
                     }
                 }
                 const int mode = (dm == 0 && mlo >= -2 && mlo <= 0) ? (mlo + 2)            // 0,1,2: same shift
                                  : (dm == 1 && mlo >= -2 && mlo <= -1) ? (mlo + 5)         // 3,4: shifts differ by one
                                                                        : 5;                // generic
-                const uint32_t row = sB + (uint32_t)(w * PB + CL_PAD * 8);
-                const uint32_t orow = sA + (uint32_t)((w + H) * PB + CL_PAD * 8);
+                KickRow2 K;
+                K.row = sB + (uint32_t)(w * PB);
+                K.orow = sA + (uint32_t)((w + H) * PB);
                 // second slots of the rows stored twice, and halo pushes (first H rows -> rank-1's
                 // lower halo, last H rows -> rank+1's upper halo)
-                const bool dupA = (w + H >= Rh), dupB = (w < H);
-                const uint32_t adupA = sA + (uint32_t)((w + H - Rh) * PB + CL_PAD * 8 + 4);
-                const uint32_t adupB = sA + (uint32_t)((w + H + Rh) * PB + CL_PAD * 8);
-                const bool up = (w < H) && (rank > 0), dn = (w >= Rh - H) && (rank < S - 1);
-                uint32_t aup = 0, mup = 0, adn = 0, mdn = 0;
-                if (up) { aup = mapa(sA + (uint32_t)((Rh + H + w) * PB + CL_PAD * 8 + 4), rank - 1); mup = mapa(mbHalo, rank - 1); }
-                if (dn) { adn = mapa(sA + (uint32_t)((w - Rh + H) * PB + CL_PAD * 8), rank + 1); mdn = mapa(mbHalo, rank + 1); }
+                K.dupA = (w + H >= Rh); K.dupB = (w < H);
+                K.adupA = sA + (uint32_t)((w + H - Rh) * PB + 4);
+                K.adupB = sA + (uint32_t)((w + H + Rh) * PB);
+                K.up = (w < H) && (rank > 0); K.dn = (w >= Rh - H) && (rank < S - 1);
+                K.aup = K.mup = K.adn = K.mdn = 0;
+                if (K.up) { K.aup = mapa(sA + (uint32_t)((Rh + H + w) * PB + 4), rank - 1); K.mup = mapa(mbHalo, rank - 1); }
+                if (K.dn) { K.adn = mapa(sA + (uint32_t)((w - Rh + H) * PB), rank + 1); K.mdn = mapa(mbHalo, rank + 1); }
                 float2 rs = f2(0.0f);
+                switch (mode) {
+                    case 0: kick_fp_row2<ORDER, N, -2, ORDER>(K, W, lane, fb2, cc2, c1p, colsum, rs); break;
+                    case 1: kick_fp_row2<ORDER, N, -1, ORDER>(K, W, lane, fb2, cc2, c1p, colsum, rs); break;
+                    case 2: kick_fp_row2<ORDER, N, 0, ORDER>(K, W, lane, fb2, cc2, c1p, colsum, rs); break;
+                    case 3: kick_fp_row2<ORDER, N, -2, ORDER + 1>(K, W, lane, fb2, cc2, c1p, colsum, rs); break;
+                    case 4: kick_fp_row2<ORDER, N, -1, ORDER + 1>(K, W, lane, fb2, cc2, c1p, colsum, rs); break;
+                    default: {
 #pragma unroll
-                for (int k = 0; k < NG; ++k) {
-                    const int g = 4 * lane + 128 * k;
-                    float2 o[4];
-                    if (mode < 5) {
-                        float2 b[12];
+                        for (int k = 0; k < NG; ++k) {
+                            const int g = 4 * lane + 128 * k;
+                            float oa[4], ob[4];
+                            kick_fp_granule_any2<ORDER, NH2>(K.row, 0, lA, mmA, g, N, G.fp_b, c2, c1p[k], oa);
+                            kick_fp_granule_any2<ORDER, NH2>(K.row, 1, lB, mmB, g, N, G.fp_b, c2, c1p[k], ob);
 #pragma unroll
-                        for (int q = 0; q < 6; ++q) {
-                            const float4 v = lds4(row + (uint32_t)((g - 4 + 2 * q) * 8));
-                            b[2 * q] = make_float2(v.x, v.y);
-                            b[2 * q + 1] = make_float2(v.z, v.w);
+                            for (int c = 0; c < 4; ++c) {
+                                const uint32_t e = col_off<NH2>(g + c);
+                                const float2 oc = make_float2(oa[c], ob[c]);
+                                sts2(K.orow + e, oc);
+                                if (K.dupA) sts(K.adupA + e, oa[c]);
+                                if (K.dupB) sts(K.adupB + e, ob[c]);
+                                if (K.up) st_async(K.aup + e, oa[c], K.mup);
+                                if (K.dn) st_async(K.adn + e, ob[c], K.mdn);
+                                rs = add2(rs, oc);
+                                colsum[k][c] = add2(colsum[k][c], oc);
+                            }
                         }
-                        const float2 fb = f2(G.fp_b), cc2 = f2(c2);
-                        switch (mode) {
-                            case 0: kick_fp_granule2<ORDER, -2, ORDER>(b, W, g, N, fb, cc2, c1p[k], o); break;
-                            case 1: kick_fp_granule2<ORDER, -1, ORDER>(b, W, g, N, fb, cc2, c1p[k], o); break;
-                            case 2: kick_fp_granule2<ORDER, 0, ORDER>(b, W, g, N, fb, cc2, c1p[k], o); break;
-                            case 3: kick_fp_granule2<ORDER, -2, ORDER + 1>(b, W, g, N, fb, cc2, c1p[k], o); break;
-                            default: kick_fp_granule2<ORDER, -1, ORDER + 1>(b, W, g, N, fb, cc2, c1p[k], o); break;
-                        }
-                    } else {
-                        float oa[4], ob[4];
-                        const float *prow = bufB + ((size_t)w * PITCH + CL_PAD) * 2;
-                        kick_fp_granule_any2<ORDER>(prow, 0, lA, mmA, g, N, G.fp_b, c2, c1p[k], oa);
-                        kick_fp_granule_any2<ORDER>(prow, 1, lB, mmB, g, N, G.fp_b, c2, c1p[k], ob);
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) o[c] = make_float2(oa[c], ob[c]);
                     }
-                    sts4(orow + (uint32_t)(g * 8), make_float4(o[0].x, o[0].y, o[1].x, o[1].y));
-                    sts4(orow + (uint32_t)(g * 8 + 16), make_float4(o[2].x, o[2].y, o[3].x, o[3].y));
-                    if (dupA) {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) sts(adupA + (uint32_t)((g + c) * 8), o[c].x);
-                    }
-                    if (dupB) {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) sts(adupB + (uint32_t)((g + c) * 8), o[c].y);
-                    }
-                    if (up) {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) st_async(aup + (uint32_t)((g + c) * 8), o[c].x, mup);
-                    }
-                    if (dn) {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) st_async(adn + (uint32_t)((g + c) * 8), o[c].y, mdn);
-                    }
-                    rs = add2(rs, add2(add2(o[0], o[1]), add2(o[2], o[3])));
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) colsum[k][c] += o[c].x + o[c].y;
                 }
-                // q moments of the END-of-step psi from the row sums (the same values in every lane)
-                const float ra = warp_sum(rs.x), rb = warp_sum(rs.y);
-                const float XA = (float)xA - xc, XB = (float)xB - xc;
-                const float ta = ra * XA, tb = rb * XB;
-                s0 += ra + rb;
-                q1 += ta + tb;
-                q2 = fmaf(ta, XA, fmaf(tb, XB, q2));
+                // q moments of the END-of-step psi: this lane's part of the two row sums
+                const float2 X2 = make_float2((float)xA - xc, (float)xB - xc);
+                const float2 tq = mul2(rs, X2);
+                q1v = add2(q1v, tq);
+                q2v = fma2(tq, X2, q2v);
             }
-            // p moments from the per-lane column sums
-            float s1 = 0.0f, s2 = 0.0f;
+            // charge and p moments from the per-lane column sums
+            float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f;
 #pragma unroll
             for (int k = 0; k < NG; ++k)
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     const float yy = (float)(4 * lane + 128 * k + c) - yc;
-                    const float tt = colsum[k][c] * yy;
-                    s1 += tt; s2 = fmaf(tt, yy, s2);
+                    const float cs = colsum[k][c].x + colsum[k][c].y;
+                    const float tt = cs * yy;
+                    s0 += cs; s1 += tt; s2 = fmaf(tt, yy, s2);
                 }
+            float q1 = q1v.x + q1v.y, q2 = q2v.x + q2v.y;
+            s0 = warp_sum(s0); q1 = warp_sum(q1); q2 = warp_sum(q2); pw = warp_sum(pw);
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 7] = clock64();
             // ================= 5. partial sums of this CTA -> every CTA
             s1 = warp_sum(s1); s2 = warp_sum(s2);
             if (lane == 0) {
@@ -585,9 +701,10 @@ k_cluster2_step(GridConst G, ClusterArgs A)
         __syncthreads();
         for (int i = tid; i < R * (N / 4); i += NT) {
             const int r = i / (N / 4), c = (i - r * (N / 4)) * 4;
-            const float *src = (r < Rh) ? bufA + ((size_t)(r + H) * PITCH + CL_PAD + c) * 2
-                                        : bufA + ((size_t)(r + H - Rh) * PITCH + CL_PAD + c) * 2 + 1;
-            *reinterpret_cast<float4 *>(gpsi + (size_t)(x0 + r) * N + c) = make_float4(src[0], src[2], src[4], src[6]);
+            const uint32_t src = (r < Rh) ? sA + (uint32_t)((r + H) * PB) : sA + (uint32_t)((r + H - Rh) * PB + 4);
+            *reinterpret_cast<float4 *>(gpsi + (size_t)(x0 + r) * N + c) =
+                make_float4(lds(src + col_off<NH2>(c)), lds(src + col_off<NH2>(c + 1)), lds(src + col_off<NH2>(c + 2)),
+                            lds(src + col_off<NH2>(c + 3)));
         }
         if (rank == 0 && tid == 0) A.scale[m] = sc;
         cluster.sync();       // every CTA is done with this member before anyone re-initialises

@@ -1,0 +1,424 @@
+// vfps_stream2.cuh -- second generation of the streaming (HBM / L2) kernels (sm_100a).
+//
+// ncu of the first generation at 2048^2 (profiles/r01_c4_stream.md): k_rotate 27.5 us, bound by
+// instruction issue (160 thread-instructions per cell, 79 % of the issue slots: tile staging with
+// bounds checks, 16 shared loads and one 5-step warp reduction per cell); k_kick_fp 26 us with
+// 12 % of the warp slots (132 KB of staged rows per CTA = one CTA of 8 warps per SM);
+// k_wake_fft 44.5 us on ONE SM (24 serial FFT stages with global twiddle loads).  Here:
+//   k_rotate2      a1 + a2: thread = column, walks down RT rows with a sliding ORDER x ORDER
+//                  register window fed by global loads that hit L1 (no staging, no bounds checks
+//                  away from the grid edge); row sums by an 8-value transposed warp reduction
+//   k_wake_direct  a3 by direct convolution (Eq. 4) on N/8 CTAs instead of one (the profile is
+//                  completed by the last CTA of every row of rotation tiles)
+//   k_kick_fp2     a4 + a5 + a6: four cells per thread in registers (12-value window, three
+//                  128-bit loads), no shared memory, thousands of warps in flight
+#pragma once
+#include "vfps_cluster.cuh"
+
+namespace vfps {
+
+constexpr int R2_RT = 16;          // rows per rotation tile (two reduction groups of 8)
+constexpr int R2_THREADS = 256;    // 8 warps = 256 columns per tile
+constexpr int R2_WARPS = R2_THREADS / 32;
+constexpr int WD_ROWS = 8;         // rows per CTA of k_wake_direct (one per warp)
+constexpr int WD_THREADS = 256;
+constexpr int K2_THREADS = 256;
+
+// 8 values per lane -> sums over the 32 lanes.  On return v[0] of lane l holds the total of input
+// value index ((l >> 4) & 1) * 4 + ((l >> 3) & 1) * 2 + ((l >> 2) & 1); 9 shuffles instead of 40.
+__device__ __forceinline__ float warp_reduce8(float (&v)[8], int lane)
+{
+    const unsigned FULL = 0xffffffffu;
+    {
+        const bool up = (lane & 16) != 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float send = up ? v[i] : v[i + 4], keep = up ? v[i + 4] : v[i];
+            v[i] = keep + __shfl_xor_sync(FULL, send, 16);
+        }
+    }
+    {
+        const bool up = (lane & 8) != 0;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const float send = up ? v[i] : v[i + 2], keep = up ? v[i + 2] : v[i];
+            v[i] = keep + __shfl_xor_sync(FULL, send, 8);
+        }
+    }
+    {
+        const bool up = (lane & 4) != 0;
+        const float send = up ? v[0] : v[1], keep = up ? v[1] : v[0];
+        v[0] = keep + __shfl_xor_sync(FULL, send, 4);
+    }
+    v[0] += __shfl_xor_sync(FULL, v[0], 2);
+    v[0] += __shfl_xor_sync(FULL, v[0], 1);
+    return v[0];
+}
+
+// read-only global load that the compiler keeps where it is written (all loads of a batch are
+// issued before the arithmetic that consumes the first one)
+__device__ __forceinline__ float ldg_nc(const float *p)
+{
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+
+// ---------------------------------------------------------------- a1 + a2: rotation + projection
+// grid = (tiles_x * tiles_y, members), block = 256.  Tile = R2_RT rows x 256 columns; thread =
+// column y, rows tx0 .. tx0 + R2_RT - 1 in groups of 8.  Taps come straight from global memory
+// (a warp reads 128 contiguous bytes per tap; the four taps of a row and the next warp's overlap
+// hit L1).  Fast path (warp-uniform): every tap of the group lies inside the grid and floor(dx),
+// floor(dy) do not change along the group for any lane -> sliding register window, ORDER loads per
+// cell.  Otherwise every cell loads its own window with per-tap range checks (psi = 0 outside, A8).
+// rho_part[m][x][tile_y] = dp * scale * sum over the tile's columns of psi'(x, .)
+template <int ORDER>
+struct GRot {
+    static constexpr int O0 = (ORDER - 1) / 2;
+    float a, d, bY, aY, Xoff;
+    const float *src;      // psi of this member
+    int N, y;
+
+    // one cell, its own floors, range-checked taps
+    __device__ __noinline__ float cell_checked(int x) const
+    {
+        const float X = (float)x + Xoff;
+        int ix, iy;
+        float tx, ty;
+        floor_frac(fmaf(a, X, bY), ix, tx);
+        floor_frac(fmaf(d, X, aY), iy, ty);
+        float lx[ORDER], ly[ORDER];
+        lagrange<ORDER>(tx, lx);
+        lagrange<ORDER>(ty, ly);
+        const int sx = x + ix - O0, sy = y + iy - O0;
+        float acc = 0.0f;
+#pragma unroll
+        for (int i = 0; i < ORDER; ++i) {
+            float rsum = 0.0f;
+#pragma unroll
+            for (int j = 0; j < ORDER; ++j) {
+                const int xx = sx + i, yy = sy + j;
+                const float v = (xx >= 0 && xx < N && yy >= 0 && yy < N) ? __ldg(src + (size_t)xx * N + yy) : 0.0f;
+                rsum = fmaf(ly[j], v, rsum);
+            }
+            acc = fmaf(lx[i], rsum, acc);
+        }
+        return acc;
+    }
+    // rows x .. x+7 with floors (ix, iy) throughout and every tap inside the grid: all
+    // (8 + ORDER - 1) x ORDER taps are requested before the first one is used (one exposed memory
+    // latency per group instead of one per row), then row r interpolates rows r .. r+ORDER-1
+    __device__ __forceinline__ void group8(const float *base, float X0, float fx, float fy, float (&out)[8]) const
+    {
+        float t[8 + ORDER - 1][ORDER];
+        const float *p = base;
+#pragma unroll
+        for (int i = 0; i < 8 + ORDER - 1; ++i) {
+#pragma unroll
+            for (int j = 0; j < ORDER; ++j) t[i][j] = ldg_nc(p + j);      // one address per row, immediate offsets
+            p += N;
+        }
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const float X = X0 + (float)r;
+            float lx[ORDER], ly[ORDER];
+            lagrange<ORDER>(fmaf(a, X, bY) - fx, lx);
+            lagrange<ORDER>(fmaf(d, X, aY) - fy, ly);
+            float acc = 0.0f;
+#pragma unroll
+            for (int i = 0; i < ORDER; ++i) {
+                float rsum = ly[0] * t[r + i][0];
+#pragma unroll
+                for (int j = 1; j < ORDER; ++j) rsum = fmaf(ly[j], t[r + i][j], rsum);
+                acc = (i == 0) ? lx[0] * rsum : fmaf(lx[i], rsum, acc);
+            }
+            out[r] = acc;
+        }
+    }
+};
+
+template <int ORDER>
+__global__ void __launch_bounds__(R2_THREADS)
+k_rotate2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_out,
+          const float *__restrict__ scale, float *__restrict__ rho_part, int tiles_y,
+          float *__restrict__ rho, unsigned *__restrict__ tilectr)
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+    constexpr unsigned FULL = 0xffffffffu;
+    __shared__ float red[R2_RT][R2_WARPS];
+    const int N = G.N, m = blockIdx.y;
+    const int tx0 = (blockIdx.x / tiles_y) * R2_RT, ty = blockIdx.x % tiles_y;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int y = ty * (32 * R2_WARPS) + warp * 32 + lane;
+    const bool yok = (y < N);
+    const float sc = G.renorm ? __ldg(scale + m) : 1.0f;
+    float *dst = psi_out + (size_t)m * N * N;
+
+    GRot<ORDER> rot;
+    rot.src = psi_in + (size_t)m * N * N;
+    rot.N = N; rot.y = min(y, N - 1);        // lanes beyond the grid compute a valid cell, never stored
+    {
+        const float Yc = (float)rot.y + G.y0c;
+        rot.a = G.a; rot.d = G.d; rot.bY = G.b * Yc; rot.aY = G.a * Yc; rot.Xoff = G.x0c;
+    }
+    if (warp * 32 + ty * (32 * R2_WARPS) < N) {       // warps entirely beyond the grid have nothing to do
+#pragma unroll 1
+        for (int grp = 0; grp < R2_RT / 8; ++grp) {
+            const int xg = tx0 + 8 * grp;             // rows xg .. xg+7 (clamped to the grid)
+            float out[8];
+            const int xl = min(xg + 7, N - 1), xf = min(xg, N - 1);
+            const float X0 = (float)xf + rot.Xoff, XL = (float)xl + rot.Xoff;
+            const float rx0 = __fadd_rd(fmaf(rot.a, X0, rot.bY), CL_MAGIC), ry0 = __fadd_rd(fmaf(rot.d, X0, rot.aY), CL_MAGIC);
+            const float rxL = __fadd_rd(fmaf(rot.a, XL, rot.bY), CL_MAGIC), ryL = __fadd_rd(fmaf(rot.d, XL, rot.aY), CL_MAGIC);
+            const int ix = __float_as_int(rx0) - CL_IMAGIC, iy = __float_as_int(ry0) - CL_IMAGIC;
+            const int sx = xg + ix - O0, sy = rot.y + iy - O0;
+            const bool fast = (rx0 == rxL) && (ry0 == ryL) && (xg + 7 < N) && (sx >= 0) && (sx + 7 + ORDER - 1 < N) &&
+                              (sy >= 0) && (sy + ORDER - 1 < N);
+            if (__all_sync(FULL, fast)) {
+                rot.group8(rot.src + (size_t)sx * N + sy, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
+            } else {
+#pragma unroll
+                for (int r = 0; r < 8; ++r) out[r] = rot.cell_checked(min(xg + r, N - 1));
+            }
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                out[r] *= sc;
+                const bool ok = yok && (xg + r < N);
+                if (ok) dst[(size_t)(xg + r) * N + y] = out[r];
+                else out[r] = 0.0f;
+            }
+            const float tot = warp_reduce8(out, lane);
+            if ((lane & 3) == 0) red[8 * grp + ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
+        }
+    } else {
+        if (lane < R2_RT) red[lane][warp] = 0.0f;
+    }
+    __syncthreads();
+    if (threadIdx.x < R2_RT) {
+        const int x = tx0 + threadIdx.x;
+        if (x < N) {
+            float s = 0.0f;
+#pragma unroll
+            for (int w = 0; w < R2_WARPS; ++w) s += red[threadIdx.x][w];
+            rho_part[((size_t)m * N + x) * tiles_y + ty] = G.dp * s;
+            __threadfence();
+        }
+    }
+    // ---- the last CTA of this row of tiles adds the tiles_y partial sums in a fixed order: the
+    // profile is complete when the kernel ends (tilectr[m][tile row] returns to zero)
+    __shared__ bool is_last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned *ctr = tilectr + (size_t)m * gridDim.x / tiles_y + blockIdx.x / tiles_y;
+        const unsigned done = atomicAdd(ctr, 1u);
+        is_last = (done == (unsigned)tiles_y - 1);
+        if (is_last) *ctr = 0u;
+    }
+    __syncthreads();
+    if (is_last && threadIdx.x < R2_RT) {
+        __threadfence();
+        const int x = tx0 + threadIdx.x;
+        if (x < N) {
+            const volatile float *pp = rho_part + ((size_t)m * N + x) * tiles_y;
+            float s = 0.0f;
+            for (int k = 0; k < tiles_y; ++k) s += pp[k];
+            rho[(size_t)m * N + x] = s;
+        }
+    }
+}
+
+// ---------------------------------------------------------------- a3: direct wake
+// grid = (ceil(N / WD_ROWS), members), block = 256 (one row per warp), dynamic shared memory
+// (2N + WD_ROWS) floats: the profile (complete after k_rotate2) and the N + WD_ROWS - 1 lags of the
+// wake function this CTA's rows touch are staged with coalesced loads, then warp w evaluates
+// V_x = sum_x' w[x - x'] rho_x' (Eq. 4; w = Re IDFT(Z) from create, lag d at index d + N - 1)
+// for x = r0 + w.  pw_part[m][cta] = sum over the CTA's rows of rho_x V_x.
+__global__ void __launch_bounds__(WD_THREADS)
+k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wfun, float *__restrict__ V,
+              float *__restrict__ pw_part)
+{
+    extern __shared__ float wd_smem[];
+    __shared__ float wpw[WD_THREADS / 32];
+    float *srho = wd_smem, *sw = wd_smem + N;
+    const int m = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int r0 = blockIdx.x * WD_ROWS;
+    const float *gr = rho + (size_t)m * N, *gw = wfun + (size_t)m * 2 * N + r0;
+    for (int i = tid; i < N; i += WD_THREADS) srho[i] = __ldg(gr + i);
+    for (int i = tid; i < N + WD_ROWS - 1; i += WD_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(gw + i) : 0.0f;
+    __syncthreads();
+    const int x = r0 + warp;
+    float v0 = 0.0f, v1 = 0.0f;
+    if (x < N) {
+        const float *wx = sw + (warp + N - 1);
+        int xp = lane;
+        for (; xp + 32 < N; xp += 64) {
+            v0 = fmaf(wx[-xp], srho[xp], v0);
+            v1 = fmaf(wx[-(xp + 32)], srho[xp + 32], v1);
+        }
+        if (xp < N) v0 = fmaf(wx[-xp], srho[xp], v0);
+    }
+    const float v = warp_sum(v0 + v1);
+    if (lane == 0) {
+        float pw = 0.0f;
+        if (x < N) {
+            V[(size_t)m * N + x] = v;
+            pw = srho[x] * v;
+        }
+        wpw[warp] = pw;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        float t = 0.0f;
+#pragma unroll
+        for (int i = 0; i < WD_THREADS / 32; ++i) t += wpw[i];
+        pw_part[(size_t)m * gridDim.x + blockIdx.x] = t;
+    }
+}
+
+// ---------------------------------------------------------------- a4 + a5 + a6: kick, FP, moments
+struct Kfp2Args {
+    const float *psi_in;    // rotated, scaled density (after a1)
+    float *psi_out;         // end-of-step density, un-normalised
+    const float *V;         // [members][N]
+    const float *qstat;     // [members][4] from k_wake_fft (P_raw in slot 3), used if pw_part == nullptr
+    const float *pw_part;   // [members][npw] from k_wake_direct, or nullptr
+    int npw;
+    float *mom_part;        // [members][gridDim.x][5]: sum psi, sum Yc psi, sum Yc^2 psi, sum Xc psi, sum Xc^2 psi
+    float *scale;           // [members] out: 1/C
+    unsigned *blkctr;       // [members], zero between launches
+    int *rowctr;            // [members] diagnostics row of this step
+    float *const *diag;     // device cell holding the caller's diag pointer (may hold NULL)
+    int members;
+    int rows_per_cta;
+};
+
+// grid = (ceil(N / rows_per_cta), members), block = 256.  Thread = granule of four cells g..g+3 of
+// one row: three 128-bit loads give the rotated density at g-4 .. g+7, kick and Fokker-Planck run
+// in registers (kick_fp_granule of vfps_cluster.cuh), one 128-bit store.  The last CTA of each
+// member finalises the diagnostics row and the renormalisation scalar (fixed summation order).
+template <int ORDER>
+__global__ void __launch_bounds__(K2_THREADS)
+k_kick_fp2(GridConst G, Kfp2Args A)
+{
+    __shared__ float red[8][K2_THREADS / 32];
+    __shared__ bool is_last;
+    const int N = G.N, m = blockIdx.y, NQ = N >> 2, lgNQ = 31 - __clz(NQ);      // N is a power of two
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const float *src = A.psi_in + (size_t)m * N * N;
+    float *dst = A.psi_out + (size_t)m * N * N;
+    const float yc = 0.5f * (float)(N - 1);
+    const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
+    const int x_begin = blockIdx.x * A.rows_per_cta;
+    const int nrows = min(N, x_begin + A.rows_per_cta) - x_begin;
+    float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 - - -
+
+    // four granules per thread and pass: every load of the pass is issued before the first use
+    const int total = nrows * NQ;
+    for (int idx0 = tid; idx0 < total; idx0 += 4 * K2_THREADS) {
+        float4 v0[4], v1[4], v2[4];
+        float Vx[4];
+        const float4 z4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int idx = idx0 + u * K2_THREADS;
+            v0[u] = v1[u] = v2[u] = z4; Vx[u] = 0.0f;
+            if (idx < total) {
+                const int x = x_begin + (idx >> lgNQ), g = (idx & (NQ - 1)) << 2;
+                const float *row = src + (size_t)x * N;
+                Vx[u] = __ldg(A.V + (size_t)m * N + x);
+                if (g >= 4) v0[u] = __ldg(reinterpret_cast<const float4 *>(row + g - 4));
+                v1[u] = __ldg(reinterpret_cast<const float4 *>(row + g));
+                if (g + 4 < N) v2[u] = __ldg(reinterpret_cast<const float4 *>(row + g + 4));
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int idx = idx0 + u * K2_THREADS;
+            if (idx < total) {
+                const int x = x_begin + (idx >> lgNQ), g = (idx & (NQ - 1)) << 2;
+                // kick of this row: y_r = y + sh, sh = (dphi/dp) V_x (Delta p = -dphi V)
+                int mm;
+                float t;
+                floor_frac(G.kick_c * Vx[u], mm, t);
+                float l[ORDER];
+                lagrange<ORDER>(t, l);
+                float c1p[4], o[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) c1p[c] = c1 * fmaf((float)(g + c), G.dp, G.p_min);
+                if (mm >= -2 && mm <= 0) {
+                    const float b[12] = {v0[u].x, v0[u].y, v0[u].z, v0[u].w, v1[u].x, v1[u].y, v1[u].z, v1[u].w,
+                                         v2[u].x, v2[u].y, v2[u].z, v2[u].w};
+                    if (mm == 0) kick_fp_granule<ORDER, 0>(b, l, g, N, G.fp_b, c2, c1p, o);
+                    else if (mm == -1) kick_fp_granule<ORDER, -1>(b, l, g, N, G.fp_b, c2, c1p, o);
+                    else kick_fp_granule<ORDER, -2>(b, l, g, N, G.fp_b, c2, c1p, o);
+                } else {
+                    kick_fp_granule_any<ORDER>(src + (size_t)x * N, l, mm, g, N, G.fp_b, c2, c1p, o);
+                }
+                *reinterpret_cast<float4 *>(dst + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
+                float rs = 0.0f;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const float yy = (float)(g + c) - yc, tt = o[c] * yy;
+                    rs += o[c]; acc[1] += tt; acc[2] = fmaf(tt, yy, acc[2]);
+                }
+                const float xx = (float)x - yc, tq = rs * xx;
+                acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+            }
+        }
+    }
+    {
+        const float tot = warp_reduce8(acc, lane);
+        if ((lane & 3) == 0) red[((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
+    }
+    __syncthreads();
+    if (tid < 5) {
+        float tsum = 0.0f;
+#pragma unroll
+        for (int w = 0; w < K2_THREADS / 32; ++w) tsum += red[tid][w];
+        A.mom_part[((size_t)m * gridDim.x + blockIdx.x) * 5 + tid] = tsum;
+        __threadfence();
+    }
+    // ---- last CTA of this member finalises the step (deterministic: fixed summation order)
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned done = atomicAdd(A.blkctr + m, 1u);
+        is_last = (done == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    if (warp == 0) {
+        double t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0, tp = 0;
+        const volatile float *mp = A.mom_part + (size_t)m * gridDim.x * 5;
+        for (int i = lane; i < (int)gridDim.x; i += 32) {
+            t0 += mp[5 * i]; t1 += mp[5 * i + 1]; t2 += mp[5 * i + 2]; t3 += mp[5 * i + 3]; t4 += mp[5 * i + 4];
+        }
+        if (A.pw_part != nullptr)
+            for (int i = lane; i < A.npw; i += 32) tp += A.pw_part[(size_t)m * A.npw + i];
+        t0 = warp_sum(t0); t1 = warp_sum(t1); t2 = warp_sum(t2); t3 = warp_sum(t3); t4 = warp_sum(t4); tp = warp_sum(tp);
+        if (lane == 0) {
+            const double C = (double)G.dq * (double)G.dp * t0;
+            const double mp_c = t1 / t0, vp = t2 / t0 - mp_c * mp_c;
+            const double mq_c = t3 / t0, vq = t4 / t0 - mq_c * mq_c;
+            const double P_raw = (A.pw_part != nullptr) ? tp * (double)G.dq : (double)A.qstat[(size_t)m * 4 + 3];
+            A.scale[m] = (float)(1.0 / C);
+            const int row = A.rowctr[m];
+            A.rowctr[m] = row + 1;
+            float *diag = *A.diag;
+            if (diag != nullptr) {
+                float *o = diag + ((size_t)row * A.members + m) * 6;
+                const double xc = 0.5 * (double)(N - 1);
+                const double cc = G.renorm ? C : 1.0;
+                o[0] = (float)C;
+                o[1] = (float)((double)G.q_min + (mq_c + xc) * (double)G.dq);
+                o[2] = (float)((double)G.p_min + (mp_c + xc) * (double)G.dp);
+                o[3] = (float)(sqrt(fmax(vq, 0.0)) * (double)G.dq);
+                o[4] = (float)(sqrt(fmax(vp, 0.0)) * (double)G.dp);
+                o[5] = (float)(P_raw / (cc * cc));
+            }
+            A.blkctr[m] = 0u;
+        }
+    }
+}
+
+}  // namespace vfps

@@ -258,22 +258,53 @@ def test_error_paths_on_gpu(vfps):
 # ---------------------------------------------------------------- engines
 def _engine_id(vfps, name):
     return {"stream": vfps.ENGINE_STREAM, "graph": vfps.ENGINE_GRAPH, "cluster": vfps.ENGINE_CLUSTER,
-            "cluster1": vfps.ENGINE_CLUSTER}[name]
+            "cluster2": vfps.ENGINE_CLUSTER}[name]
 
 
-@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster1"])
+@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster2"])
 def test_c1_every_engine_100_steps(vfps, orc, engine):
     """The same 100 steps of C1 through each engine (graph: two replays of 50 captured steps;
-    cluster: the packed kernel, which AUTO picks at 256^2; cluster1: the scalar kernel)."""
+    cluster: the scalar kernel, which AUTO picks; cluster2: the packed fp32x2 kernel)."""
     wl = get_workload("C1")
     sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 100, engine=_engine_id(vfps, engine), diag_every=1,
-                                     cluster_kernel=1 if engine == "cluster1" else None)
-    assert sim.engine_name == engine.rstrip("1")
+                                     cluster_kernel=2 if engine == "cluster2" else None)
+    assert sim.engine_name == engine.rstrip("2")
     if engine.startswith("cluster"):
-        assert sim.cluster_kernel == (1 if engine == "cluster1" else 2)
+        assert sim.cluster_kernel == (2 if engine == "cluster2" else 1)
     assert_psi(psi[0], refs[0].psi, 1e-4, f"C1 100 steps, {engine}")
     for i in (0, 1, 49, 50, 99):
         assert_diag(d[i, 0], dr[0][i])
+    sim.close()
+
+
+@pytest.mark.parametrize("gen,wake", [(1, "fft"), (2, "fft"), (2, "direct")])
+@pytest.mark.parametrize("order,N", [(4, 256), (3, 128), (2, 64), (4, 32)])
+def test_stream_generations(vfps, orc, gen, wake, order, N):
+    """Both generations of the streaming kernels and both wake evaluations (Eq. 5 FFT, Eq. 4 direct
+    convolution) on the stream and the graph engine: asymmetric box, off-centre bunch, free-space
+    wake, 300 steps per period (edge tiles, floors changing inside a tile; N = 32 and 64 are
+    narrower than one 256-column tile)."""
+    pad = 2
+    Z = make_impedance(N, pad, 12.0 / (N - 1), 0.4, None)[None, :]
+    psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
+    sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, pad, 1, Z=Z)
+    sim.set_stream_gen(gen)
+    sim.set_wake_mode({"fft": vfps.WAKE_FFT, "direct": vfps.WAKE_DIRECT}[wake])
+    sim.set_engine(vfps.ENGINE_STREAM)
+    assert sim.stream_gen == gen and sim.wake_name == wake
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, pad, Z[0])
+    o.set_psi(psi0[0])
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"stream gen {gen} {wake} N={N} order={order} 1 step")
+    assert_diag(d[0, 0], dr[0])
+    sim.set_engine(vfps.ENGINE_GRAPH)
+    d = sim.step_host(59)
+    dr = o.step(59)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"graph gen {gen} {wake} N={N} order={order} 60 steps")
+    for i in (0, 30, 58):
+        assert_diag(d[i, 0], dr[i])
     sim.close()
 
 
@@ -360,6 +391,8 @@ def test_cluster_engine_large_kick_and_switching(vfps, orc, N):
     psi0 = make_psi0(N, -6, 6, -6, 6, 1.0, 1.0, 0, 0)[None]
     spp = 100 * N // 64          # the same rotation displacement in cells on both grids
     sim = vfps.Simulation(N, -6, 6, -6, 6, spp, 1e-3, 4, 2, 1, Z=Z)
+    if N == 128:
+        sim.set_cluster_kernel(2)
     sim.set_engine(vfps.ENGINE_CLUSTER)
     assert sim.cluster_kernel == (2 if N == 128 else 1)
     sim.set_psi_host(psi0)
