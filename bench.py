@@ -46,7 +46,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--inner", type=int, default=0, help="split steps per bench step (0 = one synchrotron period)")
-    ap.add_argument("--engine", default="auto", choices=["auto", "stream", "graph", "cluster"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "stream", "graph", "cluster", "grid"])
     ap.add_argument("--wake", default="auto", choices=["auto", "fft", "direct"])
     ap.add_argument("--cluster-size", type=int, default=0, help="CTAs per cluster of the cluster engine (0 = auto)")
     ap.add_argument("--stream-gen", type=int, default=0, help="streaming kernels: 0 auto, 1 first generation, 2 second")
@@ -169,7 +169,7 @@ def run_reference(args, wl, rank, world):
 
 
 # ------------------------------------------------------------------------------------ our arm
-ENGINES = {"auto": 0, "stream": 1, "graph": 2, "cluster": 3}
+ENGINES = {"auto": 0, "stream": 1, "graph": 2, "cluster": 3, "grid": 4}
 WAKES = {"auto": 0, "fft": 1, "direct": 2}
 
 
@@ -235,7 +235,7 @@ def run_ours(args, wl, rank, local_rank, world):
     ms = dist.reduce_max(ms_local, dev)
     engine, wake = sim.engine_name, sim.wake_name
     cluster_size = sim.cluster_size if engine == "cluster" else None
-    sim_gen = sim.stream_gen if engine != "cluster" else None
+    sim_gen = sim.stream_gen if engine in ("stream", "graph") else None
     cluster_kernel = {1: "k_cluster_step (scalar fp32)", 2: "k_cluster2_step (packed fp32x2)"}.get(sim.cluster_kernel) if engine == "cluster" else None
     cluster_threads = sim.cluster_threads if engine == "cluster" else None
     diag_last = diag[-1].cpu().numpy().astype(float)
@@ -255,7 +255,7 @@ def run_ours(args, wl, rank, local_rank, world):
         sim.set_engine(ENGINES[args.engine])
     tot = sum(t for _, (t, c) in ktimes.items())
     kname, (kt, kc) = max(ktimes.items(), key=lambda kv: kv[1][0])
-    steps_per_launch = n_inner if kname.startswith("k_cluster") else 1
+    steps_per_launch = n_inner if (kname.startswith("k_cluster") or kname.startswith("k_grid")) else 1
     alg_bytes = ALG_BYTES_PER_CELL_STEP * cells * steps_per_launch
     achieved = alg_bytes / (kt / kc * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",

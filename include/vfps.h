@@ -98,14 +98,18 @@ enum {
     VFPS_KERNEL_ROTATE2 = 4,  /* a1 + a2, second-generation streaming kernel (register window)   */
     VFPS_KERNEL_WAKE_DIRECT = 5, /* a2 finish + a3 by direct convolution on N/32 CTAs             */
     VFPS_KERNEL_KICK_FP2 = 6, /* a4 + a5 + a6, second generation (four cells per thread)         */
-    VFPS_NUM_KERNELS = 7
+    VFPS_KERNEL_GRID = 7,     /* a1..a6 for all n steps of one vfps_step call (grid engine)      */
+    VFPS_NUM_KERNELS = 8
 };
 enum {
-    VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRAPH                    */
+    VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRID (one simulation) or
+                                 GRAPH (a batch)                                                 */
     VFPS_ENGINE_STREAM = 1,   /* one launch per kernel per step on the stream                    */
     VFPS_ENGINE_GRAPH = 2,    /* the same kernels replayed from a CUDA graph of many steps       */
-    VFPS_ENGINE_CLUSTER = 3   /* persistent thread-block-cluster kernel, psi resident in
+    VFPS_ENGINE_CLUSTER = 3,  /* persistent thread-block-cluster kernel, psi resident in
                                  distributed shared memory for all n steps                       */
+    VFPS_ENGINE_GRID = 4      /* persistent cooperative kernel on every SM, psi in L2 / HBM, grid
+                                 barriers where the step has global dependencies (members = 1)   */
 };
 enum {
     VFPS_WAKE_AUTO = 0,

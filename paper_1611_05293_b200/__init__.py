@@ -6,7 +6,7 @@ shared library cannot be built or loaded, importing symbols from it raises.
 """
 from .build import build, lib_path
 from .binding import (
-    ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER,
+    ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER, ENGINE_GRID,
     WAKE_AUTO, WAKE_FFT, WAKE_DIRECT, OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE,
     OPT_CLUSTER_KERNEL, OPT_CLUSTER_THREADS, OPT_STREAM_GEN,
     FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN,
@@ -15,7 +15,7 @@ from .binding import (
 
 __all__ = [
     "build", "lib_path", "load", "version", "EXPORTS",
-    "ENGINE_AUTO", "ENGINE_STREAM", "ENGINE_GRAPH", "ENGINE_CLUSTER",
+    "ENGINE_AUTO", "ENGINE_STREAM", "ENGINE_GRAPH", "ENGINE_CLUSTER", "ENGINE_GRID",
     "WAKE_AUTO", "WAKE_FFT", "WAKE_DIRECT", "OPT_ENGINE", "OPT_WAKE", "OPT_TIMING", "OPT_CLUSTER_SIZE",
     "OPT_CLUSTER_KERNEL", "OPT_CLUSTER_THREADS", "OPT_STREAM_GEN",
     "FLAG_RENORMALISE", "FLAG_CLAMP", "FLAG_ROT_MANHATTAN",

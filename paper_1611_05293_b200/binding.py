@@ -13,10 +13,10 @@ import numpy as np
 
 from .build import build, lib_path
 
-ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER = 0, 1, 2, 3
+ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER, ENGINE_GRID = 0, 1, 2, 3, 4
 WAKE_AUTO, WAKE_FFT, WAKE_DIRECT = 0, 1, 2
 OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL, OPT_CLUSTER_THREADS, OPT_STREAM_GEN = 1, 2, 3, 4, 5, 6, 7
-NUM_KERNELS = 7
+NUM_KERNELS = 8
 FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 
 # every symbol include/vfps.h declares (tests check the library exports each of them)

@@ -5,6 +5,7 @@
 #include "vfps_cluster.cuh"
 #include "vfps_cluster2.cuh"
 #include "vfps_stream2.cuh"
+#include "vfps_grid.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -61,6 +62,11 @@ struct vfps_sim {
     int gen_opt = 0;                             // 0 auto (2), 1, 2
     int tiles_x2 = 0, tiles_y2 = 0, kfp2_rows = 0, kfp2_blocks = 0, wd_blocks = 0;
     float *pw_part = nullptr;                    // [members][wd_blocks]
+    // persistent cooperative-grid engine (vfps_grid.cuh); gr_blocks = 0: not available
+    int gr_blocks = 0, gr_KR = 0;
+    size_t gr_smem = 0;
+    float *gr_mom = nullptr;                     // [gr_blocks][GR_NPART]
+    std::string gr_why;
     unsigned *tilectr = nullptr;                 // [members][tiles_x2], zero between launches
     size_t rot_smem = 0, kfp_smem = 0, fft_smem = 0;
     int fft_threads = 0;
@@ -386,6 +392,85 @@ int launch_step_stream(vfps_sim *h, bool timed)
     return VFPS_OK;
 }
 
+template <int ORDER>
+cudaError_t grid_occupancy(int *per_sm, size_t smem)
+{
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, k_grid_step<ORDER>, GR_THREADS, smem);
+}
+
+// The cooperative-grid engine needs every CTA resident at once: grid = SMs x (CTAs per SM, at most
+// two), rows of the kick phase dealt out evenly.
+void grid_configure(vfps_sim *h)
+{
+    h->gr_blocks = 0; h->gr_why.clear();
+    if (h->members != 1) { h->gr_why = "grid engine advances one simulation per handle"; return; }
+    int dev = 0, coop = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (!coop) { h->gr_why = "device does not support cooperative launches"; return; }
+    const int N = h->N;
+    int blocks = 2 * sms;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int KR = (N + blocks - 1) / blocks;
+        const size_t smem = grid_smem_floats(N, KR) * sizeof(float);
+        int per_sm = 0;
+        cudaError_t e;
+        switch (h->P.interp_order) {
+            case 2: e = grid_occupancy<2>(&per_sm, smem); break;
+            case 3: e = grid_occupancy<3>(&per_sm, smem); break;
+            default: e = grid_occupancy<4>(&per_sm, smem); break;
+        }
+        if (e != cudaSuccess || per_sm < 1) { cudaGetLastError(); h->gr_why = "grid kernel does not fit an SM"; return; }
+        const int fit = sms * (per_sm < 2 ? per_sm : 2);
+        if (fit >= blocks) { h->gr_blocks = blocks; h->gr_KR = KR; h->gr_smem = smem; return; }
+        blocks = fit;
+    }
+    h->gr_why = "grid kernel occupancy query did not converge";
+}
+
+int launch_grid_steps(vfps_sim *h, int n, float *diag)
+{
+    GridArgs A{};
+    A.psi = h->psi; A.psi_tmp = h->psi_tmp; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr;
+    A.rho_part = h->rho_part; A.mom_part = h->gr_mom; A.diag = diag; A.nsteps = n;
+    A.tiles_y = h->tiles_y2; A.KR = h->gr_KR;
+    void *args[2] = {(void *)&h->G, (void *)&A};
+    const void *kern;
+    switch (h->P.interp_order) {
+        case 2: kern = (const void *)k_grid_step<2>; break;
+        case 3: kern = (const void *)k_grid_step<3>; break;
+        default: kern = (const void *)k_grid_step<4>; break;
+    }
+    cudaError_t e;
+    // debug aid as in launch_cluster_steps: VFPS_PHASE_DUMP=<file>
+    const char *dump = std::getenv("VFPS_PHASE_DUMP");
+    const size_t ndbg = (size_t)h->gr_blocks * 64 * 8;
+    if (dump && cudaMalloc((void **)&A.dbg, ndbg * sizeof(long long)) != cudaSuccess) { A.dbg = nullptr; dump = nullptr; }
+    if (dump) cudaMemsetAsync(A.dbg, 0, ndbg * sizeof(long long), h->stream);
+    {
+        Bracket br(h, VFPS_KERNEL_GRID, h->timing);
+        e = cudaLaunchCooperativeKernel(kern, dim3((unsigned)h->gr_blocks), dim3(GR_THREADS), args, h->gr_smem, h->stream);
+    }
+    if (dump) {
+        std::vector<long long> t(ndbg);
+        cudaMemcpyAsync(t.data(), A.dbg, ndbg * sizeof(long long), cudaMemcpyDeviceToHost, h->stream);
+        cudaStreamSynchronize(h->stream);
+        cudaFree(A.dbg);
+        if (FILE *f = std::fopen(dump, "w")) {
+            for (size_t i = 0; i < ndbg; i += 8) {
+                std::fprintf(f, "%zu %zu", i / (64 * 8), (i / 8) % 64);
+                for (int k = 0; k < 8; ++k) std::fprintf(f, " %lld", t[i + k]);
+                std::fprintf(f, "\n");
+            }
+            std::fclose(f);
+        }
+    }
+    if (e != cudaSuccess) return fail(h, VFPS_ERR_CUDA, std::string("cooperative launch: ") + cudaGetErrorString(e));
+    h->launches += 1;
+    return VFPS_OK;
+}
+
 // which kernels the STREAM / GRAPH engines launch, and how they evaluate the wake
 int resolved_gen(const vfps_sim *h) { return h->gen_opt ? h->gen_opt : 2; }
 bool wake_is_direct(const vfps_sim *h)
@@ -450,7 +535,11 @@ int resolved_engine(const vfps_sim *h)
 {
     if (h->engine_opt == VFPS_ENGINE_STREAM) return VFPS_ENGINE_STREAM;
     if (h->engine_opt == VFPS_ENGINE_GRAPH) return VFPS_ENGINE_GRAPH;
-    return h->cl_S > 0 ? VFPS_ENGINE_CLUSTER : VFPS_ENGINE_GRAPH;      // AUTO, CLUSTER
+    if (h->engine_opt == VFPS_ENGINE_GRID) return VFPS_ENGINE_GRID;
+    if (h->engine_opt == VFPS_ENGINE_CLUSTER) return VFPS_ENGINE_CLUSTER;
+    // AUTO: on-chip grids -> cluster; one large simulation -> cooperative grid; else graph replay
+    if (h->cl_S > 0) return VFPS_ENGINE_CLUSTER;
+    return h->gr_blocks > 0 ? VFPS_ENGINE_GRID : VFPS_ENGINE_GRAPH;
 }
 
 // the captured graph depends on the kernel generation and the wake mode
@@ -602,6 +691,8 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
         h->launches += 1;
     }
     cluster_configure(h);
+    grid_configure(h);
+    if (h->gr_blocks > 0) CUB(dalloc(h, &h->gr_mom, (size_t)h->gr_blocks * GR_NPART));
     cudaError_t e = cudaSuccess;
     switch (p->interp_order) {
         case 2: e = set_kernel_attrs<2>(h); break;
@@ -675,6 +766,11 @@ int vfps_set_option(vfps_handle h, int option, int value)
         }
         if (value == VFPS_ENGINE_CLUSTER) {
             if (h->cl_S == 0) return fail(h, VFPS_ERR_UNSUPPORTED, "cluster engine unavailable: " + h->cl_why);
+            h->engine_opt = value;
+            return VFPS_OK;
+        }
+        if (value == VFPS_ENGINE_GRID) {
+            if (h->gr_blocks == 0) return fail(h, VFPS_ERR_UNSUPPORTED, "grid engine unavailable: " + h->gr_why);
             h->engine_opt = value;
             return VFPS_OK;
         }
@@ -755,13 +851,14 @@ const char *vfps_engine_name(vfps_handle h)
     switch (resolved_engine(h)) {
         case VFPS_ENGINE_STREAM: return "stream";
         case VFPS_ENGINE_GRAPH: return "graph";
+        case VFPS_ENGINE_GRID: return "grid";
         default: return "cluster";
     }
 }
 const char *vfps_wake_name(vfps_handle h)
 {
     if (!h) return "";
-    if (resolved_engine(h) == VFPS_ENGINE_CLUSTER) return "direct";
+    if (resolved_engine(h) == VFPS_ENGINE_CLUSTER || resolved_engine(h) == VFPS_ENGINE_GRID) return "direct";
     return wake_is_direct(h) ? "direct" : "fft";
 }
 
@@ -789,6 +886,13 @@ int vfps_step(vfps_handle h, int n, float *diag)
     if (n < 0) return fail(h, VFPS_ERR_ARG, "n must be >= 0");
     if (!h->psi_set) return fail(h, VFPS_ERR_STATE, "vfps_step before vfps_set_psi");
     if (n == 0) return VFPS_OK;
+    if (resolved_engine(h) == VFPS_ENGINE_GRID) {
+        if (h->timing) resolve_timing(h);
+        int rc = launch_grid_steps(h, n, diag);
+        if (rc != VFPS_OK) return rc;
+        h->steps += n;
+        return VFPS_OK;
+    }
     if (resolved_engine(h) == VFPS_ENGINE_CLUSTER) {
         if (h->timing) resolve_timing(h);
         int rc = launch_cluster_steps(h, n, diag);
@@ -975,6 +1079,7 @@ const char *vfps_kernel_name(int kernel)
         case VFPS_KERNEL_ROTATE2: return "k_rotate2";
         case VFPS_KERNEL_WAKE_DIRECT: return "k_wake_direct";
         case VFPS_KERNEL_KICK_FP2: return "k_kick_fp2";
+        case VFPS_KERNEL_GRID: return "k_grid_step";
         default: return nullptr;
     }
 }

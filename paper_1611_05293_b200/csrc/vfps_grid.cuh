@@ -1,0 +1,254 @@
+// vfps_grid.cuh -- persistent cooperative-grid engine for grids that do not fit on chip (sm_100a).
+//
+// The streaming engines pay three kernel launches per split step; at 2048^2 each kernel has
+// ~5-10 us of work and 3-5 us of ramp-up, tail and (for the reductions) a serial last-CTA epilogue
+// (profiles/r01_c4_stream.md).  Here ONE cooperative launch advances all n steps of a vfps_step
+// call: every SM keeps CTAs resident, psi ping-pongs between two HBM buffers that stay in the
+// 126 MB L2 (2 x 16 MB at 2048^2), and the two global dependencies of a step are grid barriers:
+//   phase 1  a1 + a2: rotation tiles of GR_RT rows x 256 columns (register window, as k_rotate2),
+//            per-tile row sums -> rho_part[tile_y][x]
+//   -- grid barrier --
+//   phase 2  every CTA sums the tile_y partial profiles (N * tiles_y coalesced L2 loads), then for
+//            its KR rows: a3 direct-convolution wake (Eq. 4), a4 + a5 kick and Fokker-Planck in
+//            registers (as k_kick_fp2), partial sums for a6 -> mom_part[cta]
+//   -- grid barrier --
+//   phase 3  every CTA adds the partial sums of all CTAs in the same fixed order -> C, 1/C;
+//            CTA 0 writes the diagnostics row.
+// One simulation per handle (members == 1); batches of on-chip grids use the cluster engine.
+#pragma once
+#include "vfps_stream2.cuh"
+
+#include <cooperative_groups.h>
+
+namespace vfps {
+
+constexpr int GR_RT = 8;            // rows per rotation tile (one reduction group)
+constexpr int GR_THREADS = 256;
+constexpr int GR_WARPS = GR_THREADS / 32;
+constexpr int GR_NPART = 8;         // partial sums per CTA per step
+
+struct GridArgs {
+    float *psi;          // [N][N] in/out, un-normalised
+    float *psi_tmp;      // [N][N] rotated density
+    float *scale;        // [1] in/out: 1/C of the last step
+    const float *wfun;   // [2N] wake function, lag d at index d + N - 1; nullptr = no wake
+    float *rho_part;     // [tiles_y][N]
+    float *mom_part;     // [GR_NPART][gridDim.x]: sum psi, sum Yc psi, sum Yc^2 psi, sum Xc psi, sum Xc^2 psi, sum rho V
+    float *diag;         // [nsteps][1][6] or nullptr
+    int nsteps;
+    int tiles_y;         // column tiles of 256
+    int KR;              // rows per CTA in phase 2
+    long long *dbg;      // nullptr, or [CTA][64 steps][8] clock64 stamps (debug aid)
+};
+
+__host__ __device__ inline size_t grid_smem_floats(int N, int KR) { return (size_t)2 * N + 2 * KR + 8; }
+
+template <int ORDER>
+__global__ void __launch_bounds__(GR_THREADS, 2)
+k_grid_step(GridConst G, GridArgs A)
+{
+    namespace cg = cooperative_groups;
+    constexpr int O0 = (ORDER - 1) / 2;
+    constexpr unsigned FULL = 0xffffffffu;
+    cg::grid_group grid = cg::this_grid();
+    extern __shared__ float gsm[];
+    __shared__ float red[8][GR_WARPS];
+    __shared__ float s_sc;
+    const int N = G.N, NQ = N >> 2, lgNQ = 31 - __clz(NQ);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    float *srho = gsm, *sw = gsm + N, *sV = gsm + 2 * N + A.KR;       // sw: N + KR - 1 lags
+    const int tiles_x = (N + GR_RT - 1) / GR_RT, ntiles = tiles_x * A.tiles_y;
+    const float yc = 0.5f * (float)(N - 1);
+    const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
+    float sc = G.renorm ? A.scale[0] : 1.0f;
+
+    for (int step = 0; step < A.nsteps; ++step) {
+        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 0] = clock64();
+        // ================= phase 1: rotation psi -> psi_tmp (times 1/C), partial profiles
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            const int xg = (t / A.tiles_y) * GR_RT, ty = t % A.tiles_y;
+            const int y = ty * (32 * GR_WARPS) + warp * 32 + lane;
+            float out[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) out[r] = 0.0f;
+            if (ty * (32 * GR_WARPS) + warp * 32 < N) {
+                GRot<ORDER, false> rot;
+                rot.src = A.psi; rot.N = N; rot.y = min(y, N - 1);
+                const float Yc = (float)rot.y + G.y0c;
+                rot.a = G.a; rot.d = G.d; rot.bY = G.b * Yc; rot.aY = G.a * Yc; rot.Xoff = G.x0c;
+                const int xl = min(xg + 7, N - 1);
+                const float X0 = (float)xg + rot.Xoff, XL = (float)xl + rot.Xoff;
+                const float rx0 = __fadd_rd(fmaf(rot.a, X0, rot.bY), CL_MAGIC), ry0 = __fadd_rd(fmaf(rot.d, X0, rot.aY), CL_MAGIC);
+                const float rxL = __fadd_rd(fmaf(rot.a, XL, rot.bY), CL_MAGIC), ryL = __fadd_rd(fmaf(rot.d, XL, rot.aY), CL_MAGIC);
+                const int ix = __float_as_int(rx0) - CL_IMAGIC, iy = __float_as_int(ry0) - CL_IMAGIC;
+                const int sx = xg + ix - O0, sy = rot.y + iy - O0;
+                const bool uni = (rx0 == rxL) && (ry0 == ryL) && (xg + 7 < N);
+                const bool inside = (sx >= 0) && (sx + 7 + ORDER - 1 < N) && (sy >= 0) && (sy + ORDER - 1 < N);
+                if (__all_sync(FULL, uni && inside)) {
+                    rot.group8(A.psi + (size_t)sx * N + sy, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
+                } else if (__all_sync(FULL, uni)) {
+                    rot.group8_edge(sx, sy, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) out[r] = rot.cell_checked(min(xg + r, N - 1));
+                }
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    out[r] *= sc;
+                    if (y < N && xg + r < N) A.psi_tmp[(size_t)(xg + r) * N + y] = out[r];
+                    else out[r] = 0.0f;
+                }
+            }
+            const float tot = warp_reduce8(out, lane);
+            if ((lane & 3) == 0) red[((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
+            __syncthreads();
+            if (tid < GR_RT && xg + tid < N) {
+                float s = 0.0f;
+#pragma unroll
+                for (int w = 0; w < GR_WARPS; ++w) s += red[tid][w];
+                A.rho_part[(size_t)ty * N + xg + tid] = G.dp * s;
+            }
+            __syncthreads();
+        }
+        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 1] = clock64();
+        grid.sync();
+        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 2] = clock64();
+        // ================= phase 2: profile, wake, kick + Fokker-Planck of the rows r0 .. r1-1
+        const int r0 = blockIdx.x * A.KR, r1 = min(N, r0 + A.KR);
+        float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 pw - -
+        if (r0 < N) {
+            for (int x4 = tid; x4 < NQ; x4 += GR_THREADS) {       // all loads of a pass in flight at once
+                float4 r = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+#pragma unroll 8
+                for (int k = 0; k < A.tiles_y; ++k) {
+                    const float4 v = __ldcg(reinterpret_cast<const float4 *>(A.rho_part + (size_t)k * N) + x4);
+                    r.x += v.x; r.y += v.y; r.z += v.z; r.w += v.w;
+                }
+                *reinterpret_cast<float4 *>(srho + 4 * x4) = r;
+            }
+            if (A.wfun != nullptr)
+                for (int i = tid; i < N + A.KR - 1; i += GR_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
+            __syncthreads();
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 3] = clock64();
+            // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4), one row per warp at a time
+            for (int r = warp; r < r1 - r0; r += GR_WARPS) {
+                float v0 = 0.0f, v1 = 0.0f;
+                if (A.wfun != nullptr) {
+                    const float *wx = sw + (r + N - 1);
+                    int xp = lane;
+                    for (; xp + 32 < N; xp += 64) {
+                        v0 = fmaf(wx[-xp], srho[xp], v0);
+                        v1 = fmaf(wx[-(xp + 32)], srho[xp + 32], v1);
+                    }
+                    if (xp < N) v0 = fmaf(wx[-xp], srho[xp], v0);
+                }
+                const float v = warp_sum(v0 + v1);
+                if (lane == 0) { sV[r] = v; acc[5] = fmaf(srho[r0 + r], v, acc[5]); }
+            }
+            __syncthreads();
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 4] = clock64();
+            // a4 + a5: four cells per thread in registers; four granules per pass, loads first
+            const int total = (r1 - r0) * NQ;
+            for (int idx0 = tid; idx0 < total; idx0 += 4 * GR_THREADS) {
+                float4 v0[4], v1[4], v2[4];
+                const float4 z4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int idx = idx0 + u * GR_THREADS;
+                    v0[u] = v1[u] = v2[u] = z4;
+                    if (idx < total) {
+                        const int x = r0 + (idx >> lgNQ), g = (idx & (NQ - 1)) << 2;
+                        const float4 *row = reinterpret_cast<const float4 *>(A.psi_tmp + (size_t)x * N + g);
+                        if (g >= 4) v0[u] = row[-1];
+                        v1[u] = row[0];
+                        if (g + 4 < N) v2[u] = row[1];
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int idx = idx0 + u * GR_THREADS;
+                    if (idx < total) {
+                        const int rr = idx >> lgNQ, x = r0 + rr, g = (idx & (NQ - 1)) << 2;
+                        int mm;
+                        float t;
+                        floor_frac(G.kick_c * sV[rr], mm, t);
+                        float l[ORDER];
+                        lagrange<ORDER>(t, l);
+                        float c1p[4], o[4];
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) c1p[c] = c1 * fmaf((float)(g + c), G.dp, G.p_min);
+                        if (mm >= -2 && mm <= 0) {
+                            const float b[12] = {v0[u].x, v0[u].y, v0[u].z, v0[u].w, v1[u].x, v1[u].y, v1[u].z, v1[u].w,
+                                                 v2[u].x, v2[u].y, v2[u].z, v2[u].w};
+                            if (mm == 0) kick_fp_granule<ORDER, 0>(b, l, g, N, G.fp_b, c2, c1p, o);
+                            else if (mm == -1) kick_fp_granule<ORDER, -1>(b, l, g, N, G.fp_b, c2, c1p, o);
+                            else kick_fp_granule<ORDER, -2>(b, l, g, N, G.fp_b, c2, c1p, o);
+                        } else {
+                            kick_fp_granule_any<ORDER>(A.psi_tmp + (size_t)x * N, l, mm, g, N, G.fp_b, c2, c1p, o);
+                        }
+                        *reinterpret_cast<float4 *>(A.psi + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
+                        float rs = 0.0f;
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            const float yy = (float)(g + c) - yc, tt = o[c] * yy;
+                            rs += o[c]; acc[1] += tt; acc[2] = fmaf(tt, yy, acc[2]);
+                        }
+                        const float xx = (float)x - yc, tq = rs * xx;
+                        acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+                    }
+                }
+            }
+        }
+        {
+            const float tot = warp_reduce8(acc, lane);
+            if ((lane & 3) == 0) red[((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
+        }
+        __syncthreads();
+        if (tid < GR_NPART) {
+            float s = 0.0f;
+#pragma unroll
+            for (int w = 0; w < GR_WARPS; ++w) s += red[tid][w];
+            A.mom_part[(size_t)tid * gridDim.x + blockIdx.x] = s;
+        }
+        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 5] = clock64();
+        grid.sync();
+        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 6] = clock64();
+        // ================= phase 3: a6 -- every CTA forms C and 1/C in the same fixed order
+        // Every CTA needs only the charge (one coalesced pass over gridDim.x floats, all loads in
+        // flight); warp w < 6 of CTA 0 also sums partial w for the diagnostics row.  fp32 sums in a
+        // fixed order (fp64 adds and shuffles cost ~10 us per step on B200), fp64 for the scalars.
+        __shared__ float s_tot[6];
+        if (warp == 0 || (blockIdx.x == 0 && warp < 6)) {
+            const float *mp = A.mom_part + (size_t)warp * gridDim.x;
+            float f = 0.0f;
+#pragma unroll 8
+            for (int i = lane; i < (int)gridDim.x; i += 32) f += __ldcg(mp + i);
+            f = warp_sum(f);
+            if (lane == 0) {
+                s_tot[warp] = f;
+                if (warp == 0) s_sc = G.renorm ? 1.0f / ((G.dq * G.dp) * f) : 1.0f;
+            }
+        }
+        __syncthreads();
+        if (blockIdx.x == 0 && tid == 0 && A.diag != nullptr) {
+            // (fp32, as in the cluster engine: fp64 divisions and square roots would hold CTA 0 back)
+            const float t0 = s_tot[0], i0 = 1.0f / t0;
+            const float C = (G.dq * G.dp) * t0;
+            const float mp_c = s_tot[1] * i0, vp = fmaf(-mp_c, mp_c, s_tot[2] * i0);
+            const float mq_c = s_tot[3] * i0, vq = fmaf(-mq_c, mq_c, s_tot[4] * i0);
+            const float cc = G.renorm ? C : 1.0f;
+            float *o = A.diag + (size_t)step * 6;
+            o[0] = C;
+            o[1] = fmaf(mq_c + yc, G.dq, G.q_min);
+            o[2] = fmaf(mp_c + yc, G.dp, G.p_min);
+            o[3] = sqrtf(fmaxf(vq, 0.0f)) * G.dq;
+            o[4] = sqrtf(fmaxf(vp, 0.0f)) * G.dp;
+            o[5] = s_tot[5] * G.dq / (cc * cc);
+        }
+        sc = s_sc;
+        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 7] = clock64();
+    }
+    if (blockIdx.x == 0 && tid == 0) A.scale[0] = sc;
+}
+
+}  // namespace vfps

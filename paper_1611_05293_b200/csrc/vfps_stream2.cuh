@@ -63,6 +63,13 @@ __device__ __forceinline__ float ldg_nc(const float *p)
     asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
     return v;
 }
+// the same through the coherent path, for data other CTAs wrote earlier in the same kernel
+__device__ __forceinline__ float ldg_co(const float *p)
+{
+    float v;
+    asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+    return v;
+}
 
 // ---------------------------------------------------------------- a1 + a2: rotation + projection
 // grid = (tiles_x * tiles_y, members), block = 256.  Tile = R2_RT rows x 256 columns; thread =
@@ -72,15 +79,16 @@ __device__ __forceinline__ float ldg_nc(const float *p)
 // floor(dy) do not change along the group for any lane -> sliding register window, ORDER loads per
 // cell.  Otherwise every cell loads its own window with per-tap range checks (psi = 0 outside, A8).
 // rho_part[m][x][tile_y] = dp * scale * sum over the tile's columns of psi'(x, .)
-template <int ORDER>
+template <int ORDER, bool NC = true>      // NC: psi is read-only for the whole kernel (ld.global.nc)
 struct GRot {
     static constexpr int O0 = (ORDER - 1) / 2;
+    static __device__ __forceinline__ float ld(const float *p) { return NC ? ldg_nc(p) : *p; }
     float a, d, bY, aY, Xoff;
     const float *src;      // psi of this member
     int N, y;
 
     // one cell, its own floors, range-checked taps
-    __device__ __noinline__ float cell_checked(int x) const
+    __device__ __forceinline__ float cell_checked(int x) const
     {
         const float X = (float)x + Xoff;
         int ix, iy;
@@ -98,7 +106,7 @@ struct GRot {
 #pragma unroll
             for (int j = 0; j < ORDER; ++j) {
                 const int xx = sx + i, yy = sy + j;
-                const float v = (xx >= 0 && xx < N && yy >= 0 && yy < N) ? __ldg(src + (size_t)xx * N + yy) : 0.0f;
+                const float v = (xx >= 0 && xx < N && yy >= 0 && yy < N) ? ld(src + (size_t)xx * N + yy) : 0.0f;
                 rsum = fmaf(ly[j], v, rsum);
             }
             acc = fmaf(lx[i], rsum, acc);
@@ -115,9 +123,39 @@ struct GRot {
 #pragma unroll
         for (int i = 0; i < 8 + ORDER - 1; ++i) {
 #pragma unroll
-            for (int j = 0; j < ORDER; ++j) t[i][j] = ldg_nc(p + j);      // one address per row, immediate offsets
+            for (int j = 0; j < ORDER; ++j) t[i][j] = ld(p + j);      // one address per row, immediate offsets
             p += N;
         }
+        interp8(t, X0, fx, fy, out);
+    }
+    // as group8 for a group whose taps may leave the grid (psi = 0 there, A8): rows and columns are
+    // clamped into the grid for the load, and a value whose tap lies outside is replaced by zero
+    __device__ __forceinline__ void group8_edge(int sx, int sy, float X0, float fx, float fy, float (&out)[8]) const
+    {
+        float t[8 + ORDER - 1][ORDER];
+        int cy[ORDER];
+        bool oky[ORDER];
+#pragma unroll
+        for (int j = 0; j < ORDER; ++j) {
+            oky[j] = (sy + j >= 0) && (sy + j < N);
+            cy[j] = min(max(sy + j, 0), N - 1);
+        }
+#pragma unroll
+        for (int i = 0; i < 8 + ORDER - 1; ++i) {
+            const bool okx = (sx + i >= 0) && (sx + i < N);
+            const float *p = src + (size_t)min(max(sx + i, 0), N - 1) * N;
+#pragma unroll
+            for (int j = 0; j < ORDER; ++j) {
+                const float v = ld(p + cy[j]);
+                t[i][j] = (okx && oky[j]) ? v : 0.0f;
+            }
+        }
+        interp8(t, X0, fx, fy, out);
+    }
+    // rows r = 0..7 from the taps t[r .. r+ORDER-1][.]
+    __device__ __forceinline__ void interp8(const float (&t)[8 + ORDER - 1][ORDER], float X0, float fx, float fy,
+                                            float (&out)[8]) const
+    {
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             const float X = X0 + (float)r;
@@ -172,10 +210,12 @@ k_rotate2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi
             const float rxL = __fadd_rd(fmaf(rot.a, XL, rot.bY), CL_MAGIC), ryL = __fadd_rd(fmaf(rot.d, XL, rot.aY), CL_MAGIC);
             const int ix = __float_as_int(rx0) - CL_IMAGIC, iy = __float_as_int(ry0) - CL_IMAGIC;
             const int sx = xg + ix - O0, sy = rot.y + iy - O0;
-            const bool fast = (rx0 == rxL) && (ry0 == ryL) && (xg + 7 < N) && (sx >= 0) && (sx + 7 + ORDER - 1 < N) &&
-                              (sy >= 0) && (sy + ORDER - 1 < N);
-            if (__all_sync(FULL, fast)) {
+            const bool uni = (rx0 == rxL) && (ry0 == ryL) && (xg + 7 < N);
+            const bool inside = (sx >= 0) && (sx + 7 + ORDER - 1 < N) && (sy >= 0) && (sy + ORDER - 1 < N);
+            if (__all_sync(FULL, uni && inside)) {
                 rot.group8(rot.src + (size_t)sx * N + sy, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
+            } else if (__all_sync(FULL, uni)) {
+                rot.group8_edge(sx, sy, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
             } else {
 #pragma unroll
                 for (int r = 0; r < 8; ++r) out[r] = rot.cell_checked(min(xg + r, N - 1));
@@ -388,15 +428,19 @@ k_kick_fp2(GridConst G, Kfp2Args A)
     if (!is_last) return;
     __threadfence();
     if (warp == 0) {
-        double t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0, tp = 0;
-        const volatile float *mp = A.mom_part + (size_t)m * gridDim.x * 5;
+        // (fp32 sums: fp64 adds and shuffles cost ~10 us of serial tail per step on B200)
+        float f0 = 0, f1 = 0, f2 = 0, f3 = 0, f4 = 0, fp = 0;
+        const float *mp = A.mom_part + (size_t)m * gridDim.x * 5;
+#pragma unroll 4
         for (int i = lane; i < (int)gridDim.x; i += 32) {
-            t0 += mp[5 * i]; t1 += mp[5 * i + 1]; t2 += mp[5 * i + 2]; t3 += mp[5 * i + 3]; t4 += mp[5 * i + 4];
+            f0 += __ldcg(mp + 5 * i); f1 += __ldcg(mp + 5 * i + 1); f2 += __ldcg(mp + 5 * i + 2);
+            f3 += __ldcg(mp + 5 * i + 3); f4 += __ldcg(mp + 5 * i + 4);
         }
         if (A.pw_part != nullptr)
-            for (int i = lane; i < A.npw; i += 32) tp += A.pw_part[(size_t)m * A.npw + i];
-        t0 = warp_sum(t0); t1 = warp_sum(t1); t2 = warp_sum(t2); t3 = warp_sum(t3); t4 = warp_sum(t4); tp = warp_sum(tp);
+            for (int i = lane; i < A.npw; i += 32) fp += __ldcg(A.pw_part + (size_t)m * A.npw + i);
+        f0 = warp_sum(f0); f1 = warp_sum(f1); f2 = warp_sum(f2); f3 = warp_sum(f3); f4 = warp_sum(f4); fp = warp_sum(fp);
         if (lane == 0) {
+            const double t0 = f0, t1 = f1, t2 = f2, t3 = f3, t4 = f4, tp = fp;
             const double C = (double)G.dq * (double)G.dp * t0;
             const double mp_c = t1 / t0, vp = t2 / t0 - mp_c * mp_c;
             const double mq_c = t3 / t0, vq = t4 / t0 - mq_c * mq_c;

@@ -258,13 +258,13 @@ def test_error_paths_on_gpu(vfps):
 # ---------------------------------------------------------------- engines
 def _engine_id(vfps, name):
     return {"stream": vfps.ENGINE_STREAM, "graph": vfps.ENGINE_GRAPH, "cluster": vfps.ENGINE_CLUSTER,
-            "cluster2": vfps.ENGINE_CLUSTER}[name]
+            "cluster2": vfps.ENGINE_CLUSTER, "grid": vfps.ENGINE_GRID}[name]
 
 
-@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster2"])
+@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster2", "grid"])
 def test_c1_every_engine_100_steps(vfps, orc, engine):
     """The same 100 steps of C1 through each engine (graph: two replays of 50 captured steps;
-    cluster: the scalar kernel, which AUTO picks; cluster2: the packed fp32x2 kernel)."""
+    cluster: the scalar kernel, which AUTO picks; cluster2: the packed fp32x2 kernel; grid: the persistent cooperative kernel)."""
     wl = get_workload("C1")
     sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 100, engine=_engine_id(vfps, engine), diag_every=1,
                                      cluster_kernel=2 if engine == "cluster2" else None)
@@ -305,6 +305,49 @@ def test_stream_generations(vfps, orc, gen, wake, order, N):
     assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"graph gen {gen} {wake} N={N} order={order} 60 steps")
     for i in (0, 30, 58):
         assert_diag(d[i, 0], dr[i])
+    sim.close()
+
+
+@pytest.mark.parametrize("order,N", [(4, 512), (4, 256), (3, 128), (2, 64), (4, 8)])
+def test_grid_engine(vfps, orc, order, N):
+    """Persistent cooperative-grid engine: asymmetric box, off-centre bunch, free-space wake, 300
+    steps per period (slow rotation paths at the edges and where a floor changes), 1 step and 60
+    steps with the diagnostics of every step; then hand-over to the stream engine and back."""
+    Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
+    psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
+    sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, 1, Z=Z)
+    sim.set_engine(vfps.ENGINE_GRID)
+    assert sim.engine_name == "grid" and sim.wake_name == "direct"
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, Z[0])
+    o.set_psi(psi0[0])
+    tol_q = 2e-3 if N == 8 else TOL_MOM          # N = 8: the bunch overflows the box (edge flux)
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"grid N={N} order={order} 1 step")
+    assert_diag(d[0, 0], dr[0], tol_q=tol_q)
+    d = sim.step_host(59)
+    dr = o.step(59)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"grid N={N} order={order} 60 steps")
+    for i in (0, 30, 58):
+        assert_diag(d[i, 0], dr[i], tol_q=tol_q)
+    sim.set_engine(vfps.ENGINE_STREAM)
+    sim.step_host(2)
+    sim.set_engine(vfps.ENGINE_GRID)
+    d = sim.step_host(2)
+    dr = o.step(4)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"grid -> stream -> grid N={N}")
+    assert_diag(d[1, 0], dr[3], tol_q=tol_q)
+    assert sim.step_count() == 64
+    sim.close()
+
+
+def test_grid_engine_rejects_batches(vfps):
+    wl = get_workload("C3")
+    sim = vfps.Simulation.from_workload(wl, [0, 1])
+    with pytest.raises(vfps.VfpsError) as e:
+        sim.set_engine(vfps.ENGINE_GRID)
+    assert e.value.code == -5
     sim.close()
 
 
