@@ -36,6 +36,15 @@ if ROOT not in sys.path:
 METRIC = "phase-space cell-updates/s"
 UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_STEP = 8.0     # one fp32 read + one fp32 write per cell per split step
+FMA_OPS_PER_CELL_STEP = 60.0      # FMA-pipe operations per cell per split step
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the ncu
+# --set full captures under profiles/ (psi is loaded once per launch and stays on chip / in L2, so
+# the figure does not depend on the number of steps in the launch)
+NCU_TRAFFIC = {
+    ("C1", "k_cluster_step"): (0.322e6, "profiles/r01_c1_cluster.md"),
+    ("C3", "k_cluster_step"): (77.7e6, "profiles/r01_c1_cluster.md"),
+    ("C4", "k_grid_step"): (18.6e6, "profiles/r01_c4_grid_and_stream.md"),
+}
 
 
 def parse_args():
@@ -258,8 +267,15 @@ def run_ours(args, wl, rank, local_rank, world):
     steps_per_launch = n_inner if (kname.startswith("k_cluster") or kname.startswith("k_grid")) else 1
     alg_bytes = ALG_BYTES_PER_CELL_STEP * cells * steps_per_launch
     achieved = alg_bytes / (kt / kc * 1e-3) / 1e9
+    traffic, traffic_src = NCU_TRAFFIC.get((wl.name, kname), (None, None)) if members == wl.members else (None, None)
+    sm_mhz = clocks.get("sm_max_mhz") or 1965
+    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e9                     # G FMA-pipe lane-operations per second
+    alu_ach = FMA_OPS_PER_CELL_STEP * cells * steps_per_launch / (kt / kc * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / hbm_peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                "alu": {"achieved": alu_ach, "peak": alu_peak, "unit": "G FMA-pipe op/s", "frac": alu_ach / alu_peak,
+                        "ops_per_cell_step": FMA_OPS_PER_CELL_STEP,
+                        "note": "the path sits at the ridge: 8 B and ~60 fp32 pipe operations per cell per step (DESIGN.md section 8)"},
                 "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": 1e3 * kt / kc,
                 "share_of_step": kt / tot if tot > 0 else None,
                 "kernels_ms": {k: {"ms": t, "launches": c} for k, (t, c) in ktimes.items()}}
