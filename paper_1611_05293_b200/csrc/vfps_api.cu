@@ -336,7 +336,7 @@ int launch_cluster_steps(vfps_sim *h, int n, float *diag)
     cudaError_t e;
     // debug aid: VFPS_PHASE_DUMP=<file> writes the packed kernel's per-phase clock stamps of the
     // first 64 steps of every CTA (synchronises; never set in measurements)
-    const char *dump = (h->cl_ver == 2) ? std::getenv("VFPS_PHASE_DUMP") : nullptr;
+    const char *dump = std::getenv("VFPS_PHASE_DUMP");
     const size_t ndbg = (size_t)A.S * nclusters * 64 * 8;
     if (dump && cudaMalloc((void **)&A.dbg, ndbg * sizeof(long long)) != cudaSuccess) { A.dbg = nullptr; dump = nullptr; }
     if (dump) cudaMemsetAsync(A.dbg, 0, ndbg * sizeof(long long), h->stream);
@@ -630,7 +630,7 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     h->kfp2_blocks = (N + h->kfp2_rows - 1) / h->kfp2_rows;
     h->wd_blocks = (N + WD_ROWS - 1) / WD_ROWS;
     h->fft_threads = h->Nf / 2 < 1024 ? (h->Nf / 2 < 32 ? 32 : h->Nf / 2) : 1024;
-    h->fft_smem = (size_t)h->Nf * sizeof(float2);
+    h->fft_smem = (size_t)(2 * h->Nf) * sizeof(float2);              // points + per-stage twiddle tables
 
 #define CUB(call)                                                                             \
     do {                                                                                      \

@@ -419,9 +419,12 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 mbar_wait(mbHalo, phase ^ 1u);
                 if (tid == 0 && !last) mbar_expect_tx(mbHalo, bytesHalo);
             }
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 0] = clock64();
             // ================= 1. rotation: bufA -> bufB
             if (!last) rot.run(rbeg, rend, x0);
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 1] = clock64();
             __syncthreads();
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 2] = clock64();
             if (step > 0) {
                 // ================= 6. a6 of step t-1: charge, scale, diagnostics
                 mbar_wait(mbPart, phase ^ 1u);
@@ -456,6 +459,7 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 }
             }
             if (last) break;
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 3] = clock64();
             // ================= 2. projection: rho_x = dp * sc * sum_y bufB(x, y), all-gathered
             for (int r = warp; r < R; r += CL_WARPS) {
                 const uint32_t row = sB + (uint32_t)((r * PITCH + CL_PAD) * 4);
@@ -485,7 +489,9 @@ k_cluster_step(GridConst G, ClusterArgs A)
                     st_async4(mapa(a, dd), lds4(a), mapa(mbRho, dd));
                 }
             }
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 4] = clock64();
             mbar_wait(mbRho, phase);
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 5] = clock64();
             if (tid == 0 && step + 1 < A.nsteps) mbar_expect_tx(mbRho, bytesRho);
             // ================= 3.+4. wake (own rows), kick + Fokker-Planck: bufB -> bufA
             // per-warp sums: s0 sum psi, s1/s2 p moments (per lane), q1/q2 q moments, pw = sum rho V
@@ -554,6 +560,7 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 const float X = (float)x - xc, tq = rs * X;
                 s0 += rs; q1 += tq; q2 = fmaf(tq, X, q2);
             }
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 6] = clock64();
             // ================= 5. partial sums of this CTA -> every CTA
             s1 = warp_sum(s1); s2 = warp_sum(s2);
             if (lane == 0) {
@@ -578,6 +585,7 @@ k_cluster_step(GridConst G, ClusterArgs A)
                     st_async4(mapa(slot + hh * 16, dd), lds4(slot + hh * 16), mapa(mbPart, dd));
                 }
             }
+            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 7] = clock64();
             phase ^= 1u;
         }
         // ---- store own rows and the scale (all remote stores into this CTA have been waited for)

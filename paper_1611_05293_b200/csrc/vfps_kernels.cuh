@@ -214,33 +214,42 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_pa
            const float2 *__restrict__ Z, const float2 *__restrict__ tw, float *__restrict__ rho_out,
            float *__restrict__ V, float *__restrict__ qstat)
 {
-    extern __shared__ float2 s[];
-    __shared__ double red[4][32];
+    extern __shared__ float2 s[];          // Nf points, then Nf - 1 twiddles, one contiguous table per stage
+    __shared__ float red[4][32];
+    float2 *stw = s + Nf;
     const int m = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
     const float xc = 0.5f * (float)(N - 1);
-    double s0 = 0, s1 = 0, s2 = 0, pw = 0;
+    float s0 = 0, s1 = 0, s2 = 0, pw = 0;
     for (int x = tid; x < Nf; x += nt) {
         float r = 0.0f;
         if (x < N) {
             const float *pp = rho_part + ((size_t)m * N + x) * nparts;
-            for (int k = 0; k < nparts; ++k) r += pp[k];
+#pragma unroll 8
+            for (int k = 0; k < nparts; ++k) r += __ldg(pp + k);
             rho_out[(size_t)m * N + x] = r;
-            const double c = (float)x - xc;
-            s0 += r; s1 += c * r; s2 += c * c * r;
+            const float c = (float)x - xc, t = c * r;
+            s0 += r; s1 += t; s2 = fmaf(t, c, s2);
         }
         s[x] = make_float2(r, 0.0f);
     }
     if (Z != nullptr) {
         const float2 *Zm = Z + (size_t)m * (Nf / 2 + 1);
+        // The twiddles are read 2 log2(Nf) times: stage them once, as one contiguous table per
+        // butterfly span (entry half - 1 + pos = tw[pos * (Nf/2) / half]): reading the single
+        // table with stride (Nf/2)/half put up to 32 lanes on one bank in most stages.
+        for (int j = tid; j < Nf - 1; j += nt) {
+            const int half = 1 << (31 - __clz(j + 1)), pos = j + 1 - half;
+            stw[j] = __ldg(tw + pos * ((Nf >> 1) / half));
+        }
         __syncthreads();
         for (int half = Nf >> 1; half >= 1; half >>= 1) {       // forward, DIF
-            const int tstride = (Nf >> 1) / half;
+            const float2 *wst = stw + (half - 1);
             for (int j = tid; j < (Nf >> 1); j += nt) {
                 const int pos = j & (half - 1);
                 const int i0 = ((j - pos) << 1) + pos, i1 = i0 + half;
                 const float2 u = s[i0], v = s[i1];
                 s[i0] = make_float2(u.x + v.x, u.y + v.y);
-                s[i1] = cmul(make_float2(u.x - v.x, u.y - v.y), __ldg(tw + pos * tstride));
+                s[i1] = cmul(make_float2(u.x - v.x, u.y - v.y), wst[pos]);
             }
             __syncthreads();
         }
@@ -255,16 +264,16 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_pa
                 z.y = -z.y;
             }
             const float2 R = s[i];
-            pw += (double)(z.x * fmaf(R.x, R.x, R.y * R.y));
+            pw = fmaf(z.x, fmaf(R.x, R.x, R.y * R.y), pw);
             s[i] = cmul(R, z);
         }
         __syncthreads();
         for (int half = 1; half <= (Nf >> 1); half <<= 1) {     // inverse, DIT
-            const int tstride = (Nf >> 1) / half;
+            const float2 *wst = stw + (half - 1);
             for (int j = tid; j < (Nf >> 1); j += nt) {
                 const int pos = j & (half - 1);
                 const int i0 = ((j - pos) << 1) + pos, i1 = i0 + half;
-                float2 w = __ldg(tw + pos * tstride);
+                float2 w = wst[pos];
                 w.y = -w.y;
                 const float2 u = s[i0], v = cmul(s[i1], w);
                 s[i0] = make_float2(u.x + v.x, u.y + v.y);
@@ -277,16 +286,17 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_pa
     } else {
         for (int x = tid; x < N; x += nt) V[(size_t)m * N + x] = 0.0f;
     }
+    // fp32 sums in a fixed order (fp64 adds and shuffles are ~50x slower on B200)
     s0 = warp_sum(s0); s1 = warp_sum(s1); s2 = warp_sum(s2); pw = warp_sum(pw);
     if ((tid & 31) == 0) {
         red[0][tid >> 5] = s0; red[1][tid >> 5] = s1; red[2][tid >> 5] = s2; red[3][tid >> 5] = pw;
     }
     __syncthreads();
     if (tid < 4) {
-        double t = 0;
+        float t = 0;
         for (int w = 0; w < (nt + 31) / 32; ++w) t += red[tid][w];
-        if (tid == 3) t *= (double)dq / (double)Nf;
-        qstat[(size_t)m * 4 + tid] = (float)t;
+        if (tid == 3) t *= dq / (float)Nf;
+        qstat[(size_t)m * 4 + tid] = t;
     }
 }
 
