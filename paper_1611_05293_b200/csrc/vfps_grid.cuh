@@ -65,7 +65,13 @@ k_grid_step(GridConst G, GridArgs A)
     for (int step = 0; step < A.nsteps; ++step) {
         if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 0] = clock64();
         // ================= phase 1: rotation psi -> psi_tmp (times 1/C), partial profiles
-        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        // round k: CTA c takes tile k*grid + (c + k) mod grid.  (With the plain c + k*grid a CTA keeps
+        // the same column tile in every round when grid is a multiple of tiles_y, so the CTAs that
+        // own the edge columns -- clamped-load path -- are slower in every round and everybody
+        // waits for them at the barrier.)
+        for (int k = 0, tb = 0; tb < ntiles; ++k, tb += gridDim.x) {
+            const int t = tb + (int)((blockIdx.x + k) % gridDim.x);
+            if (t >= ntiles) continue;
             const int xg = (t / A.tiles_y) * GR_RT, ty = t % A.tiles_y;
             const int y = ty * (32 * GR_WARPS) + warp * 32 + lane;
             float out[8];
