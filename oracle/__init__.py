@@ -32,7 +32,7 @@ class Params(C.Structure):
     _fields_ = [("N", C.c_int), ("q_min", C.c_double), ("q_max", C.c_double),
                 ("p_min", C.c_double), ("p_max", C.c_double), ("steps_per_period", C.c_int),
                 ("beta", C.c_double), ("interp_order", C.c_int), ("pad", C.c_int),
-                ("renormalise", C.c_int)]
+                ("renormalise", C.c_int), ("manhattan", C.c_int)]
 
 
 _dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
@@ -47,6 +47,8 @@ def lib():
         L.vfpo_set_num_threads.argtypes = [C.c_int]
         L.vfpo_lagrange_weights.argtypes = [C.c_int, C.c_double, _dp]
         L.vfpo_rotate.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
+        L.vfpo_drift.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
+        L.vfpo_rf_kick.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
         L.vfpo_project.argtypes = [C.c_int, C.c_double, _dp, _dp]
         L.vfpo_wake_function.argtypes = [C.c_int, C.c_int, _dp, _dp]
         L.vfpo_wake.argtypes = [C.c_int, _dp, _dp, _dp]
@@ -89,6 +91,22 @@ def rotate(psi, q_min, q_max, p_min, p_max, dphi, order) -> np.ndarray:
     psi = _f64(psi)
     out = np.empty_like(psi)
     lib().vfpo_rotate(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out)
+    return out
+
+
+def drift(psi, q_min, q_max, p_min, p_max, dphi, order) -> np.ndarray:
+    """First half of the Manhattan rotation (L136): psi_A(q, p) = psi(q - dphi p, p)."""
+    psi = _f64(psi)
+    out = np.empty_like(psi)
+    lib().vfpo_drift(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out)
+    return out
+
+
+def rf_kick(psi, q_min, q_max, p_min, p_max, dphi, order) -> np.ndarray:
+    """Second half of the Manhattan rotation (L136): psi_B(q, p) = psi_A(q, p + dphi q)."""
+    psi = _f64(psi)
+    out = np.empty_like(psi)
+    lib().vfpo_rf_kick(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out)
     return out
 
 
@@ -144,9 +162,9 @@ class Oracle:
     """One simulation (one batch member) advanced by the C oracle; state in double."""
 
     def __init__(self, N, q_min, q_max, p_min, p_max, steps_per_period, beta, interp_order,
-                 pad=2, Z: Optional[np.ndarray] = None, renormalise: bool = True):
+                 pad=2, Z: Optional[np.ndarray] = None, renormalise: bool = True, manhattan: bool = False):
         self.P = Params(N, q_min, q_max, p_min, p_max, steps_per_period, beta, interp_order, pad,
-                        1 if renormalise else 0)
+                        1 if renormalise else 0, 1 if manhattan else 0)
         self.N = N
         self.Z = None if Z is None else _z_pairs(np.asarray(Z).reshape(-1)).copy()
         if self.Z is not None and self.Z.size != 2 * (pad * N // 2 + 1):
@@ -155,10 +173,10 @@ class Oracle:
         self.steps = 0
 
     @classmethod
-    def from_workload(cls, wl, member: int = 0, renormalise: bool = True) -> "Oracle":
+    def from_workload(cls, wl, member: int = 0, renormalise: bool = True, manhattan: bool = False) -> "Oracle":
         Z = wl.impedance([member])
         o = cls(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
-                wl.interp_order, wl.pad, None if Z is None else Z[0], renormalise)
+                wl.interp_order, wl.pad, None if Z is None else Z[0], renormalise, manhattan)
         o.set_psi(wl.psi0([member])[0])
         return o
 

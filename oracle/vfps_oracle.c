@@ -114,6 +114,48 @@ void vfpo_rotate(int N, double q_min, double q_max, double p_min, double p_max, 
     }
 }
 
+/* 1-D interpolation along q of column y at real grid coordinate x_r (Eq. 10). */
+static double interp_q(const double *psi, int N, int order, double x_r, int y)
+{
+    double l[VFPO_MAX_ORDER];
+    double m = floor(x_r);
+    vfpo_lagrange_weights(order, x_r - m, l);
+    double acc = 0.0;
+    for (int i = 0; i < order; ++i)
+        acc += l[i] * at(psi, N, (int)m + node_offset(order, i), y);
+    return acc;
+}
+
+/* ---- O1' "Manhattan rotation" (the symplectic map "splits the rotation into a
+ * energy-dependent drift followed by a location dependent RF kick.  Each requires a
+ * one-dimensional interpolation").  With the flow of Eq. 1 (dq/dtheta = +p, dp/dtheta = -q) and
+ * the first-order symplectic (Euler) map of the paper's ref. [23] (reading A15):
+ *   drift    q' = q + dphi p      psi_A(q, p) = psi(q - dphi p, p)       interpolation along q
+ *   RF kick  p' = p - dphi q'     psi_B(q, p) = psi_A(q, p + dphi q)     interpolation along p */
+void vfpo_drift(int N, double q_min, double q_max, double p_min, double p_max, double dphi, int order,
+                const double *psi, double *out)
+{
+    const double dq = (q_max - q_min) / (N - 1), dp = (p_max - p_min) / (N - 1);
+#pragma omp parallel for schedule(static)
+    for (int x = 0; x < N; ++x)
+        for (int y = 0; y < N; ++y) {
+            double p = p_min + y * dp;
+            out[(size_t)N * x + y] = interp_q(psi, N, order, (double)x - dphi * p / dq, y);
+        }
+}
+
+void vfpo_rf_kick(int N, double q_min, double q_max, double p_min, double p_max, double dphi, int order,
+                  const double *psi, double *out)
+{
+    const double dq = (q_max - q_min) / (N - 1), dp = (p_max - p_min) / (N - 1);
+#pragma omp parallel for schedule(static)
+    for (int x = 0; x < N; ++x) {
+        double q = q_min + x * dq;
+        for (int y = 0; y < N; ++y)
+            out[(size_t)N * x + y] = interp_p(psi, N, order, x, (double)y + dphi * q / dp);
+    }
+}
+
 /* ---- O2 projection: bunch profile rho_x = dp * sum_y psi(x,y). */
 void vfpo_project(int N, double dp, const double *psi, double *rho)
 {
@@ -248,6 +290,7 @@ typedef struct {
     int interp_order;  /* 2, 3, 4 */
     int pad;           /* N_f = pad * N */
     int renormalise;   /* 1: psi_{t+1} = psi''' / C */
+    int manhattan;     /* 1: a1 is the Manhattan rotation (drift, RF kick) instead of the standard one */
 } vfpo_params;
 
 /* psi: in/out [N][N] double.  Z: (N_f/2+1) (re,im) pairs or NULL (no wake).  w: wake function
@@ -267,7 +310,12 @@ void vfpo_step(const vfpo_params *P, const double *Z, const double *w, double *p
     double *rho = (double *)malloc(N * sizeof(double));
     double *V = (double *)calloc(N, sizeof(double));
 
-    vfpo_rotate(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, psi, t1); /* a1 */
+    if (P->manhattan) {                                                                      /* a1 */
+        vfpo_drift(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, psi, t2);
+        vfpo_rf_kick(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, t2, t1);
+    } else {
+        vfpo_rotate(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, psi, t1);
+    }
     vfpo_project(N, dp, t1, rho);                                                            /* a2 */
     if (Z) vfpo_wake(N, w, rho, V);                                                          /* a3 */
     vfpo_kick(N, dp, dphi, P->interp_order, V, t1, t2);                                      /* a4 */

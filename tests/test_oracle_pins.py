@@ -336,3 +336,70 @@ def test_p13_converged_bunch_length_close_to_one(orc):
     o.set_psi(gauss(N, L, 1.3, 1.3))
     d = o.step(40 * spp, diag_every=spp)
     assert abs(d[-1, 3] - 1.0) < 1e-3 and abs(d[-1, 4] - 1.0) < 1e-3
+
+
+# ---------------------------------------------------------------- P14 Manhattan rotation (L136)
+def _cov(psi, L):
+    """<q>, <p> and the covariance matrix of psi on the box [-L, L]^2, formed here in numpy."""
+    N = psi.shape[0]
+    q = np.linspace(-L, L, N)
+    w = psi / psi.sum()
+    mq, mp = (w.sum(1) * q).sum(), (w.sum(0) * q).sum()
+    dq, dp = q - mq, q - mp
+    return np.array([mq, mp]), np.array([[(w.sum(1) * dq * dq).sum(), (w * np.outer(dq, dp)).sum()],
+                                         [(w * np.outer(dq, dp)).sum(), (w.sum(0) * dp * dp).sum()]])
+
+
+def test_p14_manhattan_moments_follow_the_symplectic_map(orc):
+    """Drift q' = q + dphi p, RF kick p' = p - dphi q' (Eq. 1 signs, L25; symplectic split, L136).
+    A 1-D Lagrange shift of order >= 3 moves the mean of every line by exactly the shift and keeps
+    its variance, so means and covariances of psi follow the linear map M = [[1, dphi],
+    [-dphi, 1 - dphi^2]] exactly: m_n = M^n m_0, S_n = M^n S_0 (M^n)^T; det M = 1 (area
+    preserved: the emittance det S is invariant)."""
+    N, L, spp, n = 128, 6.0, 400, 100
+    dphi = TWO_PI / spp
+    psi = gauss(N, L, 0.8, 0.6, 0.5, -0.3)          # 7 sigma inside the box: no edge loss
+    m0, S0 = _cov(psi, L)
+    M = np.array([[1.0, dphi], [-dphi, 1.0 - dphi * dphi]])
+    assert abs(np.linalg.det(M) - 1.0) < 1e-15
+    o = orc.Oracle(N, -L, L, -L, L, spp, 0.0, 4, 2, None, renormalise=False, manhattan=True)
+    o.set_psi(psi)
+    o.step(n, diag=False)
+    Mn = np.linalg.matrix_power(M, n)
+    m, S = _cov(o.psi, L)
+    np.testing.assert_allclose(m, Mn @ m0, atol=2e-9)
+    np.testing.assert_allclose(S, Mn @ S0 @ Mn.T, atol=2e-8)
+    assert abs(np.linalg.det(S) - np.linalg.det(S0)) < 1e-7
+    # and it IS a rotation to O(dphi): a quarter period takes (q, p) to (p, -q)
+    assert abs(m[0] - m0[1]) < 0.01 and abs(m[1] + m0[0]) < 0.01
+
+
+@pytest.mark.parametrize("order", [2, 3, 4])
+def test_p14_manhattan_substeps_conserve_charge_and_shift_lines(orc, order):
+    """Each half is a family of 1-D shifts: charge is conserved to rounding (interior support) and
+    the line at p_y (resp. q_x) moves by exactly dphi p_y (resp. -dphi q_x)."""
+    N, L = 64, 6.0
+    dphi = TWO_PI / 150
+    q = np.linspace(-L, L, N)
+    psi = gauss(N, L, 0.6, 0.7, 0.4, 0.2)           # > 8 sigma inside the box: no edge loss
+    a = orc.drift(psi, -L, L, -L, L, dphi, order)
+    b = orc.rf_kick(a, -L, L, -L, L, dphi, order)
+    assert abs(a.sum() / psi.sum() - 1.0) < 1e-12 and abs(b.sum() / psi.sum() - 1.0) < 1e-12
+    y = 40                                                        # the line p = q[y]
+    mean_q = lambda f: (f[:, y] * q).sum() / f[:, y].sum()
+    assert abs(mean_q(a) - mean_q(psi) - dphi * q[y]) < 1e-10
+    x = 22                                                        # the line q = q[x]
+    mean_p = lambda f: (f[x, :] * q).sum() / f[x, :].sum()
+    assert abs(mean_p(b) - mean_p(a) + dphi * q[x]) < 1e-10
+
+
+def test_p14_manhattan_keeps_the_gaussian(orc):
+    """L196 / Fig. 5: with Manhattan rotation a sigma = 1 Gaussian stays put (sigma_p within 1 %
+    over a period, Table II), here 256^2 at 1000 steps per period without damping."""
+    N, L, spp = 256, 6.0, 1000
+    o = orc.Oracle(N, -L, L, -L, L, spp, 0.0, 4, 2, None, renormalise=False, manhattan=True)
+    o.set_psi(gauss(N, L))
+    d = o.step(spp, diag_every=100)
+    rows = d[~np.isnan(d[:, 0])]
+    assert np.all(np.abs(rows[:, 3] - 1.0) < 0.01) and np.all(np.abs(rows[:, 4] - 1.0) < 0.01)
+    assert abs(rows[-1, 0] - 1.0) < 1e-7          # only the 6-sigma tails leave through the box edge
