@@ -131,7 +131,6 @@ int validate(const vfps_params *p, std::string &why)
     if (p->members < 1) { why = "members must be >= 1"; return VFPS_ERR_ARG; }
     if (p->flags & ~(VFPS_FLAG_RENORMALISE | VFPS_FLAG_CLAMP | VFPS_FLAG_ROT_MANHATTAN)) { why = "unknown flag"; return VFPS_ERR_ARG; }
     if (p->flags & VFPS_FLAG_CLAMP) { why = "clamped interpolation (Eq. 14) is not implemented"; return VFPS_ERR_UNSUPPORTED; }
-    if (p->flags & VFPS_FLAG_ROT_MANHATTAN) { why = "Manhattan rotation is not implemented"; return VFPS_ERR_UNSUPPORTED; }
     if (p->N % 4 != 0) { why = "N must be a multiple of 4 (float4 rows)"; return VFPS_ERR_UNSUPPORTED; }
     if ((long long)p->N * p->pad > 8192) { why = "N*pad > 8192: wake FFT does not fit one CTA's shared memory"; return VFPS_ERR_UNSUPPORTED; }
     return VFPS_OK;
@@ -153,6 +152,8 @@ void grid_constants(vfps_sim *h)
     G.x0c = (float)x0c; G.y0c = (float)y0c;
     G.dq = (float)dq; G.dp = (float)dp;
     G.kick_c = (float)(dphi / dp);
+    G.mh_q = (float)(-dphi * dp / dq);
+    G.mh_p = (float)(dphi * dq / dp);
     G.fp_b = (float)(P.beta / P.steps_per_period);
     G.p_min = (float)P.p_min; G.q_min = (float)P.q_min;
     G.renorm = (P.flags & VFPS_FLAG_RENORMALISE) ? 1 : 0;
@@ -290,6 +291,7 @@ cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, boo
 void cluster_configure(vfps_sim *h)
 {
     h->cl_S = 0; h->cl_max_clusters = 0; h->cl_ver = 0; h->cl_why.clear();
+    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) { h->cl_why = "the cluster engine implements the standard rotation only"; return; }
     const int N = h->N, H = h->G.H;
     if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
     if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
@@ -403,6 +405,7 @@ cudaError_t grid_occupancy(int *per_sm, size_t smem)
 void grid_configure(vfps_sim *h)
 {
     h->gr_blocks = 0; h->gr_why.clear();
+    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) { h->gr_why = "the grid engine implements the standard rotation only"; return; }
     if (h->members != 1) { h->gr_why = "grid engine advances one simulation per handle"; return; }
     int dev = 0, coop = 0, sms = 0;
     cudaGetDevice(&dev);
@@ -472,7 +475,11 @@ int launch_grid_steps(vfps_sim *h, int n, float *diag)
 }
 
 // which kernels the STREAM / GRAPH engines launch, and how they evaluate the wake
-int resolved_gen(const vfps_sim *h) { return h->gen_opt ? h->gen_opt : 2; }
+int resolved_gen(const vfps_sim *h)
+{
+    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) return 2;      // only the second generation has it
+    return h->gen_opt ? h->gen_opt : 2;
+}
 bool wake_is_direct(const vfps_sim *h)
 {
     if (resolved_gen(h) == 1) return false;
@@ -484,10 +491,15 @@ int launch_step_stream2(vfps_sim *h, bool timed)
 {
     const int N = h->N;
     const bool direct = wake_is_direct(h);
+    const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0;
     {
         Bracket br(h, VFPS_KERNEL_ROTATE2, timed);
-        k_rotate2<ORDER><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
-            h->G, h->psi, h->psi_tmp, h->scale, h->rho_part, h->tiles_y2, h->rho, h->tilectr);
+        if (manh)
+            k_drift2<ORDER><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
+                h->G, h->psi, h->psi_tmp, h->scale, h->rho_part, h->tiles_y2, h->rho, h->tilectr);
+        else
+            k_rotate2<ORDER><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
+                h->G, h->psi, h->psi_tmp, h->scale, h->rho_part, h->tiles_y2, h->rho, h->tilectr);
     }
     if (!direct) {
         Bracket br(h, VFPS_KERNEL_WAKE, timed);
@@ -508,7 +520,8 @@ int launch_step_stream2(vfps_sim *h, bool timed)
     A.diag = h->diag_cell; A.members = h->members; A.rows_per_cta = h->kfp2_rows;
     {
         Bracket br(h, VFPS_KERNEL_KICK_FP2, timed);
-        k_kick_fp2<ORDER><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
+        if (manh) k_kick_fp2<ORDER, true><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
+        else k_kick_fp2<ORDER, false><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
     }
     h->launches += 2;
     return VFPS_OK;
@@ -823,6 +836,8 @@ int vfps_set_option(vfps_handle h, int option, int value)
     }
     if (option == VFPS_OPT_STREAM_GEN) {
         if (value < 0 || value > 2) return fail(h, VFPS_ERR_ARG, "stream generation must be 0 (auto), 1 or 2");
+        if (value == 1 && (h->P.flags & VFPS_FLAG_ROT_MANHATTAN))
+            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels implement the standard rotation only");
         if (value == 1 && h->wake_opt == VFPS_WAKE_DIRECT)
             return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels have no direct-convolution wake");
         if (value != h->gen_opt) drop_graph(h);

@@ -35,6 +35,8 @@ struct GridConst {
     float p_min;
     float q_min;
     int H;             // rotation halo
+    float mh_q;        // Manhattan drift:   shift along q in cells = mh_q * Y,  mh_q = -dphi * dp/dq
+    float mh_p;        // Manhattan RF kick: shift along p in cells = mh_p * X,  mh_p = +dphi * dq/dp
     int renorm;
 };
 

@@ -267,6 +267,92 @@ k_rotate2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi
     }
 }
 
+// ---------------------------------------------------------------- a1' Manhattan rotation, first half
+// Drift psi_A(q, p) = psi(q - dphi p, p) (reading A15): column y is shifted along q
+// by s_y = mh_q * Y cells (Y = y + y0c), one 1-D Lagrange interpolation with per-column weights.
+// Same tiling, stores, row sums and last-CTA profile as k_rotate2; thread = column, 8 rows per
+// group from a window of 8 + ORDER - 1 loads (rows outside the grid read as zero, A8).  The
+// second half (RF kick, a shift along p by mh_p * X cells) does not change the profile and is
+// applied by k_kick_fp2<ORDER, true> together with the wake kick.
+template <int ORDER>
+__global__ void __launch_bounds__(R2_THREADS)
+k_drift2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_out,
+         const float *__restrict__ scale, float *__restrict__ rho_part, int tiles_y,
+         float *__restrict__ rho, unsigned *__restrict__ tilectr)
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+    __shared__ float red[R2_RT][R2_WARPS];
+    const int N = G.N, m = blockIdx.y;
+    const int tx0 = (blockIdx.x / tiles_y) * R2_RT, ty = blockIdx.x % tiles_y;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int y = ty * (32 * R2_WARPS) + warp * 32 + lane, yl = min(y, N - 1);
+    const float sc = G.renorm ? __ldg(scale + m) : 1.0f;
+    const float *src = psi_in + (size_t)m * N * N + yl;
+    float *dst = psi_out + (size_t)m * N * N;
+    int mm;
+    float t;
+    floor_frac(G.mh_q * ((float)yl + G.y0c), mm, t);
+    float l[ORDER];
+    lagrange<ORDER>(t, l);
+#pragma unroll
+    for (int i = 0; i < ORDER; ++i) l[i] *= sc;
+    if (warp * 32 + ty * (32 * R2_WARPS) < N) {
+#pragma unroll 1
+        for (int grp = 0; grp < R2_RT / 8; ++grp) {
+            const int xg = tx0 + 8 * grp, sx = xg + mm - O0;       // first source row of the group
+            float w[8 + ORDER - 1], out[8];
+#pragma unroll
+            for (int i = 0; i < 8 + ORDER - 1; ++i) {
+                const int xx = sx + i;
+                w[i] = (xx >= 0 && xx < N) ? __ldg(src + (size_t)xx * N) : 0.0f;
+            }
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                float acc = l[0] * w[r];
+#pragma unroll
+                for (int i = 1; i < ORDER; ++i) acc = fmaf(l[i], w[r + i], acc);
+                const bool ok = (y < N) && (xg + r < N);
+                if (ok) dst[(size_t)(xg + r) * N + y] = acc;
+                out[r] = ok ? acc : 0.0f;
+            }
+            const float tot = warp_reduce8(out, lane);
+            if ((lane & 3) == 0) red[8 * grp + ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
+        }
+    } else {
+        if (lane < R2_RT) red[lane][warp] = 0.0f;
+    }
+    __syncthreads();
+    if (threadIdx.x < R2_RT) {
+        const int x = tx0 + threadIdx.x;
+        if (x < N) {
+            float s = 0.0f;
+#pragma unroll
+            for (int w = 0; w < R2_WARPS; ++w) s += red[threadIdx.x][w];
+            rho_part[((size_t)m * N + x) * tiles_y + ty] = G.dp * s;
+            __threadfence();
+        }
+    }
+    __shared__ bool is_last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned *ctr = tilectr + (size_t)m * gridDim.x / tiles_y + blockIdx.x / tiles_y;
+        const unsigned done = atomicAdd(ctr, 1u);
+        is_last = (done == (unsigned)tiles_y - 1);
+        if (is_last) *ctr = 0u;
+    }
+    __syncthreads();
+    if (is_last && threadIdx.x < R2_RT) {
+        __threadfence();
+        const int x = tx0 + threadIdx.x;
+        if (x < N) {
+            const volatile float *pp = rho_part + ((size_t)m * N + x) * tiles_y;
+            float s = 0.0f;
+            for (int k = 0; k < tiles_y; ++k) s += pp[k];
+            rho[(size_t)m * N + x] = s;
+        }
+    }
+}
+
 // ---------------------------------------------------------------- a3: direct wake
 // grid = (ceil(N / WD_ROWS), members), block = 256 (one row per warp), dynamic shared memory
 // (2N + WD_ROWS) floats: the profile (complete after k_rotate2) and the N + WD_ROWS - 1 lags of the
@@ -315,6 +401,62 @@ k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wf
     }
 }
 
+// Manhattan rotation, second half (RF kick): psi_B(x, y) = psi_A(x, y + s1),
+// s1 = mh_p * X cells, for the 12 columns g-4 .. g+7 that the wake kick of the granule g..g+3
+// reads.  a[i] = psi_A(x, g - 8 + i), i = 0..19; MM1 = floor(s1) (compile time), l1 = weights of
+// its fraction; columns outside the grid are zero before and after (A8).
+template <int ORDER, int MM1>
+__device__ __forceinline__ void rf_stage(const float (&a)[20], const float (&l1)[ORDER], int g, int N, float (&r)[12])
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+#pragma unroll
+    for (int i = 0; i < 12; ++i) {
+        const int i0 = i + 4 + MM1 - O0;
+        float acc = l1[0] * a[i0];
+#pragma unroll
+        for (int j = 1; j < ORDER; ++j) acc = fmaf(l1[j], a[i0 + j], acc);
+        const int y = g - 4 + i;
+        r[i] = (y >= 0 && y < N) ? acc : 0.0f;
+    }
+}
+// any integer parts: psi_B at column s of the row (bounds-checked loads), and the whole granule
+template <int ORDER>
+__device__ __forceinline__ float rf_value(const float *row, int N, int s, int mm1, const float (&l1)[ORDER])
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+    if (s < 0 || s >= N) return 0.0f;
+    float acc = 0.0f;
+#pragma unroll
+    for (int j = 0; j < ORDER; ++j) {
+        const int c = s + mm1 - O0 + j;
+        acc = fmaf(l1[j], (c >= 0 && c < N) ? row[c] : 0.0f, acc);
+    }
+    return acc;
+}
+template <int ORDER>
+__device__ __noinline__ void rf_kick_fp_granule_any(const float *row, const float (&l1)[ORDER], int mm1,
+                                                    const float (&l2)[ORDER], int mm2, int g, int N, float fp_b,
+                                                    float c2, const float (&c1p)[4], float (&out)[4])
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+    float k[7];
+#pragma unroll 1
+    for (int i = 0; i < 7; ++i) {
+        const int y = g - 1 + i;
+        float acc = 0.0f;
+        for (int j = 0; j < ORDER; ++j) acc = fmaf(l2[j], rf_value<ORDER>(row, N, y + mm2 - O0 + j, mm1, l1), acc);
+        k[i] = (y >= 0 && y < N) ? acc : 0.0f;
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const float fm1 = k[c], f0 = k[c + 1], fp1 = k[c + 2], fp2 = k[c + 3];
+        const float d1 = fmaf(-2.0f, fm1, fmaf(-3.0f, f0, fmaf(6.0f, fp1, -fp2)));
+        const float d2 = (fm1 + fp1) - 2.0f * f0;
+        const float incr = fmaf(fp_b, f0, fmaf(c1p[c], d1, c2 * d2));
+        out[c] = f0 + incr;
+    }
+}
+
 // ---------------------------------------------------------------- a4 + a5 + a6: kick, FP, moments
 struct Kfp2Args {
     const float *psi_in;    // rotated, scaled density (after a1)
@@ -336,7 +478,7 @@ struct Kfp2Args {
 // one row: three 128-bit loads give the rotated density at g-4 .. g+7, kick and Fokker-Planck run
 // in registers (kick_fp_granule of vfps_cluster.cuh), one 128-bit store.  The last CTA of each
 // member finalises the diagnostics row and the renormalisation scalar (fixed summation order).
-template <int ORDER>
+template <int ORDER, bool MANH = false>
 __global__ void __launch_bounds__(K2_THREADS)
 k_kick_fp2(GridConst G, Kfp2Args A)
 {
@@ -352,6 +494,54 @@ k_kick_fp2(GridConst G, Kfp2Args A)
     const int nrows = min(N, x_begin + A.rows_per_cta) - x_begin;
     float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 - - -
 
+    if constexpr (MANH) {
+        // Manhattan rotation: RF kick (shift s1 = mh_p X) then wake kick (shift kick_c V_x), two
+        // successive 1-D interpolations along p in registers, then Fokker-Planck
+        const int total = nrows * NQ;
+        for (int idx = tid; idx < total; idx += K2_THREADS) {
+            const int x = x_begin + (idx >> lgNQ), g = (idx & (NQ - 1)) << 2;
+            const float *row = src + (size_t)x * N;
+            const float4 z4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            float4 v[5];
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                const int c = g - 8 + 4 * q;
+                v[q] = (c >= 0 && c < N) ? __ldg(reinterpret_cast<const float4 *>(row + c)) : z4;
+            }
+            int mm1, mm2;
+            float t1, t2;
+            floor_frac(G.mh_p * ((float)x + G.x0c), mm1, t1);
+            floor_frac(G.kick_c * __ldg(A.V + (size_t)m * N + x), mm2, t2);
+            float l1[ORDER], l2[ORDER], c1p[4], o[4];
+            lagrange<ORDER>(t1, l1);
+            lagrange<ORDER>(t2, l2);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) c1p[c] = c1 * fmaf((float)(g + c), G.dp, G.p_min);
+            if (mm1 >= -2 && mm1 <= 1 && mm2 >= -2 && mm2 <= 0) {
+                float a[20], r[12];
+#pragma unroll
+                for (int q = 0; q < 5; ++q) { a[4 * q] = v[q].x; a[4 * q + 1] = v[q].y; a[4 * q + 2] = v[q].z; a[4 * q + 3] = v[q].w; }
+                if (mm1 == 0) rf_stage<ORDER, 0>(a, l1, g, N, r);
+                else if (mm1 == -1) rf_stage<ORDER, -1>(a, l1, g, N, r);
+                else if (mm1 == 1) rf_stage<ORDER, 1>(a, l1, g, N, r);
+                else rf_stage<ORDER, -2>(a, l1, g, N, r);
+                if (mm2 == 0) kick_fp_granule<ORDER, 0>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                else if (mm2 == -1) kick_fp_granule<ORDER, -1>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                else kick_fp_granule<ORDER, -2>(r, l2, g, N, G.fp_b, c2, c1p, o);
+            } else {
+                rf_kick_fp_granule_any<ORDER>(row, l1, mm1, l2, mm2, g, N, G.fp_b, c2, c1p, o);
+            }
+            *reinterpret_cast<float4 *>(dst + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
+            float rs = 0.0f;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float yy = (float)(g + c) - yc, tt = o[c] * yy;
+                rs += o[c]; acc[1] += tt; acc[2] = fmaf(tt, yy, acc[2]);
+            }
+            const float xx = (float)x - yc, tq = rs * xx;
+            acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+        }
+    } else {
     // four granules per thread and pass: every load of the pass is issued before the first use
     const int total = nrows * NQ;
     for (int idx0 = tid; idx0 < total; idx0 += 4 * K2_THREADS) {
@@ -405,6 +595,7 @@ k_kick_fp2(GridConst G, Kfp2Args A)
                 acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
             }
         }
+    }
     }
     {
         const float tot = warp_reduce8(acc, lane);

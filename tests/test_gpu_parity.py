@@ -367,6 +367,70 @@ def test_stream_generations(vfps, orc, gen, wake, order, N):
     sim.close()
 
 
+@pytest.mark.parametrize("wake", ["direct", "fft"])
+@pytest.mark.parametrize("order,N", [(4, 256), (3, 128), (2, 64), (4, 32)])
+def test_manhattan_rotation(vfps, orc, order, N, wake):
+    """VFPS_FLAG_ROT_MANHATTAN (drift along q, RF kick along p) against the oracle's
+    Manhattan step: asymmetric box, off-centre bunch, free-space wake, 300 steps per period (the
+    drift and the RF kick move the outer lines by more than one cell: integer parts -2..1), stream
+    engine for 1 step, graph engine for 59 more; the on-chip engines refuse the flag."""
+    Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
+    psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
+    flags = vfps.FLAG_RENORMALISE | vfps.FLAG_ROT_MANHATTAN
+    sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, 1, Z=Z, flags=flags)
+    for eng in (vfps.ENGINE_CLUSTER, vfps.ENGINE_GRID):
+        with pytest.raises(vfps.VfpsError) as e:
+            sim.set_engine(eng)
+        assert e.value.code == -5
+    sim.set_wake_mode({"fft": vfps.WAKE_FFT, "direct": vfps.WAKE_DIRECT}[wake])
+    sim.set_engine(vfps.ENGINE_STREAM)
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, Z[0], manhattan=True)
+    o.set_psi(psi0[0])
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"manhattan N={N} order={order} 1 step")
+    assert_diag(d[0, 0], dr[0])
+    sim.set_engine(vfps.ENGINE_AUTO)
+    assert sim.engine_name == "graph"
+    d = sim.step_host(59)
+    dr = o.step(59)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"manhattan N={N} order={order} 60 steps")
+    for i in (0, 30, 58):
+        assert_diag(d[i, 0], dr[i])
+    sim.close()
+
+
+def test_manhattan_c1_and_large_kick(vfps, orc):
+    """C1 physics with the Manhattan rotation (100 steps), and a resistive impedance strong enough
+    for wake shifts of several cells (generic two-stage path)."""
+    wl = get_workload("C1")
+    flags = vfps.FLAG_RENORMALISE | vfps.FLAG_ROT_MANHATTAN
+    sim = vfps.Simulation(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
+                          wl.interp_order, wl.pad, 1, Z=wl.impedance([0]), flags=flags)
+    sim.set_psi_host(wl.psi0([0]))
+    o = orc.Oracle.from_workload(wl, 0, manhattan=True)
+    d = sim.step_host(100)
+    dr = o.step(100)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, "manhattan C1 100 steps")
+    for i in (0, 49, 99):
+        assert_diag(d[i, 0], dr[i])
+    sim.close()
+    N = 64
+    Z = np.full((1, N + 1), 60.0 + 0j, dtype=np.complex64)
+    psi0 = make_psi0(N, -6, 6, -6, 6, 1.0, 1.0, 0, 0)[None]
+    sim = vfps.Simulation(N, -6, 6, -6, 6, 100, 1e-3, 4, 2, 1, Z=Z, flags=flags)
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, -6, 6, -6, 6, 100, 1e-3, 4, 2, Z[0], manhattan=True)
+    o.set_psi(psi0[0])
+    d = sim.step_host(3)
+    dr = o.step(3)
+    # three steps of three successive fp32 interpolations with shifts of up to 8 cells on a 64^2 grid
+    assert_psi(sim.get_psi_host()[0], o.psi, 6e-5, "manhattan large kick")
+    assert_diag(d[2, 0], dr[2], tol_p=0.1)
+    sim.close()
+
+
 @pytest.mark.parametrize("order,N", [(4, 512), (4, 256), (3, 128), (2, 64), (4, 8)])
 def test_grid_engine(vfps, orc, order, N):
     """Persistent cooperative-grid engine: asymmetric box, off-centre bunch, free-space wake, 300
