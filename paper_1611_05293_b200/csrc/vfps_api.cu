@@ -395,9 +395,18 @@ int launch_step_stream(vfps_sim *h, bool timed)
 }
 
 template <int ORDER>
-cudaError_t grid_occupancy(int *per_sm, size_t smem)
+const void *grid_kernel(bool manh)
 {
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, k_grid_step<ORDER>, GR_THREADS, smem);
+    return manh ? (const void *)k_grid_step<ORDER, true> : (const void *)k_grid_step<ORDER, false>;
+}
+const void *grid_kernel(const vfps_sim *h)
+{
+    const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0;
+    switch (h->P.interp_order) {
+        case 2: return grid_kernel<2>(manh);
+        case 3: return grid_kernel<3>(manh);
+        default: return grid_kernel<4>(manh);
+    }
 }
 
 // The cooperative-grid engine needs every CTA resident at once: grid = SMs x (CTAs per SM, at most
@@ -405,7 +414,6 @@ cudaError_t grid_occupancy(int *per_sm, size_t smem)
 void grid_configure(vfps_sim *h)
 {
     h->gr_blocks = 0; h->gr_why.clear();
-    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) { h->gr_why = "the grid engine implements the standard rotation only"; return; }
     if (h->members != 1) { h->gr_why = "grid engine advances one simulation per handle"; return; }
     int dev = 0, coop = 0, sms = 0;
     cudaGetDevice(&dev);
@@ -418,12 +426,7 @@ void grid_configure(vfps_sim *h)
         const int KR = (N + blocks - 1) / blocks;
         const size_t smem = grid_smem_floats(N, KR) * sizeof(float);
         int per_sm = 0;
-        cudaError_t e;
-        switch (h->P.interp_order) {
-            case 2: e = grid_occupancy<2>(&per_sm, smem); break;
-            case 3: e = grid_occupancy<3>(&per_sm, smem); break;
-            default: e = grid_occupancy<4>(&per_sm, smem); break;
-        }
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, grid_kernel(h), GR_THREADS, smem);
         if (e != cudaSuccess || per_sm < 1) { cudaGetLastError(); h->gr_why = "grid kernel does not fit an SM"; return; }
         const int fit = sms * (per_sm < 2 ? per_sm : 2);
         if (fit >= blocks) { h->gr_blocks = blocks; h->gr_KR = KR; h->gr_smem = smem; return; }
@@ -439,12 +442,7 @@ int launch_grid_steps(vfps_sim *h, int n, float *diag)
     A.rho_part = h->rho_part; A.mom_part = h->gr_mom; A.diag = diag; A.nsteps = n;
     A.tiles_y = h->tiles_y2; A.KR = h->gr_KR;
     void *args[2] = {(void *)&h->G, (void *)&A};
-    const void *kern;
-    switch (h->P.interp_order) {
-        case 2: kern = (const void *)k_grid_step<2>; break;
-        case 3: kern = (const void *)k_grid_step<3>; break;
-        default: kern = (const void *)k_grid_step<4>; break;
-    }
+    const void *kern = grid_kernel(h);
     cudaError_t e;
     // debug aid as in launch_cluster_steps: VFPS_PHASE_DUMP=<file>
     const char *dump = std::getenv("VFPS_PHASE_DUMP");

@@ -14,6 +14,8 @@
 //   -- grid barrier --
 //   phase 3  every CTA adds the partial sums of all CTAs in the same fixed order -> C, 1/C;
 //            CTA 0 writes the diagnostics row.
+// With VFPS_FLAG_ROT_MANHATTAN (template MANH) phase 1 is the drift (1-D shift along q) and phase 2
+// applies the RF kick before the wake kick (vfps_stream2.cuh: k_drift2, rf_stage).
 // One simulation per handle (members == 1); batches of on-chip grids use the cluster engine.
 #pragma once
 #include "vfps_stream2.cuh"
@@ -43,7 +45,7 @@ struct GridArgs {
 
 __host__ __device__ inline size_t grid_smem_floats(int N, int KR) { return (size_t)2 * N + 2 * KR + 8; }
 
-template <int ORDER>
+template <int ORDER, bool MANH = false>
 __global__ void __launch_bounds__(GR_THREADS, 2)
 k_grid_step(GridConst G, GridArgs A)
 {
@@ -78,6 +80,29 @@ k_grid_step(GridConst G, GridArgs A)
 #pragma unroll
             for (int r = 0; r < 8; ++r) out[r] = 0.0f;
             if (ty * (32 * GR_WARPS) + warp * 32 < N) {
+                if constexpr (MANH) {
+                    // Manhattan drift (L136): column y shifted along q by mh_q * Y cells
+                    const int yl = min(y, N - 1);
+                    int mm;
+                    float t;
+                    floor_frac(G.mh_q * ((float)yl + G.y0c), mm, t);
+                    float l[ORDER], w[8 + ORDER - 1];
+                    lagrange<ORDER>(t, l);
+                    const int sx = xg + mm - O0;
+                    const float *src = A.psi + yl;
+#pragma unroll
+                    for (int i = 0; i < 8 + ORDER - 1; ++i) {
+                        const int xx = sx + i;
+                        w[i] = (xx >= 0 && xx < N) ? src[(size_t)xx * N] : 0.0f;
+                    }
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) {
+                        float a = l[0] * w[r];
+#pragma unroll
+                        for (int i = 1; i < ORDER; ++i) a = fmaf(l[i], w[r + i], a);
+                        out[r] = a;
+                    }
+                } else {
                 GRot<ORDER, false> rot;
                 rot.src = A.psi; rot.N = N; rot.y = min(y, N - 1);
                 const float Yc = (float)rot.y + G.y0c;
@@ -97,6 +122,7 @@ k_grid_step(GridConst G, GridArgs A)
                 } else {
 #pragma unroll
                     for (int r = 0; r < 8; ++r) out[r] = rot.cell_checked(min(xg + r, N - 1));
+                }
                 }
 #pragma unroll
                 for (int r = 0; r < 8; ++r) {
@@ -153,6 +179,53 @@ k_grid_step(GridConst G, GridArgs A)
             }
             __syncthreads();
             if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 4] = clock64();
+            if constexpr (MANH) {
+                // Manhattan: RF kick, wake kick (two 1-D interpolations along p), Fokker-Planck
+                const int total = (r1 - r0) * NQ;
+                for (int idx = tid; idx < total; idx += GR_THREADS) {
+                    const int rr = idx >> lgNQ, x = r0 + rr, g = (idx & (NQ - 1)) << 2;
+                    const float *row = A.psi_tmp + (size_t)x * N;
+                    const float4 z4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                    float4 v[5];
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) {
+                        const int c = g - 8 + 4 * q;
+                        v[q] = (c >= 0 && c < N) ? *reinterpret_cast<const float4 *>(row + c) : z4;
+                    }
+                    int mm1, mm2;
+                    float t1, t2;
+                    floor_frac(G.mh_p * ((float)x + G.x0c), mm1, t1);
+                    floor_frac(G.kick_c * sV[rr], mm2, t2);
+                    float l1[ORDER], l2[ORDER], c1p[4], o[4];
+                    lagrange<ORDER>(t1, l1);
+                    lagrange<ORDER>(t2, l2);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) c1p[c] = c1 * fmaf((float)(g + c), G.dp, G.p_min);
+                    if (mm1 >= -2 && mm1 <= 1 && mm2 >= -2 && mm2 <= 0) {
+                        float a[20], r[12];
+#pragma unroll
+                        for (int q = 0; q < 5; ++q) { a[4 * q] = v[q].x; a[4 * q + 1] = v[q].y; a[4 * q + 2] = v[q].z; a[4 * q + 3] = v[q].w; }
+                        if (mm1 == 0) rf_stage<ORDER, 0>(a, l1, g, N, r);
+                        else if (mm1 == -1) rf_stage<ORDER, -1>(a, l1, g, N, r);
+                        else if (mm1 == 1) rf_stage<ORDER, 1>(a, l1, g, N, r);
+                        else rf_stage<ORDER, -2>(a, l1, g, N, r);
+                        if (mm2 == 0) kick_fp_granule<ORDER, 0>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                        else if (mm2 == -1) kick_fp_granule<ORDER, -1>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                        else kick_fp_granule<ORDER, -2>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                    } else {
+                        rf_kick_fp_granule_any<ORDER>(row, l1, mm1, l2, mm2, g, N, G.fp_b, c2, c1p, o);
+                    }
+                    *reinterpret_cast<float4 *>(A.psi + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
+                    float rs = 0.0f;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const float yy = (float)(g + c) - yc, tt = o[c] * yy;
+                        rs += o[c]; acc[1] += tt; acc[2] = fmaf(tt, yy, acc[2]);
+                    }
+                    const float xx = (float)x - yc, tq = rs * xx;
+                    acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+                }
+            } else {
             // a4 + a5: four cells per thread in registers; four granules per pass, loads first
             const int total = (r1 - r0) * NQ;
             for (int idx0 = tid; idx0 < total; idx0 += 4 * GR_THREADS) {
@@ -203,6 +276,7 @@ k_grid_step(GridConst G, GridArgs A)
                         acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
                     }
                 }
+            }
             }
         }
         {
