@@ -18,7 +18,8 @@
  * Pins (tests/test_oracle_pins.py, all independent of this file's formulas): polynomial
  * exactness of the interpolation, closed-form moment laws of rotation / kick / Fokker-Planck,
  * Parseval identity wake <-> CSR power, free-space radiated-power closed form, quarter-period
- * displacement of a blob, stationarity of the Gaussian.  The full nonlinear CSR run has no closed
+ * displacement of a blob, stationarity of the Gaussian, and for the Manhattan rotation the exact
+ * linear symplectic map of means and covariances (P14).  The full nonlinear CSR run has no closed
  * form: "parity unpinned" beyond those pins.
  */
 #include <math.h>
