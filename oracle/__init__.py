@@ -32,7 +32,7 @@ class Params(C.Structure):
     _fields_ = [("N", C.c_int), ("q_min", C.c_double), ("q_max", C.c_double),
                 ("p_min", C.c_double), ("p_max", C.c_double), ("steps_per_period", C.c_int),
                 ("beta", C.c_double), ("interp_order", C.c_int), ("pad", C.c_int),
-                ("renormalise", C.c_int), ("manhattan", C.c_int)]
+                ("renormalise", C.c_int), ("manhattan", C.c_int), ("clamp", C.c_int)]
 
 
 _dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
@@ -46,13 +46,13 @@ def lib():
         L.vfpo_num_threads.restype = C.c_int
         L.vfpo_set_num_threads.argtypes = [C.c_int]
         L.vfpo_lagrange_weights.argtypes = [C.c_int, C.c_double, _dp]
-        L.vfpo_rotate.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
-        L.vfpo_drift.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
-        L.vfpo_rf_kick.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
+        L.vfpo_rotate.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp, C.c_int]
+        L.vfpo_drift.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp, C.c_int]
+        L.vfpo_rf_kick.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp, C.c_int]
         L.vfpo_project.argtypes = [C.c_int, C.c_double, _dp, _dp]
         L.vfpo_wake_function.argtypes = [C.c_int, C.c_int, _dp, _dp]
         L.vfpo_wake.argtypes = [C.c_int, _dp, _dp, _dp]
-        L.vfpo_kick.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp]
+        L.vfpo_kick.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp, C.c_int]
         L.vfpo_fokker_planck.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp]
         L.vfpo_moments.argtypes = [C.c_int] + [C.c_double] * 4 + [_dp, _dp]
         L.vfpo_csr_power.argtypes = [C.c_int, C.c_int, C.c_double, _dp, _dp]
@@ -87,26 +87,26 @@ def lagrange_weights(order: int, t: float) -> np.ndarray:
     return out
 
 
-def rotate(psi, q_min, q_max, p_min, p_max, dphi, order) -> np.ndarray:
+def rotate(psi, q_min, q_max, p_min, p_max, dphi, order, clamp: bool = False) -> np.ndarray:
     psi = _f64(psi)
     out = np.empty_like(psi)
-    lib().vfpo_rotate(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out)
+    lib().vfpo_rotate(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out, int(clamp))
     return out
 
 
-def drift(psi, q_min, q_max, p_min, p_max, dphi, order) -> np.ndarray:
+def drift(psi, q_min, q_max, p_min, p_max, dphi, order, clamp: bool = False) -> np.ndarray:
     """First half of the Manhattan rotation (L136): psi_A(q, p) = psi(q - dphi p, p)."""
     psi = _f64(psi)
     out = np.empty_like(psi)
-    lib().vfpo_drift(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out)
+    lib().vfpo_drift(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out, int(clamp))
     return out
 
 
-def rf_kick(psi, q_min, q_max, p_min, p_max, dphi, order) -> np.ndarray:
+def rf_kick(psi, q_min, q_max, p_min, p_max, dphi, order, clamp: bool = False) -> np.ndarray:
     """Second half of the Manhattan rotation (L136): psi_B(q, p) = psi_A(q, p + dphi q)."""
     psi = _f64(psi)
     out = np.empty_like(psi)
-    lib().vfpo_rf_kick(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out)
+    lib().vfpo_rf_kick(psi.shape[0], q_min, q_max, p_min, p_max, dphi, order, psi, out, int(clamp))
     return out
 
 
@@ -131,10 +131,10 @@ def wake(w, rho) -> np.ndarray:
     return V
 
 
-def kick(psi, dp, dphi, order, V) -> np.ndarray:
+def kick(psi, dp, dphi, order, V, clamp: bool = False) -> np.ndarray:
     psi = _f64(psi)
     out = np.empty_like(psi)
-    lib().vfpo_kick(psi.shape[0], dp, dphi, order, _f64(V), psi, out)
+    lib().vfpo_kick(psi.shape[0], dp, dphi, order, _f64(V), psi, out, int(clamp))
     return out
 
 
@@ -162,9 +162,10 @@ class Oracle:
     """One simulation (one batch member) advanced by the C oracle; state in double."""
 
     def __init__(self, N, q_min, q_max, p_min, p_max, steps_per_period, beta, interp_order,
-                 pad=2, Z: Optional[np.ndarray] = None, renormalise: bool = True, manhattan: bool = False):
+                 pad=2, Z: Optional[np.ndarray] = None, renormalise: bool = True, manhattan: bool = False,
+                 clamp: bool = False):
         self.P = Params(N, q_min, q_max, p_min, p_max, steps_per_period, beta, interp_order, pad,
-                        1 if renormalise else 0, 1 if manhattan else 0)
+                        1 if renormalise else 0, 1 if manhattan else 0, 1 if clamp else 0)
         self.N = N
         self.Z = None if Z is None else _z_pairs(np.asarray(Z).reshape(-1)).copy()
         if self.Z is not None and self.Z.size != 2 * (pad * N // 2 + 1):
@@ -173,10 +174,11 @@ class Oracle:
         self.steps = 0
 
     @classmethod
-    def from_workload(cls, wl, member: int = 0, renormalise: bool = True, manhattan: bool = False) -> "Oracle":
+    def from_workload(cls, wl, member: int = 0, renormalise: bool = True, manhattan: bool = False,
+                      clamp: bool = False) -> "Oracle":
         Z = wl.impedance([member])
         o = cls(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
-                wl.interp_order, wl.pad, None if Z is None else Z[0], renormalise, manhattan)
+                wl.interp_order, wl.pad, None if Z is None else Z[0], renormalise, manhattan, clamp)
         o.set_psi(wl.psi0([member])[0])
         return o
 

@@ -75,8 +75,13 @@ static double at(const double *psi, int N, int x, int y)
     return psi[(size_t)N * x + y];
 }
 
+/* Eq. 14 as read in DESIGN.md A9: the printed formula always returns
+ * max(a, b); the intended "clamped or saturated" interpolation limits the interpolated value to
+ * the interval spanned by the nodes that bracket the evaluation point. */
+static double clamp_to(double v, double lo, double hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
 /* 1-D interpolation along p of column x at real grid coordinate y_r (Eq. 10). */
-static double interp_p(const double *psi, int N, int order, int x, double y_r)
+static double interp_p(const double *psi, int N, int order, int x, double y_r, int clamp)
 {
     double l[VFPO_MAX_ORDER];
     double m = floor(y_r);
@@ -84,6 +89,10 @@ static double interp_p(const double *psi, int N, int order, int x, double y_r)
     double acc = 0.0;
     for (int j = 0; j < order; ++j)
         acc += l[j] * at(psi, N, x, (int)m + node_offset(order, j));
+    if (clamp) {
+        double a = at(psi, N, x, (int)m), b = at(psi, N, x, (int)m + 1);
+        acc = clamp_to(acc, fmin(a, b), fmax(a, b));
+    }
     return acc;
 }
 
@@ -91,7 +100,7 @@ static double interp_p(const double *psi, int N, int order, int x, double y_r)
  * dp/dtheta = -q).  Target (x,y) takes the value interpolated (N_i x N_i taps) at the
  * back-rotated source point q_s = c q - s p, p_s = s q + c p with exact cos/sin (reading A3). */
 void vfpo_rotate(int N, double q_min, double q_max, double p_min, double p_max, double dphi,
-                 int order, const double *psi, double *out)
+                 int order, const double *psi, double *out, int clamp)
 {
     const double dq = (q_max - q_min) / (N - 1), dp = (p_max - p_min) / (N - 1);
     const double c = cos(dphi), s = sin(dphi);
@@ -110,13 +119,18 @@ void vfpo_rotate(int N, double q_min, double q_max, double p_min, double p_max, 
                 for (int j = 0; j < order; ++j)
                     acc += lx[i] * ly[j] *
                            at(psi, N, (int)mx + node_offset(order, i), (int)my + node_offset(order, j));
+            if (clamp) {          /* the 2 x 2 nodes around the source point */
+                double a = at(psi, N, (int)mx, (int)my), b = at(psi, N, (int)mx, (int)my + 1);
+                double c2 = at(psi, N, (int)mx + 1, (int)my), d2 = at(psi, N, (int)mx + 1, (int)my + 1);
+                acc = clamp_to(acc, fmin(fmin(a, b), fmin(c2, d2)), fmax(fmax(a, b), fmax(c2, d2)));
+            }
             out[(size_t)N * x + y] = acc;
         }
     }
 }
 
 /* 1-D interpolation along q of column y at real grid coordinate x_r (Eq. 10). */
-static double interp_q(const double *psi, int N, int order, double x_r, int y)
+static double interp_q(const double *psi, int N, int order, double x_r, int y, int clamp)
 {
     double l[VFPO_MAX_ORDER];
     double m = floor(x_r);
@@ -124,6 +138,10 @@ static double interp_q(const double *psi, int N, int order, double x_r, int y)
     double acc = 0.0;
     for (int i = 0; i < order; ++i)
         acc += l[i] * at(psi, N, (int)m + node_offset(order, i), y);
+    if (clamp) {
+        double a = at(psi, N, (int)m, y), b = at(psi, N, (int)m + 1, y);
+        acc = clamp_to(acc, fmin(a, b), fmax(a, b));
+    }
     return acc;
 }
 
@@ -134,26 +152,26 @@ static double interp_q(const double *psi, int N, int order, double x_r, int y)
  *   drift    q' = q + dphi p      psi_A(q, p) = psi(q - dphi p, p)       interpolation along q
  *   RF kick  p' = p - dphi q'     psi_B(q, p) = psi_A(q, p + dphi q)     interpolation along p */
 void vfpo_drift(int N, double q_min, double q_max, double p_min, double p_max, double dphi, int order,
-                const double *psi, double *out)
+                const double *psi, double *out, int clamp)
 {
     const double dq = (q_max - q_min) / (N - 1), dp = (p_max - p_min) / (N - 1);
 #pragma omp parallel for schedule(static)
     for (int x = 0; x < N; ++x)
         for (int y = 0; y < N; ++y) {
             double p = p_min + y * dp;
-            out[(size_t)N * x + y] = interp_q(psi, N, order, (double)x - dphi * p / dq, y);
+            out[(size_t)N * x + y] = interp_q(psi, N, order, (double)x - dphi * p / dq, y, clamp);
         }
 }
 
 void vfpo_rf_kick(int N, double q_min, double q_max, double p_min, double p_max, double dphi, int order,
-                  const double *psi, double *out)
+                  const double *psi, double *out, int clamp)
 {
     const double dq = (q_max - q_min) / (N - 1), dp = (p_max - p_min) / (N - 1);
 #pragma omp parallel for schedule(static)
     for (int x = 0; x < N; ++x) {
         double q = q_min + x * dq;
         for (int y = 0; y < N; ++y)
-            out[(size_t)N * x + y] = interp_p(psi, N, order, x, (double)y + dphi * q / dp);
+            out[(size_t)N * x + y] = interp_p(psi, N, order, x, (double)y + dphi * q / dp, clamp);
     }
 }
 
@@ -206,13 +224,13 @@ void vfpo_wake(int N, const double *w, const double *rho, double *V)
  * Delta p_x = -dphi * V_x (readings A1, A6), so psi''(x,p) = psi'(x, p - Delta p_x):
  * y_r = y - Delta p_x / dp, 1-D interpolation along p. */
 void vfpo_kick(int N, double dp, double dphi, int order, const double *V, const double *psi,
-               double *out)
+               double *out, int clamp)
 {
 #pragma omp parallel for schedule(static)
     for (int x = 0; x < N; ++x) {
         double delta_p = -dphi * V[x];
         for (int y = 0; y < N; ++y)
-            out[(size_t)N * x + y] = interp_p(psi, N, order, x, (double)y - delta_p / dp);
+            out[(size_t)N * x + y] = interp_p(psi, N, order, x, (double)y - delta_p / dp, clamp);
     }
 }
 
@@ -292,6 +310,7 @@ typedef struct {
     int pad;           /* N_f = pad * N */
     int renormalise;   /* 1: psi_{t+1} = psi''' / C */
     int manhattan;     /* 1: a1 is the Manhattan rotation (drift, RF kick) instead of the standard one */
+    int clamp;         /* 1: every interpolation is clamped (Eq. 14, reading A9) */
 } vfpo_params;
 
 /* psi: in/out [N][N] double.  Z: (N_f/2+1) (re,im) pairs or NULL (no wake).  w: wake function
@@ -312,14 +331,14 @@ void vfpo_step(const vfpo_params *P, const double *Z, const double *w, double *p
     double *V = (double *)calloc(N, sizeof(double));
 
     if (P->manhattan) {                                                                      /* a1 */
-        vfpo_drift(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, psi, t2);
-        vfpo_rf_kick(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, t2, t1);
+        vfpo_drift(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, psi, t2, P->clamp);
+        vfpo_rf_kick(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, t2, t1, P->clamp);
     } else {
-        vfpo_rotate(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, psi, t1);
+        vfpo_rotate(N, P->q_min, P->q_max, P->p_min, P->p_max, dphi, P->interp_order, psi, t1, P->clamp);
     }
     vfpo_project(N, dp, t1, rho);                                                            /* a2 */
     if (Z) vfpo_wake(N, w, rho, V);                                                          /* a3 */
-    vfpo_kick(N, dp, dphi, P->interp_order, V, t1, t2);                                      /* a4 */
+    vfpo_kick(N, dp, dphi, P->interp_order, V, t1, t2, P->clamp);                                      /* a4 */
     vfpo_fokker_planck(N, P->p_min, P->p_max, b, t2, t1);                                    /* a5 */
     double C = 0.0;                                                                          /* a6 */
     for (size_t z = 0; z < cells; ++z) C += t1[z];

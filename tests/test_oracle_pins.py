@@ -403,3 +403,54 @@ def test_p14_manhattan_keeps_the_gaussian(orc):
     rows = d[~np.isnan(d[:, 0])]
     assert np.all(np.abs(rows[:, 3] - 1.0) < 0.01) and np.all(np.abs(rows[:, 4] - 1.0) < 0.01)
     assert abs(rows[-1, 0] - 1.0) < 1e-7          # only the 6-sigma tails leave through the box edge
+
+
+# ---------------------------------------------------------------- P15 clamped interpolation (Eq. 14)
+@pytest.mark.parametrize("order", [3, 4])
+def test_p15_clamped_interpolation_has_no_overshoot(orc, order):
+    """L110-116: "Interpolation using these polynomials sometimes overshoots the values of the
+    neighboring grid cells ... To avoid overshooting, one has to use clamped ... interpolation"
+    (Eq. 14, read as clamp to the interval of the bracketing nodes, A9).  On a step
+    the unclamped quadratic / cubic shift over- and undershoots; the clamped one stays inside
+    [min, max] of the data, creates no new extremum, and equals the unclamped one wherever that
+    already lies between its two bracketing nodes."""
+    N, L = 32, 6.0
+    dp = 2 * L / (N - 1)
+    psi = np.zeros((N, N))
+    psi[:, 10:20] = 1.0                                           # a box along p in every column
+    V = np.full(N, -0.37 * dp / (TWO_PI / 100))                   # shift of +0.37 cell... (sign per A6)
+    free = orc.kick(psi, dp, TWO_PI / 100, order, V)
+    clamped = orc.kick(psi, dp, TWO_PI / 100, order, V, clamp=True)
+    assert free.max() > 1.0 + 1e-3 and free.min() < -1e-3         # the artifact the paper describes
+    assert clamped.max() <= 1.0 and clamped.min() >= 0.0
+    row_f, row_c = free[5], clamped[5]
+    inside = (row_f >= 0.0) & (row_f <= 1.0)
+    # away from the two edges the interpolant is exact (constant data) and untouched
+    np.testing.assert_allclose(row_c[:8], 0.0, atol=0)
+    np.testing.assert_allclose(row_c[13:17], 1.0, atol=1e-15)
+    assert np.count_nonzero(~inside) >= 2
+    # linear interpolation never leaves the bracket: clamping is the identity
+    lin = orc.kick(psi, dp, TWO_PI / 100, 2, V)
+    np.testing.assert_array_equal(lin, orc.kick(psi, dp, TWO_PI / 100, 2, V, clamp=True))
+
+
+def test_p15_clamp_is_identity_on_smooth_data_and_bounds_the_rotation(orc):
+    """On a smooth Gaussian the cubic interpolant lies between its bracketing nodes almost
+    everywhere, so clamped and free rotation agree to the interpolation error; on a 2-D box the
+    clamped rotation stays within [0, 1] while the free one does not."""
+    N, L = 64, 6.0
+    g = gauss(N, L)
+    dphi = TWO_PI / 500
+    a = orc.rotate(g, -L, L, -L, L, dphi, 4)
+    b = orc.rotate(g, -L, L, -L, L, dphi, 4, clamp=True)
+    assert np.max(np.abs(a - b)) < 2e-4 * g.max()
+    box = np.zeros((N, N))
+    box[20:40, 24:44] = 1.0
+    a = orc.rotate(box, -L, L, -L, L, 25 * dphi, 4)
+    b = orc.rotate(box, -L, L, -L, L, 25 * dphi, 4, clamp=True)
+    assert a.max() > 1.01 and a.min() < -0.01
+    assert b.max() <= 1.0 and b.min() >= 0.0
+    # Manhattan halves: same statement line by line
+    for f in (orc.drift, orc.rf_kick):
+        c = f(box, -L, L, -L, L, 25 * dphi, 4, clamp=True)
+        assert c.max() <= 1.0 and c.min() >= 0.0
