@@ -59,6 +59,7 @@ def parse_args():
     ap.add_argument("--wake", default="auto", choices=["auto", "fft", "direct"])
     ap.add_argument("--cluster-size", type=int, default=0, help="CTAs per cluster of the cluster engine (0 = auto)")
     ap.add_argument("--manhattan", action="store_true", help="Manhattan (symplectic) rotation instead of the standard one")
+    ap.add_argument("--clamp", action="store_true", help="clamped interpolation (Eq. 14)")
     ap.add_argument("--stream-gen", type=int, default=0, help="streaming kernels: 0 auto, 1 first generation, 2 second")
     ap.add_argument("--cluster-kernel", type=int, default=0, help="cluster engine kernel: 0 auto, 1 scalar, 2 packed fp32x2")
     ap.add_argument("--cluster-threads", type=int, default=0, help="threads per CTA of the packed cluster kernel (0 = auto)")
@@ -205,7 +206,8 @@ def run_ours(args, wl, rank, local_rank, world):
     Z = wl.impedance(idx)
     sim = pkg.Simulation(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
                          wl.interp_order, wl.pad, members, Z=Z,
-                         flags=pkg.FLAG_RENORMALISE | (pkg.FLAG_ROT_MANHATTAN if args.manhattan else 0))
+                         flags=pkg.FLAG_RENORMALISE | (pkg.FLAG_ROT_MANHATTAN if args.manhattan else 0)
+                         | (pkg.FLAG_CLAMP if args.clamp else 0))
     if args.stream_gen:
         sim.set_stream_gen(args.stream_gen)
     if args.cluster_kernel:
@@ -320,7 +322,7 @@ def run_ours(args, wl, rank, local_rank, world):
             "config": {"workload": wl.name, "N": wl.N, "members": members, "split_steps_per_bench_step": n_inner,
                        "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
                        "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size, "stream_gen": sim_gen,
-                       "rotation": "manhattan" if args.manhattan else "standard",
+                       "rotation": "manhattan" if args.manhattan else "standard", "clamp": bool(args.clamp),
                        "cluster_kernel": cluster_kernel, "cluster_threads": cluster_threads,
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                        "l2": "256 MB buffer written between timed bench steps (L2 flush)"},

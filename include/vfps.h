@@ -57,7 +57,9 @@ typedef struct vfps_complex { float re, im; } vfps_complex;
 
 enum {
     VFPS_FLAG_RENORMALISE = 1,   /* psi <- psi / C after every step (BASELINE north_star (6)) */
-    VFPS_FLAG_CLAMP = 2,         /* Eq. 14 clamped interpolation -- not implemented yet */
+    VFPS_FLAG_CLAMP = 2,         /* clamped interpolation (Eq. 14, read as: limit every
+                                    interpolated value to the interval of its bracketing nodes);
+                                    STREAM / GRAPH / GRID engines                                 */
     VFPS_FLAG_ROT_MANHATTAN = 4  /* a1 is the symplectic "Manhattan" rotation (L136): drift along q then
                                     RF kick along p, two 1-D interpolations; STREAM / GRAPH engines  */
 };

@@ -130,7 +130,6 @@ int validate(const vfps_params *p, std::string &why)
     if (!is_pow2((long long)p->N * p->pad)) { why = "N*pad must be a power of two"; return VFPS_ERR_ARG; }
     if (p->members < 1) { why = "members must be >= 1"; return VFPS_ERR_ARG; }
     if (p->flags & ~(VFPS_FLAG_RENORMALISE | VFPS_FLAG_CLAMP | VFPS_FLAG_ROT_MANHATTAN)) { why = "unknown flag"; return VFPS_ERR_ARG; }
-    if (p->flags & VFPS_FLAG_CLAMP) { why = "clamped interpolation (Eq. 14) is not implemented"; return VFPS_ERR_UNSUPPORTED; }
     if (p->N % 4 != 0) { why = "N must be a multiple of 4 (float4 rows)"; return VFPS_ERR_UNSUPPORTED; }
     if ((long long)p->N * p->pad > 8192) { why = "N*pad > 8192: wake FFT does not fit one CTA's shared memory"; return VFPS_ERR_UNSUPPORTED; }
     return VFPS_OK;
@@ -291,7 +290,7 @@ cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, boo
 void cluster_configure(vfps_sim *h)
 {
     h->cl_S = 0; h->cl_max_clusters = 0; h->cl_ver = 0; h->cl_why.clear();
-    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) { h->cl_why = "the cluster engine implements the standard rotation only"; return; }
+    if (h->P.flags & (VFPS_FLAG_ROT_MANHATTAN | VFPS_FLAG_CLAMP)) { h->cl_why = "the cluster engine implements the standard rotation with free interpolation only"; return; }
     const int N = h->N, H = h->G.H;
     if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
     if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
@@ -395,17 +394,18 @@ int launch_step_stream(vfps_sim *h, bool timed)
 }
 
 template <int ORDER>
-const void *grid_kernel(bool manh)
+const void *grid_kernel(bool manh, bool clamp)
 {
-    return manh ? (const void *)k_grid_step<ORDER, true> : (const void *)k_grid_step<ORDER, false>;
+    if (clamp) return manh ? (const void *)k_grid_step<ORDER, true, true> : (const void *)k_grid_step<ORDER, false, true>;
+    return manh ? (const void *)k_grid_step<ORDER, true, false> : (const void *)k_grid_step<ORDER, false, false>;
 }
 const void *grid_kernel(const vfps_sim *h)
 {
-    const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0;
+    const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0, clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0;
     switch (h->P.interp_order) {
-        case 2: return grid_kernel<2>(manh);
-        case 3: return grid_kernel<3>(manh);
-        default: return grid_kernel<4>(manh);
+        case 2: return grid_kernel<2>(manh, clamp);
+        case 3: return grid_kernel<3>(manh, clamp);
+        default: return grid_kernel<4>(manh, clamp);
     }
 }
 
@@ -414,6 +414,10 @@ const void *grid_kernel(const vfps_sim *h)
 void grid_configure(vfps_sim *h)
 {
     h->gr_blocks = 0; h->gr_why.clear();
+    if ((h->P.flags & VFPS_FLAG_ROT_MANHATTAN) && (h->P.flags & VFPS_FLAG_CLAMP)) {
+        h->gr_why = "Manhattan rotation with clamped interpolation needs the profile after the RF kick (stream / graph engines)";
+        return;
+    }
     if (h->members != 1) { h->gr_why = "grid engine advances one simulation per handle"; return; }
     int dev = 0, coop = 0, sms = 0;
     cudaGetDevice(&dev);
@@ -475,7 +479,7 @@ int launch_grid_steps(vfps_sim *h, int n, float *diag)
 // which kernels the STREAM / GRAPH engines launch, and how they evaluate the wake
 int resolved_gen(const vfps_sim *h)
 {
-    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) return 2;      // only the second generation has it
+    if (h->P.flags & (VFPS_FLAG_ROT_MANHATTAN | VFPS_FLAG_CLAMP)) return 2;      // only the second generation has them
     return h->gen_opt ? h->gen_opt : 2;
 }
 bool wake_is_direct(const vfps_sim *h)
@@ -484,7 +488,7 @@ bool wake_is_direct(const vfps_sim *h)
     return h->wake_opt != VFPS_WAKE_FFT;
 }
 
-template <int ORDER>
+template <int ORDER, bool CLAMP>
 int launch_step_stream2(vfps_sim *h, bool timed)
 {
     const int N = h->N;
@@ -493,17 +497,24 @@ int launch_step_stream2(vfps_sim *h, bool timed)
     {
         Bracket br(h, VFPS_KERNEL_ROTATE2, timed);
         if (manh)
-            k_drift2<ORDER><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
+            k_drift2<ORDER, CLAMP><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
                 h->G, h->psi, h->psi_tmp, h->scale, h->rho_part, h->tiles_y2, h->rho, h->tilectr);
         else
-            k_rotate2<ORDER><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
+            k_rotate2<ORDER, CLAMP><<<dim3(h->tiles_x2 * h->tiles_y2, h->members), R2_THREADS, 0, h->stream>>>(
                 h->G, h->psi, h->psi_tmp, h->scale, h->rho_part, h->tiles_y2, h->rho, h->tilectr);
+    }
+    // Manhattan + clamp: the clamped RF kick changes the profile (k_rf_profile); rho then replaces
+    // the drift's partial sums as the wake's input
+    const bool rfp = manh && CLAMP && h->has_wake;
+    if (rfp) {
+        k_rf_profile<ORDER><<<dim3((N + 7) / 8, h->members), 256, 0, h->stream>>>(h->G, h->psi_tmp, h->rho);
+        h->launches += 1;
     }
     if (!direct) {
         Bracket br(h, VFPS_KERNEL_WAKE, timed);
         k_wake_fft<<<h->members, h->fft_threads, h->fft_smem, h->stream>>>(
-            N, h->Nf, h->log2Nf, h->G.dq, h->rho_part, h->tiles_y2, h->has_wake ? h->Z : nullptr, h->tw,
-            h->rho, h->V, h->qstat);
+            N, h->Nf, h->log2Nf, h->G.dq, rfp ? h->rho : h->rho_part, rfp ? 1 : h->tiles_y2,
+            h->has_wake ? h->Z : nullptr, h->tw, h->rho, h->V, h->qstat);
         h->launches += 1;
     } else if (h->has_wake) {      // without an impedance V stays 0 (set at create) and P = 0
         Bracket br(h, VFPS_KERNEL_WAKE_DIRECT, timed);
@@ -518,8 +529,8 @@ int launch_step_stream2(vfps_sim *h, bool timed)
     A.diag = h->diag_cell; A.members = h->members; A.rows_per_cta = h->kfp2_rows;
     {
         Bracket br(h, VFPS_KERNEL_KICK_FP2, timed);
-        if (manh) k_kick_fp2<ORDER, true><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
-        else k_kick_fp2<ORDER, false><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
+        if (manh) k_kick_fp2<ORDER, true, CLAMP><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
+        else k_kick_fp2<ORDER, false, CLAMP><<<dim3(h->kfp2_blocks, h->members), K2_THREADS, 0, h->stream>>>(h->G, A);
     }
     h->launches += 2;
     return VFPS_OK;
@@ -528,10 +539,11 @@ int launch_step_stream2(vfps_sim *h, bool timed)
 int launch_step(vfps_sim *h, bool timed)
 {
     if (resolved_gen(h) == 2) {
+        const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0;
         switch (h->P.interp_order) {
-            case 2: return launch_step_stream2<2>(h, timed);
-            case 3: return launch_step_stream2<3>(h, timed);
-            default: return launch_step_stream2<4>(h, timed);
+            case 2: return clamp ? launch_step_stream2<2, true>(h, timed) : launch_step_stream2<2, false>(h, timed);
+            case 3: return clamp ? launch_step_stream2<3, true>(h, timed) : launch_step_stream2<3, false>(h, timed);
+            default: return clamp ? launch_step_stream2<4, true>(h, timed) : launch_step_stream2<4, false>(h, timed);
         }
     }
     switch (h->P.interp_order) {
@@ -834,8 +846,8 @@ int vfps_set_option(vfps_handle h, int option, int value)
     }
     if (option == VFPS_OPT_STREAM_GEN) {
         if (value < 0 || value > 2) return fail(h, VFPS_ERR_ARG, "stream generation must be 0 (auto), 1 or 2");
-        if (value == 1 && (h->P.flags & VFPS_FLAG_ROT_MANHATTAN))
-            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels implement the standard rotation only");
+        if (value == 1 && (h->P.flags & (VFPS_FLAG_ROT_MANHATTAN | VFPS_FLAG_CLAMP)))
+            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels implement the standard rotation with free interpolation only");
         if (value == 1 && h->wake_opt == VFPS_WAKE_DIRECT)
             return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels have no direct-convolution wake");
         if (value != h->gen_opt) drop_graph(h);

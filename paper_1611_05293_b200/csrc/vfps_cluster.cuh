@@ -141,7 +141,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity)
 // cells g..g+3 of one row held in registers: b[i] = psi'(g - 4 + i), i = 0..11.
 // MM = integer part of the shift (compile time).  Returns the four new values and adds to the
 // moment sums.  k[i] = kicked value at position g - 1 + i, zero outside the grid (ghosts, A8).
-template <int ORDER, int MM>
+// CLAMP: Eq. 14 (reading A9) -- the kicked value is limited to the interval of its two bracketing
+// nodes (taps O0 and O0 + 1 of its stencil); only valid with un-scaled weights.
+template <int ORDER, int MM, bool CLAMP = false>
 __device__ __forceinline__ void kick_fp_granule(const float (&b)[12], const float (&l)[ORDER], int g, int N,
                                                 float fp_b, float c2, const float (&c1p)[4],
                                                 float (&out)[4])
@@ -155,6 +157,7 @@ __device__ __forceinline__ void kick_fp_granule(const float (&b)[12], const floa
         float acc = l[0] * b[i0];
 #pragma unroll
         for (int j = 1; j < ORDER; ++j) acc = fmaf(l[j], b[i0 + j], acc);
+        if (CLAMP) acc = fminf(fmaxf(acc, fminf(b[i0 + O0], b[i0 + O0 + 1])), fmaxf(b[i0 + O0], b[i0 + O0 + 1]));
         k[i] = acc;
     }
     if (g == 0) k[0] = 0.0f;
@@ -170,7 +173,7 @@ __device__ __forceinline__ void kick_fp_granule(const float (&b)[12], const floa
 }
 
 // generic (any integer shift) version reading the staged row with bounds checks
-template <int ORDER>
+template <int ORDER, bool CLAMP = false>
 __device__ __forceinline__ void kick_fp_granule_any(const float *row /* index 0 = y 0 */, const float (&l)[ORDER],
                                                     int mm, int g, int N, float fp_b, float c2,
                                                     const float (&c1p)[4], float (&out)[4])
@@ -180,13 +183,16 @@ __device__ __forceinline__ void kick_fp_granule_any(const float *row /* index 0 
 #pragma unroll
     for (int i = 0; i < 7; ++i) {
         const int y = g - 1 + i;
-        float acc = 0.0f;
+        float acc = 0.0f, lo = 0.0f, hi = 0.0f;
 #pragma unroll
         for (int j = 0; j < ORDER; ++j) {
             const int s = y + mm - O0 + j;
             const float v = (s >= 0 && s < N) ? row[s] : 0.0f;
             acc = fmaf(l[j], v, acc);
+            if (j == O0) { lo = v; hi = v; }
+            if (j == O0 + 1) { lo = fminf(lo, v); hi = fmaxf(hi, v); }
         }
+        if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
         k[i] = (y >= 0 && y < N) ? acc : 0.0f;
     }
 #pragma unroll

@@ -16,6 +16,7 @@
 //            CTA 0 writes the diagnostics row.
 // With VFPS_FLAG_ROT_MANHATTAN (template MANH) phase 1 is the drift (1-D shift along q) and phase 2
 // applies the RF kick before the wake kick (vfps_stream2.cuh: k_drift2, rf_stage).
+// Template CLAMP: clamped interpolation (Eq. 14, reading A9) in every interpolation of the step.
 // One simulation per handle (members == 1); batches of on-chip grids use the cluster engine.
 #pragma once
 #include "vfps_stream2.cuh"
@@ -45,7 +46,7 @@ struct GridArgs {
 
 __host__ __device__ inline size_t grid_smem_floats(int N, int KR) { return (size_t)2 * N + 2 * KR + 8; }
 
-template <int ORDER, bool MANH = false>
+template <int ORDER, bool MANH = false, bool CLAMP = false>
 __global__ void __launch_bounds__(GR_THREADS, 2)
 k_grid_step(GridConst G, GridArgs A)
 {
@@ -100,10 +101,11 @@ k_grid_step(GridConst G, GridArgs A)
                         float a = l[0] * w[r];
 #pragma unroll
                         for (int i = 1; i < ORDER; ++i) a = fmaf(l[i], w[r + i], a);
+                        if (CLAMP) a = fminf(fmaxf(a, fminf(w[r + O0], w[r + O0 + 1])), fmaxf(w[r + O0], w[r + O0 + 1]));
                         out[r] = a;
                     }
                 } else {
-                GRot<ORDER, false> rot;
+                GRot<ORDER, false, CLAMP> rot;
                 rot.src = A.psi; rot.N = N; rot.y = min(y, N - 1);
                 const float Yc = (float)rot.y + G.y0c;
                 rot.a = G.a; rot.d = G.d; rot.bY = G.b * Yc; rot.aY = G.a * Yc; rot.Xoff = G.x0c;
@@ -205,15 +207,15 @@ k_grid_step(GridConst G, GridArgs A)
                         float a[20], r[12];
 #pragma unroll
                         for (int q = 0; q < 5; ++q) { a[4 * q] = v[q].x; a[4 * q + 1] = v[q].y; a[4 * q + 2] = v[q].z; a[4 * q + 3] = v[q].w; }
-                        if (mm1 == 0) rf_stage<ORDER, 0>(a, l1, g, N, r);
-                        else if (mm1 == -1) rf_stage<ORDER, -1>(a, l1, g, N, r);
-                        else if (mm1 == 1) rf_stage<ORDER, 1>(a, l1, g, N, r);
-                        else rf_stage<ORDER, -2>(a, l1, g, N, r);
-                        if (mm2 == 0) kick_fp_granule<ORDER, 0>(r, l2, g, N, G.fp_b, c2, c1p, o);
-                        else if (mm2 == -1) kick_fp_granule<ORDER, -1>(r, l2, g, N, G.fp_b, c2, c1p, o);
-                        else kick_fp_granule<ORDER, -2>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                        if (mm1 == 0) rf_stage<ORDER, 0, CLAMP>(a, l1, g, N, r);
+                        else if (mm1 == -1) rf_stage<ORDER, -1, CLAMP>(a, l1, g, N, r);
+                        else if (mm1 == 1) rf_stage<ORDER, 1, CLAMP>(a, l1, g, N, r);
+                        else rf_stage<ORDER, -2, CLAMP>(a, l1, g, N, r);
+                        if (mm2 == 0) kick_fp_granule<ORDER, 0, CLAMP>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                        else if (mm2 == -1) kick_fp_granule<ORDER, -1, CLAMP>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                        else kick_fp_granule<ORDER, -2, CLAMP>(r, l2, g, N, G.fp_b, c2, c1p, o);
                     } else {
-                        rf_kick_fp_granule_any<ORDER>(row, l1, mm1, l2, mm2, g, N, G.fp_b, c2, c1p, o);
+                        rf_kick_fp_granule_any<ORDER, CLAMP>(row, l1, mm1, l2, mm2, g, N, G.fp_b, c2, c1p, o);
                     }
                     *reinterpret_cast<float4 *>(A.psi + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
                     float rs = 0.0f;
@@ -259,11 +261,11 @@ k_grid_step(GridConst G, GridArgs A)
                         if (mm >= -2 && mm <= 0) {
                             const float b[12] = {v0[u].x, v0[u].y, v0[u].z, v0[u].w, v1[u].x, v1[u].y, v1[u].z, v1[u].w,
                                                  v2[u].x, v2[u].y, v2[u].z, v2[u].w};
-                            if (mm == 0) kick_fp_granule<ORDER, 0>(b, l, g, N, G.fp_b, c2, c1p, o);
-                            else if (mm == -1) kick_fp_granule<ORDER, -1>(b, l, g, N, G.fp_b, c2, c1p, o);
-                            else kick_fp_granule<ORDER, -2>(b, l, g, N, G.fp_b, c2, c1p, o);
+                            if (mm == 0) kick_fp_granule<ORDER, 0, CLAMP>(b, l, g, N, G.fp_b, c2, c1p, o);
+                            else if (mm == -1) kick_fp_granule<ORDER, -1, CLAMP>(b, l, g, N, G.fp_b, c2, c1p, o);
+                            else kick_fp_granule<ORDER, -2, CLAMP>(b, l, g, N, G.fp_b, c2, c1p, o);
                         } else {
-                            kick_fp_granule_any<ORDER>(A.psi_tmp + (size_t)x * N, l, mm, g, N, G.fp_b, c2, c1p, o);
+                            kick_fp_granule_any<ORDER, CLAMP>(A.psi_tmp + (size_t)x * N, l, mm, g, N, G.fp_b, c2, c1p, o);
                         }
                         *reinterpret_cast<float4 *>(A.psi + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
                         float rs = 0.0f;

@@ -79,7 +79,9 @@ __device__ __forceinline__ float ldg_co(const float *p)
 // floor(dy) do not change along the group for any lane -> sliding register window, ORDER loads per
 // cell.  Otherwise every cell loads its own window with per-tap range checks (psi = 0 outside, A8).
 // rho_part[m][x][tile_y] = dp * scale * sum over the tile's columns of psi'(x, .)
-template <int ORDER, bool NC = true>      // NC: psi is read-only for the whole kernel (ld.global.nc)
+// NC: psi is read-only for the whole kernel (ld.global.nc); CLAMP: Eq. 14 (reading A9) -- the
+// interpolated value is limited to the interval of the 2 x 2 nodes around the source point
+template <int ORDER, bool NC = true, bool CLAMP = false>
 struct GRot {
     static constexpr int O0 = (ORDER - 1) / 2;
     static __device__ __forceinline__ float ld(const float *p) { return NC ? ldg_nc(p) : *p; }
@@ -99,7 +101,7 @@ struct GRot {
         lagrange<ORDER>(tx, lx);
         lagrange<ORDER>(ty, ly);
         const int sx = x + ix - O0, sy = y + iy - O0;
-        float acc = 0.0f;
+        float acc = 0.0f, lo = 0.0f, hi = 0.0f;
 #pragma unroll
         for (int i = 0; i < ORDER; ++i) {
             float rsum = 0.0f;
@@ -108,9 +110,14 @@ struct GRot {
                 const int xx = sx + i, yy = sy + j;
                 const float v = (xx >= 0 && xx < N && yy >= 0 && yy < N) ? ld(src + (size_t)xx * N + yy) : 0.0f;
                 rsum = fmaf(ly[j], v, rsum);
+                if (CLAMP && (i == O0 || i == O0 + 1) && (j == O0 || j == O0 + 1)) {
+                    if (i == O0 && j == O0) { lo = v; hi = v; }
+                    else { lo = fminf(lo, v); hi = fmaxf(hi, v); }
+                }
             }
             acc = fmaf(lx[i], rsum, acc);
         }
+        if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
         return acc;
     }
     // rows x .. x+7 with floors (ix, iy) throughout and every tap inside the grid: all
@@ -170,12 +177,16 @@ struct GRot {
                 for (int j = 1; j < ORDER; ++j) rsum = fmaf(ly[j], t[r + i][j], rsum);
                 acc = (i == 0) ? lx[0] * rsum : fmaf(lx[i], rsum, acc);
             }
+            if (CLAMP) {
+                const float a0 = t[r + O0][O0], a1 = t[r + O0][O0 + 1], b0 = t[r + O0 + 1][O0], b1 = t[r + O0 + 1][O0 + 1];
+                acc = fminf(fmaxf(acc, fminf(fminf(a0, a1), fminf(b0, b1))), fmaxf(fmaxf(a0, a1), fmaxf(b0, b1)));
+            }
             out[r] = acc;
         }
     }
 };
 
-template <int ORDER>
+template <int ORDER, bool CLAMP = false>
 __global__ void __launch_bounds__(R2_THREADS)
 k_rotate2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_out,
           const float *__restrict__ scale, float *__restrict__ rho_part, int tiles_y,
@@ -192,7 +203,7 @@ k_rotate2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi
     const float sc = G.renorm ? __ldg(scale + m) : 1.0f;
     float *dst = psi_out + (size_t)m * N * N;
 
-    GRot<ORDER> rot;
+    GRot<ORDER, true, CLAMP> rot;
     rot.src = psi_in + (size_t)m * N * N;
     rot.N = N; rot.y = min(y, N - 1);        // lanes beyond the grid compute a valid cell, never stored
     {
@@ -274,7 +285,7 @@ k_rotate2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi
 // group from a window of 8 + ORDER - 1 loads (rows outside the grid read as zero, A8).  The
 // second half (RF kick, a shift along p by mh_p * X cells) does not change the profile and is
 // applied by k_kick_fp2<ORDER, true> together with the wake kick.
-template <int ORDER>
+template <int ORDER, bool CLAMP = false>
 __global__ void __launch_bounds__(R2_THREADS)
 k_drift2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_out,
          const float *__restrict__ scale, float *__restrict__ rho_part, int tiles_y,
@@ -311,6 +322,8 @@ k_drift2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_
                 float acc = l[0] * w[r];
 #pragma unroll
                 for (int i = 1; i < ORDER; ++i) acc = fmaf(l[i], w[r + i], acc);
+                if (CLAMP)      // the weights carry the scale 1/C > 0, so do the bounds
+                    acc = fminf(fmaxf(acc, sc * fminf(w[r + O0], w[r + O0 + 1])), sc * fmaxf(w[r + O0], w[r + O0 + 1]));
                 const bool ok = (y < N) && (xg + r < N);
                 if (ok) dst[(size_t)(xg + r) * N + y] = acc;
                 out[r] = ok ? acc : 0.0f;
@@ -405,7 +418,7 @@ k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wf
 // s1 = mh_p * X cells, for the 12 columns g-4 .. g+7 that the wake kick of the granule g..g+3
 // reads.  a[i] = psi_A(x, g - 8 + i), i = 0..19; MM1 = floor(s1) (compile time), l1 = weights of
 // its fraction; columns outside the grid are zero before and after (A8).
-template <int ORDER, int MM1>
+template <int ORDER, int MM1, bool CLAMP = false>
 __device__ __forceinline__ void rf_stage(const float (&a)[20], const float (&l1)[ORDER], int g, int N, float (&r)[12])
 {
     constexpr int O0 = (ORDER - 1) / 2;
@@ -415,25 +428,30 @@ __device__ __forceinline__ void rf_stage(const float (&a)[20], const float (&l1)
         float acc = l1[0] * a[i0];
 #pragma unroll
         for (int j = 1; j < ORDER; ++j) acc = fmaf(l1[j], a[i0 + j], acc);
+        if (CLAMP) acc = fminf(fmaxf(acc, fminf(a[i0 + O0], a[i0 + O0 + 1])), fmaxf(a[i0 + O0], a[i0 + O0 + 1]));
         const int y = g - 4 + i;
         r[i] = (y >= 0 && y < N) ? acc : 0.0f;
     }
 }
 // any integer parts: psi_B at column s of the row (bounds-checked loads), and the whole granule
-template <int ORDER>
+template <int ORDER, bool CLAMP = false>
 __device__ __forceinline__ float rf_value(const float *row, int N, int s, int mm1, const float (&l1)[ORDER])
 {
     constexpr int O0 = (ORDER - 1) / 2;
     if (s < 0 || s >= N) return 0.0f;
-    float acc = 0.0f;
+    float acc = 0.0f, lo = 0.0f, hi = 0.0f;
 #pragma unroll
     for (int j = 0; j < ORDER; ++j) {
         const int c = s + mm1 - O0 + j;
-        acc = fmaf(l1[j], (c >= 0 && c < N) ? row[c] : 0.0f, acc);
+        const float v = (c >= 0 && c < N) ? row[c] : 0.0f;
+        acc = fmaf(l1[j], v, acc);
+        if (j == O0) { lo = v; hi = v; }
+        if (j == O0 + 1) { lo = fminf(lo, v); hi = fmaxf(hi, v); }
     }
+    if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
     return acc;
 }
-template <int ORDER>
+template <int ORDER, bool CLAMP = false>
 __device__ __noinline__ void rf_kick_fp_granule_any(const float *row, const float (&l1)[ORDER], int mm1,
                                                     const float (&l2)[ORDER], int mm2, int g, int N, float fp_b,
                                                     float c2, const float (&c1p)[4], float (&out)[4])
@@ -443,8 +461,14 @@ __device__ __noinline__ void rf_kick_fp_granule_any(const float *row, const floa
 #pragma unroll 1
     for (int i = 0; i < 7; ++i) {
         const int y = g - 1 + i;
-        float acc = 0.0f;
-        for (int j = 0; j < ORDER; ++j) acc = fmaf(l2[j], rf_value<ORDER>(row, N, y + mm2 - O0 + j, mm1, l1), acc);
+        float acc = 0.0f, lo = 0.0f, hi = 0.0f;
+        for (int j = 0; j < ORDER; ++j) {
+            const float v = rf_value<ORDER, CLAMP>(row, N, y + mm2 - O0 + j, mm1, l1);
+            acc = fmaf(l2[j], v, acc);
+            if (j == O0) { lo = v; hi = v; }
+            if (j == O0 + 1) { lo = fminf(lo, v); hi = fmaxf(hi, v); }
+        }
+        if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
         k[i] = (y >= 0 && y < N) ? acc : 0.0f;
     }
 #pragma unroll
@@ -455,6 +479,30 @@ __device__ __noinline__ void rf_kick_fp_granule_any(const float *row, const floa
         const float incr = fmaf(fp_b, f0, fmaf(c1p[c], d1, c2 * d2));
         out[c] = f0 + incr;
     }
+}
+
+// ---------------------------------------------------------------- a2 for Manhattan + clamp
+// The RF kick is a shift along p and leaves the profile alone -- unless its interpolation is
+// clamped (Eq. 14), which is not conservative.  Then the profile the wake needs is that of psi_B:
+// one warp per row evaluates the RF stage of its row once more and sums it (nothing is stored).
+// grid = (ceil(N / 8), members), block = 256.
+template <int ORDER>
+__global__ void __launch_bounds__(256)
+k_rf_profile(GridConst G, const float *__restrict__ psi_A, float *__restrict__ rho)
+{
+    const int N = G.N, m = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int x = blockIdx.x * 8 + warp;
+    if (x >= N) return;
+    const float *row = psi_A + ((size_t)m * N + x) * N;
+    int mm1;
+    float t1;
+    floor_frac(G.mh_p * ((float)x + G.x0c), mm1, t1);
+    float l1[ORDER];
+    lagrange<ORDER>(t1, l1);
+    float s = 0.0f;
+    for (int y = lane; y < N; y += 32) s += rf_value<ORDER, true>(row, N, y, mm1, l1);
+    s = warp_sum(s);
+    if (lane == 0) rho[(size_t)m * N + x] = G.dp * s;
 }
 
 // ---------------------------------------------------------------- a4 + a5 + a6: kick, FP, moments
@@ -478,7 +526,7 @@ struct Kfp2Args {
 // one row: three 128-bit loads give the rotated density at g-4 .. g+7, kick and Fokker-Planck run
 // in registers (kick_fp_granule of vfps_cluster.cuh), one 128-bit store.  The last CTA of each
 // member finalises the diagnostics row and the renormalisation scalar (fixed summation order).
-template <int ORDER, bool MANH = false>
+template <int ORDER, bool MANH = false, bool CLAMP = false>
 __global__ void __launch_bounds__(K2_THREADS)
 k_kick_fp2(GridConst G, Kfp2Args A)
 {
@@ -521,15 +569,15 @@ k_kick_fp2(GridConst G, Kfp2Args A)
                 float a[20], r[12];
 #pragma unroll
                 for (int q = 0; q < 5; ++q) { a[4 * q] = v[q].x; a[4 * q + 1] = v[q].y; a[4 * q + 2] = v[q].z; a[4 * q + 3] = v[q].w; }
-                if (mm1 == 0) rf_stage<ORDER, 0>(a, l1, g, N, r);
-                else if (mm1 == -1) rf_stage<ORDER, -1>(a, l1, g, N, r);
-                else if (mm1 == 1) rf_stage<ORDER, 1>(a, l1, g, N, r);
-                else rf_stage<ORDER, -2>(a, l1, g, N, r);
-                if (mm2 == 0) kick_fp_granule<ORDER, 0>(r, l2, g, N, G.fp_b, c2, c1p, o);
-                else if (mm2 == -1) kick_fp_granule<ORDER, -1>(r, l2, g, N, G.fp_b, c2, c1p, o);
-                else kick_fp_granule<ORDER, -2>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                if (mm1 == 0) rf_stage<ORDER, 0, CLAMP>(a, l1, g, N, r);
+                else if (mm1 == -1) rf_stage<ORDER, -1, CLAMP>(a, l1, g, N, r);
+                else if (mm1 == 1) rf_stage<ORDER, 1, CLAMP>(a, l1, g, N, r);
+                else rf_stage<ORDER, -2, CLAMP>(a, l1, g, N, r);
+                if (mm2 == 0) kick_fp_granule<ORDER, 0, CLAMP>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                else if (mm2 == -1) kick_fp_granule<ORDER, -1, CLAMP>(r, l2, g, N, G.fp_b, c2, c1p, o);
+                else kick_fp_granule<ORDER, -2, CLAMP>(r, l2, g, N, G.fp_b, c2, c1p, o);
             } else {
-                rf_kick_fp_granule_any<ORDER>(row, l1, mm1, l2, mm2, g, N, G.fp_b, c2, c1p, o);
+                rf_kick_fp_granule_any<ORDER, CLAMP>(row, l1, mm1, l2, mm2, g, N, G.fp_b, c2, c1p, o);
             }
             *reinterpret_cast<float4 *>(dst + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
             float rs = 0.0f;
@@ -578,11 +626,11 @@ k_kick_fp2(GridConst G, Kfp2Args A)
                 if (mm >= -2 && mm <= 0) {
                     const float b[12] = {v0[u].x, v0[u].y, v0[u].z, v0[u].w, v1[u].x, v1[u].y, v1[u].z, v1[u].w,
                                          v2[u].x, v2[u].y, v2[u].z, v2[u].w};
-                    if (mm == 0) kick_fp_granule<ORDER, 0>(b, l, g, N, G.fp_b, c2, c1p, o);
-                    else if (mm == -1) kick_fp_granule<ORDER, -1>(b, l, g, N, G.fp_b, c2, c1p, o);
-                    else kick_fp_granule<ORDER, -2>(b, l, g, N, G.fp_b, c2, c1p, o);
+                    if (mm == 0) kick_fp_granule<ORDER, 0, CLAMP>(b, l, g, N, G.fp_b, c2, c1p, o);
+                    else if (mm == -1) kick_fp_granule<ORDER, -1, CLAMP>(b, l, g, N, G.fp_b, c2, c1p, o);
+                    else kick_fp_granule<ORDER, -2, CLAMP>(b, l, g, N, G.fp_b, c2, c1p, o);
                 } else {
-                    kick_fp_granule_any<ORDER>(src + (size_t)x * N, l, mm, g, N, G.fp_b, c2, c1p, o);
+                    kick_fp_granule_any<ORDER, CLAMP>(src + (size_t)x * N, l, mm, g, N, G.fp_b, c2, c1p, o);
                 }
                 *reinterpret_cast<float4 *>(dst + (size_t)x * N + g) = make_float4(o[0], o[1], o[2], o[3]);
                 float rs = 0.0f;

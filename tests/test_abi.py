@@ -48,8 +48,10 @@ def test_version_and_error_strings_without_gpu(vfps):
     P = vfps.VfpsParams(7, -6, 6, -6, 6, 100, 1e-3, 4, 2, 1, 1)
     assert L.vfps_create(ctypes.byref(P), None, None, ctypes.byref(h)) == -1      # VFPS_ERR_ARG
     assert b"N must be" in L.vfps_last_error(None)
-    P = vfps.VfpsParams(64, -6, 6, -6, 6, 100, 1e-3, 4, 2, 1, 1 | 2)
-    assert L.vfps_create(ctypes.byref(P), None, None, ctypes.byref(h)) == -5      # UNSUPPORTED (clamp)
+    P = vfps.VfpsParams(8192, -6, 6, -6, 6, 100000, 1e-3, 4, 2, 1, 1)
+    assert L.vfps_create(ctypes.byref(P), None, None, ctypes.byref(h)) == -5      # UNSUPPORTED (FFT length)
+    P = vfps.VfpsParams(64, -6, 6, -6, 6, 100, 1e-3, 4, 2, 1, 1 | 64)
+    assert L.vfps_create(ctypes.byref(P), None, None, ctypes.byref(h)) == -1      # unknown flag
     assert L.vfps_destroy(None) == 0
 
 
