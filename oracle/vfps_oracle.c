@@ -19,7 +19,7 @@
  * exactness of the interpolation, closed-form moment laws of rotation / kick / Fokker-Planck,
  * Parseval identity wake <-> CSR power, free-space radiated-power closed form, quarter-period
  * displacement of a blob, stationarity of the Gaussian, and for the Manhattan rotation the exact
- * linear symplectic map of means and covariances (P14).  The full nonlinear CSR run has no closed
+ * linear symplectic map of means and covariances (P14), no-overshoot of the clamped interpolation (P15).  The full nonlinear CSR run has no closed
  * form: "parity unpinned" beyond those pins.
  */
 #include <math.h>
