@@ -138,6 +138,13 @@ int vfps_destroy(vfps_handle h);
 int vfps_set_option(vfps_handle h, int option, int value);
 int vfps_get_option(vfps_handle h, int option, int *value);
 
+/* Replace the impedance of a simulation that was created with one (same layout as in vfps_create);
+ * psi and the step counter are kept.  This is the paper's adiabatic current scan (L239, L290-298,
+ * App. A): the final distribution of one bunch current is the starting distribution of the next.
+ * VFPS_ERR_STATE if the handle was created with Z = NULL. */
+int vfps_set_impedance(vfps_handle h, const vfps_complex *Z);
+int vfps_set_impedance_host(vfps_handle h, const vfps_complex *Z_host);
+
 /* Copy psi [members][N][N] into the simulation; no renormalisation; step counter := 0. */
 int vfps_set_psi(vfps_handle h, const float *psi);
 int vfps_set_psi_host(vfps_handle h, const float *psi_host);

@@ -22,6 +22,7 @@ FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 # every symbol include/vfps.h declares (tests check the library exports each of them)
 EXPORTS = [
     "vfps_create", "vfps_create_host", "vfps_destroy", "vfps_set_option", "vfps_get_option",
+    "vfps_set_impedance", "vfps_set_impedance_host",
     "vfps_set_psi", "vfps_set_psi_host", "vfps_step", "vfps_step_host",
     "vfps_get_psi", "vfps_get_psi_host", "vfps_get_profile", "vfps_get_profile_host",
     "vfps_get_wake", "vfps_get_wake_host", "vfps_get_moments", "vfps_get_moments_host",
@@ -60,7 +61,8 @@ def load():
     L.vfps_destroy.argtypes = [vp]
     L.vfps_set_option.argtypes = [vp, ip, ip]
     L.vfps_get_option.argtypes = [vp, ip, C.POINTER(ip)]
-    for name in ("vfps_set_psi", "vfps_set_psi_host", "vfps_get_psi", "vfps_get_psi_host",
+    for name in ("vfps_set_impedance", "vfps_set_impedance_host",
+                 "vfps_set_psi", "vfps_set_psi_host", "vfps_get_psi", "vfps_get_psi_host",
                  "vfps_get_profile", "vfps_get_profile_host", "vfps_get_wake", "vfps_get_wake_host",
                  "vfps_get_moments", "vfps_get_moments_host"):
         getattr(L, name).argtypes = [vp, vp]
@@ -262,6 +264,11 @@ class Simulation:
         return out
 
     # ---------------------------------------------------------------- host-pointer calls
+    def set_impedance_host(self, Z) -> None:
+        """New impedance [members][Nf/2+1] for the running simulation (adiabatic current scan)."""
+        zh = _host_arr(Z, np.complex64, self.members * (self.Nf // 2 + 1), "Z")
+        self._check(self._L.vfps_set_impedance_host(self._h, zh.ctypes.data_as(C.c_void_p)))
+
     def set_psi_host(self, psi) -> None:
         a = _host_arr(psi, np.float32, self.members * self.N * self.N, "psi")
         self._check(self._L.vfps_set_psi_host(self._h, a.ctypes.data_as(C.c_void_p)))

@@ -902,6 +902,24 @@ static int set_psi_impl(vfps_handle h, const float *psi, cudaMemcpyKind kind)
     return VFPS_OK;
 }
 
+static int set_impedance_impl(vfps_handle h, const vfps_complex *Z, cudaMemcpyKind kind)
+{
+    if (!h) return fail(nullptr, VFPS_ERR_ARG, "handle is NULL");
+    if (!Z) return fail(h, VFPS_ERR_ARG, "Z is NULL");
+    if (!h->has_wake) return fail(h, VFPS_ERR_STATE, "the simulation was created without an impedance");
+    const size_t nz = (size_t)h->members * (h->Nf / 2 + 1);
+    CU(cudaMemcpyAsync(h->Z, Z, nz * sizeof(float2), kind, h->stream));
+    const int nw = h->members * 2 * h->N;
+    k_wake_function<<<(nw + 127) / 128, 128, 0, h->stream>>>(h->N, h->Nf, h->members, h->Z, h->wfun);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    if (kind == cudaMemcpyHostToDevice) CU(cudaStreamSynchronize(h->stream));
+    return VFPS_OK;
+}
+
+int vfps_set_impedance(vfps_handle h, const vfps_complex *Z) { return set_impedance_impl(h, Z, cudaMemcpyDeviceToDevice); }
+int vfps_set_impedance_host(vfps_handle h, const vfps_complex *Z) { return set_impedance_impl(h, Z, cudaMemcpyHostToDevice); }
+
 int vfps_set_psi(vfps_handle h, const float *psi) { return set_psi_impl(h, psi, cudaMemcpyDeviceToDevice); }
 int vfps_set_psi_host(vfps_handle h, const float *psi) { return set_psi_impl(h, psi, cudaMemcpyHostToDevice); }
 

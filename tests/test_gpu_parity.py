@@ -495,6 +495,41 @@ def test_clamped_interpolation(vfps, orc, order, N, manhattan):
     sim.close()
 
 
+def test_adiabatic_scan_set_impedance(vfps, orc):
+    """The paper's adiabatic current scan (L239, L290-298): the final distribution of one current
+    seeds the next.  vfps_set_impedance swaps Z (and the wake function) of a running simulation:
+    three currents S_csr = 0.6 -> 0.5 -> 0.4 of the C1 physics, 150 steps each, on every engine in
+    turn, against the oracle chained the same way."""
+    wl = get_workload("C1")
+    dq = (wl.q_max - wl.q_min) / (wl.N - 1)
+    sim = vfps.Simulation.from_workload(wl.with_(S_csr=(0.6,)))
+    o = orc.Oracle.from_workload(wl.with_(S_csr=(0.6,)))
+    engines = [vfps.ENGINE_CLUSTER, vfps.ENGINE_GRID, vfps.ENGINE_GRAPH]
+    P = []
+    for S, eng in zip((0.6, 0.5, 0.4), engines):
+        Z = make_impedance(wl.N, wl.pad, dq, S, 1.0)
+        if S != 0.6:
+            sim.set_impedance_host(Z[None, :])
+            psi_prev = o.psi.copy()
+            o = orc.Oracle(wl.N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta,
+                           wl.interp_order, wl.pad, Z)
+            o.set_psi(psi_prev)
+        sim.set_engine(eng)
+        d = sim.step_host(150)
+        dr = o.step(150)
+        assert_psi(sim.get_psi_host()[0], o.psi, 2e-4, f"adiabatic scan, S = {S}")
+        assert_diag(d[149, 0], dr[149])
+        P.append(d[149, 0, 5])
+    assert P[0] > P[1] > P[2] > 0                    # the radiated power follows the current down
+    assert sim.step_count() == 450
+    sim.close()
+    nowake = vfps.Simulation(64, -6, 6, -6, 6, 500, 1e-3, 2)
+    with pytest.raises(vfps.VfpsError) as e:
+        nowake.set_impedance_host(np.zeros((1, 65), dtype=np.complex64))
+    assert e.value.code == -2
+    nowake.close()
+
+
 @pytest.mark.parametrize("order,N", [(4, 512), (4, 256), (3, 128), (2, 64), (4, 8)])
 def test_grid_engine(vfps, orc, order, N):
     """Persistent cooperative-grid engine: asymmetric box, off-centre bunch, free-space wake, 300
