@@ -61,7 +61,7 @@ enum {
                                     interpolated value to the interval of its bracketing nodes);
                                     STREAM / GRAPH / GRID engines                                 */
     VFPS_FLAG_ROT_MANHATTAN = 4  /* a1 is the symplectic "Manhattan" rotation (L136): drift along q then
-                                    RF kick along p, two 1-D interpolations; STREAM / GRAPH engines  */
+                                    RF kick along p, two 1-D interpolations; every engine            */
 };
 
 typedef struct vfps_params {

@@ -264,14 +264,19 @@ cudaError_t cluster_launch_o(vfps_sim *h, const ClusterArgs &A, int nclusters, b
             default: return cudaErrorInvalidValue;
         }
     }
+    const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0;
+#define VFPS_CL1(NN)                                                                                      \
+    (manh ? cluster_launch_k(h, k_cluster_step<ORDER, NN, true>, CL_THREADS, A, nclusters, query, mc)    \
+          : cluster_launch_k(h, k_cluster_step<ORDER, NN, false>, CL_THREADS, A, nclusters, query, mc))
     switch (h->N) {
-        case 32: return cluster_launch_k(h, k_cluster_step<ORDER, 32>, CL_THREADS, A, nclusters, query, mc);
-        case 64: return cluster_launch_k(h, k_cluster_step<ORDER, 64>, CL_THREADS, A, nclusters, query, mc);
-        case 128: return cluster_launch_k(h, k_cluster_step<ORDER, 128>, CL_THREADS, A, nclusters, query, mc);
-        case 256: return cluster_launch_k(h, k_cluster_step<ORDER, 256>, CL_THREADS, A, nclusters, query, mc);
-        case 512: return cluster_launch_k(h, k_cluster_step<ORDER, 512>, CL_THREADS, A, nclusters, query, mc);
+        case 32: return VFPS_CL1(32);
+        case 64: return VFPS_CL1(64);
+        case 128: return VFPS_CL1(128);
+        case 256: return VFPS_CL1(256);
+        case 512: return VFPS_CL1(512);
         default: return cudaErrorInvalidValue;
     }
+#undef VFPS_CL1
 }
 
 cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *mc)
@@ -290,7 +295,7 @@ cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, boo
 void cluster_configure(vfps_sim *h)
 {
     h->cl_S = 0; h->cl_max_clusters = 0; h->cl_ver = 0; h->cl_why.clear();
-    if (h->P.flags & (VFPS_FLAG_ROT_MANHATTAN | VFPS_FLAG_CLAMP)) { h->cl_why = "the cluster engine implements the standard rotation with free interpolation only"; return; }
+    if (h->P.flags & VFPS_FLAG_CLAMP) { h->cl_why = "the cluster engine implements free (un-clamped) interpolation only"; return; }
     const int N = h->N, H = h->G.H;
     if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
     if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
@@ -304,6 +309,7 @@ void cluster_configure(vfps_sim *h)
     for (int ver = 1; ver <= 2; ++ver) {
         if (ver != (h->cl_ver_opt ? h->cl_ver_opt : 1)) continue;
         if (ver == 2 && !(N == 128 || N == 256 || N == 512)) continue;
+        if (ver == 2 && (h->P.flags & VFPS_FLAG_ROT_MANHATTAN)) continue;      // packed kernel: standard rotation only
         for (int c = 0; c < 5; ++c) {
             const int S = cand[c];
             if (h->cl_S_opt && S != h->cl_S_opt) continue;

@@ -205,6 +205,73 @@ __device__ __forceinline__ void kick_fp_granule_any(const float *row /* index 0 
     }
 }
 
+// Manhattan rotation, second half (RF kick): psi_B(x, y) = psi_A(x, y + s1),
+// s1 = mh_p * X cells, for the 12 columns g-4 .. g+7 that the wake kick of the granule g..g+3
+// reads.  a[i] = psi_A(x, g - 8 + i), i = 0..19; MM1 = floor(s1) (compile time), l1 = weights of
+// its fraction; columns outside the grid are zero before and after (A8).
+template <int ORDER, int MM1, bool CLAMP = false>
+__device__ __forceinline__ void rf_stage(const float (&a)[20], const float (&l1)[ORDER], int g, int N, float (&r)[12])
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+#pragma unroll
+    for (int i = 0; i < 12; ++i) {
+        const int i0 = i + 4 + MM1 - O0;
+        float acc = l1[0] * a[i0];
+#pragma unroll
+        for (int j = 1; j < ORDER; ++j) acc = fmaf(l1[j], a[i0 + j], acc);
+        if (CLAMP) acc = fminf(fmaxf(acc, fminf(a[i0 + O0], a[i0 + O0 + 1])), fmaxf(a[i0 + O0], a[i0 + O0 + 1]));
+        const int y = g - 4 + i;
+        r[i] = (y >= 0 && y < N) ? acc : 0.0f;
+    }
+}
+// any integer parts: psi_B at column s of the row (bounds-checked loads), and the whole granule
+template <int ORDER, bool CLAMP = false>
+__device__ __forceinline__ float rf_value(const float *row, int N, int s, int mm1, const float (&l1)[ORDER])
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+    if (s < 0 || s >= N) return 0.0f;
+    float acc = 0.0f, lo = 0.0f, hi = 0.0f;
+#pragma unroll
+    for (int j = 0; j < ORDER; ++j) {
+        const int c = s + mm1 - O0 + j;
+        const float v = (c >= 0 && c < N) ? row[c] : 0.0f;
+        acc = fmaf(l1[j], v, acc);
+        if (j == O0) { lo = v; hi = v; }
+        if (j == O0 + 1) { lo = fminf(lo, v); hi = fmaxf(hi, v); }
+    }
+    if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
+    return acc;
+}
+template <int ORDER, bool CLAMP = false>
+__device__ __noinline__ void rf_kick_fp_granule_any(const float *row, const float (&l1)[ORDER], int mm1,
+                                                    const float (&l2)[ORDER], int mm2, int g, int N, float fp_b,
+                                                    float c2, const float (&c1p)[4], float (&out)[4])
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+    float k[7];
+#pragma unroll 1
+    for (int i = 0; i < 7; ++i) {
+        const int y = g - 1 + i;
+        float acc = 0.0f, lo = 0.0f, hi = 0.0f;
+        for (int j = 0; j < ORDER; ++j) {
+            const float v = rf_value<ORDER, CLAMP>(row, N, y + mm2 - O0 + j, mm1, l1);
+            acc = fmaf(l2[j], v, acc);
+            if (j == O0) { lo = v; hi = v; }
+            if (j == O0 + 1) { lo = fminf(lo, v); hi = fmaxf(hi, v); }
+        }
+        if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
+        k[i] = (y >= 0 && y < N) ? acc : 0.0f;
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const float fm1 = k[c], f0 = k[c + 1], fp1 = k[c + 2], fp2 = k[c + 3];
+        const float d1 = fmaf(-2.0f, fm1, fmaf(-3.0f, f0, fmaf(6.0f, fp1, -fp2)));
+        const float d2 = (fm1 + fp1) - 2.0f * f0;
+        const float incr = fmaf(fp_b, f0, fmaf(c1p[c], d1, c2 * d2));
+        out[c] = f0 + incr;
+    }
+}
+
 // ---------------------------------------------------------------- rotation of a range of rows
 // Thread = column y; rows r0..r1-1 (local indices) of bufA -> bufB.  aA / aB: shared addresses of
 // bufA[row 0][CL_PAD + y - O0] and bufB[row 0][CL_PAD + y].  Rows are taken in chunks of ORDER:
@@ -339,7 +406,7 @@ struct Rotator {
 // from every CTA, which each CTA sends after it has consumed rho(t); halo(t+1) and part(t+1) are
 // sent after rho(t+1) has arrived from every CTA, which each CTA sends after it has consumed
 // halo(t) and part(t).
-template <int ORDER, int N>
+template <int ORDER, int N, bool MANH = false>
 __global__ void __launch_bounds__(CL_THREADS, 1)
 k_cluster_step(GridConst G, ClusterArgs A)
 {
@@ -385,6 +452,15 @@ k_cluster_step(GridConst G, ClusterArgs A)
         asm volatile("" : "+r"(rot.aA), "+r"(rot.aB));      // opaque: do not re-derive per use
     }
 
+    // ---- Manhattan drift: shift of this thread's column and its weights (un-scaled)
+    int mmq = 0;
+    float lq[ORDER];
+    {
+        float tq;
+        floor_frac(G.mh_q * ((float)y + G.y0c), mmq, tq);
+        lagrange<ORDER>(tq, lq);
+    }
+
     // ---- kick / Fokker-Planck: lane = granules g = 4*lane + 128*k of one row per warp
     const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
     const float yc = 0.5f * (float)(N - 1), xc = 0.5f * (float)(N - 1);
@@ -427,7 +503,25 @@ k_cluster_step(GridConst G, ClusterArgs A)
             }
             if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 0] = clock64();
             // ================= 1. rotation: bufA -> bufB
-            if (!last) rot.run(rbeg, rend, x0);
+            if (!last) {
+                if constexpr (MANH) {
+                    // Manhattan drift (L136): column y shifted along q by mh_q * Y cells -- one 1-D
+                    // interpolation with per-column weights; the taps of row r are the rows
+                    // r + mmq - O0 .. r + mmq - O0 + ORDER - 1 of bufA (|shift| <= the halo, as for
+                    // the standard rotation)
+                    uint32_t src = sA + (uint32_t)(((rbeg + H + mmq - O0) * PITCH + CL_PAD + y) * 4);
+                    uint32_t dstb = sB + (uint32_t)((rbeg * PITCH + CL_PAD + y) * 4);
+                    for (int r = rbeg; r < rend; ++r) {
+                        float acc = lq[0] * lds(src);
+#pragma unroll
+                        for (int i = 1; i < ORDER; ++i) acc = fmaf(lq[i], lds(src + i * PITCH * 4), acc);
+                        sts(dstb, acc);
+                        src += PITCH * 4; dstb += PITCH * 4;
+                    }
+                } else {
+                    rot.run(rbeg, rend, x0);
+                }
+            }
             if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 1] = clock64();
             __syncthreads();
             if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 2] = clock64();
@@ -522,6 +616,13 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 lagrange<ORDER>(t, l);
 #pragma unroll
                 for (int j = 0; j < ORDER; ++j) l[j] *= sc;
+                int mm1 = 0;
+                float l1[ORDER];
+                if constexpr (MANH) {
+                    float t1;
+                    floor_frac(G.mh_p * ((float)x + G.x0c), mm1, t1);
+                    lagrange<ORDER>(t1, l1);
+                }
                 const uint32_t row = sB + (uint32_t)((r * PITCH + CL_PAD) * 4);
                 const uint32_t orow = sA + (uint32_t)(((r + H) * PITCH + CL_PAD) * 4);
                 // halo pushes: the first H rows go to rank-1's lower halo, the last H to rank+1's upper
@@ -535,6 +636,27 @@ k_cluster_step(GridConst G, ClusterArgs A)
                     const int g = 4 * lane + 128 * k;
                     if (g < N) {
                         float o[4];
+                        if constexpr (MANH) {
+                            // RF kick (shift mh_p * X cells, weights l1) then wake kick, both along p
+                            if (mm >= -2 && mm <= 0 && mm1 >= -2 && mm1 <= 1) {
+                                const float4 z4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                                const float4 v0 = (g >= 4) ? lds4(row + (g - 8) * 4) : z4;
+                                const float4 v1 = lds4(row + (g - 4) * 4), v2 = lds4(row + g * 4), v3 = lds4(row + (g + 4) * 4);
+                                const float4 v4 = (g <= N - 8) ? lds4(row + (g + 8) * 4) : z4;
+                                const float a[20] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w, v2.x, v2.y,
+                                                     v2.z, v2.w, v3.x, v3.y, v3.z, v3.w, v4.x, v4.y, v4.z, v4.w};
+                                float rr[12];
+                                if (mm1 == 0) rf_stage<ORDER, 0>(a, l1, g, N, rr);
+                                else if (mm1 == -1) rf_stage<ORDER, -1>(a, l1, g, N, rr);
+                                else if (mm1 == 1) rf_stage<ORDER, 1>(a, l1, g, N, rr);
+                                else rf_stage<ORDER, -2>(a, l1, g, N, rr);
+                                if (mm == 0) kick_fp_granule<ORDER, 0>(rr, l, g, N, G.fp_b, c2, c1p[k], o);
+                                else if (mm == -1) kick_fp_granule<ORDER, -1>(rr, l, g, N, G.fp_b, c2, c1p[k], o);
+                                else kick_fp_granule<ORDER, -2>(rr, l, g, N, G.fp_b, c2, c1p[k], o);
+                            } else {
+                                rf_kick_fp_granule_any<ORDER>(bufB + r * PITCH + CL_PAD, l1, mm1, l, mm, g, N, G.fp_b, c2, c1p[k], o);
+                            }
+                        } else
                         if (mm >= -2 && mm <= 0) {
                             float b[12];
                             const float4 v0 = lds4(row + (g - 4) * 4), v1 = lds4(row + g * 4), v2 = lds4(row + (g + 4) * 4);

@@ -414,72 +414,8 @@ k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wf
     }
 }
 
-// Manhattan rotation, second half (RF kick): psi_B(x, y) = psi_A(x, y + s1),
-// s1 = mh_p * X cells, for the 12 columns g-4 .. g+7 that the wake kick of the granule g..g+3
-// reads.  a[i] = psi_A(x, g - 8 + i), i = 0..19; MM1 = floor(s1) (compile time), l1 = weights of
-// its fraction; columns outside the grid are zero before and after (A8).
-template <int ORDER, int MM1, bool CLAMP = false>
-__device__ __forceinline__ void rf_stage(const float (&a)[20], const float (&l1)[ORDER], int g, int N, float (&r)[12])
-{
-    constexpr int O0 = (ORDER - 1) / 2;
-#pragma unroll
-    for (int i = 0; i < 12; ++i) {
-        const int i0 = i + 4 + MM1 - O0;
-        float acc = l1[0] * a[i0];
-#pragma unroll
-        for (int j = 1; j < ORDER; ++j) acc = fmaf(l1[j], a[i0 + j], acc);
-        if (CLAMP) acc = fminf(fmaxf(acc, fminf(a[i0 + O0], a[i0 + O0 + 1])), fmaxf(a[i0 + O0], a[i0 + O0 + 1]));
-        const int y = g - 4 + i;
-        r[i] = (y >= 0 && y < N) ? acc : 0.0f;
-    }
-}
-// any integer parts: psi_B at column s of the row (bounds-checked loads), and the whole granule
-template <int ORDER, bool CLAMP = false>
-__device__ __forceinline__ float rf_value(const float *row, int N, int s, int mm1, const float (&l1)[ORDER])
-{
-    constexpr int O0 = (ORDER - 1) / 2;
-    if (s < 0 || s >= N) return 0.0f;
-    float acc = 0.0f, lo = 0.0f, hi = 0.0f;
-#pragma unroll
-    for (int j = 0; j < ORDER; ++j) {
-        const int c = s + mm1 - O0 + j;
-        const float v = (c >= 0 && c < N) ? row[c] : 0.0f;
-        acc = fmaf(l1[j], v, acc);
-        if (j == O0) { lo = v; hi = v; }
-        if (j == O0 + 1) { lo = fminf(lo, v); hi = fmaxf(hi, v); }
-    }
-    if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
-    return acc;
-}
-template <int ORDER, bool CLAMP = false>
-__device__ __noinline__ void rf_kick_fp_granule_any(const float *row, const float (&l1)[ORDER], int mm1,
-                                                    const float (&l2)[ORDER], int mm2, int g, int N, float fp_b,
-                                                    float c2, const float (&c1p)[4], float (&out)[4])
-{
-    constexpr int O0 = (ORDER - 1) / 2;
-    float k[7];
-#pragma unroll 1
-    for (int i = 0; i < 7; ++i) {
-        const int y = g - 1 + i;
-        float acc = 0.0f, lo = 0.0f, hi = 0.0f;
-        for (int j = 0; j < ORDER; ++j) {
-            const float v = rf_value<ORDER, CLAMP>(row, N, y + mm2 - O0 + j, mm1, l1);
-            acc = fmaf(l2[j], v, acc);
-            if (j == O0) { lo = v; hi = v; }
-            if (j == O0 + 1) { lo = fminf(lo, v); hi = fmaxf(hi, v); }
-        }
-        if (CLAMP) acc = fminf(fmaxf(acc, lo), hi);
-        k[i] = (y >= 0 && y < N) ? acc : 0.0f;
-    }
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        const float fm1 = k[c], f0 = k[c + 1], fp1 = k[c + 2], fp2 = k[c + 3];
-        const float d1 = fmaf(-2.0f, fm1, fmaf(-3.0f, f0, fmaf(6.0f, fp1, -fp2)));
-        const float d2 = (fm1 + fp1) - 2.0f * f0;
-        const float incr = fmaf(fp_b, f0, fmaf(c1p[c], d1, c2 * d2));
-        out[c] = f0 + incr;
-    }
-}
+// (rf_stage, rf_value, rf_kick_fp_granule_any: the RF-kick stage of the Manhattan rotation, live in
+// vfps_cluster.cuh beside kick_fp_granule)
 
 // ---------------------------------------------------------------- a2 for Manhattan + clamp
 // The RF kick is a shift along p and leaves the profile alone -- unless its interpolation is

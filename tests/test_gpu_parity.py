@@ -373,15 +373,12 @@ def test_manhattan_rotation(vfps, orc, order, N, wake):
     """VFPS_FLAG_ROT_MANHATTAN (drift along q, RF kick along p) against the oracle's
     Manhattan step: asymmetric box, off-centre bunch, free-space wake, 300 steps per period (the
     drift and the RF kick move the outer lines by more than one cell: integer parts -2..1), stream
-    engine for 1 step, graph engine for 59 more, grid engine for 20 more; the cluster engine
-    refuses the flag."""
+    engine for 1 step, graph engine for 59 more, grid engine for 20 more, then the cluster engine
+    (scalar kernel) at several cluster sizes."""
     Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
     psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
     flags = vfps.FLAG_RENORMALISE | vfps.FLAG_ROT_MANHATTAN
     sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, 1, Z=Z, flags=flags)
-    with pytest.raises(vfps.VfpsError) as e:
-        sim.set_engine(vfps.ENGINE_CLUSTER)
-    assert e.value.code == -5
     sim.set_wake_mode({"fft": vfps.WAKE_FFT, "direct": vfps.WAKE_DIRECT}[wake])
     sim.set_engine(vfps.ENGINE_STREAM)
     sim.set_psi_host(psi0)
@@ -397,13 +394,32 @@ def test_manhattan_rotation(vfps, orc, order, N, wake):
     assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"manhattan N={N} order={order} 60 steps")
     for i in (0, 30, 58):
         assert_diag(d[i, 0], dr[i])
-    sim.set_engine(vfps.ENGINE_AUTO)                 # no cluster engine with this flag: the grid engine
-    assert sim.engine_name == "grid"
+    sim.set_engine(vfps.ENGINE_GRID)
     d = sim.step_host(20)
     dr = o.step(20)
     assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"manhattan N={N} order={order} 80 steps, grid engine")
     for i in (0, 19):
         assert_diag(d[i, 0], dr[i])
+    try:
+        sim.set_engine(vfps.ENGINE_CLUSTER)          # scalar kernel; needs halo <= 4 rows (not N = 256 here)
+    except vfps.VfpsError as err:
+        assert err.code == -5 and N == 256
+        sim.close()
+        return
+    assert sim.engine_name == "cluster" and sim.cluster_kernel == 1
+    for S in (16, 4, 1):
+        try:
+            sim.set_cluster_size(S)
+        except vfps.VfpsError:
+            continue
+        d = sim.step_host(20)
+        dr = o.step(20)
+        assert_psi(sim.get_psi_host()[0], o.psi, 2e-4, f"manhattan N={N} order={order}, cluster engine S={S}")
+        for i in (0, 19):
+            assert_diag(d[i, 0], dr[i])
+    with pytest.raises(vfps.VfpsError) as e:
+        sim.set_cluster_kernel(2)                    # the packed kernel has the standard rotation only
+    assert e.value.code == -5
     sim.close()
 
 
