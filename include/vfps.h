@@ -115,7 +115,8 @@ enum {
                                  barriers where the step has global dependencies (members = 1)   */
 };
 enum {
-    VFPS_WAKE_AUTO = 0,
+    VFPS_WAKE_AUTO = 0,       /* DIRECT (the CLUSTER and GRID engines always; STREAM / GRAPH with the
+                                 second-generation kernels), FFT with the first generation      */
     VFPS_WAKE_FFT = 1,        /* zero-padded length-Nf FFT, x Z, inverse FFT, every step (Eq. 5) */
     VFPS_WAKE_DIRECT = 2      /* w = Re IDFT(Z) once at create; V = w * rho by direct convolution
                                  (Eq. 4) -- identical result, no serial FFT chain per step  */

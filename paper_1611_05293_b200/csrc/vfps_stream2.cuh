@@ -5,9 +5,11 @@
 // bounds checks, 16 shared loads and one 5-step warp reduction per cell); k_kick_fp 26 us with
 // 12 % of the warp slots (132 KB of staged rows per CTA = one CTA of 8 warps per SM);
 // k_wake_fft 44.5 us on ONE SM (24 serial FFT stages with global twiddle loads).  Here:
-//   k_rotate2      a1 + a2: thread = column, walks down RT rows with a sliding ORDER x ORDER
-//                  register window fed by global loads that hit L1 (no staging, no bounds checks
-//                  away from the grid edge); row sums by an 8-value transposed warp reduction
+//   k_rotate2      a1 + a2: thread = column, 8 rows at a time from a register window of
+//                  (8 + ORDER - 1) x ORDER taps fed by global loads that hit L1 (no staging, no
+//                  bounds checks away from the grid edge; clamped loads at the edge); row sums by
+//                  an 8-value transposed warp reduction
+//   k_drift2       a1' first half of the Manhattan rotation (1-D shift along q) + a2
 //   k_wake_direct  a3 by direct convolution (Eq. 4) on N/8 CTAs instead of one (the profile is
 //                  completed by the last CTA of every row of rotation tiles)
 //   k_kick_fp2     a4 + a5 + a6: four cells per thread in registers (12-value window, three
@@ -63,21 +65,15 @@ __device__ __forceinline__ float ldg_nc(const float *p)
     asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
     return v;
 }
-// the same through the coherent path, for data other CTAs wrote earlier in the same kernel
-__device__ __forceinline__ float ldg_co(const float *p)
-{
-    float v;
-    asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
-    return v;
-}
-
 // ---------------------------------------------------------------- a1 + a2: rotation + projection
 // grid = (tiles_x * tiles_y, members), block = 256.  Tile = R2_RT rows x 256 columns; thread =
 // column y, rows tx0 .. tx0 + R2_RT - 1 in groups of 8.  Taps come straight from global memory
 // (a warp reads 128 contiguous bytes per tap; the four taps of a row and the next warp's overlap
 // hit L1).  Fast path (warp-uniform): every tap of the group lies inside the grid and floor(dx),
-// floor(dy) do not change along the group for any lane -> sliding register window, ORDER loads per
-// cell.  Otherwise every cell loads its own window with per-tap range checks (psi = 0 outside, A8).
+// floor(dy) do not change along the group for any lane -> one register window for the 8 rows,
+// (8 + ORDER - 1) * ORDER / 8 loads per cell.  Groups at the grid edge load clamped addresses and
+// zero the outside taps; groups where a floor changes load every cell's own window with per-tap
+// range checks (psi = 0 outside, A8).
 // rho_part[m][x][tile_y] = dp * scale * sum over the tile's columns of psi'(x, .)
 // NC: psi is read-only for the whole kernel (ld.global.nc); CLAMP: Eq. 14 (reading A9) -- the
 // interpolated value is limited to the interval of the 2 x 2 nodes around the source point
