@@ -201,7 +201,8 @@ k_project(GridConst G, const float *__restrict__ psi, const float *__restrict__ 
 
 // ---------------------------------------------------------------- a3: wake by FFT (Eq. 5)
 // One CTA per member, blockDim = min(1024, Nf/2).  Complex radix-2 FFT of length Nf in shared
-// memory: forward decimation-in-frequency (natural in, bit-reversed out), multiply by the
+// memory (two radix-2 stages per pass in registers): forward decimation-in-frequency (natural in,
+// bit-reversed out), multiply by the
 // Hermitian-extended impedance at the bit-reversed positions, inverse decimation-in-time
 // (bit-reversed in, natural out) -- no permutation pass.  tw[j] = exp(-2 pi i j/Nf), j < Nf/2.
 // Outputs: rho[m][x] (summed partials), V[m][x], qstat[m] = { sum rho, sum Xc rho, sum Xc^2 rho,
@@ -244,14 +245,31 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_pa
             stw[j] = __ldg(tw + pos * ((Nf >> 1) / half));
         }
         __syncthreads();
-        for (int half = Nf >> 1; half >= 1; half >>= 1) {       // forward, DIF
-            const float2 *wst = stw + (half - 1);
+        // forward, decimation in frequency; two radix-2 stages (spans 2q and q) per pass in registers:
+        // half as many passes over shared memory and half as many barriers
+        int half = Nf >> 1;
+        for (; half >= 2; half >>= 2) {
+            const int q = half >> 1;
+            const float2 *w2 = stw + (half - 1), *w1 = stw + (q - 1);
+            for (int j = tid; j < (Nf >> 2); j += nt) {
+                const int pos = j & (q - 1), i0 = ((j - pos) << 2) + pos, i1 = i0 + q, i2 = i1 + q, i3 = i2 + q;
+                const float2 x0 = s[i0], x1 = s[i1], x2 = s[i2], x3 = s[i3];
+                const float2 u0 = make_float2(x0.x + x2.x, x0.y + x2.y), u1 = make_float2(x1.x + x3.x, x1.y + x3.y);
+                const float2 u2 = cmul(make_float2(x0.x - x2.x, x0.y - x2.y), w2[pos]);
+                const float2 u3 = cmul(make_float2(x1.x - x3.x, x1.y - x3.y), w2[pos + q]);
+                const float2 wq = w1[pos];
+                s[i0] = make_float2(u0.x + u1.x, u0.y + u1.y);
+                s[i1] = cmul(make_float2(u0.x - u1.x, u0.y - u1.y), wq);
+                s[i2] = make_float2(u2.x + u3.x, u2.y + u3.y);
+                s[i3] = cmul(make_float2(u2.x - u3.x, u2.y - u3.y), wq);
+            }
+            __syncthreads();
+        }
+        if (half == 1) {                                          // odd log2(Nf): one radix-2 stage left (w = 1)
             for (int j = tid; j < (Nf >> 1); j += nt) {
-                const int pos = j & (half - 1);
-                const int i0 = ((j - pos) << 1) + pos, i1 = i0 + half;
-                const float2 u = s[i0], v = s[i1];
-                s[i0] = make_float2(u.x + v.x, u.y + v.y);
-                s[i1] = cmul(make_float2(u.x - v.x, u.y - v.y), wst[pos]);
+                const float2 u = s[2 * j], v = s[2 * j + 1];
+                s[2 * j] = make_float2(u.x + v.x, u.y + v.y);
+                s[2 * j + 1] = make_float2(u.x - v.x, u.y - v.y);
             }
             __syncthreads();
         }
@@ -270,16 +288,33 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_pa
             s[i] = cmul(R, z);
         }
         __syncthreads();
-        for (int half = 1; half <= (Nf >> 1); half <<= 1) {     // inverse, DIT
-            const float2 *wst = stw + (half - 1);
+        // inverse, decimation in time, mirrored: the single radix-2 stage first if log2(Nf) is odd,
+        // then spans q and 2q per pass
+        int hq = 1;
+        if (log2Nf & 1) {
             for (int j = tid; j < (Nf >> 1); j += nt) {
-                const int pos = j & (half - 1);
-                const int i0 = ((j - pos) << 1) + pos, i1 = i0 + half;
-                float2 w = wst[pos];
-                w.y = -w.y;
-                const float2 u = s[i0], v = cmul(s[i1], w);
-                s[i0] = make_float2(u.x + v.x, u.y + v.y);
-                s[i1] = make_float2(u.x - v.x, u.y - v.y);
+                const float2 u = s[2 * j], v = s[2 * j + 1];
+                s[2 * j] = make_float2(u.x + v.x, u.y + v.y);
+                s[2 * j + 1] = make_float2(u.x - v.x, u.y - v.y);
+            }
+            __syncthreads();
+            hq = 2;
+        }
+        for (int q = hq; q <= (Nf >> 2); q <<= 2) {
+            const float2 *w1 = stw + (q - 1), *w2 = stw + (2 * q - 1);
+            for (int j = tid; j < (Nf >> 2); j += nt) {
+                const int pos = j & (q - 1), i0 = ((j - pos) << 2) + pos, i1 = i0 + q, i2 = i1 + q, i3 = i2 + q;
+                float2 wq = w1[pos], wa = w2[pos], wb = w2[pos + q];
+                wq.y = -wq.y; wa.y = -wa.y; wb.y = -wb.y;
+                const float2 x0 = s[i0], x2 = s[i2];
+                const float2 v1 = cmul(s[i1], wq), v3 = cmul(s[i3], wq);
+                const float2 y0 = make_float2(x0.x + v1.x, x0.y + v1.y), y1 = make_float2(x0.x - v1.x, x0.y - v1.y);
+                const float2 y2 = make_float2(x2.x + v3.x, x2.y + v3.y), y3 = make_float2(x2.x - v3.x, x2.y - v3.y);
+                const float2 t2 = cmul(y2, wa), t3 = cmul(y3, wb);
+                s[i0] = make_float2(y0.x + t2.x, y0.y + t2.y);
+                s[i2] = make_float2(y0.x - t2.x, y0.y - t2.y);
+                s[i1] = make_float2(y1.x + t3.x, y1.y + t3.y);
+                s[i3] = make_float2(y1.x - t3.x, y1.y - t3.y);
             }
             __syncthreads();
         }
