@@ -56,11 +56,13 @@ k_grid_step(GridConst G, GridArgs A)
     cg::grid_group grid = cg::this_grid();
     extern __shared__ float gsm[];
     __shared__ float red[8][GR_WARPS];
+    __shared__ float redt[2][8][GR_WARPS];     // rotation tiles: two buffers, one barrier per tile
     __shared__ float s_sc;
     const int N = G.N, NQ = N >> 2, lgNQ = 31 - __clz(NQ);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     float *srho = gsm, *sw = gsm + N, *sV = gsm + 2 * N + A.KR;       // sw: N + KR - 1 lags
     const int tiles_x = (N + GR_RT - 1) / GR_RT, ntiles = tiles_x * A.tiles_y;
+    const int lg_ty = 31 - __clz(A.tiles_y);           // tiles_y is a power of two (N is; 256 columns per tile)
     const float yc = 0.5f * (float)(N - 1);
     const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
     float sc = G.renorm ? A.scale[0] : 1.0f;
@@ -73,9 +75,11 @@ k_grid_step(GridConst G, GridArgs A)
         // own the edge columns -- clamped-load path -- are slower in every round and everybody
         // waits for them at the barrier.)
         for (int k = 0, tb = 0; tb < ntiles; ++k, tb += gridDim.x) {
-            const int t = tb + (int)((blockIdx.x + k) % gridDim.x);
+            int rot_c = (int)blockIdx.x + k;
+            while (rot_c >= (int)gridDim.x) rot_c -= (int)gridDim.x;
+            const int t = tb + rot_c;
             if (t >= ntiles) continue;
-            const int xg = (t / A.tiles_y) * GR_RT, ty = t % A.tiles_y;
+            const int xg = (t >> lg_ty) * GR_RT, ty = t & (A.tiles_y - 1);
             const int y = ty * (32 * GR_WARPS) + warp * 32 + lane;
             float out[8];
 #pragma unroll
@@ -126,23 +130,33 @@ k_grid_step(GridConst G, GridArgs A)
                     for (int r = 0; r < 8; ++r) out[r] = rot.cell_checked(min(xg + r, N - 1));
                 }
                 }
+                float *orow = A.psi_tmp + (size_t)xg * N + y;
+                if (__all_sync(FULL, y < N) && xg + 8 <= N) {           // whole 8 x 32 patch inside the grid
 #pragma unroll
-                for (int r = 0; r < 8; ++r) {
-                    out[r] *= sc;
-                    if (y < N && xg + r < N) A.psi_tmp[(size_t)(xg + r) * N + y] = out[r];
-                    else out[r] = 0.0f;
+                    for (int r = 0; r < 8; ++r) {
+                        out[r] *= sc;
+                        *orow = out[r];
+                        orow += N;
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) {
+                        out[r] *= sc;
+                        if (y < N && xg + r < N) orow[(size_t)r * N] = out[r];
+                        else out[r] = 0.0f;
+                    }
                 }
             }
+            // (buffer k & 1 was last read two tiles ago, i.e. before the barrier of the previous tile)
             const float tot = warp_reduce8(out, lane);
-            if ((lane & 3) == 0) red[((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
+            if ((lane & 3) == 0) redt[k & 1][((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
             __syncthreads();
             if (tid < GR_RT && xg + tid < N) {
                 float s = 0.0f;
 #pragma unroll
-                for (int w = 0; w < GR_WARPS; ++w) s += red[tid][w];
+                for (int w = 0; w < GR_WARPS; ++w) s += redt[k & 1][tid][w];
                 A.rho_part[(size_t)ty * N + xg + tid] = G.dp * s;
             }
-            __syncthreads();
         }
         if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 1] = clock64();
         grid.sync();
