@@ -220,9 +220,11 @@ __device__ __forceinline__ void rf_stage(const float (&a)[20], const float (&l1)
 #pragma unroll
         for (int j = 1; j < ORDER; ++j) acc = fmaf(l1[j], a[i0 + j], acc);
         if (CLAMP) acc = fminf(fmaxf(acc, fminf(a[i0 + O0], a[i0 + O0 + 1])), fmaxf(a[i0 + O0], a[i0 + O0 + 1]));
-        const int y = g - 4 + i;
-        r[i] = (y >= 0 && y < N) ? acc : 0.0f;
+        r[i] = acc;
     }
+    // columns g-4 .. g-1 lie outside the grid only for the first granule, g+4 .. g+7 only for the last
+    if (g == 0) { r[0] = 0.0f; r[1] = 0.0f; r[2] = 0.0f; r[3] = 0.0f; }
+    if (g == N - 4) { r[8] = 0.0f; r[9] = 0.0f; r[10] = 0.0f; r[11] = 0.0f; }
 }
 // any integer parts: psi_B at column s of the row (bounds-checked loads), and the whole granule
 template <int ORDER, bool CLAMP = false>
