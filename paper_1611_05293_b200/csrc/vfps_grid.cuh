@@ -41,6 +41,8 @@ struct GridArgs {
     int nsteps;
     int tiles_y;         // column tiles of 256
     int KR;              // rows per CTA in phase 2
+    unsigned long long *qacc;   // [2] charge of the step in 32.32 fixed point (integer atomics: exact,
+                                // order-independent), zero at launch; parity = step & 1
     long long *dbg;      // nullptr, or [CTA][64 steps][8] clock64 stamps (debug aid)
 };
 
@@ -305,25 +307,32 @@ k_grid_step(GridConst G, GridArgs A)
 #pragma unroll
             for (int w = 0; w < GR_WARPS; ++w) s += red[tid][w];
             A.mom_part[(size_t)tid * gridDim.x + blockIdx.x] = s;
+            // the charge also goes into one 64-bit fixed-point accumulator: after the barrier every CTA
+            // needs just one load for 1/C (re-reading gridDim.x partials from every CTA at once cost
+            // 3-4 k cycles per step); integer addition is associative, so the sum is deterministic
+            if (tid == 0) atomicAdd(A.qacc + (step & 1), (unsigned long long)__float2ll_rn(s * 4294967296.0f));
         }
         if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 5] = clock64();
         grid.sync();
         if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 6] = clock64();
         // ================= phase 3: a6 -- every CTA forms C and 1/C in the same fixed order
-        // Every CTA needs only the charge (one coalesced pass over gridDim.x floats, all loads in
-        // flight); warp w < 6 of CTA 0 also sums partial w for the diagnostics row.  fp32 sums in a
-        // fixed order (fp64 adds and shuffles cost ~10 us per step on B200), fp64 for the scalars.
+        // Every CTA needs only the charge: one load of the fixed-point accumulator.  Warps 1-5 of
+        // CTA 0 sum the other partials for the diagnostics row (fp32, fixed order).
         __shared__ float s_tot[6];
-        if (warp == 0 || (blockIdx.x == 0 && warp < 6)) {
+        if (tid == 0) {
+            const long long q = (long long)__ldcg(A.qacc + (step & 1));
+            const float f = (float)((double)q * (1.0 / 4294967296.0));
+            s_tot[0] = f;
+            s_sc = G.renorm ? 1.0f / ((G.dq * G.dp) * f) : 1.0f;
+            if (blockIdx.x == 0) A.qacc[(step + 1) & 1] = 0ull;      // nobody touches it before the next barrier
+        }
+        if (blockIdx.x == 0 && warp >= 1 && warp < 6) {              // the other sums, for the diagnostics row
             const float *mp = A.mom_part + (size_t)warp * gridDim.x;
             float f = 0.0f;
 #pragma unroll 8
             for (int i = lane; i < (int)gridDim.x; i += 32) f += __ldcg(mp + i);
             f = warp_sum(f);
-            if (lane == 0) {
-                s_tot[warp] = f;
-                if (warp == 0) s_sc = G.renorm ? 1.0f / ((G.dq * G.dp) * f) : 1.0f;
-            }
+            if (lane == 0) s_tot[warp] = f;
         }
         __syncthreads();
         if (blockIdx.x == 0 && tid == 0 && A.diag != nullptr) {
