@@ -12,8 +12,9 @@
 //            its KR rows: a3 direct-convolution wake (Eq. 4), a4 + a5 kick and Fokker-Planck in
 //            registers (as k_kick_fp2), partial sums for a6 -> mom_part[cta]
 //   -- grid barrier --
-//   phase 3  every CTA adds the partial sums of all CTAs in the same fixed order -> C, 1/C;
-//            CTA 0 writes the diagnostics row.
+//   phase 3  every CTA reads the charge of the step from a 32.32 fixed-point accumulator that the
+//            CTAs fed with integer atomics in phase 2 (exact, order-independent) -> C, 1/C;
+//            CTA 0 sums the other partial sums in a fixed order and writes the diagnostics row.
 // With VFPS_FLAG_ROT_MANHATTAN (template MANH) phase 1 is the drift (1-D shift along q) and phase 2
 // applies the RF kick before the wake kick (vfps_stream2.cuh: k_drift2, rf_stage).
 // Template CLAMP: clamped interpolation (Eq. 14, reading A9) in every interpolation of the step.
