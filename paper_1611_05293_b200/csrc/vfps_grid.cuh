@@ -2,7 +2,7 @@
 //
 // The streaming engines pay three kernel launches per split step; at 2048^2 each kernel has
 // ~5-10 us of work and 3-5 us of ramp-up, tail and (for the reductions) a serial last-CTA epilogue
-// (profiles/r01_c4_stream.md).  Here ONE cooperative launch advances all n steps of a vfps_step
+// (profiles/r01_c4_grid_and_stream.md).  Here ONE cooperative launch advances all n steps of a vfps_step
 // call: every SM keeps CTAs resident, psi ping-pongs between two HBM buffers that stay in the
 // 126 MB L2 (2 x 16 MB at 2048^2), and the two global dependencies of a step are grid barriers:
 //   phase 1  a1 + a2: rotation tiles of GR_RT rows x 256 columns (register window, as k_rotate2),

@@ -1,6 +1,6 @@
 // vfps_stream2.cuh -- second generation of the streaming (HBM / L2) kernels (sm_100a).
 //
-// ncu of the first generation at 2048^2 (profiles/r01_c4_stream.md): k_rotate 27.5 us, bound by
+// ncu of the first generation at 2048^2 (profiles/r01_c4_grid_and_stream.md): k_rotate 27.5 us, bound by
 // instruction issue (160 thread-instructions per cell, 79 % of the issue slots: tile staging with
 // bounds checks, 16 shared loads and one 5-step warp reduction per cell); k_kick_fp 26 us with
 // 12 % of the warp slots (132 KB of staged rows per CTA = one CTA of 8 warps per SM);
