@@ -168,14 +168,20 @@ k_grid_step(GridConst G, GridArgs A)
         const int r0 = blockIdx.x * A.KR, r1 = min(N, r0 + A.KR);
         float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 pw - -
         if (r0 < N) {
-            for (int x4 = tid; x4 < NQ; x4 += GR_THREADS) {       // all loads of a pass in flight at once
-                float4 r = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            for (int x4 = tid; x4 < NQ; x4 += 2 * GR_THREADS) {   // two columns of float4 per pass: up to
+                const int x4b = x4 + GR_THREADS;                   // 16 loads in flight per thread
+                const bool two = (x4b < NQ);
+                float4 r = make_float4(0.0f, 0.0f, 0.0f, 0.0f), q = r;
 #pragma unroll 8
                 for (int k = 0; k < A.tiles_y; ++k) {
-                    const float4 v = __ldcg(reinterpret_cast<const float4 *>(A.rho_part + (size_t)k * N) + x4);
+                    const float4 *pk = reinterpret_cast<const float4 *>(A.rho_part + (size_t)k * N);
+                    const float4 v = __ldcg(pk + x4);
+                    const float4 u = two ? __ldcg(pk + x4b) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
                     r.x += v.x; r.y += v.y; r.z += v.z; r.w += v.w;
+                    q.x += u.x; q.y += u.y; q.z += u.z; q.w += u.w;
                 }
                 *reinterpret_cast<float4 *>(srho + 4 * x4) = r;
+                if (two) *reinterpret_cast<float4 *>(srho + 4 * x4b) = q;
             }
             if (A.wfun != nullptr)
                 for (int i = tid; i < N + A.KR - 1; i += GR_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
