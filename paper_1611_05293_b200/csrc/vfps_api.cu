@@ -67,6 +67,7 @@ struct vfps_sim {
     size_t gr_smem = 0;
     float *gr_mom = nullptr;                     // [gr_blocks][GR_NPART]
     unsigned long long *gr_qacc = nullptr;       // [2] fixed-point charge accumulators
+    float *gr_zrow = nullptr;                    // [N] zeros
     std::string gr_why;
     unsigned *tilectr = nullptr;                 // [members][tiles_x2], zero between launches
     size_t rot_smem = 0, kfp_smem = 0, fft_smem = 0;
@@ -451,7 +452,7 @@ int launch_grid_steps(vfps_sim *h, int n, float *diag)
     GridArgs A{};
     A.psi = h->psi; A.psi_tmp = h->psi_tmp; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr;
     A.rho_part = h->rho_part; A.mom_part = h->gr_mom; A.diag = diag; A.nsteps = n;
-    A.tiles_y = h->tiles_y2; A.KR = h->gr_KR; A.qacc = h->gr_qacc;
+    A.tiles_y = h->tiles_y2; A.KR = h->gr_KR; A.qacc = h->gr_qacc; A.zrow = h->gr_zrow;
     if (cudaMemsetAsync(h->gr_qacc, 0, 2 * sizeof(unsigned long long), h->stream) != cudaSuccess)
         return fail(h, VFPS_ERR_CUDA, "cudaMemsetAsync failed");
     void *args[2] = {(void *)&h->G, (void *)&A};
@@ -726,6 +727,10 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     grid_configure(h);
     if (h->gr_blocks > 0) CUB(dalloc(h, &h->gr_mom, (size_t)h->gr_blocks * GR_NPART));
     if (h->gr_blocks > 0) CUB(dalloc(h, &h->gr_qacc, (size_t)2));
+    if (h->gr_blocks > 0) {
+        CUB(dalloc(h, &h->gr_zrow, (size_t)N));
+        CUB(cudaMemsetAsync(h->gr_zrow, 0, (size_t)N * sizeof(float), h->stream));
+    }
     cudaError_t e = cudaSuccess;
     switch (p->interp_order) {
         case 2: e = set_kernel_attrs<2>(h); break;

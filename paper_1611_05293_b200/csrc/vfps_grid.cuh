@@ -42,6 +42,7 @@ struct GridArgs {
     int nsteps;
     int tiles_y;         // column tiles of 256
     int KR;              // rows per CTA in phase 2
+    const float *zrow;          // N zeros: stands in for the rows outside the grid (A8)
     unsigned long long *qacc;   // [2] charge of the step in 32.32 fixed point (integer atomics: exact,
                                 // order-independent), zero at launch; parity = step & 1
     long long *dbg;      // nullptr, or [CTA][64 steps][8] clock64 stamps (debug aid)
@@ -126,6 +127,8 @@ k_grid_step(GridConst G, GridArgs A)
                 const bool inside = (sx >= 0) && (sx + 7 + ORDER - 1 < N) && (sy >= 0) && (sy + ORDER - 1 < N);
                 if (__all_sync(FULL, uni && inside)) {
                     rot.group8(A.psi + (size_t)sx * N + sy, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
+                } else if (__all_sync(FULL, uni && (sy >= 0) && (sy + ORDER - 1 < N))) {
+                    rot.group8_rows(sx, sy, A.zrow, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
                 } else if (__all_sync(FULL, uni)) {
                     rot.group8_edge(sx, sy, X0, rx0 - CL_MAGIC, ry0 - CL_MAGIC, out);
                 } else {

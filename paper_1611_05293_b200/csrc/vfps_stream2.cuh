@@ -155,6 +155,22 @@ struct GRot {
         }
         interp8(t, X0, fx, fy, out);
     }
+    // as group8 for a group at the top or bottom edge of the grid whose columns all lie inside:
+    // rows outside the grid are read from a row of zeros (zrow, at least N floats) -- no per-tap
+    // clamping or selection
+    __device__ __forceinline__ void group8_rows(int sx, int sy, const float *zrow, float X0, float fx, float fy,
+                                                float (&out)[8]) const
+    {
+        float t[8 + ORDER - 1][ORDER];
+#pragma unroll
+        for (int i = 0; i < 8 + ORDER - 1; ++i) {
+            const int xx = sx + i;
+            const float *p = ((xx >= 0 && xx < N) ? src + (size_t)xx * N : zrow) + sy;
+#pragma unroll
+            for (int j = 0; j < ORDER; ++j) t[i][j] = ld(p + j);
+        }
+        interp8(t, X0, fx, fy, out);
+    }
     // rows r = 0..7 from the taps t[r .. r+ORDER-1][.]
     __device__ __forceinline__ void interp8(const float (&t)[8 + ORDER - 1][ORDER], float X0, float fx, float fy,
                                             float (&out)[8]) const
