@@ -228,6 +228,34 @@ def test_kick_sign_energy_loss(orc):
     assert orc.moments(out, -L, L, -L, L)[2] < -1e-3
 
 
+# ---------------------------------------------------------------- O2 projection (L56)
+def test_projection_is_the_marginal_over_p(orc):
+    """rho_x = dp * sum_y psi(x, y) ("bunch profile"), pinned without the oracle on
+    the other side: (i) a separable psi = f(x) g(y) with asymmetric, different f and g has the
+    profile dp * f(x) * sum(g) -- a sum over x instead of y, or dq in place of dp, fails;
+    (ii) the marginal of a bivariate Gaussian with sigma_q != sigma_p on a box with dq != dp is
+    the 1-D Gaussian exp(-q^2 / 2 sigma_q^2) / (sqrt(2 pi) sigma_q) (the trapezoid sum of a
+    Gaussian over +-8 sigma is exact to rounding)."""
+    N = 24
+    x = np.arange(N, dtype=np.float64)
+    f = 1.0 + 0.3 * x + 0.01 * x ** 2                      # not symmetric, not equal to g
+    g = np.exp(-0.2 * x) * (2.0 + np.sin(0.7 * x))
+    psi = f[:, None] * g[None, :]
+    dp, dq = 0.37, 0.91
+    rho = orc.project(psi, dp)
+    np.testing.assert_allclose(rho, dp * f * g.sum(), rtol=1e-14)
+    wrong_axis = dp * g * f.sum()                          # what a transposed sum would give
+    assert np.max(np.abs(rho - wrong_axis)) > 0.1 * np.max(np.abs(rho))
+    assert np.max(np.abs(rho - dq * f * g.sum())) > 0.1 * np.max(np.abs(rho))
+    # (ii) closed-form marginal, non-square box and spacings
+    N, sq, sp = 96, 0.8, 1.3
+    q = grid_axis(N, -7.0, 6.0)
+    p = grid_axis(N, -10.4, 10.4)
+    psi = (np.exp(-0.5 * (q[:, None] / sq) ** 2 - 0.5 * (p[None, :] / sp) ** 2) / (TWO_PI * sq * sp))
+    rho = orc.project(psi, p[1] - p[0])
+    np.testing.assert_allclose(rho, np.exp(-0.5 * (q / sq) ** 2) / (math.sqrt(TWO_PI) * sq), rtol=0, atol=1e-13)
+
+
 # ---------------------------------------------------------------- wake: Eq. 4 == Eq. 5
 def test_wake_matches_library_fft_convolution(orc):
     """Direct convolution with w (Eq. 4) equals Re IDFT(Z . DFT(zero-padded rho)) (Eq. 5,
