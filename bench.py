@@ -61,12 +61,13 @@ def parse_args():
     ap.add_argument("--manhattan", action="store_true", help="Manhattan (symplectic) rotation instead of the standard one")
     ap.add_argument("--clamp", action="store_true", help="clamped interpolation (Eq. 14)")
     ap.add_argument("--stream-gen", type=int, default=0, help="streaming kernels: 0 auto, 1 first generation, 2 second")
-    ap.add_argument("--cluster-kernel", type=int, default=0, help="cluster engine kernel: 0 auto, 1 scalar, 2 packed fp32x2")
-    ap.add_argument("--cluster-threads", type=int, default=0, help="threads per CTA of the packed cluster kernel (0 = auto)")
+    ap.add_argument("--cluster-kernel", type=int, default=0, help="cluster engine kernel: 0 auto, 1 first design (k_cluster_step), 3 in-place design (k_onchip_step)")
     ap.add_argument("--members", type=int, default=0, help="batch members (0 = the workload's own count)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU-oracle sample budget")
+    ap.add_argument("--peaks", action="store_true",
+                    help="only run the on-chip / L2 / FMA micro-benchmarks (libvfps_peaks.so) and print them")
     return ap.parse_args()
 
 
@@ -80,6 +81,29 @@ def peaks():
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+PEAK_KEYS = ["sms", "smem_read_B_per_clk_sm", "smem_read_GBs", "smem_rw_B_per_clk_sm", "smem_rw_GBs",
+             "ffma_lanes_per_clk_sm", "ffma_G_per_s", "ffma2_lanes_per_clk_sm", "ffma2_G_per_s",
+             "ffma_with_lds_lanes_per_clk_sm", "l2_copy_16MB_GBs", "l2_copy_32MB_GBs", "l2_copy_64MB_GBs",
+             "hbm_copy_512MB_GBs", "sm_mhz_during_ffma", "ffma_shared_operands_lanes_per_clk_sm"]
+
+
+def measure_peaks():
+    """Run the micro-benchmarks of csrc/peaks/vfps_peaks.cu on the current device (a second or
+    two): measured shared-memory, L2 and FMA-pipe rates and resident clusters per cluster size."""
+    import ctypes
+    import paper_1611_05293_b200 as pkg
+    lib = ctypes.CDLL(pkg.build_peaks())
+    lib.vfps_peaks_measure.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+    lib.vfps_peaks_measure.restype = ctypes.c_int
+    out = (ctypes.c_double * 32)()
+    rc = lib.vfps_peaks_measure(out, 32)
+    if rc != 0:
+        raise RuntimeError(f"vfps_peaks_measure failed with CUDA error {rc}")
+    d = {k: float(out[i]) for i, k in enumerate(PEAK_KEYS)}
+    d["max_resident_clusters_200KB"] = {str(S): int(out[16 + S - 1]) for S in range(1, 17)}
+    return d
 
 
 class ClockSampler(threading.Thread):
@@ -212,8 +236,6 @@ def run_ours(args, wl, rank, local_rank, world):
         sim.set_stream_gen(args.stream_gen)
     if args.cluster_kernel:
         sim.set_cluster_kernel(args.cluster_kernel)
-    if args.cluster_threads:
-        sim.set_cluster_threads(args.cluster_threads)
     if args.cluster_size:
         sim.set_cluster_size(args.cluster_size)
     sim.set_engine(ENGINES[args.engine])
@@ -249,8 +271,7 @@ def run_ours(args, wl, rank, local_rank, world):
     engine, wake = sim.engine_name, sim.wake_name
     cluster_size = sim.cluster_size if engine == "cluster" else None
     sim_gen = sim.stream_gen if engine in ("stream", "graph") else None
-    cluster_kernel = {1: "k_cluster_step (scalar fp32)", 2: "k_cluster2_step (packed fp32x2)"}.get(sim.cluster_kernel) if engine == "cluster" else None
-    cluster_threads = sim.cluster_threads if engine == "cluster" else None
+    cluster_kernel = {1: "k_cluster_step", 3: "k_onchip_step"}.get(sim.cluster_kernel) if engine == "cluster" else None
     diag_last = diag[-1].cpu().numpy().astype(float)
     value = cells * n_inner * args.steps * world / (ms * 1e-3)
 
@@ -323,7 +344,7 @@ def run_ours(args, wl, rank, local_rank, world):
                        "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
                        "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size, "stream_gen": sim_gen,
                        "rotation": "manhattan" if args.manhattan else "standard", "clamp": bool(args.clamp),
-                       "cluster_kernel": cluster_kernel, "cluster_threads": cluster_threads,
+                       "cluster_kernel": cluster_kernel,
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                        "l2": "256 MB buffer written between timed bench steps (L2 flush)"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
@@ -336,6 +357,16 @@ def run_ours(args, wl, rank, local_rank, world):
 
 def main():
     args = parse_args()
+    if args.peaks:
+        import torch
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        torch.zeros(1, device="cuda")
+        sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+        sampler.start()
+        d = measure_peaks()
+        d["clocks"] = sampler.stop()
+        print(json.dumps({"peaks": d}), flush=True)
+        return
     from workloads import get_workload
     wl = get_workload(args.workload)
     if args.impl == "reference":

@@ -4,7 +4,7 @@ Argument marshalling only: every step of the hot path runs in the CUDA kernels o
 ``csrc/``.  PyTorch supplies device memory and streams.  There is no CPU fallback: if the
 shared library cannot be built or loaded, importing symbols from it raises.
 """
-from .build import build, lib_path
+from .build import build, build_peaks, lib_path
 from .binding import (
     ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER, ENGINE_GRID,
     WAKE_AUTO, WAKE_FFT, WAKE_DIRECT, OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE,
@@ -14,7 +14,7 @@ from .binding import (
 )
 
 __all__ = [
-    "build", "lib_path", "load", "version", "EXPORTS",
+    "build", "build_peaks", "lib_path", "load", "version", "EXPORTS",
     "ENGINE_AUTO", "ENGINE_STREAM", "ENGINE_GRAPH", "ENGINE_CLUSTER", "ENGINE_GRID",
     "WAKE_AUTO", "WAKE_FFT", "WAKE_DIRECT", "OPT_ENGINE", "OPT_WAKE", "OPT_TIMING", "OPT_CLUSTER_SIZE",
     "OPT_CLUSTER_KERNEL", "OPT_CLUSTER_THREADS", "OPT_STREAM_GEN",

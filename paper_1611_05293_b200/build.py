@@ -9,6 +9,8 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libvfps.so")
+_PEAKS_SRC = os.path.join(_CSRC, "peaks", "vfps_peaks.cu")
+_PEAKS_LIB = os.path.join(_HERE, "libvfps_peaks.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -57,5 +59,23 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return _LIB
 
 
+def build_peaks(force: bool = False) -> str:
+    """Compile the measurement harness csrc/peaks/vfps_peaks.cu into libvfps_peaks.so (its own
+    library: nothing of it is linked into libvfps.so)."""
+    if not force and os.path.exists(_PEAKS_LIB) and os.path.getmtime(_PEAKS_LIB) >= os.path.getmtime(_PEAKS_SRC):
+        return _PEAKS_LIB
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        if os.path.exists(_PEAKS_LIB):
+            return _PEAKS_LIB
+        raise RuntimeError("nvcc not found and libvfps_peaks.so is missing")
+    cmd = [nvcc] + NVCC_FLAGS + ["-o", _PEAKS_LIB, _PEAKS_SRC]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + res.stderr[-4000:])
+    return _PEAKS_LIB
+
+
 if __name__ == "__main__":
     print(build(force=True, verbose=True))
+    print(build_peaks(force=True))

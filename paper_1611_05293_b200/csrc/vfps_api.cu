@@ -3,7 +3,7 @@
 #include "../../include/vfps.h"
 #include "vfps_kernels.cuh"
 #include "vfps_cluster.cuh"
-#include "vfps_cluster2.cuh"
+#include "vfps_onchip.cuh"
 #include "vfps_stream2.cuh"
 #include "vfps_grid.cuh"
 
@@ -56,6 +56,15 @@ struct vfps_sim {
     int cl_ver = 0, cl_ver_opt = 0, cl_threads = 0, cl_threads_opt = 0;   // kernel in use (1 scalar, 2 packed), request, block size
     size_t cl_smem = 0;
     std::string cl_why;                          // why the cluster engine is unavailable
+    // second cluster design (vfps_onchip.cuh, cl_ver == 3): geometry tables and the work queue
+    bool oc_tab = false;                         // per-launch weight tables are accurate enough
+    int oc_tab_S = 0;                            // cluster size the tables on the device were built for
+    float *oc_coltab = nullptr, *oc_rowtab = nullptr;
+    int *oc_colix = nullptr;
+    unsigned long long *oc_item_ctr = nullptr;
+    unsigned int *oc_member_done = nullptr;
+    unsigned long long oc_item_base = 0;
+    unsigned int oc_done_base = 0;
 
     int tiles_x = 0, tiles_y = 0, kfp_rows = 0, kfp_blocks = 0;
     // second-generation streaming kernels (vfps_stream2.cuh)
@@ -255,17 +264,6 @@ cudaError_t cluster_launch_k(vfps_sim *h, K kern, int threads, const ClusterArgs
 template <int ORDER>
 cudaError_t cluster_launch_o(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *mc)
 {
-    if (h->cl_ver == 2) {
-        // packed kernel: block size chosen in cluster_configure (cl_threads)
-        switch (h->N * 4 + (h->cl_threads == 512 ? 1 : 0)) {
-            case 128 * 4: return cluster_launch_k(h, k_cluster2_step<ORDER, 128, 256>, 256, A, nclusters, query, mc);
-            case 128 * 4 + 1: return cluster_launch_k(h, k_cluster2_step<ORDER, 128, 512>, 512, A, nclusters, query, mc);
-            case 256 * 4: return cluster_launch_k(h, k_cluster2_step<ORDER, 256, 256>, 256, A, nclusters, query, mc);
-            case 256 * 4 + 1: return cluster_launch_k(h, k_cluster2_step<ORDER, 256, 512>, 512, A, nclusters, query, mc);
-            case 512 * 4 + 1: return cluster_launch_k(h, k_cluster2_step<ORDER, 512, 512>, 512, A, nclusters, query, mc);
-            default: return cudaErrorInvalidValue;
-        }
-    }
     const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0;
 #define VFPS_CL1(NN)                                                                                      \
     (manh ? cluster_launch_k(h, k_cluster_step<ORDER, NN, true>, CL_THREADS, A, nclusters, query, mc)    \
@@ -290,6 +288,253 @@ cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, boo
     }
 }
 
+// ---------------------------------------------------------------- second cluster design: host side
+// Lagrange weights l_k(t) and their derivatives (Eq. 13, nodes k - floor((order-1)/2)), double.
+void lagrange_d(int order, double t, double *l, double *lp)
+{
+    if (order == 2) {
+        l[0] = 1.0 - t; l[1] = t; lp[0] = -1.0; lp[1] = 1.0;
+    } else if (order == 3) {
+        l[0] = 0.5 * t * (t - 1.0); l[1] = 1.0 - t * t; l[2] = 0.5 * t * (t + 1.0);
+        lp[0] = t - 0.5; lp[1] = -2.0 * t; lp[2] = t + 0.5;
+    } else {
+        l[0] = -t * (t - 1.0) * (t - 2.0) / 6.0;
+        l[1] = (t + 1.0) * (t - 1.0) * (t - 2.0) / 2.0;
+        l[2] = -(t + 1.0) * t * (t - 2.0) / 2.0;
+        l[3] = (t + 1.0) * t * (t - 1.0) / 6.0;
+        lp[0] = -(3.0 * t * t - 6.0 * t + 2.0) / 6.0;
+        lp[1] = (3.0 * t * t - 4.0 * t - 1.0) / 2.0;
+        lp[2] = -(3.0 * t * t - 2.0 * t - 2.0) / 2.0;
+        lp[3] = (3.0 * t * t - 1.0) / 6.0;
+    }
+}
+
+// Geometry of the rotation in double precision (the same formulas as grid_constants)
+struct RotGeomD {
+    double a, b, d, x0c, y0c;
+};
+RotGeomD rot_geom_d(const vfps_params &P)
+{
+    const double PI = 3.14159265358979323846;
+    const double dq = (P.q_max - P.q_min) / (P.N - 1), dp = (P.p_max - P.p_min) / (P.N - 1);
+    const double dphi = 2.0 * PI / P.steps_per_period;
+    const double sh = std::sin(0.5 * dphi), s = std::sin(dphi);
+    RotGeomD g;
+    g.a = -2.0 * sh * sh; g.b = -s * dp / dq; g.d = s * dq / dp;
+    g.x0c = P.q_min / dq; g.y0c = P.p_min / dp;
+    return g;
+}
+
+// First-order weight tables are used when the neglected term (a * half-span)^2 |l''| / 2 stays
+// at the level of one fp32 ulp of a weight (|l''| <= 2 for the cubic basis).
+bool onchip_tab_ok(const vfps_sim *h, int S)
+{
+    const RotGeomD g = rot_geom_d(h->P);
+    const double span = 0.5 * (double)((h->N / S > h->N / 2 ? h->N / S : h->N) );
+    (void)span;
+    const double ex = std::fabs(g.a) * 0.5 * (double)(h->N / S), ey = std::fabs(g.a) * 0.5 * (double)h->N;
+    const double e = ex > ey ? ex : ey;
+    return e * e <= 1.2e-7;
+}
+
+// Column table (per rank and column), row table (per row), built in double and rounded once:
+//   dx(x, y) = a X + b Y,  dy(x, y) = d X + a Y,  X = x + x0c, Y = y + y0c
+//   column y of rank r is "good" if floor(dx) is the same for all rows of the rank (ix),
+//   row x is "good" if floor(dy) is the same for all columns (iy)
+//   TAB:  M_i(y) = l_i(t0x), M'_i = l_i'(t0x), t0x = a Xc(r) + b Y - ix, Xc = centre row of the rank
+//         L_j(x) = l_j(t0y), L'_j = l_j'(t0y), t0y = d X + a Ymid - iy;  e_x(x) = a (X - Xc)
+//         (the kernel forms e_y(y) = a (y - (N-1)/2) itself)
+//   else: column {b Y - ix, a Y}, row {X, d X - iy}: the kernel evaluates the weights per cell
+int onchip_tables(vfps_sim *h, int S)
+{
+    const int N = h->N, R = N / S, order = h->P.interp_order;
+    const RotGeomD g = rot_geom_d(h->P);
+    const bool tab = onchip_tab_ok(h, S);
+    std::vector<float> col((size_t)S * N * OC_COLTAB, 0.0f), row((size_t)N * OC_ROWTAB, 0.0f);
+    std::vector<int> cix((size_t)S * N, OC_BAD);
+    const double Ymid = 0.5 * (double)(N - 1) + g.y0c;
+    for (int r = 0; r < S; ++r) {
+        const double Xlo = (double)(r * R) + g.x0c, Xhi = (double)(r * R + R - 1) + g.x0c, Xc = 0.5 * (Xlo + Xhi);
+        for (int y = 0; y < N; ++y) {
+            const double Y = (double)y + g.y0c;
+            const double f0 = std::floor(g.a * Xlo + g.b * Y), f1 = std::floor(g.a * Xhi + g.b * Y);
+            float *c = &col[((size_t)r * N + y) * OC_COLTAB];
+            if (f0 != f1) continue;                                   // dx is monotonic in x
+            cix[(size_t)r * N + y] = (int)f0;
+            if (tab) {
+                double l[4] = {0, 0, 0, 0}, lp[4] = {0, 0, 0, 0};
+                lagrange_d(order, g.a * Xc + g.b * Y - f0, l, lp);
+                for (int i = 0; i < 4; ++i) { c[i] = (float)l[i]; c[4 + i] = (float)lp[i]; }
+            } else {
+                c[0] = (float)(g.b * Y - f0);
+                c[1] = (float)(g.a * Y);
+            }
+        }
+    }
+    for (int x = 0; x < N; ++x) {
+        const double X = (double)x + g.x0c;
+        const double Ylo = g.y0c, Yhi = (double)(N - 1) + g.y0c;
+        const double f0 = std::floor(g.d * X + g.a * Ylo), f1 = std::floor(g.d * X + g.a * Yhi);
+        float *t = &row[(size_t)x * OC_ROWTAB];
+        int iy = OC_BAD;
+        if (f0 == f1) {
+            iy = (int)f0;
+            const int r = x / R;
+            const double Xc = 0.5 * ((double)(r * R) + (double)(r * R + R - 1)) + g.x0c;
+            if (tab) {
+                double l[4] = {0, 0, 0, 0}, lp[4] = {0, 0, 0, 0};
+                lagrange_d(order, g.d * X + g.a * Ymid - f0, l, lp);
+                for (int j = 0; j < 4; ++j) { t[j] = (float)l[j]; t[4 + j] = (float)lp[j]; }
+                t[8] = (float)(g.a * (X - Xc));
+            } else {
+                t[8] = (float)X;
+                t[9] = (float)(g.d * X - f0);
+            }
+        }
+        std::memcpy(&t[10], &iy, sizeof(int));
+    }
+    if (!h->oc_coltab) {
+        CU(dalloc(h, &h->oc_coltab, (size_t)OC_MAX_S * N * OC_COLTAB));
+        CU(dalloc(h, &h->oc_colix, (size_t)OC_MAX_S * N));
+        CU(dalloc(h, &h->oc_rowtab, (size_t)N * OC_ROWTAB));
+        CU(dalloc(h, &h->oc_item_ctr, (size_t)1));
+        CU(dalloc(h, &h->oc_member_done, (size_t)h->members));
+        CU(cudaMemsetAsync(h->oc_item_ctr, 0, sizeof(unsigned long long), h->stream));
+        CU(cudaMemsetAsync(h->oc_member_done, 0, (size_t)h->members * sizeof(unsigned int), h->stream));
+    }
+    // pageable host memory: the copies are staged before the calls return
+    CU(cudaMemcpyAsync(h->oc_coltab, col.data(), col.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->oc_colix, cix.data(), cix.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->oc_rowtab, row.data(), row.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    h->oc_tab = tab;
+    h->oc_tab_S = S;
+    return VFPS_OK;
+}
+
+template <int ORDER, int NN>
+cudaError_t onchip_launch_n(vfps_sim *h, const OnchipArgs &A, int nclusters, bool query, int *mc)
+{
+    // cluster_launch_k passes (G, A) -- same launch helper, different argument struct
+    auto go = [&](auto kern) -> cudaError_t {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->cl_smem);
+        if (e != cudaSuccess) return e;
+        if (A.S > 8) {
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (e != cudaSuccess) return e;
+        }
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(A.S * nclusters));
+        cfg.blockDim = dim3((unsigned)OC_THREADS);
+        cfg.dynamicSmemBytes = h->cl_smem;
+        cfg.stream = h->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)A.S;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        if (query) return cudaOccupancyMaxActiveClusters(mc, kern, &cfg);
+        return cudaLaunchKernelEx(&cfg, kern, h->G, A);
+    };
+    return h->oc_tab ? go(k_onchip_step<ORDER, NN, true>) : go(k_onchip_step<ORDER, NN, false>);
+}
+
+template <int ORDER>
+cudaError_t onchip_launch_o(vfps_sim *h, const OnchipArgs &A, int nclusters, bool query, int *mc)
+{
+    switch (h->N) {
+        case 64: return onchip_launch_n<ORDER, 64>(h, A, nclusters, query, mc);
+        case 128: return onchip_launch_n<ORDER, 128>(h, A, nclusters, query, mc);
+        case 256: return onchip_launch_n<ORDER, 256>(h, A, nclusters, query, mc);
+        case 512: return onchip_launch_n<ORDER, 512>(h, A, nclusters, query, mc);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+cudaError_t onchip_launch(vfps_sim *h, const OnchipArgs &A, int nclusters, bool query, int *mc)
+{
+    switch (h->P.interp_order) {
+        case 2: return onchip_launch_o<2>(h, A, nclusters, query, mc);
+        case 3: return onchip_launch_o<3>(h, A, nclusters, query, mc);
+        default: return onchip_launch_o<4>(h, A, nclusters, query, mc);
+    }
+}
+
+// feasibility of the second cluster design for cluster size S; fills cl_smem / cl_max_clusters
+bool onchip_try(vfps_sim *h, int S, int smem_max)
+{
+    const int N = h->N, H = h->G.H;
+    if (!(N == 64 || N == 128 || N == 256 || N == 512)) return false;
+    if (h->P.flags & (VFPS_FLAG_CLAMP | VFPS_FLAG_ROT_MANHATTAN)) return false;
+    if (H > OC_MAX_H || N % S) return false;
+    const int R = N / S;
+    if (R < 4 || (R & 3) || R < H) return false;
+    const OnchipLayout L = onchip_layout(N, S, H, h->P.interp_order);
+    if (L.RPW < H) return false;
+    const size_t bytes = L.total_floats * sizeof(float);
+    if (bytes > (size_t)smem_max) return false;
+    const size_t keep = h->cl_smem;
+    const bool keep_tab = h->oc_tab;
+    h->cl_smem = bytes;
+    h->oc_tab = onchip_tab_ok(h, S);
+    OnchipArgs A{};
+    A.S = S; A.R = R;
+    int mc = 0;
+    cudaError_t e = onchip_launch(h, A, 1, true, &mc);
+    if (e != cudaSuccess || mc < 1) { cudaGetLastError(); h->cl_smem = keep; h->oc_tab = keep_tab; return false; }
+    h->cl_max_clusters = mc;
+    return true;
+}
+
+// split the n steps of a call into chunks so that (chunks x members) work items fill the
+// resident clusters evenly (a 256-member batch on 74 clusters: 2 chunks -> 512 items, 98.8 %)
+void onchip_chunks(const vfps_sim *h, int n, int nclusters, int *nchunks, int *chunk)
+{
+    *nchunks = 1; *chunk = n;
+    if (h->members <= nclusters) return;
+    double best = 0.0;
+    for (int c = 1; c <= 8 && n / c >= 32; ++c) {
+        const long long items = (long long)c * h->members;
+        const long long rounds = (items + nclusters - 1) / nclusters;
+        const double eff = (double)items / (double)(rounds * nclusters);
+        if (eff > best + 1e-9) { best = eff; *nchunks = c; }
+        if (eff >= 0.97) break;
+    }
+    *chunk = (n + *nchunks - 1) / *nchunks;
+    *nchunks = (n + *chunk - 1) / *chunk;
+}
+
+int launch_onchip_steps(vfps_sim *h, int n, float *diag)
+{
+    if (h->oc_tab_S != h->cl_S) {
+        int rc = onchip_tables(h, h->cl_S);
+        if (rc != VFPS_OK) return rc;
+    }
+    OnchipArgs A{};
+    A.psi = h->psi; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr; A.diag = diag;
+    A.coltab = h->oc_coltab; A.colix = h->oc_colix; A.rowtab = h->oc_rowtab;
+    A.members = h->members; A.S = h->cl_S; A.R = h->N / h->cl_S;
+    const int nclusters = h->members < h->cl_max_clusters ? h->members : h->cl_max_clusters;
+    int nchunks = 1, chunk = n;
+    onchip_chunks(h, n, nclusters, &nchunks, &chunk);
+    A.nsteps = chunk; A.nchunks = nchunks; A.last_steps = n - (nchunks - 1) * chunk;
+    A.item_ctr = h->oc_item_ctr; A.item_base = h->oc_item_base;
+    A.member_done = h->oc_member_done; A.done_base = h->oc_done_base;
+    cudaError_t e;
+    {
+        Bracket br(h, VFPS_KERNEL_CLUSTER, h->timing);
+        e = onchip_launch(h, A, nclusters, false, nullptr);
+    }
+    if (e != cudaSuccess) return fail(h, VFPS_ERR_CUDA, std::string("cluster launch: ") + cudaGetErrorString(e));
+    // every cluster fetches until it draws an item past the end: nclusters extra fetches per launch
+    h->oc_item_base += (unsigned long long)nchunks * (unsigned long long)h->members + (unsigned long long)nclusters;
+    h->oc_done_base += (unsigned int)nchunks;
+    h->launches += 1;
+    return VFPS_OK;
+}
+
 // Pick the cluster kernel and size.  Kernel: the request (cl_ver_opt) or, on AUTO, the scalar
 // kernel (1).  Size: the request (cl_S_opt) if
 // feasible; otherwise the largest feasible size for a single simulation (shortest step), the
@@ -297,40 +542,44 @@ cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, boo
 void cluster_configure(vfps_sim *h)
 {
     h->cl_S = 0; h->cl_max_clusters = 0; h->cl_ver = 0; h->cl_why.clear();
-    if (h->P.flags & VFPS_FLAG_CLAMP) { h->cl_why = "the cluster engine implements free (un-clamped) interpolation only"; return; }
     const int N = h->N, H = h->G.H;
-    if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
-    if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
     int dev = 0, smem_max = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const int cand_single[5] = {16, 8, 4, 2, 1}, cand_batch[5] = {1, 2, 4, 8, 16};
     const int *cand = (h->members == 1) ? cand_single : cand_batch;
-    // AUTO takes the scalar kernel: on B200 the packed one is not faster yet (C1 4.5 vs 3.5 us per
-    // step, C3 79 vs 79 us; profiles/r01_cluster2.md), it is there to be selected and measured
-    for (int ver = 1; ver <= 2; ++ver) {
-        if (ver != (h->cl_ver_opt ? h->cl_ver_opt : 1)) continue;
-        if (ver == 2 && !(N == 128 || N == 256 || N == 512)) continue;
-        if (ver == 2 && (h->P.flags & VFPS_FLAG_ROT_MANHATTAN)) continue;      // packed kernel: standard rotation only
+    // second design (k_onchip_step, kernel id 3): standard rotation, free interpolation; AUTO takes it
+    if (h->cl_ver_opt == 0 || h->cl_ver_opt == 3) {
         for (int c = 0; c < 5; ++c) {
             const int S = cand[c];
             if (h->cl_S_opt && S != h->cl_S_opt) continue;
-            if (N / S < (H > 1 ? H : 1) || N % S) continue;
-            const int R = N / S;
-            if (ver == 2 && ((R & 3) != 0 || R < 2 * H)) continue;
-            const size_t bytes = (ver == 2 ? cluster2_smem_floats(N, S, H) : cluster_smem_floats(N, S, H)) * sizeof(float);
-            if (bytes > (size_t)smem_max) continue;
-            h->cl_smem = bytes;
-            h->cl_ver = ver;
-            h->cl_threads = (ver == 2) ? ((N == 512 || h->cl_threads_opt == 512) ? 512 : 256) : CL_THREADS;
-            ClusterArgs A{};
-            A.S = S; A.R = R;
-            int mc = 0;
-            cudaError_t e = cluster_launch(h, A, 1, true, &mc);
-            if (e != cudaSuccess || mc < 1) { cudaGetLastError(); continue; }
-            h->cl_S = S; h->cl_max_clusters = mc;
+            if (!onchip_try(h, S, smem_max)) continue;
+            h->cl_S = S; h->cl_ver = 3; h->cl_threads = OC_THREADS;
             return;
         }
+        if (h->cl_ver_opt == 3) { h->cl_why = "second cluster design not feasible for this grid / flags / cluster size"; return; }
+    }
+    // first design (k_cluster_step, kernel id 1): also the Manhattan rotation
+    if (h->P.flags & VFPS_FLAG_CLAMP) { h->cl_why = "the cluster engine implements free (un-clamped) interpolation only"; return; }
+    if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
+    if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
+    for (int c = 0; c < 5; ++c) {
+        const int S = cand[c];
+        if (h->cl_S_opt && S != h->cl_S_opt) continue;
+        if (N / S < (H > 1 ? H : 1) || N % S) continue;
+        const int R = N / S;
+        const size_t bytes = cluster_smem_floats(N, S, H) * sizeof(float);
+        if (bytes > (size_t)smem_max) continue;
+        h->cl_smem = bytes;
+        h->cl_ver = 1;
+        h->cl_threads = CL_THREADS;
+        ClusterArgs A{};
+        A.S = S; A.R = R;
+        int mc = 0;
+        cudaError_t e = cluster_launch(h, A, 1, true, &mc);
+        if (e != cudaSuccess || mc < 1) { cudaGetLastError(); continue; }
+        h->cl_S = S; h->cl_max_clusters = mc;
+        return;
     }
     h->cl_ver = 0;
     h->cl_why = "no feasible cluster size (shared memory or cluster scheduling)";
@@ -338,6 +587,7 @@ void cluster_configure(vfps_sim *h)
 
 int launch_cluster_steps(vfps_sim *h, int n, float *diag)
 {
+    if (h->cl_ver == 3) return launch_onchip_steps(h, n, diag);
     ClusterArgs A{};
     A.psi = h->psi; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr; A.diag = diag;
     A.members = h->members; A.nsteps = n; A.S = h->cl_S; A.R = h->N / h->cl_S;
@@ -830,8 +1080,8 @@ int vfps_set_option(vfps_handle h, int option, int value)
     }
     if (option == VFPS_OPT_CLUSTER_KERNEL || option == VFPS_OPT_CLUSTER_THREADS) {
         const bool is_k = (option == VFPS_OPT_CLUSTER_KERNEL);
-        if (is_k ? !(value >= 0 && value <= 2) : !(value == 0 || value == 256 || value == 512))
-            return fail(h, VFPS_ERR_ARG, is_k ? "cluster kernel must be 0 (auto), 1 or 2" : "cluster threads must be 0 (auto), 256 or 512");
+        if (is_k ? !(value >= 0 && value <= 3) : !(value == 0 || value == 256 || value == 512))
+            return fail(h, VFPS_ERR_ARG, is_k ? "cluster kernel must be 0 (auto), 1, 2 or 3" : "cluster threads must be 0 (auto), 256 or 512");
         int &slot = is_k ? h->cl_ver_opt : h->cl_threads_opt;
         const int old = slot;
         slot = value;
