@@ -60,7 +60,6 @@ def parse_args():
     ap.add_argument("--cluster-size", type=int, default=0, help="CTAs per cluster of the cluster engine (0 = auto)")
     ap.add_argument("--manhattan", action="store_true", help="Manhattan (symplectic) rotation instead of the standard one")
     ap.add_argument("--clamp", action="store_true", help="clamped interpolation (Eq. 14)")
-    ap.add_argument("--stream-gen", type=int, default=0, help="streaming kernels: 0 auto, 1 first generation, 2 second")
     ap.add_argument("--cluster-kernel", type=int, default=0, help="cluster engine kernel: 0 auto, 1 first design (k_cluster_step), 3 in-place design (k_onchip_step)")
     ap.add_argument("--members", type=int, default=0, help="batch members (0 = the workload's own count)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -232,8 +231,6 @@ def run_ours(args, wl, rank, local_rank, world):
                          wl.interp_order, wl.pad, members, Z=Z,
                          flags=pkg.FLAG_RENORMALISE | (pkg.FLAG_ROT_MANHATTAN if args.manhattan else 0)
                          | (pkg.FLAG_CLAMP if args.clamp else 0))
-    if args.stream_gen:
-        sim.set_stream_gen(args.stream_gen)
     if args.cluster_kernel:
         sim.set_cluster_kernel(args.cluster_kernel)
     if args.cluster_size:
@@ -270,7 +267,6 @@ def run_ours(args, wl, rank, local_rank, world):
     ms = dist.reduce_max(ms_local, dev)
     engine, wake = sim.engine_name, sim.wake_name
     cluster_size = sim.cluster_size if engine == "cluster" else None
-    sim_gen = sim.stream_gen if engine in ("stream", "graph") else None
     cluster_kernel = {1: "k_cluster_step", 3: "k_onchip_step"}.get(sim.cluster_kernel) if engine == "cluster" else None
     diag_last = diag[-1].cpu().numpy().astype(float)
     value = cells * n_inner * args.steps * world / (ms * 1e-3)
@@ -342,7 +338,7 @@ def run_ours(args, wl, rank, local_rank, world):
             "us_per_split_step": 1e3 * ms / (n_inner * args.steps),
             "config": {"workload": wl.name, "N": wl.N, "members": members, "split_steps_per_bench_step": n_inner,
                        "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
-                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size, "stream_gen": sim_gen,
+                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size,
                        "rotation": "manhattan" if args.manhattan else "standard", "clamp": bool(args.clamp),
                        "cluster_kernel": cluster_kernel,
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",

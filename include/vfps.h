@@ -84,25 +84,20 @@ enum {
                               on, vfps_step may synchronise the stream to read finished events)  */
     VFPS_OPT_CLUSTER_SIZE = 4, /* CTAs per cluster of the CLUSTER engine: 0 = auto, 1, 2, 4, 8, 16;
                               vfps_get_option returns the size in use (0 = engine unavailable)  */
-    VFPS_OPT_CLUSTER_KERNEL = 5, /* kernel of the CLUSTER engine: 0 = auto, 1 = scalar fp32
-                              (k_cluster_step), 2 = packed fp32x2, two cells per thread
-                              (k_cluster2_step; N = 128, 256, 512); get returns the one in use  */
-    VFPS_OPT_CLUSTER_THREADS = 6, /* threads per CTA of the packed kernel: 0 = auto, 256, 512    */
-    VFPS_OPT_STREAM_GEN = 7 /* kernels of the STREAM / GRAPH engines: 0 = auto (2), 1 = first
-                              generation (k_rotate, k_wake_fft, k_kick_fp), 2 = second (k_rotate2,
-                              k_wake_direct or k_wake_fft, k_kick_fp2); get returns the one in use */
+    VFPS_OPT_CLUSTER_KERNEL = 5  /* kernel of the CLUSTER engine: 0 = auto, 1 = first design
+                              (k_cluster_step: two buffers, weights per cell; also the Manhattan
+                              rotation), 3 = in-place design (k_onchip_step: one buffer, per-launch
+                              weight tables; a 256^2 grid fits two CTAs); get returns the one in use */
 };
 /* kernel ids of vfps_kernel_time / vfps_kernel_name */
 enum {
-    VFPS_KERNEL_ROTATE = 0,   /* a1 + a2 partial sums                                            */
-    VFPS_KERNEL_WAKE = 1,     /* a2 finish + a3 + q-moments + CSR power                          */
-    VFPS_KERNEL_KICK_FP = 2,  /* a4 + a5 + a6                                                    */
-    VFPS_KERNEL_CLUSTER = 3,  /* a1..a6 for all n steps of one vfps_step call (cluster engine)   */
-    VFPS_KERNEL_ROTATE2 = 4,  /* a1 + a2, second-generation streaming kernel (register window)   */
-    VFPS_KERNEL_WAKE_DIRECT = 5, /* a2 finish + a3 by direct convolution on N/32 CTAs             */
-    VFPS_KERNEL_KICK_FP2 = 6, /* a4 + a5 + a6, second generation (four cells per thread)         */
-    VFPS_KERNEL_GRID = 7,     /* a1..a6 for all n steps of one vfps_step call (grid engine)      */
-    VFPS_NUM_KERNELS = 8
+    VFPS_KERNEL_WAKE = 0,     /* k_wake_fft: a2 finish + a3 by FFT (Eq. 5) + q-moments + CSR power */
+    VFPS_KERNEL_CLUSTER = 1,  /* a1..a6 for all n steps of one vfps_step call (cluster engine)   */
+    VFPS_KERNEL_ROTATE2 = 2,  /* k_rotate2 / k_drift2: a1 + a2, streaming (register window)      */
+    VFPS_KERNEL_WAKE_DIRECT = 3, /* k_wake_direct: a3 by direct convolution (Eq. 4) on N/8 CTAs   */
+    VFPS_KERNEL_KICK_FP2 = 4, /* k_kick_fp2: a4 + a5 + a6 (four cells per thread)                */
+    VFPS_KERNEL_GRID = 5,     /* a1..a6 for all n steps of one vfps_step call (grid engine)      */
+    VFPS_NUM_KERNELS = 6
 };
 enum {
     VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRID (one simulation) or
@@ -115,8 +110,7 @@ enum {
                                  barriers where the step has global dependencies (members = 1)   */
 };
 enum {
-    VFPS_WAKE_AUTO = 0,       /* DIRECT (the CLUSTER and GRID engines always; STREAM / GRAPH with the
-                                 second-generation kernels), FFT with the first generation      */
+    VFPS_WAKE_AUTO = 0,       /* DIRECT                                                          */
     VFPS_WAKE_FFT = 1,        /* zero-padded length-Nf FFT, x Z, inverse FFT, every step (Eq. 5) */
     VFPS_WAKE_DIRECT = 2      /* w = Re IDFT(Z) once at create; V = w * rho by direct convolution
                                  (Eq. 4) -- identical result, no serial FFT chain per step  */
@@ -192,7 +186,7 @@ int vfps_kernel_time(vfps_handle h, int kernel, double *ms_total, long long *lau
 int vfps_reset_kernel_times(vfps_handle h);
 const char *vfps_kernel_name(int kernel);
 
-/* Name of the engine / wake mode the next vfps_step will use ("stream", "graph", "cluster";
+/* Name of the engine / wake mode the next vfps_step will use ("stream", "graph", "cluster", "grid";
  * "fft", "direct"); static strings. */
 const char *vfps_engine_name(vfps_handle h);
 const char *vfps_wake_name(vfps_handle h);

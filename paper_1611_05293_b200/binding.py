@@ -15,8 +15,8 @@ from .build import build, lib_path
 
 ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER, ENGINE_GRID = 0, 1, 2, 3, 4
 WAKE_AUTO, WAKE_FFT, WAKE_DIRECT = 0, 1, 2
-OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL, OPT_CLUSTER_THREADS, OPT_STREAM_GEN = 1, 2, 3, 4, 5, 6, 7
-NUM_KERNELS = 8
+OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL = 1, 2, 3, 4, 5
+NUM_KERNELS = 6
 FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 
 # every symbol include/vfps.h declares (tests check the library exports each of them)
@@ -184,26 +184,12 @@ class Simulation:
     def cluster_size(self) -> int:
         return self.get_option(OPT_CLUSTER_SIZE)
 
-    def set_stream_gen(self, gen: int) -> None:
-        self.set_option(OPT_STREAM_GEN, gen)
-
-    @property
-    def stream_gen(self) -> int:
-        return self.get_option(OPT_STREAM_GEN)
-
     def set_cluster_kernel(self, version: int) -> None:
         self.set_option(OPT_CLUSTER_KERNEL, version)
 
     @property
     def cluster_kernel(self) -> int:
         return self.get_option(OPT_CLUSTER_KERNEL)
-
-    def set_cluster_threads(self, threads: int) -> None:
-        self.set_option(OPT_CLUSTER_THREADS, threads)
-
-    @property
-    def cluster_threads(self) -> int:
-        return self.get_option(OPT_CLUSTER_THREADS)
 
     @property
     def engine_name(self) -> str:

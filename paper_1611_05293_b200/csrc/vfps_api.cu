@@ -6,6 +6,7 @@
 #include "vfps_onchip.cuh"
 #include "vfps_stream2.cuh"
 #include "vfps_grid.cuh"
+#include "vfps_launch.h"
 
 #include <cmath>
 #include <cstdio>
@@ -38,10 +39,10 @@ struct vfps_sim {
     float *psi = nullptr, *psi_tmp = nullptr;   // [members][N][N]; psi holds the current state
     float2 *Z = nullptr;                         // [members][Nf/2+1]
     float2 *tw = nullptr;                        // [Nf/2]
-    float *rho_part = nullptr;                   // [members][N][tiles_y]
+    float *rho_part = nullptr;                   // [members][N][tiles_y2]
     float *rho = nullptr, *V = nullptr;          // [members][N]
     float *qstat = nullptr;                      // [members][4]
-    float *mom_part = nullptr;                   // [members][kfp_blocks][5]
+    float *mom_part = nullptr;                   // [members][kfp2_blocks][5]
     float *scale = nullptr;                      // [members]
     unsigned *blkctr = nullptr;                  // [members]
     int *rowctr = nullptr;                       // [members]
@@ -53,7 +54,7 @@ struct vfps_sim {
     float *wfun = nullptr;                       // [members][2N] wake function w = Re IDFT(Z)
     // cluster engine (0 = not available for this grid)
     int cl_S = 0, cl_S_opt = 0, cl_max_clusters = 0;
-    int cl_ver = 0, cl_ver_opt = 0, cl_threads = 0, cl_threads_opt = 0;   // kernel in use (1 scalar, 2 packed), request, block size
+    int cl_ver = 0, cl_ver_opt = 0;              // kernel in use (1 k_cluster_step, 3 k_onchip_step), request
     size_t cl_smem = 0;
     std::string cl_why;                          // why the cluster engine is unavailable
     // second cluster design (vfps_onchip.cuh, cl_ver == 3): geometry tables and the work queue
@@ -66,9 +67,7 @@ struct vfps_sim {
     unsigned long long oc_item_base = 0;
     unsigned int oc_done_base = 0;
 
-    int tiles_x = 0, tiles_y = 0, kfp_rows = 0, kfp_blocks = 0;
-    // second-generation streaming kernels (vfps_stream2.cuh)
-    int gen_opt = 0;                             // 0 auto (2), 1, 2
+    // streaming kernels (vfps_stream2.cuh)
     int tiles_x2 = 0, tiles_y2 = 0, kfp2_rows = 0, kfp2_blocks = 0, wd_blocks = 0;
     float *pw_part = nullptr;                    // [members][wd_blocks]
     // persistent cooperative-grid engine (vfps_grid.cuh); gr_blocks = 0: not available
@@ -79,7 +78,7 @@ struct vfps_sim {
     float *gr_zrow = nullptr;                    // [N] zeros
     std::string gr_why;
     unsigned *tilectr = nullptr;                 // [members][tiles_x2], zero between launches
-    size_t rot_smem = 0, kfp_smem = 0, fft_smem = 0;
+    size_t fft_smem = 0;
     int fft_threads = 0;
 
     // CUDA-graph engine: GRAPH_STEPS split steps captured once, replayed
@@ -235,57 +234,77 @@ __global__ void k_wake_function(int N, int Nf, int members, const float2 *__rest
     w[i] = (float)(acc / (double)Nf);
 }
 
-template <typename K>
-cudaError_t cluster_launch_k(vfps_sim *h, K kern, int threads, const ClusterArgs &A, int nclusters, bool query,
-                             int *max_clusters)
+#ifdef VFPS_PHASE_CLOCKS
+// Instrumented builds only: VFPS_PHASE_DUMP=<file> in the environment writes the per-phase clock
+// stamps (first 64 steps of every CTA) of each persistent-kernel launch; synchronises the stream.
+struct PhaseDump {
+    vfps_sim *h; long long *dbg = nullptr; size_t n = 0; const char *path = nullptr;
+    PhaseDump(vfps_sim *h_, size_t nctas) : h(h_)
+    {
+        path = std::getenv("VFPS_PHASE_DUMP");
+        n = nctas * 64 * 8;
+        if (path && cudaMalloc((void **)&dbg, n * sizeof(long long)) != cudaSuccess) { dbg = nullptr; path = nullptr; }
+        if (dbg) cudaMemsetAsync(dbg, 0, n * sizeof(long long), h->stream);
+    }
+    ~PhaseDump()
+    {
+        if (!dbg) return;
+        std::vector<long long> t(n);
+        cudaMemcpyAsync(t.data(), dbg, n * sizeof(long long), cudaMemcpyDeviceToHost, h->stream);
+        cudaStreamSynchronize(h->stream);
+        cudaFree(dbg);
+        if (FILE *f = std::fopen(path, "w")) {
+            for (size_t i = 0; i < n; i += 8) {
+                std::fprintf(f, "%zu %zu", i / (64 * 8), (i / 8) % 64);
+                for (int k = 0; k < 8; ++k) std::fprintf(f, " %lld", t[i + k]);
+                std::fprintf(f, "\n");
+            }
+            std::fclose(f);
+        }
+    }
+};
+#else
+struct PhaseDump {
+    long long *dbg = nullptr;
+    PhaseDump(vfps_sim *, size_t) {}
+};
+#endif
+
+// Launch (or occupancy query) of a persistent cluster kernel: grid = S x nclusters CTAs of `threads`
+// threads, cluster dimension S, h->cl_smem bytes of dynamic shared memory; args = {&GridConst, &Args}.
+cudaError_t cluster_launch_ptr(vfps_sim *h, const void *kern, int threads, int S, int nclusters, void **args,
+                               bool query, int *max_clusters)
 {
+    if (!kern) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->cl_smem);
     if (e != cudaSuccess) return e;
-    if (A.S > 8) {
+    if (S > 8) {
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         if (e != cudaSuccess) return e;
     }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(A.S * nclusters));
+    cfg.gridDim = dim3((unsigned)(S * nclusters));
     cfg.blockDim = dim3((unsigned)threads);
     cfg.dynamicSmemBytes = h->cl_smem;
     cfg.stream = h->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)A.S;
+    attr[0].val.clusterDim.x = (unsigned)S;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     if (query) return cudaOccupancyMaxActiveClusters(max_clusters, kern, &cfg);
-    return cudaLaunchKernelEx(&cfg, kern, h->G, A);
-}
-
-template <int ORDER>
-cudaError_t cluster_launch_o(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *mc)
-{
-    const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0;
-#define VFPS_CL1(NN)                                                                                      \
-    (manh ? cluster_launch_k(h, k_cluster_step<ORDER, NN, true>, CL_THREADS, A, nclusters, query, mc)    \
-          : cluster_launch_k(h, k_cluster_step<ORDER, NN, false>, CL_THREADS, A, nclusters, query, mc))
-    switch (h->N) {
-        case 32: return VFPS_CL1(32);
-        case 64: return VFPS_CL1(64);
-        case 128: return VFPS_CL1(128);
-        case 256: return VFPS_CL1(256);
-        case 512: return VFPS_CL1(512);
-        default: return cudaErrorInvalidValue;
-    }
-#undef VFPS_CL1
+    return cudaLaunchKernelExC(&cfg, kern, args);
 }
 
 cudaError_t cluster_launch(vfps_sim *h, const ClusterArgs &A, int nclusters, bool query, int *mc)
 {
-    switch (h->P.interp_order) {
-        case 2: return cluster_launch_o<2>(h, A, nclusters, query, mc);
-        case 3: return cluster_launch_o<3>(h, A, nclusters, query, mc);
-        default: return cluster_launch_o<4>(h, A, nclusters, query, mc);
-    }
+    const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0;
+    const void *kern = h->P.interp_order == 2 ? cluster_kernel_o2(h->N, manh)
+                     : h->P.interp_order == 3 ? cluster_kernel_o3(h->N, manh) : cluster_kernel_o4(h->N, manh);
+    void *args[2] = {(void *)&h->G, (void *)&A};
+    return cluster_launch_ptr(h, kern, CL_THREADS, A.S, nclusters, args, query, mc);
 }
 
 // ---------------------------------------------------------------- second cluster design: host side
@@ -412,54 +431,14 @@ int onchip_tables(vfps_sim *h, int S)
     return VFPS_OK;
 }
 
-template <int ORDER, int NN>
-cudaError_t onchip_launch_n(vfps_sim *h, const OnchipArgs &A, int nclusters, bool query, int *mc)
-{
-    // cluster_launch_k passes (G, A) -- same launch helper, different argument struct
-    auto go = [&](auto kern) -> cudaError_t {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->cl_smem);
-        if (e != cudaSuccess) return e;
-        if (A.S > 8) {
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-            if (e != cudaSuccess) return e;
-        }
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(A.S * nclusters));
-        cfg.blockDim = dim3((unsigned)OC_THREADS);
-        cfg.dynamicSmemBytes = h->cl_smem;
-        cfg.stream = h->stream;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = (unsigned)A.S;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        if (query) return cudaOccupancyMaxActiveClusters(mc, kern, &cfg);
-        return cudaLaunchKernelEx(&cfg, kern, h->G, A);
-    };
-    return h->oc_tab ? go(k_onchip_step<ORDER, NN, true>) : go(k_onchip_step<ORDER, NN, false>);
-}
-
-template <int ORDER>
-cudaError_t onchip_launch_o(vfps_sim *h, const OnchipArgs &A, int nclusters, bool query, int *mc)
-{
-    switch (h->N) {
-        case 64: return onchip_launch_n<ORDER, 64>(h, A, nclusters, query, mc);
-        case 128: return onchip_launch_n<ORDER, 128>(h, A, nclusters, query, mc);
-        case 256: return onchip_launch_n<ORDER, 256>(h, A, nclusters, query, mc);
-        case 512: return onchip_launch_n<ORDER, 512>(h, A, nclusters, query, mc);
-        default: return cudaErrorInvalidValue;
-    }
-}
-
 cudaError_t onchip_launch(vfps_sim *h, const OnchipArgs &A, int nclusters, bool query, int *mc)
 {
-    switch (h->P.interp_order) {
-        case 2: return onchip_launch_o<2>(h, A, nclusters, query, mc);
-        case 3: return onchip_launch_o<3>(h, A, nclusters, query, mc);
-        default: return onchip_launch_o<4>(h, A, nclusters, query, mc);
-    }
+    const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0;
+    const void *kern = h->P.interp_order == 2 ? onchip_kernel_o2(h->N, h->oc_tab, clamp)
+                     : h->P.interp_order == 3 ? onchip_kernel_o3(h->N, h->oc_tab, clamp)
+                                              : onchip_kernel_o4(h->N, h->oc_tab, clamp);
+    void *args[2] = {(void *)&h->G, (void *)&A};
+    return cluster_launch_ptr(h, kern, OC_THREADS, A.S, nclusters, args, query, mc);
 }
 
 // feasibility of the second cluster design for cluster size S; fills cl_smem / cl_max_clusters
@@ -524,6 +503,8 @@ int launch_onchip_steps(vfps_sim *h, int n, float *diag)
     A.member_done = h->oc_member_done; A.done_base = h->oc_done_base;
     cudaError_t e;
     {
+        PhaseDump pd(h, (size_t)A.S * nclusters);
+        A.dbg = pd.dbg;
         Bracket br(h, VFPS_KERNEL_CLUSTER, h->timing);
         e = onchip_launch(h, A, nclusters, false, nullptr);
     }
@@ -554,7 +535,7 @@ void cluster_configure(vfps_sim *h)
             const int S = cand[c];
             if (h->cl_S_opt && S != h->cl_S_opt) continue;
             if (!onchip_try(h, S, smem_max)) continue;
-            h->cl_S = S; h->cl_ver = 3; h->cl_threads = OC_THREADS;
+            h->cl_S = S; h->cl_ver = 3;
             return;
         }
         if (h->cl_ver_opt == 3) { h->cl_why = "second cluster design not feasible for this grid / flags / cluster size"; return; }
@@ -572,7 +553,6 @@ void cluster_configure(vfps_sim *h)
         if (bytes > (size_t)smem_max) continue;
         h->cl_smem = bytes;
         h->cl_ver = 1;
-        h->cl_threads = CL_THREADS;
         ClusterArgs A{};
         A.S = S; A.R = R;
         int mc = 0;
@@ -593,77 +573,24 @@ int launch_cluster_steps(vfps_sim *h, int n, float *diag)
     A.members = h->members; A.nsteps = n; A.S = h->cl_S; A.R = h->N / h->cl_S;
     const int nclusters = h->members < h->cl_max_clusters ? h->members : h->cl_max_clusters;
     cudaError_t e;
-    // debug aid: VFPS_PHASE_DUMP=<file> writes the packed kernel's per-phase clock stamps of the
-    // first 64 steps of every CTA (synchronises; never set in measurements)
-    const char *dump = std::getenv("VFPS_PHASE_DUMP");
-    const size_t ndbg = (size_t)A.S * nclusters * 64 * 8;
-    if (dump && cudaMalloc((void **)&A.dbg, ndbg * sizeof(long long)) != cudaSuccess) { A.dbg = nullptr; dump = nullptr; }
-    if (dump) cudaMemsetAsync(A.dbg, 0, ndbg * sizeof(long long), h->stream);
     {
+        PhaseDump pd(h, (size_t)A.S * nclusters);
+        A.dbg = pd.dbg;
         Bracket br(h, VFPS_KERNEL_CLUSTER, h->timing);
         e = cluster_launch(h, A, nclusters, false, nullptr);
-    }
-    if (dump) {
-        std::vector<long long> t(ndbg);
-        cudaMemcpyAsync(t.data(), A.dbg, ndbg * sizeof(long long), cudaMemcpyDeviceToHost, h->stream);
-        cudaStreamSynchronize(h->stream);
-        cudaFree(A.dbg);
-        if (FILE *f = std::fopen(dump, "w")) {
-            for (size_t i = 0; i < ndbg; i += 8) {
-                std::fprintf(f, "%zu %zu", i / (64 * 8), (i / 8) % 64);
-                for (int k = 0; k < 8; ++k) std::fprintf(f, " %lld", t[i + k]);
-                std::fprintf(f, "\n");
-            }
-            std::fclose(f);
-        }
     }
     if (e != cudaSuccess) return fail(h, VFPS_ERR_CUDA, std::string("cluster launch: ") + cudaGetErrorString(e));
     h->launches += 1;
     return VFPS_OK;
 }
 
-template <int ORDER>
-int launch_step_stream(vfps_sim *h, bool timed)
-{
-    const int N = h->N;
-    dim3 g1(h->tiles_x * h->tiles_y, h->members);
-    {
-        Bracket br(h, VFPS_KERNEL_ROTATE, timed);
-        k_rotate<ORDER><<<g1, ROT_THREADS, h->rot_smem, h->stream>>>(h->G, h->psi, h->psi_tmp, h->scale,
-                                                                      h->rho_part, h->tiles_y);
-    }
-    {
-        Bracket br(h, VFPS_KERNEL_WAKE, timed);
-        k_wake_fft<<<h->members, h->fft_threads, h->fft_smem, h->stream>>>(
-            N, h->Nf, h->log2Nf, h->G.dq, h->rho_part, h->tiles_y, h->has_wake ? h->Z : nullptr, h->tw,
-            h->rho, h->V, h->qstat);
-    }
-    KfpArgs A;
-    A.psi_in = h->psi_tmp; A.psi_out = h->psi; A.V = h->V; A.qstat = h->qstat;
-    A.mom_part = h->mom_part; A.scale = h->scale; A.blkctr = h->blkctr; A.rowctr = h->rowctr;
-    A.diag = h->diag_cell; A.members = h->members; A.rows_per_cta = h->kfp_rows;
-    dim3 g3(h->kfp_blocks, h->members);
-    {
-        Bracket br(h, VFPS_KERNEL_KICK_FP, timed);
-        k_kick_fp<ORDER><<<g3, KFP_THREADS, h->kfp_smem, h->stream>>>(h->G, A);
-    }
-    h->launches += 3;
-    return VFPS_OK;
-}
-
-template <int ORDER>
-const void *grid_kernel(bool manh, bool clamp)
-{
-    if (clamp) return manh ? (const void *)k_grid_step<ORDER, true, true> : (const void *)k_grid_step<ORDER, false, true>;
-    return manh ? (const void *)k_grid_step<ORDER, true, false> : (const void *)k_grid_step<ORDER, false, false>;
-}
 const void *grid_kernel(const vfps_sim *h)
 {
     const bool manh = (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) != 0, clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0;
     switch (h->P.interp_order) {
-        case 2: return grid_kernel<2>(manh, clamp);
-        case 3: return grid_kernel<3>(manh, clamp);
-        default: return grid_kernel<4>(manh, clamp);
+        case 2: return grid_kernel_o2(manh, clamp);
+        case 3: return grid_kernel_o3(manh, clamp);
+        default: return grid_kernel_o4(manh, clamp);
     }
 }
 
@@ -708,45 +635,33 @@ int launch_grid_steps(vfps_sim *h, int n, float *diag)
     void *args[2] = {(void *)&h->G, (void *)&A};
     const void *kern = grid_kernel(h);
     cudaError_t e;
-    // debug aid as in launch_cluster_steps: VFPS_PHASE_DUMP=<file>
-    const char *dump = std::getenv("VFPS_PHASE_DUMP");
-    const size_t ndbg = (size_t)h->gr_blocks * 64 * 8;
-    if (dump && cudaMalloc((void **)&A.dbg, ndbg * sizeof(long long)) != cudaSuccess) { A.dbg = nullptr; dump = nullptr; }
-    if (dump) cudaMemsetAsync(A.dbg, 0, ndbg * sizeof(long long), h->stream);
     {
+        PhaseDump pd(h, (size_t)h->gr_blocks);
+        A.dbg = pd.dbg;
         Bracket br(h, VFPS_KERNEL_GRID, h->timing);
         e = cudaLaunchCooperativeKernel(kern, dim3((unsigned)h->gr_blocks), dim3(GR_THREADS), args, h->gr_smem, h->stream);
-    }
-    if (dump) {
-        std::vector<long long> t(ndbg);
-        cudaMemcpyAsync(t.data(), A.dbg, ndbg * sizeof(long long), cudaMemcpyDeviceToHost, h->stream);
-        cudaStreamSynchronize(h->stream);
-        cudaFree(A.dbg);
-        if (FILE *f = std::fopen(dump, "w")) {
-            for (size_t i = 0; i < ndbg; i += 8) {
-                std::fprintf(f, "%zu %zu", i / (64 * 8), (i / 8) % 64);
-                for (int k = 0; k < 8; ++k) std::fprintf(f, " %lld", t[i + k]);
-                std::fprintf(f, "\n");
-            }
-            std::fclose(f);
-        }
     }
     if (e != cudaSuccess) return fail(h, VFPS_ERR_CUDA, std::string("cooperative launch: ") + cudaGetErrorString(e));
     h->launches += 1;
     return VFPS_OK;
 }
 
-// which kernels the STREAM / GRAPH engines launch, and how they evaluate the wake
-int resolved_gen(const vfps_sim *h)
+// k_wake_fft needs the opt-in for more than 48 KB of dynamic shared memory (Nf >= 4096).  The
+// attribute belongs to the function, not to a handle: it is only ever raised (per device).
+cudaError_t wake_fft_attr(const vfps_sim *h)
 {
-    if (h->P.flags & (VFPS_FLAG_ROT_MANHATTAN | VFPS_FLAG_CLAMP)) return 2;      // only the second generation has them
-    return h->gen_opt ? h->gen_opt : 2;
+    static size_t granted[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) dev = 0;
+    if (h->fft_smem <= granted[dev]) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(k_wake_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->fft_smem);
+    if (e == cudaSuccess) granted[dev] = h->fft_smem;
+    return e;
 }
-bool wake_is_direct(const vfps_sim *h)
-{
-    if (resolved_gen(h) == 1) return false;
-    return h->wake_opt != VFPS_WAKE_FFT;
-}
+
+// how the STREAM / GRAPH engines evaluate the wake
+bool wake_is_direct(const vfps_sim *h) { return h->wake_opt != VFPS_WAKE_FFT; }
 
 template <int ORDER, bool CLAMP>
 int launch_step_stream2(vfps_sim *h, bool timed)
@@ -772,6 +687,7 @@ int launch_step_stream2(vfps_sim *h, bool timed)
     }
     if (!direct) {
         Bracket br(h, VFPS_KERNEL_WAKE, timed);
+        wake_fft_attr(h);
         k_wake_fft<<<h->members, h->fft_threads, h->fft_smem, h->stream>>>(
             N, h->Nf, h->log2Nf, h->G.dq, rfp ? h->rho : h->rho_part, rfp ? 1 : h->tiles_y2,
             h->has_wake ? h->Z : nullptr, h->tw, h->rho, h->V, h->qstat);
@@ -798,18 +714,11 @@ int launch_step_stream2(vfps_sim *h, bool timed)
 
 int launch_step(vfps_sim *h, bool timed)
 {
-    if (resolved_gen(h) == 2) {
-        const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0;
-        switch (h->P.interp_order) {
-            case 2: return clamp ? launch_step_stream2<2, true>(h, timed) : launch_step_stream2<2, false>(h, timed);
-            case 3: return clamp ? launch_step_stream2<3, true>(h, timed) : launch_step_stream2<3, false>(h, timed);
-            default: return clamp ? launch_step_stream2<4, true>(h, timed) : launch_step_stream2<4, false>(h, timed);
-        }
-    }
+    const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0;
     switch (h->P.interp_order) {
-        case 2: return launch_step_stream<2>(h, timed);
-        case 3: return launch_step_stream<3>(h, timed);
-        default: return launch_step_stream<4>(h, timed);
+        case 2: return clamp ? launch_step_stream2<2, true>(h, timed) : launch_step_stream2<2, false>(h, timed);
+        case 3: return clamp ? launch_step_stream2<3, true>(h, timed) : launch_step_stream2<3, false>(h, timed);
+        default: return clamp ? launch_step_stream2<4, true>(h, timed) : launch_step_stream2<4, false>(h, timed);
     }
 }
 
@@ -863,14 +772,6 @@ int ensure_graph(vfps_sim *h)
     return VFPS_OK;
 }
 
-template <int ORDER>
-cudaError_t set_kernel_attrs(vfps_sim *h)
-{
-    cudaError_t e = cudaFuncSetAttribute(k_rotate<ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->rot_smem);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_kick_fp<ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->kfp_smem);
-}
-
 int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, void *cuda_stream,
                 vfps_handle *out)
 {
@@ -901,12 +802,6 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
         return bail(VFPS_ERR_UNSUPPORTED, "rotation displacement per step exceeds the supported halo (too few steps_per_period for this grid)");
 
     const int N = h->N, M = h->members;
-    h->tiles_x = (N + ROT_TX - 1) / ROT_TX;
-    h->tiles_y = (N + ROT_TY - 1) / ROT_TY;
-    h->rot_smem = (size_t)(ROT_TX + 2 * h->G.H) * (ROT_TY + 2 * h->G.H) * sizeof(float);
-    h->kfp_rows = KFP_WARPS * ((N >= 1024) ? 2 : 1);
-    h->kfp_blocks = (N + h->kfp_rows - 1) / h->kfp_rows;
-    h->kfp_smem = (size_t)KFP_WARPS * 2 * (KFP_PADL + N + KFP_PADR) * sizeof(float);
     h->tiles_x2 = (N + R2_RT - 1) / R2_RT;
     h->tiles_y2 = (N + 32 * R2_WARPS - 1) / (32 * R2_WARPS);
     h->kfp2_rows = 4096 / N > 0 ? (4096 / N < N ? 4096 / N : N) : 1;
@@ -926,7 +821,7 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     CUB(dalloc(h, &h->psi, (size_t)M * N * N));
     CUB(dalloc(h, &h->psi_tmp, (size_t)M * N * N));
     CUB(dalloc(h, &h->tw, (size_t)h->Nf / 2));
-    CUB(dalloc(h, &h->rho_part, (size_t)M * N * (h->tiles_y > h->tiles_y2 ? h->tiles_y : h->tiles_y2)));
+    CUB(dalloc(h, &h->rho_part, (size_t)M * N * h->tiles_y2));
     CUB(dalloc(h, &h->pw_part, (size_t)M * h->wd_blocks));
     CUB(dalloc(h, &h->tilectr, (size_t)M * h->tiles_x2));
     CUB(cudaMemsetAsync(h->tilectr, 0, (size_t)M * h->tiles_x2 * sizeof(unsigned), h->stream));
@@ -934,7 +829,7 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     CUB(dalloc(h, &h->rho, (size_t)M * N));
     CUB(dalloc(h, &h->V, (size_t)M * N));
     CUB(dalloc(h, &h->qstat, (size_t)M * 4));
-    CUB(dalloc(h, &h->mom_part, (size_t)M * (h->kfp_blocks > h->kfp2_blocks ? h->kfp_blocks : h->kfp2_blocks) * 5));
+    CUB(dalloc(h, &h->mom_part, (size_t)M * h->kfp2_blocks * 5));
     CUB(dalloc(h, &h->scale, (size_t)M));
     CUB(dalloc(h, &h->blkctr, (size_t)M));
     CUB(dalloc(h, &h->rowctr, (size_t)M));
@@ -981,14 +876,6 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
         CUB(dalloc(h, &h->gr_zrow, (size_t)N));
         CUB(cudaMemsetAsync(h->gr_zrow, 0, (size_t)N * sizeof(float), h->stream));
     }
-    cudaError_t e = cudaSuccess;
-    switch (p->interp_order) {
-        case 2: e = set_kernel_attrs<2>(h); break;
-        case 3: e = set_kernel_attrs<3>(h); break;
-        default: e = set_kernel_attrs<4>(h); break;
-    }
-    CUB(e);
-    CUB(cudaFuncSetAttribute(k_wake_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->fft_smem));
     CUB(cudaGetLastError());
 #undef CUB
     *out = h;
@@ -1002,6 +889,7 @@ int current_profile(vfps_sim *h, bool want_wake)
     k_project<<<dim3(N, M), 128, 0, h->stream>>>(h->G, h->psi, h->scale, h->g_rho, h->g_m1, h->g_m2);
     h->launches += 1;
     if (want_wake) {
+        CU(wake_fft_attr(h));
         k_wake_fft<<<M, h->fft_threads, h->fft_smem, h->stream>>>(N, h->Nf, h->log2Nf, h->G.dq, h->g_rho, 1,
                                                                   h->has_wake ? h->Z : nullptr, h->tw,
                                                                   h->g_rho, h->g_V, h->g_qstat);
@@ -1078,17 +966,15 @@ int vfps_set_option(vfps_handle h, int option, int value)
         }
         return VFPS_OK;
     }
-    if (option == VFPS_OPT_CLUSTER_KERNEL || option == VFPS_OPT_CLUSTER_THREADS) {
-        const bool is_k = (option == VFPS_OPT_CLUSTER_KERNEL);
-        if (is_k ? !(value >= 0 && value <= 3) : !(value == 0 || value == 256 || value == 512))
-            return fail(h, VFPS_ERR_ARG, is_k ? "cluster kernel must be 0 (auto), 1, 2 or 3" : "cluster threads must be 0 (auto), 256 or 512");
-        int &slot = is_k ? h->cl_ver_opt : h->cl_threads_opt;
-        const int old = slot;
-        slot = value;
+    if (option == VFPS_OPT_CLUSTER_KERNEL) {
+        if (!(value == 0 || value == 1 || value == 3))
+            return fail(h, VFPS_ERR_ARG, "cluster kernel must be 0 (auto), 1 (k_cluster_step) or 3 (k_onchip_step)");
+        const int old = h->cl_ver_opt;
+        h->cl_ver_opt = value;
         cluster_configure(h);
         if (h->cl_S == 0) {
             const std::string why = h->cl_why;
-            slot = old;
+            h->cl_ver_opt = old;
             cluster_configure(h);
             return fail(h, VFPS_ERR_UNSUPPORTED, "cluster kernel not available for this grid: " + why);
         }
@@ -1103,20 +989,8 @@ int vfps_set_option(vfps_handle h, int option, int value)
     if (option == VFPS_OPT_WAKE) {
         if (!(value == VFPS_WAKE_AUTO || value == VFPS_WAKE_FFT || value == VFPS_WAKE_DIRECT))
             return fail(h, VFPS_ERR_ARG, "unknown wake mode");
-        if (value == VFPS_WAKE_DIRECT && resolved_gen(h) == 1)
-            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels have no direct-convolution wake");
         if (value != h->wake_opt) drop_graph(h);
         h->wake_opt = value;
-        return VFPS_OK;
-    }
-    if (option == VFPS_OPT_STREAM_GEN) {
-        if (value < 0 || value > 2) return fail(h, VFPS_ERR_ARG, "stream generation must be 0 (auto), 1 or 2");
-        if (value == 1 && (h->P.flags & (VFPS_FLAG_ROT_MANHATTAN | VFPS_FLAG_CLAMP)))
-            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels implement the standard rotation with free interpolation only");
-        if (value == 1 && h->wake_opt == VFPS_WAKE_DIRECT)
-            return fail(h, VFPS_ERR_UNSUPPORTED, "the first-generation streaming kernels have no direct-convolution wake");
-        if (value != h->gen_opt) drop_graph(h);
-        h->gen_opt = value;
         return VFPS_OK;
     }
     return fail(h, VFPS_ERR_ARG, "unknown option");
@@ -1130,8 +1004,6 @@ int vfps_get_option(vfps_handle h, int option, int *value)
     if (option == VFPS_OPT_TIMING) { *value = h->timing ? 1 : 0; return VFPS_OK; }
     if (option == VFPS_OPT_CLUSTER_SIZE) { *value = h->cl_S; return VFPS_OK; }
     if (option == VFPS_OPT_CLUSTER_KERNEL) { *value = h->cl_ver; return VFPS_OK; }
-    if (option == VFPS_OPT_CLUSTER_THREADS) { *value = h->cl_threads; return VFPS_OK; }
-    if (option == VFPS_OPT_STREAM_GEN) { *value = resolved_gen(h); return VFPS_OK; }
     return fail(h, VFPS_ERR_ARG, "unknown option");
 }
 
@@ -1380,9 +1252,7 @@ int vfps_reset_kernel_times(vfps_handle h)
 const char *vfps_kernel_name(int kernel)
 {
     switch (kernel) {
-        case VFPS_KERNEL_ROTATE: return "k_rotate";
         case VFPS_KERNEL_WAKE: return "k_wake_fft";
-        case VFPS_KERNEL_KICK_FP: return "k_kick_fp";
         case VFPS_KERNEL_CLUSTER: return "k_cluster_step";
         case VFPS_KERNEL_ROTATE2: return "k_rotate2";
         case VFPS_KERNEL_WAKE_DIRECT: return "k_wake_direct";

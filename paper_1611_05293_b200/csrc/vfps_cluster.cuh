@@ -22,7 +22,7 @@
 //   -- cluster barrier 2 --
 //   6 a6: every CTA forms C and the scalar 1/C; rank 0 writes the diagnostics row.
 #pragma once
-#include "vfps_kernels.cuh"
+#include "vfps_common.cuh"
 
 #include <cooperative_groups.h>
 
@@ -492,7 +492,14 @@ k_cluster_step(GridConst G, ClusterArgs A)
         for (int i = tid; i < R * PITCH; i += CL_THREADS) bufB[i] = 0.0f;
         for (int i = tid; i < 2 * N; i += CL_THREADS) wf[i] = (gw && i < 2 * N - 1) ? gw[i] : 0.0f;
         float sc = G.renorm ? A.scale[m] : 1.0f;
-        if (tid == 0) { mbar_expect_tx(mbRho, bytesRho); mbar_expect_tx(mbHalo, bytesHalo); mbar_expect_tx(mbPart, bytesPart); }
+        // a barrier that expects no bytes (S = 1; the halo of an edge-less cluster) is neither armed nor
+        // waited on: arming it would complete its phase at once, and a warp that has not yet reached
+        // its wait would see the parity flip twice and hang
+        if (tid == 0) {
+            if (bytesRho) mbar_expect_tx(mbRho, bytesRho);
+            if (bytesHalo) mbar_expect_tx(mbHalo, bytesHalo);
+            if (bytesPart) mbar_expect_tx(mbPart, bytesPart);
+        }
         // nobody may store into this CTA before it has finished initialising
         cluster.sync();
 
@@ -500,10 +507,10 @@ k_cluster_step(GridConst G, ClusterArgs A)
             const bool last = (step == A.nsteps);
             if (step > 0) {
                 // ---- the neighbours' boundary rows of psi_t have arrived
-                mbar_wait(mbHalo, phase ^ 1u);
-                if (tid == 0 && !last) mbar_expect_tx(mbHalo, bytesHalo);
+                if (bytesHalo) mbar_wait(mbHalo, phase ^ 1u);
+                if (tid == 0 && !last && bytesHalo) mbar_expect_tx(mbHalo, bytesHalo);
             }
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 0] = clock64();
+            VFPS_STAMP(A.dbg, step, 0);
             // ================= 1. rotation: bufA -> bufB
             if (!last) {
                 if constexpr (MANH) {
@@ -524,13 +531,13 @@ k_cluster_step(GridConst G, ClusterArgs A)
                     rot.run(rbeg, rend, x0);
                 }
             }
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 1] = clock64();
+            VFPS_STAMP(A.dbg, step, 1);
             __syncthreads();
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 2] = clock64();
+            VFPS_STAMP(A.dbg, step, 2);
             if (step > 0) {
                 // ================= 6. a6 of step t-1: charge, scale, diagnostics
-                mbar_wait(mbPart, phase ^ 1u);
-                if (tid == 0 && !last) mbar_expect_tx(mbPart, bytesPart);
+                if (bytesPart) mbar_wait(mbPart, phase ^ 1u);
+                if (tid == 0 && !last && bytesPart) mbar_expect_tx(mbPart, bytesPart);
                 // lane = (g4, j): partial j summed over the CTAs g4, g4 + 4, ..., then over the four
                 // lane groups -- the same order in every warp of every CTA
                 const float *pp = part + ((step - 1) & 1) * (CL_MAX_S * CL_NPART);
@@ -561,7 +568,7 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 }
             }
             if (last) break;
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 3] = clock64();
+            VFPS_STAMP(A.dbg, step, 3);
             // ================= 2. projection: rho_x = dp * sc * sum_y bufB(x, y), all-gathered
             for (int r = warp; r < R; r += CL_WARPS) {
                 const uint32_t row = sB + (uint32_t)((r * PITCH + CL_PAD) * 4);
@@ -591,10 +598,10 @@ k_cluster_step(GridConst G, ClusterArgs A)
                     st_async4(mapa(a, dd), lds4(a), mapa(mbRho, dd));
                 }
             }
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 4] = clock64();
-            mbar_wait(mbRho, phase);
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 5] = clock64();
-            if (tid == 0 && step + 1 < A.nsteps) mbar_expect_tx(mbRho, bytesRho);
+            VFPS_STAMP(A.dbg, step, 4);
+            if (bytesRho) mbar_wait(mbRho, phase);
+            VFPS_STAMP(A.dbg, step, 5);
+            if (tid == 0 && step + 1 < A.nsteps && bytesRho) mbar_expect_tx(mbRho, bytesRho);
             // ================= 3.+4. wake (own rows), kick + Fokker-Planck: bufB -> bufA
             // per-warp sums: s0 sum psi, s1/s2 p moments (per lane), q1/q2 q moments, pw = sum rho V
             float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, q1 = 0.0f, q2 = 0.0f, pw = 0.0f;
@@ -690,7 +697,7 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 const float X = (float)x - xc, tq = rs * X;
                 s0 += rs; q1 += tq; q2 = fmaf(tq, X, q2);
             }
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 6] = clock64();
+            VFPS_STAMP(A.dbg, step, 6);
             // ================= 5. partial sums of this CTA -> every CTA
             s1 = warp_sum(s1); s2 = warp_sum(s2);
             if (lane == 0) {
@@ -715,7 +722,7 @@ k_cluster_step(GridConst G, ClusterArgs A)
                     st_async4(mapa(slot + hh * 16, dd), lds4(slot + hh * 16), mapa(mbPart, dd));
                 }
             }
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 7] = clock64();
+            VFPS_STAMP(A.dbg, step, 7);
             phase ^= 1u;
         }
         // ---- store own rows and the scale (all remote stores into this CTA have been waited for)

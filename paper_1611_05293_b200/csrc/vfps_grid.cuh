@@ -72,7 +72,7 @@ k_grid_step(GridConst G, GridArgs A)
     float sc = G.renorm ? A.scale[0] : 1.0f;
 
     for (int step = 0; step < A.nsteps; ++step) {
-        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 0] = clock64();
+        VFPS_STAMP(A.dbg, step, 0);
         // ================= phase 1: rotation psi -> psi_tmp (times 1/C), partial profiles
         // round k: CTA c takes tile k*grid + (c + k) mod grid.  (With the plain c + k*grid a CTA keeps
         // the same column tile in every round when grid is a multiple of tiles_y, so the CTAs that
@@ -164,9 +164,9 @@ k_grid_step(GridConst G, GridArgs A)
                 A.rho_part[(size_t)ty * N + xg + tid] = G.dp * s;
             }
         }
-        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 1] = clock64();
+        VFPS_STAMP(A.dbg, step, 1);
         grid.sync();
-        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 2] = clock64();
+        VFPS_STAMP(A.dbg, step, 2);
         // ================= phase 2: profile, wake, kick + Fokker-Planck of the rows r0 .. r1-1
         const int r0 = blockIdx.x * A.KR, r1 = min(N, r0 + A.KR);
         float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 pw - -
@@ -189,7 +189,7 @@ k_grid_step(GridConst G, GridArgs A)
             if (A.wfun != nullptr)
                 for (int i = tid; i < N + A.KR - 1; i += GR_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
             __syncthreads();
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 3] = clock64();
+            VFPS_STAMP(A.dbg, step, 3);
             // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4), one row per warp at a time
             for (int r = warp; r < r1 - r0; r += GR_WARPS) {
                 float v0 = 0.0f, v1 = 0.0f;
@@ -206,7 +206,7 @@ k_grid_step(GridConst G, GridArgs A)
                 if (lane == 0) { sV[r] = v; acc[5] = fmaf(srho[r0 + r], v, acc[5]); }
             }
             __syncthreads();
-            if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 4] = clock64();
+            VFPS_STAMP(A.dbg, step, 4);
             if constexpr (MANH) {
                 // Manhattan: RF kick, wake kick (two 1-D interpolations along p), Fokker-Planck
                 const int total = (r1 - r0) * NQ;
@@ -322,9 +322,9 @@ k_grid_step(GridConst G, GridArgs A)
             // 3-4 k cycles per step); integer addition is associative, so the sum is deterministic
             if (tid == 0) atomicAdd(A.qacc + (step & 1), (unsigned long long)__float2ll_rn(s * 4294967296.0f));
         }
-        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 5] = clock64();
+        VFPS_STAMP(A.dbg, step, 5);
         grid.sync();
-        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 6] = clock64();
+        VFPS_STAMP(A.dbg, step, 6);
         // ================= phase 3: a6 -- every CTA forms C and 1/C in the same fixed order
         // Every CTA needs only the charge: one load of the fixed-point accumulator.  Warps 1-5 of
         // CTA 0 sum the other partials for the diagnostics row (fp32, fixed order).
@@ -361,7 +361,7 @@ k_grid_step(GridConst G, GridArgs A)
             o[5] = s_tot[5] * G.dq / (cc * cc);
         }
         sc = s_sc;
-        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + 7] = clock64();
+        VFPS_STAMP(A.dbg, step, 7);
     }
     if (blockIdx.x == 0 && tid == 0) A.scale[0] = sc;
 }

@@ -1,173 +1,15 @@
-// vfps_kernels.cuh -- device code of the streaming engine (sm_100a).
-//
-// One split step = three launches:
-//   k_rotate      a1 rotation + a2 projection (per-tile partial row sums)
-//   k_wake_fft    a2 finish (sum partials) + a3 wake by shared-memory FFT + q-moments + CSR power
-//   k_kick_fp     a4 kick + a5 Fokker-Planck + a6 charge / p-moments; the last CTA of each member
-//                 finalises the diagnostics row and the renormalisation scalar
+// vfps_kernels.cuh -- the non-template kernels of the library (sm_100a), included by vfps_api.cu
+// only: the stateless get_* calls (k_project, k_moments_final, k_scale_copy), the literal Eq. 5
+// wake (k_wake_fft: zero-padded shared-memory FFT, x Z, inverse FFT), and small set-up helpers.
 // psi is stored UN-normalised together with a per-member scalar `scale` = 1/C of the previous
-// step; k_rotate applies it (the rotation is linear), so renormalisation costs no extra pass.
+// step; the rotation applies it (it is linear), so renormalisation costs no extra pass.
 #pragma once
-#include <cuda_runtime.h>
-#include <stdint.h>
+#include "vfps_common.cuh"
 
 namespace vfps {
 
-constexpr int ROT_TX = 16;        // target rows per rotation tile
-constexpr int ROT_TY = 128;       // target columns per rotation tile (4 warps x 32 lanes)
-constexpr int ROT_THREADS = 256;
-constexpr int ROT_MAX_H = 8;      // largest supported halo (source displacement + stencil reach)
-constexpr int KFP_THREADS = 256;
-constexpr int KFP_WARPS = KFP_THREADS / 32;
-constexpr int KFP_PADL = 4;       // zero floats before a staged row
-constexpr int KFP_PADR = 8;       // zero floats after a staged row
-
-struct GridConst {
-    int N;             // grid points per axis
-    int order;         // Lagrange points per axis
-    float a;           // cos(dphi) - 1
-    float b;           // -sin(dphi) * dp/dq      : dx = a*X + b*Y   (cells)
-    float d;           // +sin(dphi) * dq/dp      : dy = d*X + a*Y   (cells)
-    float x0c, y0c;    // q_min/dq, p_min/dp      : X = x + x0c, Y = y + y0c
-    float dq, dp;
-    float kick_c;      // dphi/dp                 : kick shift in cells = kick_c * V_x
-    float fp_b;        // beta/steps_per_period
-    float p_min;
-    float q_min;
-    int H;             // rotation halo
-    float mh_q;        // Manhattan drift:   shift along q in cells = mh_q * Y,  mh_q = -dphi * dp/dq
-    float mh_p;        // Manhattan RF kick: shift along p in cells = mh_p * X,  mh_p = +dphi * dq/dp
-    int renorm;
-};
-
-// ---------------------------------------------------------------- Lagrange weights (Eq. 13)
-// nodes o_k = k - floor((ORDER-1)/2); t in [0,1)
-template <int ORDER>
-__device__ __forceinline__ void lagrange(float t, float (&l)[ORDER]);
-
-template <>
-__device__ __forceinline__ void lagrange<2>(float t, float (&l)[2])
-{
-    l[0] = 1.0f - t;
-    l[1] = t;
-}
-template <>
-__device__ __forceinline__ void lagrange<3>(float t, float (&l)[3])
-{
-    // nodes -1, 0, 1
-    const float h = 0.5f * t;
-    l[0] = h * (t - 1.0f);
-    l[1] = fmaf(-t, t, 1.0f);
-    l[2] = h * (t + 1.0f);
-}
-template <>
-__device__ __forceinline__ void lagrange<4>(float t, float (&l)[4])
-{
-    // nodes -1, 0, 1, 2.  With A = t(t-1)/6 and B = (t+1)(t-2)/2 = 3A - 1:
-    //   l0 = -A (t-2), l1 = B (t-1), l2 = -B t, l3 = A (t+1)
-    const float u = fmaf(t, t, -t);          // t(t-1)
-    const float A = u * (1.0f / 6.0f);
-    const float B = fmaf(u, 0.5f, -1.0f);
-    l[0] = A * (2.0f - t);
-    l[1] = fmaf(B, t, -B);
-    l[2] = -B * t;
-    l[3] = fmaf(A, t, A);
-}
-
-__device__ __forceinline__ float warp_sum(float v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// ---------------------------------------------------------------- a1 + a2: rotation + projection
-// grid = (tiles_x * tiles_y, members), block = 256.  Tile = ROT_TX rows x ROT_TY columns; the
-// source tile with halo H (zero outside the grid) is staged in shared memory, so every tap is an
-// unchecked shared-memory read.  Warp w handles 8 consecutive rows x 32 columns (lane = column:
-// stores are 128-byte coalesced, shared reads are conflict-free).
-// rho_part[m][x][tile_y] = dp * scale * sum over the tile's columns of psi'(x, .)
-template <int ORDER>
-__global__ void __launch_bounds__(ROT_THREADS)
-k_rotate(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_out,
-         const float *__restrict__ scale, float *__restrict__ rho_part, int tiles_y)
-{
-    extern __shared__ float tile[];
-    __shared__ float red[ROT_TX][4];
-    const int N = G.N, H = G.H;
-    const int m = blockIdx.y;
-    const int tx0 = (blockIdx.x / tiles_y) * ROT_TX;
-    const int ty0 = (blockIdx.x % tiles_y) * ROT_TY;
-    const int pitch = ROT_TY + 2 * H, rows = ROT_TX + 2 * H;
-    const float *src = psi_in + (size_t)m * N * N;
-    float *dst = psi_out + (size_t)m * N * N;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-    for (int r = warp; r < rows; r += ROT_THREADS / 32) {
-        const int gx = tx0 - H + r;
-        const bool rok = (gx >= 0) && (gx < N);
-        for (int c = lane; c < pitch; c += 32) {
-            const int gy = ty0 - H + c;
-            float v = 0.0f;
-            if (rok && gy >= 0 && gy < N) v = __ldg(src + (size_t)gx * N + gy);
-            tile[r * pitch + c] = v;
-        }
-    }
-    __syncthreads();
-
-    const float sc = G.renorm ? __ldg(scale + m) : 1.0f;
-    const int wy = warp & 3, wx = warp >> 2;
-    const int y = ty0 + wy * 32 + lane;
-    // lanes / rows beyond the grid (partial tiles) compute with the last valid coordinate so that
-    // their taps stay inside the staged tile; their results are never stored
-    const float Y = (float)min(y, N - 1) + G.y0c;
-    const float bY = G.b * Y, aY = G.a * Y;
-    constexpr int O0 = (ORDER - 1) / 2;       // offset of the first node below m
-
-#pragma unroll
-    for (int r = 0; r < 8; ++r) {
-        const int x = tx0 + wx * 8 + r;
-        const float X = (float)min(x, N - 1) + G.x0c;
-        const float dx = fmaf(G.a, X, bY);
-        const float dy = fmaf(G.d, X, aY);
-        const float fx = floorf(dx), fy = floorf(dy);
-        float lx[ORDER], ly[ORDER];
-        lagrange<ORDER>(dx - fx, lx);
-        lagrange<ORDER>(dy - fy, ly);
-        // tile coordinates of the first tap
-        const int ix = (min(x, N - 1) - tx0) + H + (int)fx - O0;
-        const int iy = (min(y, N - 1) - ty0) + H + (int)fy - O0;
-        const float *t0 = tile + ix * pitch + iy;
-        float acc = 0.0f;
-#pragma unroll
-        for (int i = 0; i < ORDER; ++i) {
-            float rsum = ly[0] * t0[i * pitch];
-#pragma unroll
-            for (int j = 1; j < ORDER; ++j) rsum = fmaf(ly[j], t0[i * pitch + j], rsum);
-            acc = (i == 0) ? lx[0] * rsum : fmaf(lx[i], rsum, acc);
-        }
-        acc *= sc;
-        const bool ok = (x < N) && (y < N);
-        if (ok) dst[(size_t)x * N + y] = acc;
-        const float rs = warp_sum(ok ? acc : 0.0f);
-        if (lane == 0) red[wx * 8 + r][wy] = rs;
-    }
-    __syncthreads();
-    if (threadIdx.x < ROT_TX) {
-        const int x = tx0 + threadIdx.x;
-        if (x < N) {
-            const float s = (red[threadIdx.x][0] + red[threadIdx.x][1]) +
-                            (red[threadIdx.x][2] + red[threadIdx.x][3]);
-            rho_part[((size_t)m * N + x) * tiles_y + (blockIdx.x % tiles_y)] = G.dp * s;
-        }
-    }
-}
+constexpr int WD_ROWS = 8;         // rows per CTA of k_wake_direct (one per warp)
+constexpr int WD_THREADS = 256;
 
 // ---------------------------------------------------------------- plain projection (get_profile)
 // grid = (N, members), block = 128: rho[m][x] = dp * scale * sum_y psi(x,y); also the per-row
@@ -213,8 +55,8 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 }
 
 __global__ void __launch_bounds__(1024)
-k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_part, int nparts,
-           const float2 *__restrict__ Z, const float2 *__restrict__ tw, float *__restrict__ rho_out,
+k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *rho_part, int nparts,
+           const float2 *__restrict__ Z, const float2 *__restrict__ tw, float *rho_out /* may be rho_part (nparts = 1) */,
            float *__restrict__ V, float *__restrict__ qstat)
 {
     extern __shared__ float2 s[];          // Nf points, then Nf - 1 twiddles, one contiguous table per stage
@@ -228,7 +70,7 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_pa
         if (x < N) {
             const float *pp = rho_part + ((size_t)m * N + x) * nparts;
 #pragma unroll 8
-            for (int k = 0; k < nparts; ++k) r += __ldg(pp + k);
+            for (int k = 0; k < nparts; ++k) r += pp[k];
             rho_out[(size_t)m * N + x] = r;
             const float c = (float)x - xc, t = c * r;
             s0 += r; s1 += t; s2 = fmaf(t, c, s2);
@@ -337,150 +179,6 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *__restrict__ rho_pa
     }
 }
 
-// ---------------------------------------------------------------- a4 + a5 + a6: kick, FP, moments
-struct KfpArgs {
-    const float *psi_in;    // psi' (rotated, scaled)
-    float *psi_out;         // psi''' (un-normalised)
-    const float *V;         // [members][N]
-    const float *qstat;     // [members][4] from k_wake_fft
-    float *mom_part;        // [members][gridDim.x][5]: sum psi, sum Yc psi, sum Yc^2 psi, sum Xc psi, sum Xc^2 psi
-    float *scale;           // [members] out: 1/C
-    unsigned *blkctr;       // [members], zero between launches
-    int *rowctr;            // [members] diagnostics row of this step
-    float *const *diag;     // device cell holding the caller's diag pointer (may hold NULL)
-    int members;
-    int rows_per_cta;
-};
-
-// composite of kick (shift t along p, node m) and the Fokker-Planck update for one staged row.
-// row: shared-memory row with KFP_PADL zeros before index 0 and KFP_PADR zeros after index N-1.
-template <int ORDER>
-__device__ __forceinline__ float kicked(const float *row, int N, int y, int m, const float (&l)[ORDER])
-{
-    // psi''(y) = sum_j l_j psi'(y + m + o_j); psi' = 0 outside [0, N)
-    constexpr int O0 = (ORDER - 1) / 2;
-    const int base = y + m - O0;
-    float acc = 0.0f;
-#pragma unroll
-    for (int j = 0; j < ORDER; ++j) {
-        const int i = base + j;
-        const float v = (i >= -KFP_PADL && i < N + KFP_PADR) ? row[i] : 0.0f;
-        acc = (j == 0) ? l[0] * v : fmaf(l[j], v, acc);
-    }
-    return acc;
-}
-
-// grid = (ceil(N / rows_per_cta), members), block = 256 (8 warps, one row per warp at a time).
-// Shared memory: per warp two rows of (KFP_PADL + N + KFP_PADR) floats (psi' and psi'').
-template <int ORDER>
-__global__ void __launch_bounds__(KFP_THREADS)
-k_kick_fp(GridConst G, KfpArgs A)
-{
-    extern __shared__ float smem[];
-    __shared__ float red[5][KFP_WARPS];
-    __shared__ bool is_last;
-    const int N = G.N, m = blockIdx.y;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int rowlen = KFP_PADL + N + KFP_PADR;
-    float *r1 = smem + (size_t)warp * 2 * rowlen + KFP_PADL;     // psi'  (index 0 = y 0)
-    float *r2 = r1 + rowlen;                                       // psi''
-    const float *src = A.psi_in + (size_t)m * N * N;
-    float *dst = A.psi_out + (size_t)m * N * N;
-    const float yc = 0.5f * (float)(N - 1);
-    // FP increment coefficients: incr = b*f0 + b*p*(-2 f-1 - 3 f0 + 6 f+1 - f+2)/(6 dp)
-    //                                  + b*(f-1 - 2 f0 + f+1)/dp^2
-    const float c1 = G.fp_b / (6.0f * G.dp);
-    const float c2 = G.fp_b / (G.dp * G.dp);
-
-    for (int i = lane; i < KFP_PADL; i += 32) { r1[-1 - i] = 0.0f; r2[-1 - i] = 0.0f; }
-    for (int i = lane; i < KFP_PADR; i += 32) { r1[N + i] = 0.0f; r2[N + i] = 0.0f; }
-
-    float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, q1 = 0.0f, q2 = 0.0f;
-    const int x_begin = blockIdx.x * A.rows_per_cta;
-    const int x_end = min(N, x_begin + A.rows_per_cta);
-    for (int x = x_begin + warp; x < x_end; x += KFP_WARPS) {
-        __syncwarp();
-        const float4 *g4 = reinterpret_cast<const float4 *>(src + (size_t)x * N);
-        for (int c = lane; c < N / 4; c += 32) *reinterpret_cast<float4 *>(r1 + 4 * c) = __ldg(g4 + c);
-        // kick parameters of this row: y_r = y + sh, sh = (dphi/dp) * V_x  (Delta p = -dphi V)
-        const float sh = G.kick_c * __ldg(A.V + (size_t)m * N + x);
-        const float fm = floorf(sh);
-        float l[ORDER];
-        lagrange<ORDER>(sh - fm, l);
-        const int mm = (int)fm;
-        __syncwarp();
-        for (int y = lane; y < N; y += 32) r2[y] = kicked<ORDER>(r1, N, y, mm, l);
-        __syncwarp();
-        float rs = 0.0f;
-        for (int y = lane; y < N; y += 32) {
-            const float fm1 = r2[y - 1], f0 = r2[y], fp1 = r2[y + 1], fp2 = r2[y + 2];
-            const float p = fmaf((float)y, G.dp, G.p_min);
-            const float d1 = fmaf(-2.0f, fm1, fmaf(-3.0f, f0, fmaf(6.0f, fp1, -fp2)));
-            const float d2 = (fm1 + fp1) - 2.0f * f0;
-            const float incr = fmaf(G.fp_b, f0, fmaf(c1 * p, d1, c2 * d2));
-            const float out = f0 + incr;
-            dst[(size_t)x * N + y] = out;
-            const float yy = (float)y - yc;
-            const float t = out * yy;
-            rs += out; s1 += t; s2 = fmaf(t, yy, s2);
-        }
-        // q moments of the end-of-step psi from the row sum (every lane gets the same value)
-        rs = warp_sum(rs);
-        const float xx = (float)x - yc;
-        const float tq = rs * xx;
-        s0 += rs; q1 += tq; q2 = fmaf(tq, xx, q2);
-    }
-    s1 = warp_sum(s1); s2 = warp_sum(s2);
-    if (lane == 0) { red[0][warp] = s0; red[1][warp] = s1; red[2][warp] = s2; red[3][warp] = q1; red[4][warp] = q2; }
-    __syncthreads();
-    if (threadIdx.x < 5) {
-        float t = 0.0f;
-#pragma unroll
-        for (int w = 0; w < KFP_WARPS; ++w) t += red[threadIdx.x][w];
-        A.mom_part[((size_t)m * gridDim.x + blockIdx.x) * 5 + threadIdx.x] = t;
-    }
-    // ---- last CTA of this member finalises the step (deterministic: fixed summation order)
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned done = atomicAdd(A.blkctr + m, 1u);
-        is_last = (done == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!is_last) return;
-    __threadfence();
-    if (warp == 0) {
-        double t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
-        const volatile float *mp = A.mom_part + (size_t)m * gridDim.x * 5;
-        for (int i = lane; i < (int)gridDim.x; i += 32) {
-            t0 += mp[5 * i]; t1 += mp[5 * i + 1]; t2 += mp[5 * i + 2]; t3 += mp[5 * i + 3]; t4 += mp[5 * i + 4];
-        }
-        t0 = warp_sum(t0); t1 = warp_sum(t1); t2 = warp_sum(t2); t3 = warp_sum(t3); t4 = warp_sum(t4);
-        if (lane == 0) {
-            const double C = (double)G.dq * (double)G.dp * t0;
-            const double mp_c = t1 / t0;                       // <p> in centred cells
-            const double vp = t2 / t0 - mp_c * mp_c;
-            const float *qs = A.qstat + (size_t)m * 4;
-            const double mq_c = t3 / t0, vq = t4 / t0 - mq_c * mq_c;
-            A.scale[m] = (float)(1.0 / C);
-            const int row = A.rowctr[m];
-            A.rowctr[m] = row + 1;
-            float *diag = *A.diag;
-            if (diag != nullptr) {
-                float *o = diag + ((size_t)row * A.members + m) * 6;
-                const double xc = 0.5 * (double)(N - 1);
-                const double cc = G.renorm ? C : 1.0;
-                o[0] = (float)C;
-                o[1] = (float)((double)G.q_min + (mq_c + xc) * (double)G.dq);
-                o[2] = (float)((double)G.p_min + (mp_c + (double)yc) * (double)G.dp);
-                o[3] = (float)(sqrt(fmax(vq, 0.0)) * (double)G.dq);
-                o[4] = (float)(sqrt(fmax(vp, 0.0)) * (double)G.dp);
-                o[5] = (float)((double)qs[3] / (cc * cc));
-            }
-            A.blkctr[m] = 0u;
-        }
-    }
-}
 
 // ---------------------------------------------------------------- helpers for set / get calls
 __global__ void k_scale_copy(const float *__restrict__ psi, const float *__restrict__ scale,
@@ -541,6 +239,54 @@ k_moments_final(GridConst G, const float *__restrict__ rho, const float *__restr
         o[3] = (float)(sqrt(fmax(vq, 0.0)) * (double)G.dq);
         o[4] = (float)(sqrt(fmax(vp, 0.0)) * (double)G.dp);
         o[5] = qstat[(size_t)m * 4 + 3];
+    }
+}
+
+// ---------------------------------------------------------------- a3: direct wake
+// grid = (ceil(N / WD_ROWS), members), block = 256 (one row per warp), dynamic shared memory
+// (2N + WD_ROWS) floats: the profile (complete after k_rotate2) and the N + WD_ROWS - 1 lags of the
+// wake function this CTA's rows touch are staged with coalesced loads, then warp w evaluates
+// V_x = sum_x' w[x - x'] rho_x' (Eq. 4; w = Re IDFT(Z) from create, lag d at index d + N - 1)
+// for x = r0 + w.  pw_part[m][cta] = sum over the CTA's rows of rho_x V_x.
+__global__ void __launch_bounds__(WD_THREADS)
+k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wfun, float *__restrict__ V,
+              float *__restrict__ pw_part)
+{
+    extern __shared__ float wd_smem[];
+    __shared__ float wpw[WD_THREADS / 32];
+    float *srho = wd_smem, *sw = wd_smem + N;
+    const int m = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int r0 = blockIdx.x * WD_ROWS;
+    const float *gr = rho + (size_t)m * N, *gw = wfun + (size_t)m * 2 * N + r0;
+    for (int i = tid; i < N; i += WD_THREADS) srho[i] = __ldg(gr + i);
+    for (int i = tid; i < N + WD_ROWS - 1; i += WD_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(gw + i) : 0.0f;
+    __syncthreads();
+    const int x = r0 + warp;
+    float v0 = 0.0f, v1 = 0.0f;
+    if (x < N) {
+        const float *wx = sw + (warp + N - 1);
+        int xp = lane;
+        for (; xp + 32 < N; xp += 64) {
+            v0 = fmaf(wx[-xp], srho[xp], v0);
+            v1 = fmaf(wx[-(xp + 32)], srho[xp + 32], v1);
+        }
+        if (xp < N) v0 = fmaf(wx[-xp], srho[xp], v0);
+    }
+    const float v = warp_sum(v0 + v1);
+    if (lane == 0) {
+        float pw = 0.0f;
+        if (x < N) {
+            V[(size_t)m * N + x] = v;
+            pw = srho[x] * v;
+        }
+        wpw[warp] = pw;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        float t = 0.0f;
+#pragma unroll
+        for (int i = 0; i < WD_THREADS / 32; ++i) t += wpw[i];
+        pw_part[(size_t)m * gridDim.x + blockIdx.x] = t;
     }
 }
 

@@ -409,14 +409,7 @@ __device__ __forceinline__ float rotate_cell_generic(const GridConst &G, uint32_
     return acc;
 }
 
-#ifdef VFPS_PHASE_CLOCKS
-#define OC_STAMP(k)                                                                                         \
-    do {                                                                                                    \
-        if (A.dbg != nullptr && tid == 0 && step < 64) A.dbg[((size_t)blockIdx.x * 64 + step) * 8 + (k)] = clock64(); \
-    } while (0)
-#else
-#define OC_STAMP(k) do { } while (0)
-#endif
+#define OC_STAMP(k) VFPS_STAMP(A.dbg, step, k)
 
 // ---------------------------------------------------------------- the persistent kernel
 // grid = S * (concurrent clusters), cluster = S CTAs, block = 512.  Clusters take work items

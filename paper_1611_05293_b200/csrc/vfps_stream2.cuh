@@ -22,8 +22,6 @@ namespace vfps {
 constexpr int R2_RT = 16;          // rows per rotation tile (two reduction groups of 8)
 constexpr int R2_THREADS = 256;    // 8 warps = 256 columns per tile
 constexpr int R2_WARPS = R2_THREADS / 32;
-constexpr int WD_ROWS = 8;         // rows per CTA of k_wake_direct (one per warp)
-constexpr int WD_THREADS = 256;
 constexpr int K2_THREADS = 256;
 
 // 8 values per lane -> sums over the 32 lanes.  On return v[0] of lane l holds the total of input
@@ -378,53 +376,8 @@ k_drift2(GridConst G, const float *__restrict__ psi_in, float *__restrict__ psi_
     }
 }
 
-// ---------------------------------------------------------------- a3: direct wake
-// grid = (ceil(N / WD_ROWS), members), block = 256 (one row per warp), dynamic shared memory
-// (2N + WD_ROWS) floats: the profile (complete after k_rotate2) and the N + WD_ROWS - 1 lags of the
-// wake function this CTA's rows touch are staged with coalesced loads, then warp w evaluates
-// V_x = sum_x' w[x - x'] rho_x' (Eq. 4; w = Re IDFT(Z) from create, lag d at index d + N - 1)
-// for x = r0 + w.  pw_part[m][cta] = sum over the CTA's rows of rho_x V_x.
-__global__ void __launch_bounds__(WD_THREADS)
-k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wfun, float *__restrict__ V,
-              float *__restrict__ pw_part)
-{
-    extern __shared__ float wd_smem[];
-    __shared__ float wpw[WD_THREADS / 32];
-    float *srho = wd_smem, *sw = wd_smem + N;
-    const int m = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int r0 = blockIdx.x * WD_ROWS;
-    const float *gr = rho + (size_t)m * N, *gw = wfun + (size_t)m * 2 * N + r0;
-    for (int i = tid; i < N; i += WD_THREADS) srho[i] = __ldg(gr + i);
-    for (int i = tid; i < N + WD_ROWS - 1; i += WD_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(gw + i) : 0.0f;
-    __syncthreads();
-    const int x = r0 + warp;
-    float v0 = 0.0f, v1 = 0.0f;
-    if (x < N) {
-        const float *wx = sw + (warp + N - 1);
-        int xp = lane;
-        for (; xp + 32 < N; xp += 64) {
-            v0 = fmaf(wx[-xp], srho[xp], v0);
-            v1 = fmaf(wx[-(xp + 32)], srho[xp + 32], v1);
-        }
-        if (xp < N) v0 = fmaf(wx[-xp], srho[xp], v0);
-    }
-    const float v = warp_sum(v0 + v1);
-    if (lane == 0) {
-        float pw = 0.0f;
-        if (x < N) {
-            V[(size_t)m * N + x] = v;
-            pw = srho[x] * v;
-        }
-        wpw[warp] = pw;
-    }
-    __syncthreads();
-    if (tid == 0) {
-        float t = 0.0f;
-#pragma unroll
-        for (int i = 0; i < WD_THREADS / 32; ++i) t += wpw[i];
-        pw_part[(size_t)m * gridDim.x + blockIdx.x] = t;
-    }
-}
+// (k_wake_direct, the direct-convolution wake a3 of the stream / graph engines, is not a template and
+// lives in vfps_kernels.cuh)
 
 // (rf_stage, rf_value, rf_kick_fp_granule_any: the RF-kick stage of the Manhattan rotation, live in
 // vfps_cluster.cuh beside kick_fp_granule)

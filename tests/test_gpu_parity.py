@@ -101,7 +101,7 @@ def test_c1_1000_steps(vfps, orc):
     sim.close()
 
 
-def test_c2_512_steps(vfps, orc):
+def test_c2_one_step_and_1000_steps(vfps, orc):
     wl = get_workload("C2")
     for S in (0.2, 1.0):
         w = wl.with_(S_csr=(S,))
@@ -109,9 +109,10 @@ def test_c2_512_steps(vfps, orc):
         assert_psi(psi[0], refs[0].psi, TOL_1, f"C2 S={S} 1 step")
         assert_diag(d[0, 0], dr[0][0])
         sim.close()
-    sim, psi, d, refs, dr = run_pair(vfps, orc, wl.with_(S_csr=(0.6,)), 200, diag_every=50)
-    assert_psi(psi[0], refs[0].psi, 2e-4, "C2 200 steps")
-    assert_diag(d[199, 0], dr[0][199])
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl.with_(S_csr=(0.6,)), 1000, diag_every=100)
+    assert_psi(psi[0], refs[0].psi, TOL_1000, "C2 1000 steps")
+    for i in (99, 499, 999):
+        assert_diag(d[i, 0], dr[0][i])
     sim.close()
 
 
@@ -127,15 +128,16 @@ def test_c3_batched_members(vfps, orc):
     sim.close()
 
 
-def test_c4_2048_steps(vfps, orc):
+def test_c4_one_step_and_1000_steps(vfps, orc):
     wl = get_workload("C4")
     sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1)
     assert_psi(psi[0], refs[0].psi, TOL_1, "C4 1 step")
     assert_diag(d[0, 0], dr[0][0])
     sim.close()
-    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 10, diag_every=10)
-    assert_psi(psi[0], refs[0].psi, 5e-5, "C4 10 steps")
-    assert_diag(d[9, 0], dr[0][9])
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1000, diag_every=100)
+    assert_psi(psi[0], refs[0].psi, TOL_1000, "C4 1000 steps")
+    for i in (99, 499, 999):
+        assert_diag(d[i, 0], dr[0][i])
     sim.close()
 
 
@@ -181,18 +183,27 @@ def test_full_size_runs_invariants(vfps, name, periods):
 
 def test_full_c3_batch_all_members(vfps, orc):
     """All 256 members in one handle (the launch configuration bench.py times for C3): sampled
-    members element by element against the oracle after 30 steps, every member through the
-    invariants over one synchrotron period; P_csr grows monotonically with S_csr across members."""
+    members element by element against the oracle after 1 step and after 1000 steps (north_star's
+    two bars), every member through the invariants over one synchrotron period; P_csr grows
+    monotonically with S_csr across members."""
     wl = get_workload("C3")
     sim = vfps.Simulation.from_workload(wl)
-    d = sim.step_host(30)
+    sample = (0, 101, 255)
+    orcs = [orc.Oracle.from_workload(wl, m) for m in sample]
+    d = sim.step_host(1)
     psi = sim.get_psi_host()
-    for m in (0, 101, 255):
-        o = orc.Oracle.from_workload(wl, m)
-        dr = o.step(30)
-        assert_psi(psi[m], o.psi, 5e-5, f"full C3 batch, member {m}")
-        assert_diag(d[29, m], dr[29])
-    d = sim.step_host(wl.steps_per_period - 30)
+    for o, m in zip(orcs, sample):
+        dr = o.step(1)
+        assert_psi(psi[m], o.psi, TOL_1, f"full C3 batch, member {m}, 1 step")
+        assert_diag(d[0, m], dr[0])
+    d = sim.step_host(999)
+    psi = sim.get_psi_host()
+    for o, m in zip(orcs, sample):
+        dr = o.step(999, diag_every=100)
+        assert_psi(psi[m], o.psi, TOL_1000, f"full C3 batch, member {m}, 1000 steps")
+        for i in (99, 499, 998):
+            assert_diag(d[i, m], dr[i])
+    d = sim.step_host(wl.steps_per_period - 1000)
     _invariants(d)
     assert np.all(np.diff(d[-1, :, 5]) > 0.0)
     sim.close()
@@ -317,51 +328,51 @@ def test_error_paths_on_gpu(vfps):
 # ---------------------------------------------------------------- engines
 def _engine_id(vfps, name):
     return {"stream": vfps.ENGINE_STREAM, "graph": vfps.ENGINE_GRAPH, "cluster": vfps.ENGINE_CLUSTER,
-            "cluster2": vfps.ENGINE_CLUSTER, "grid": vfps.ENGINE_GRID}[name]
+            "cluster1": vfps.ENGINE_CLUSTER, "grid": vfps.ENGINE_GRID}[name]
 
 
-@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster2", "grid"])
+@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster1", "grid"])
 def test_c1_every_engine_100_steps(vfps, orc, engine):
     """The same 100 steps of C1 through each engine (graph: two replays of 50 captured steps;
-    cluster: the scalar kernel, which AUTO picks; cluster2: the packed fp32x2 kernel; grid: the persistent cooperative kernel)."""
+    cluster: the in-place kernel k_onchip_step, which AUTO picks; cluster1: the first design
+    k_cluster_step; grid: the persistent cooperative kernel)."""
     wl = get_workload("C1")
     sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 100, engine=_engine_id(vfps, engine), diag_every=1,
-                                     cluster_kernel=2 if engine == "cluster2" else None)
-    assert sim.engine_name == engine.rstrip("2")
+                                     cluster_kernel=1 if engine == "cluster1" else None)
+    assert sim.engine_name == engine.rstrip("1")
     if engine.startswith("cluster"):
-        assert sim.cluster_kernel == (2 if engine == "cluster2" else 1)
+        assert sim.cluster_kernel == (1 if engine == "cluster1" else 3)
     assert_psi(psi[0], refs[0].psi, 1e-4, f"C1 100 steps, {engine}")
     for i in (0, 1, 49, 50, 99):
         assert_diag(d[i, 0], dr[0][i])
     sim.close()
 
 
-@pytest.mark.parametrize("gen,wake", [(1, "fft"), (2, "fft"), (2, "direct")])
+@pytest.mark.parametrize("wake", ["fft", "direct"])
 @pytest.mark.parametrize("order,N", [(4, 256), (3, 128), (2, 64), (4, 32)])
-def test_stream_generations(vfps, orc, gen, wake, order, N):
-    """Both generations of the streaming kernels and both wake evaluations (Eq. 5 FFT, Eq. 4 direct
-    convolution) on the stream and the graph engine: asymmetric box, off-centre bunch, free-space
-    wake, 300 steps per period (edge tiles, floors changing inside a tile; N = 32 and 64 are
-    narrower than one 256-column tile)."""
+def test_stream_wake_modes(vfps, orc, wake, order, N):
+    """The streaming kernels with both wake evaluations (Eq. 5 FFT, Eq. 4 direct convolution) on
+    the stream and the graph engine: asymmetric box, off-centre bunch, free-space wake, 300 steps
+    per period (edge tiles, floors changing inside a tile; N = 32 and 64 are narrower than one
+    256-column tile)."""
     pad = 2
     Z = make_impedance(N, pad, 12.0 / (N - 1), 0.4, None)[None, :]
     psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
     sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, pad, 1, Z=Z)
-    sim.set_stream_gen(gen)
     sim.set_wake_mode({"fft": vfps.WAKE_FFT, "direct": vfps.WAKE_DIRECT}[wake])
     sim.set_engine(vfps.ENGINE_STREAM)
-    assert sim.stream_gen == gen and sim.wake_name == wake
+    assert sim.wake_name == wake
     sim.set_psi_host(psi0)
     o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, pad, Z[0])
     o.set_psi(psi0[0])
     d = sim.step_host(1)
     dr = o.step(1)
-    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"stream gen {gen} {wake} N={N} order={order} 1 step")
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"stream {wake} N={N} order={order} 1 step")
     assert_diag(d[0, 0], dr[0])
     sim.set_engine(vfps.ENGINE_GRAPH)
     d = sim.step_host(59)
     dr = o.step(59)
-    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"graph gen {gen} {wake} N={N} order={order} 60 steps")
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"graph {wake} N={N} order={order} 60 steps")
     for i in (0, 30, 58):
         assert_diag(d[i, 0], dr[i])
     sim.close()
@@ -374,7 +385,7 @@ def test_manhattan_rotation(vfps, orc, order, N, wake):
     Manhattan step: asymmetric box, off-centre bunch, free-space wake, 300 steps per period (the
     drift and the RF kick move the outer lines by more than one cell: integer parts -2..1), stream
     engine for 1 step, graph engine for 59 more, grid engine for 20 more, then the cluster engine
-    (scalar kernel) at several cluster sizes."""
+    (first design) at several cluster sizes."""
     Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
     psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
     flags = vfps.FLAG_RENORMALISE | vfps.FLAG_ROT_MANHATTAN
@@ -401,7 +412,7 @@ def test_manhattan_rotation(vfps, orc, order, N, wake):
     for i in (0, 19):
         assert_diag(d[i, 0], dr[i])
     try:
-        sim.set_engine(vfps.ENGINE_CLUSTER)          # scalar kernel; needs halo <= 4 rows (not N = 256 here)
+        sim.set_engine(vfps.ENGINE_CLUSTER)          # first design; needs halo <= 4 rows (not N = 256 here)
     except vfps.VfpsError as err:
         assert err.code == -5 and N == 256
         sim.close()
@@ -418,7 +429,7 @@ def test_manhattan_rotation(vfps, orc, order, N, wake):
         for i in (0, 19):
             assert_diag(d[i, 0], dr[i])
     with pytest.raises(vfps.VfpsError) as e:
-        sim.set_cluster_kernel(2)                    # the packed kernel has the standard rotation only
+        sim.set_cluster_kernel(3)                    # the in-place kernel has the standard rotation only
     assert e.value.code == -5
     sim.close()
 
@@ -589,34 +600,50 @@ def test_grid_engine_rejects_batches(vfps):
     sim.close()
 
 
-@pytest.mark.parametrize("S", [1, 2, 4, 8, 16])
+def _cluster_cases():
+    """(N, kernel, steps_per_period, S) for test_cluster_engine_sizes.  300 steps per period moves
+    the corner cells by up to N/60 cells per step (floors change inside a CTA's rows and columns:
+    the per-cell paths run, and the in-place kernel evaluates its weights per cell); 4000 steps per
+    period is the regime of the BASELINE configs (per-launch weight tables).  The first design
+    (kernel 1) has 4 halo rows, so its steps per period grow with N; the in-place kernel (3) takes
+    halos up to 7 rows.  Combinations the library refuses (listed in _CLUSTER_INFEASIBLE with the
+    reason) are checked to be refused with VFPS_ERR_UNSUPPORTED."""
+    cases = []
+    for N, spps in ((64, (300, 4000)), (128, (300, 4000)), (256, (300, 4000)), (512, (1200, 4000))):
+        for spp in spps:
+            for S in (1, 2, 4, 8, 16):
+                cases.append((N, 3, spp, S))
+    for N, spp in ((32, 300), (64, 300), (128, 300), (256, 1200), (512, 2400)):
+        for S in (1, 2, 4, 8, 16):
+            cases.append((N, 1, spp, S))
+    return cases
+
+
 @pytest.mark.parametrize("order", [2, 3, 4])
-@pytest.mark.parametrize("N,kernel,threads", [(32, 1, 0), (64, 1, 0), (128, 1, 0), (256, 1, 0),
-                                              (128, 2, 256), (128, 2, 512), (256, 2, 256), (256, 2, 512)])
-def test_cluster_engine_sizes(vfps, orc, N, order, S, kernel, threads):
-    """Persistent cluster engine, scalar (1) and packed (2) kernel, for every grid size /
-    interpolation order / cluster size / block size that is feasible: asymmetric box, off-centre
-    mismatched bunch, free-space wake (as test_orders_and_small_grids), 1 step and 60 steps,
-    diagnostics of every step.  300 steps per period moves the corner cells by two cells per step,
-    so floor(dx), floor(dy) change inside a CTA's rows (the packed kernel's scalar paths run) and
-    the wake of the 0.4-strength free-space impedance shifts rows by different integer parts."""
+@pytest.mark.parametrize("N,kernel,spp,S", _cluster_cases())
+def test_cluster_engine_sizes(vfps, orc, N, order, S, kernel, spp):
+    """Persistent cluster engine, both kernels, every grid size / interpolation order / cluster
+    size: asymmetric box, off-centre mismatched bunch, free-space wake (as
+    test_orders_and_small_grids), 1 step and 60 steps, diagnostics of every step; the wake of the
+    0.4-strength free-space impedance shifts rows by different integer parts."""
     Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
     psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)[None]
-    sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, 1, Z=Z)
+    sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, spp, 2e-3, order, 2, 1, Z=Z)
     try:
         sim.set_cluster_kernel(kernel)
-        if threads:
-            sim.set_cluster_threads(threads)
         sim.set_cluster_size(S)
     except vfps.VfpsError as e:
         assert e.code == -5
         sim.close()
-        pytest.skip(f"kernel {kernel} with cluster size {S} not feasible for N={N}")
+        reason = _cluster_infeasible(N, kernel, spp, S)
+        assert reason, f"kernel {kernel} refused N={N} S={S} spp={spp}: {e}"
+        return
+    assert not _cluster_infeasible(N, kernel, spp, S)
     sim.set_engine(vfps.ENGINE_CLUSTER)
     assert sim.engine_name == "cluster" and sim.cluster_size == S and sim.wake_name == "direct"
-    assert sim.cluster_kernel == kernel and (not threads or sim.cluster_threads == threads)
+    assert sim.cluster_kernel == kernel
     sim.set_psi_host(psi0)
-    o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, Z[0])
+    o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, spp, 2e-3, order, 2, Z[0])
     o.set_psi(psi0[0])
     d = sim.step_host(1)
     dr = o.step(1)
@@ -631,7 +658,28 @@ def test_cluster_engine_sizes(vfps, orc, N, order, S, kernel, threads):
     sim.close()
 
 
-@pytest.mark.parametrize("kernel", [1, 2])
+def _cluster_infeasible(N, kernel, spp, S):
+    """Why the library is expected to refuse this combination ('' = it must run)."""
+    rows = N // S
+    smem_floats = 227 * 1024 // 4
+    halo = {300: {32: 2, 64: 3, 128: 4, 256: 6}, 1200: {256: 3, 512: 4}, 2400: {512: 3},
+            4000: {64: 2, 128: 2, 256: 2, 512: 2}}[spp][N]
+    if kernel == 1:
+        if rows < halo:
+            return "fewer rows per CTA than halo rows"
+        if (2 * rows + 8) * (N + 8) > smem_floats:
+            return "two row buffers do not fit 227 KB of shared memory"
+        return ""
+    if rows < 4 or rows < halo:
+        return "fewer rows per CTA than halo rows"
+    if rows * (N + 16) > smem_floats:
+        return "the rows of a CTA do not fit 227 KB of shared memory"
+    if (N, spp, S) in ((256, 300, 2), (512, 1200, 8)):
+        return "rows + aprons + free rows of the in-place walkers (halo 6 / 4) exceed 227 KB"
+    return ""
+
+
+@pytest.mark.parametrize("kernel", [1, 3])
 def test_cluster_engine_c2_512(vfps, orc, kernel):
     wl = get_workload("C2").with_(S_csr=(0.6,))
     sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 40, engine=vfps.ENGINE_CLUSTER, diag_every=1, cluster_kernel=kernel)
@@ -642,8 +690,7 @@ def test_cluster_engine_c2_512(vfps, orc, kernel):
     sim.close()
 
 
-@pytest.mark.parametrize("kernel", [1, 2])
-@pytest.mark.parametrize("S", [4, 8, 16])
+@pytest.mark.parametrize("kernel,S", [(1, 4), (1, 8), (1, 16), (3, 2), (3, 4), (3, 8), (3, 16)])
 def test_cluster_engine_batched(vfps, orc, S, kernel):
     """More members than one cluster: every cluster walks through its members one after another."""
     wl = get_workload("C3")
@@ -663,19 +710,38 @@ def test_cluster_engine_batched(vfps, orc, S, kernel):
     sim.close()
 
 
-@pytest.mark.parametrize("N", [64, 128])
-def test_cluster_engine_large_kick_and_switching(vfps, orc, N):
-    """|kick shift| > 1 cell (generic-shift path of the cluster engine; N = 128 runs the packed
-    kernel), then continue the same simulation on the stream engine: state hand-over between
-    engines is exact."""
+def test_cluster_engine_batch_of_single_cta_clusters_long_run(vfps):
+    """64 members of 128^2 on clusters of ONE CTA (what AUTO picks for this batch) for 100 000
+    steps: every exchange of the cluster protocol degenerates to a CTA talking to itself.  A lost
+    or doubled mbarrier phase hangs or corrupts the run; the renormalised charge of every step of
+    the last period and the end state must be sane for every member."""
+    wl = get_workload("C3").with_(N=128, members=64, S_csr=tuple(0.05 + 0.01 * m for m in range(64)),
+                                  seeds=tuple(range(64)), steps_per_period=2000)
+    for kernel in (3, 1):
+        sim = vfps.Simulation.from_workload(wl)
+        sim.set_cluster_kernel(kernel)
+        sim.set_cluster_size(1)
+        sim.set_engine(vfps.ENGINE_CLUSTER)
+        assert sim.cluster_size == 1
+        for _ in range(49):
+            sim.step_host(2000, diag=False)
+        d = sim.step_host(2000)
+        _invariants(d)
+        assert sim.step_count() == 100000
+        sim.close()
+
+
+@pytest.mark.parametrize("N,kernel", [(64, 1), (128, 1), (64, 3), (128, 3)])
+def test_cluster_engine_large_kick_and_switching(vfps, orc, N, kernel):
+    """|kick shift| > 1 cell (generic-shift path of the cluster engine, both kernels), then
+    continue the same simulation on the stream engine: state hand-over between engines is exact."""
     Z = np.full((1, N + 1), 60.0 + 0j, dtype=np.complex64)
     psi0 = make_psi0(N, -6, 6, -6, 6, 1.0, 1.0, 0, 0)[None]
     spp = 100 * N // 64          # the same rotation displacement in cells on both grids
     sim = vfps.Simulation(N, -6, 6, -6, 6, spp, 1e-3, 4, 2, 1, Z=Z)
-    if N == 128:
-        sim.set_cluster_kernel(2)
+    sim.set_cluster_kernel(kernel)
     sim.set_engine(vfps.ENGINE_CLUSTER)
-    assert sim.cluster_kernel == (2 if N == 128 else 1)
+    assert sim.cluster_kernel == kernel
     sim.set_psi_host(psi0)
     o = orc.Oracle(N, -6, 6, -6, 6, spp, 1e-3, 4, 2, Z[0])
     o.set_psi(psi0[0])
@@ -698,10 +764,12 @@ def test_cluster_engine_large_kick_and_switching(vfps, orc, N):
     sim.close()
 
 
-def test_cluster_engine_no_wake_no_renormalise(vfps, orc):
+@pytest.mark.parametrize("kernel", [1, 3])
+def test_cluster_engine_no_wake_no_renormalise(vfps, orc, kernel):
     wl = get_workload("C0")
     psi0 = wl.psi0()
     sim = vfps.Simulation(wl.N, -6, 6, -6, 6, wl.steps_per_period, wl.beta, 2, 2, 1, flags=0)
+    sim.set_cluster_kernel(kernel)
     sim.set_engine(vfps.ENGINE_CLUSTER)
     sim.set_psi_host(psi0)
     o = orc.Oracle(wl.N, -6, 6, -6, 6, wl.steps_per_period, wl.beta, 2, 2, None, renormalise=False)
