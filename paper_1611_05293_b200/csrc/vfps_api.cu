@@ -362,6 +362,7 @@ bool onchip_tab_ok(const vfps_sim *h, int S)
 //   row x is "good" if floor(dy) is the same for all columns (iy)
 //   TAB:  M_i(y) = l_i(t0x), M'_i = l_i'(t0x), t0x = a Xc(r) + b Y - ix, Xc = centre row of the rank
 //         L_j(x) = l_j(t0y), L'_j = l_j'(t0y), t0y = d X + a Ymid - iy;  e_x(x) = a (X - Xc)
+//         packed per order so that the kernel fetches a row with two or three vector loads
 //         (the kernel forms e_y(y) = a (y - (N-1)/2) itself)
 //   else: column {b Y - ix, a Y}, row {X, d X - iy}: the kernel evaluates the weights per cell
 int onchip_tables(vfps_sim *h, int S)
@@ -401,10 +402,12 @@ int onchip_tables(vfps_sim *h, int S)
             const int r = x / R;
             const double Xc = 0.5 * ((double)(r * R) + (double)(r * R + R - 1)) + g.x0c;
             if (tab) {
+                // order 4: L[0..3] L'[0..3] ex;  order 3: L[0..2] ex L'[0..2];  order 2: L[0..1] L'[0..1] ex
                 double l[4] = {0, 0, 0, 0}, lp[4] = {0, 0, 0, 0};
                 lagrange_d(order, g.d * X + g.a * Ymid - f0, l, lp);
-                for (int j = 0; j < 4; ++j) { t[j] = (float)l[j]; t[4 + j] = (float)lp[j]; }
-                t[8] = (float)(g.a * (X - Xc));
+                const int olp = (order == 2) ? 2 : 4, oex = (order == 4) ? 8 : (order == 3) ? 3 : 4;
+                for (int j = 0; j < order; ++j) { t[j] = (float)l[j]; t[olp + j] = (float)lp[j]; }
+                t[oex] = (float)(g.a * (X - Xc));
             } else {
                 t[8] = (float)X;
                 t[9] = (float)(g.d * X - f0);

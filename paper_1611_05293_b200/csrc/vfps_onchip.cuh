@@ -1,10 +1,10 @@
-// vfps_onchip.cuh -- persistent thread-block-cluster engine, second design (sm_100a).
+// vfps_onchip.cuh -- persistent thread-block-cluster engine, in-place design (sm_100a).
 //
 // One cluster of S CTAs advances one simulation with psi resident in (distributed) shared memory;
 // HBM is touched when a work item starts (load psi) and ends (store psi) and for the six
 // diagnostics floats per step.  CTA `rank` owns the q-rows x in [rank*R, (rank+1)*R), R = N/S.
 //
-// What differs from the first design (one buffer pair, weights recomputed per cell):
+// What differs from the first design (vfps_cluster.cuh: one buffer pair, weights recomputed per cell):
 //  * ONE buffer.  The rotation a1 works in place: a CTA's rows are cut into W "walker" segments
 //    (W = 16 warps / (N/64) warps per row); segment w is stored as
 //        [H apron rows][its rows][H apron rows] plus D free rows,
@@ -25,13 +25,17 @@
 //    (a thread keeps its two columns for the whole launch), L, L' in shared memory; the host
 //    builds them in double precision (vfps_api.cu: onchip_tables).  4 + 4 FMAs per cell replace
 //    ~18 operations for floors, fractions and two cubic weight sets.
-//  * A thread rotates TWO adjacent columns: the 4 x 6 register window slides down the rows with
-//    three 64-bit shared loads per row (1.5 loads per cell instead of 4), one 64-bit store.
+//  * A thread rotates TWO adjacent columns: the ORDER x 6 register window slides along the rows
+//    with three 64-bit shared loads per row (1.5 loads per cell instead of 4), one 64-bit store.
+//    The loads of the NEXT target row (its entering window row, its table row) are issued in the
+//    middle of the current row's arithmetic -- the window row that leaves is consumed first -- so
+//    the shared-memory latency hides behind ~45 FMAs instead of stalling every row.
 //  * Row sums (projection a2) are formed in the rotation pass in registers (transposed warp
-//    reduction of 8 rows at a time); no second pass over psi'.
+//    reduction of one chunk of rows at a time); no second pass over psi'.
 //  * The wake a3 is a Toeplitz product done by one warp per four rows with 128-bit loads of the
-//    wake function (1.1 instructions per multiply-add); kick a4 + Fokker-Planck a5 own eight
-//    consecutive cells per lane, with the Fokker-Planck stencil folded into four per-column
+//    wake function (1.1 instructions per multiply-add); kick a4 + Fokker-Planck a5: a lane owns
+//    the 4-cell granules 4 lane + 128 k of a row (128-bit loads with a lane stride of 16 bytes:
+//    free of bank conflicts), with the Fokker-Planck stencil folded into four per-column
 //    coefficients (5 operations per cell instead of 9) and column-sum moments.
 //  * One DSMEM exchange fewer per step: the partial sums of step t travel with the profile of
 //    step t+1 (double-buffered by step parity, one mbarrier per parity).
@@ -75,6 +79,9 @@ constexpr int OC_COLTAB = 8;          // floats per column of the column table
 constexpr int OC_BAD = (int)0x80000000;
 constexpr int OC_MAX_H = 7;
 
+// rows a walker rotates between two checks of its floors (a multiple of the window period ORDER)
+__host__ __device__ constexpr int oc_chunk_rows(int order) { return order == 3 ? 3 : 4; }
+
 struct OnchipArgs {
     float *psi;            // [members][N][N] in/out, un-normalised
     float *scale;          // [members] in/out: 1/C of the last step
@@ -82,7 +89,7 @@ struct OnchipArgs {
     float *diag;           // [nsteps][members][6] or nullptr
     const float *coltab;   // [S][N][8]   TAB: M[4], M'[4] of column y for the rows of rank r; else {b Y - ix, a Y, ...}
     const int *colix;      // [S][N]      floor(dx) of column y over the rows of rank r, or OC_BAD
-    const float *rowtab;   // [N][12]     TAB: L[4], L'[4], a (X - Xc), -, iy, -; else {-, ..., X (slot 8), d X - iy (slot 9), iy (slot 10)}
+    const float *rowtab;   // [N][12]     per-row weights along p, see onchip_tables (vfps_api.cu)
     int members;
     int nsteps;            // steps per work item of this launch (chunk)
     int S, R;
@@ -95,7 +102,9 @@ struct OnchipArgs {
     long long *dbg;        // VFPS_PHASE_CLOCKS builds only: [CTA][64 steps][8] clock64 stamps
 };
 
-// ---- layout shared by host and device
+// ---- layout shared by host and device.  The psi buffer comes last, after at least one row's
+// worth of tables and before one spare row: the rotation prefetches one window row past either
+// end of a walker's range (the value is never used, the address must be inside the allocation).
 struct OnchipLayout {
     int CW, W, RPW, H, KC, K, D, seg_rows, phys_rows, pitch, nch;
     size_t off_buf, off_rowtab, off_gtab, off_wf, off_rho, off_part, off_rowpart, off_vtab, off_rowaddr,
@@ -105,34 +114,34 @@ struct OnchipLayout {
 __host__ __device__ inline OnchipLayout onchip_layout(int N, int S, int H, int order)
 {
     OnchipLayout L;
-    const int R = N / S;
+    const int R = N / S, CH = oc_chunk_rows(order);
     L.CW = N / 64;
     const int Wmax = OC_WARPS / L.CW;
     L.W = Wmax < R ? Wmax : R;                 // active walkers
     while (L.W > 1 && R / L.W < H) L.W /= 2;   // a walker's aprons come from its direct neighbours only
     L.RPW = R / L.W;
     L.H = H;
-    L.KC = (order == 2) ? 4 : 2;               // chunks (of `order` rows) per named-barrier block
-    L.K = L.KC * order;
-    const int kb = L.K < L.RPW ? L.K : ((L.RPW + order - 1) / order) * order;
+    L.KC = 2;                                  // chunks per named-barrier block
+    L.K = L.KC * CH;
+    const int kb = L.K < L.RPW ? L.K : ((L.RPW + CH - 1) / CH) * CH;
     L.D = kb + H;
     L.seg_rows = L.RPW + 2 * H + L.D;
     L.phys_rows = L.W * L.seg_rows;
     L.pitch = N + 2 * OC_PADC;
-    L.nch = (L.RPW + order - 1) / order;
+    L.nch = (L.RPW + CH - 1) / CH;
     size_t o = 0;
-    L.off_buf = o;      o += (size_t)L.phys_rows * L.pitch;
-    L.off_rowtab = o;   o += (size_t)R * OC_ROWTAB;
-    L.off_gtab = o;     o += (size_t)N * 4;
+    L.off_misc = o;     o += 32;               // own partial sums (8), three mbarriers (6), work item (2)
+    L.off_gtab = o;     o += (size_t)N * 4;    // [4 coefficients][N columns]
     L.off_wf = o;       o += (size_t)2 * N;
     L.off_rho = o;      o += (size_t)2 * N;
     L.off_part = o;     o += (size_t)2 * OC_MAX_S * OC_NPART;
-    L.off_rowpart = o;  o += (size_t)R * L.CW;
+    L.off_rowpart = o;  o += (size_t)((R * L.CW + 3) & ~3);
     L.off_vtab = o;     o += (size_t)R * 8;
     L.off_rowaddr = o;  o += (size_t)R * 4;
     L.off_chunk = o;    o += (size_t)((L.W * L.nch + 3) & ~3);
     L.off_wred = o;     o += (size_t)OC_WARPS * 8;
-    L.off_misc = o;     o += 32;               // own partial sums (8), three mbarriers (6), spare
+    L.off_rowtab = o;   o += (size_t)(R + 2) * OC_ROWTAB;      // one spare entry before and after (prefetch)
+    L.off_buf = o;      o += (size_t)(L.phys_rows + 1) * L.pitch;
     L.total_floats = o;
     return L;
 }
@@ -146,12 +155,6 @@ __device__ __forceinline__ float2 lds2(uint32_t a)
 __device__ __forceinline__ void sts2(uint32_t a, float x, float y)
 {
     asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(a), "f"(x), "f"(y) : "memory");
-}
-__device__ __forceinline__ int ldsi(uint32_t a)
-{
-    int v;
-    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a));
-    return v;
 }
 __device__ __forceinline__ int4 ldsi4(uint32_t a)
 {
@@ -174,7 +177,6 @@ __device__ __forceinline__ float warp_reduce_transposed(float (&v)[NV], int lane
     if constexpr (NV == 1) {
         return warp_sum(v[0]);
     } else {
-        constexpr int LOG = (NV == 8) ? 3 : (NV == 4) ? 2 : 1;
         // level with xor offset 16, 8, 4: keep the half of the values selected by that lane bit
         float u[NV / 2];
         const bool hi = (lane & 16) != 0;
@@ -210,26 +212,25 @@ __device__ __forceinline__ float warp_reduce_transposed(float (&v)[NV], int lane
             }
             r += __shfl_xor_sync(FULL, r, 2);
             r += __shfl_xor_sync(FULL, r, 1);
-            (void)LOG;
             return r;
         }
     }
 }
 
 // kick (shift by MM + t cells, Lagrange weights l already scaled by 1/C) and Fokker-Planck for the
-// GW cells g..g+GW-1 of one row: b[i] = psi'(g - 4 + i), i = 0..GW+7.  k[i] = kicked value at
+// four cells g..g+3 of one row: b[i] = psi'(g - 4 + i), i = 0..11.  k[i] = kicked value at
 // position g - 1 + i (zero outside the grid, A8).  The Fokker-Planck update (Eq. 15 + 3-point
 // second difference, explicit Euler) is  out = k0 + G[-1] k[-1] + G[0] k0 + G[1] k[1] + G[2] k[2]
-// with the per-column coefficients gc[c] = (G-1, G0, G1, G2) of column g + c (all <= 1e-3, so the
-// sum is exact to well below one ulp of k0).
-template <int ORDER, int MM, int GW>
-__device__ __forceinline__ void kick_fp_wide(const float (&b)[GW + 8], const float (&l)[ORDER], int g, int N,
-                                             const float4 (&gc)[GW], float (&out)[GW])
+// with the per-column coefficients (G-1, G0, G1, G2): gt[j] holds coefficient j of the columns
+// g..g+3 (all <= 1e-3, so the sum is exact to well below one ulp of k0).
+template <int ORDER, int MM>
+__device__ __forceinline__ void kick_fp4(const float (&b)[12], const float (&l)[ORDER], int g, int N,
+                                         const float4 (&gt)[4], float (&out)[4])
 {
     constexpr int O0 = (ORDER - 1) / 2;
-    float k[GW + 3];
+    float k[7];
 #pragma unroll
-    for (int i = 0; i < GW + 3; ++i) {
+    for (int i = 0; i < 7; ++i) {
         const int i0 = 3 + i + MM - O0;
         float acc = l[0] * b[i0];
 #pragma unroll
@@ -237,25 +238,27 @@ __device__ __forceinline__ void kick_fp_wide(const float (&b)[GW + 8], const flo
         k[i] = acc;
     }
     if (g == 0) k[0] = 0.0f;
-    if (g == N - GW) { k[GW + 1] = 0.0f; k[GW + 2] = 0.0f; }
+    if (g == N - 4) { k[5] = 0.0f; k[6] = 0.0f; }
+    const float gm[4] = {gt[0].x, gt[0].y, gt[0].z, gt[0].w}, g0[4] = {gt[1].x, gt[1].y, gt[1].z, gt[1].w};
+    const float g1[4] = {gt[2].x, gt[2].y, gt[2].z, gt[2].w}, g2[4] = {gt[3].x, gt[3].y, gt[3].z, gt[3].w};
 #pragma unroll
-    for (int c = 0; c < GW; ++c) {
-        const float incr = fmaf(gc[c].w, k[c + 3], fmaf(gc[c].z, k[c + 2], fmaf(gc[c].y, k[c + 1], gc[c].x * k[c])));
+    for (int c = 0; c < 4; ++c) {
+        const float incr = fmaf(g2[c], k[c + 3], fmaf(g1[c], k[c + 2], fmaf(g0[c], k[c + 1], gm[c] * k[c])));
         out[c] = k[c + 1] + incr;
     }
 }
 // any integer shift: reads the row in shared memory with bounds checks (rare: |shift| > 1 cell).
-// Not inlined; weights by value, coefficients from the shared table, results through local memory,
-// so that the fast path keeps its operands in registers.
-template <int ORDER, int GW>
-__device__ __noinline__ void kick_fp_wide_any(const float *row /* index 0 = y 0 */, float4 lw, int mm, int g, int N,
-                                              const float4 *gtab, float *out)
+// Not inlined; weights by value, coefficients from the shared table [4][N], results through local
+// memory, so that the fast path keeps its operands in registers.
+template <int ORDER>
+__device__ __noinline__ void kick_fp4_any(const float *row /* index 0 = y 0 */, float4 lw, int mm, int g, int N,
+                                          const float *gtab, float *out)
 {
     constexpr int O0 = (ORDER - 1) / 2;
     const float l[4] = {lw.x, lw.y, lw.z, lw.w};
-    float k[GW + 3];
+    float k[7];
 #pragma unroll 1
-    for (int i = 0; i < GW + 3; ++i) {
+    for (int i = 0; i < 7; ++i) {
         const int y = g - 1 + i;
         float acc = 0.0f;
         for (int j = 0; j < ORDER; ++j) {
@@ -266,9 +269,10 @@ __device__ __noinline__ void kick_fp_wide_any(const float *row /* index 0 = y 0 
         k[i] = (y >= 0 && y < N) ? acc : 0.0f;
     }
 #pragma unroll 1
-    for (int c = 0; c < GW; ++c) {
-        const float4 gc = gtab[g + c];
-        out[c] = k[c + 1] + fmaf(gc.w, k[c + 3], fmaf(gc.z, k[c + 2], fmaf(gc.y, k[c + 1], gc.x * k[c])));
+    for (int c = 0; c < 4; ++c) {
+        const int y = g + c;
+        out[c] = k[c + 1] + fmaf(gtab[3 * N + y], k[c + 3], fmaf(gtab[2 * N + y], k[c + 2],
+                                                                  fmaf(gtab[N + y], k[c + 1], gtab[y] * k[c])));
     }
 }
 
@@ -276,17 +280,22 @@ __device__ __noinline__ void kick_fp_wide_any(const float *row /* index 0 = y 0 
 // A thread owns the columns y0 = 64 cw + 2 lane and y0 + 1.  The ORDER x (2 NP) register window
 // holds ORDER source rows of the aligned column pairs that cover both cells' taps; it slides one
 // row per target row.  PAR = (iy - O0) & 1 is the offset of cell y0's first tap inside the window,
-// DIR the walk direction (+1: rows ascending).
+// DIR the walk direction (+1: rows ascending).  At the start of a target row the window and the
+// table row `tb` of that target are complete; its step loads those of the next target.
 template <int ORDER, int PITCH, bool TAB>
 struct Walker {
     static constexpr int O0 = (ORDER - 1) / 2;
     static constexpr int NPMAX = (ORDER + 3) / 2;          // column pairs of the window (PAR = 1)
+    static constexpr int CH = oc_chunk_rows(ORDER);
+    static constexpr int NTB = TAB ? 2 * ORDER + 1 : 2;
+    static constexpr int P4 = PITCH * 4;
     float win[ORDER][2 * NPMAX];
     float M0[ORDER], M0p[ORDER], M1[ORDER], M1p[ORDER];    // TAB: weights along q of both columns and their t-derivatives
                                                            // !TAB: M0[0] = b Y0 - ix, M1[0] = b Y1 - ix
     float ey0, ey1;                                        // TAB: a (Y - Ymid); else a Y
     float a;                                               // cos(dphi) - 1 (only !TAB)
-    float rs[8];                                           // row sums of the current barrier block
+    float tb[NTB];                                         // TAB: L[ORDER], L'[ORDER], a (X - Xc); else X, d X - iy
+    float rs[4];                                           // row sums of the current chunk
 
     template <int PAR>
     __device__ __forceinline__ void load_row(int slot, uint32_t addr)
@@ -298,87 +307,98 @@ struct Walker {
             win[slot][2 * k] = v.x; win[slot][2 * k + 1] = v.y;
         }
     }
-    // weights of both cells for the target row whose table entry is at `tab`
-    __device__ __forceinline__ void weights(uint32_t tab, float (&lx0)[ORDER], float (&lx1)[ORDER], float (&ly0)[ORDER],
+    // the table row at `tab` (layouts: onchip_tables in vfps_api.cu)
+    __device__ __forceinline__ void load_tab(uint32_t tab)
+    {
+        if (TAB) {
+            if (ORDER == 4) {
+                const float4 v = lds4(tab), w = lds4(tab + 16);
+                tb[0] = v.x; tb[1] = v.y; tb[2] = v.z; tb[3] = v.w; tb[4] = w.x; tb[5] = w.y; tb[6] = w.z; tb[7] = w.w;
+                tb[2 * ORDER] = lds(tab + 32);
+            } else if (ORDER == 3) {
+                const float4 v = lds4(tab), w = lds4(tab + 16);            // L0 L1 L2 ex | L'0 L'1 L'2 -
+                tb[0] = v.x; tb[1] = v.y; tb[2] = v.z; tb[2 * ORDER] = v.w; tb[3] = w.x; tb[4] = w.y; tb[5] = w.z;
+            } else {
+                const float4 v = lds4(tab);                                 // L0 L1 L'0 L'1
+                tb[0] = v.x; tb[1] = v.y; tb[2] = v.z; tb[3] = v.w;
+                tb[2 * ORDER] = lds(tab + 16);
+            }
+        } else {
+            const float2 xv = lds2(tab + 32);                               // X, d X - iy
+            tb[0] = xv.x; tb[1] = xv.y;
+        }
+    }
+    // weights of both cells from the table row in tb
+    __device__ __forceinline__ void weights(float (&lx0)[ORDER], float (&lx1)[ORDER], float (&ly0)[ORDER],
                                             float (&ly1)[ORDER]) const
     {
         if (TAB) {
-            float L[4], Lp[4];
-            if (ORDER == 4) {
-                const float4 v = lds4(tab), w = lds4(tab + 16);
-                L[0] = v.x; L[1] = v.y; L[2] = v.z; L[3] = v.w; Lp[0] = w.x; Lp[1] = w.y; Lp[2] = w.z; Lp[3] = w.w;
-            } else if (ORDER == 3) {
-                const float4 v = lds4(tab); const float2 w = lds2(tab + 16);
-                L[0] = v.x; L[1] = v.y; L[2] = v.z; Lp[0] = w.x; Lp[1] = w.y; Lp[2] = lds(tab + 24);
-            } else {
-                const float2 v = lds2(tab), w = lds2(tab + 16);
-                L[0] = v.x; L[1] = v.y; Lp[0] = w.x; Lp[1] = w.y;
-            }
-            const float ex = lds(tab + 32);
+            const float ex = tb[2 * ORDER];
 #pragma unroll
             for (int j = 0; j < ORDER; ++j) {
-                ly0[j] = fmaf(ey0, Lp[j], L[j]);
-                ly1[j] = fmaf(ey1, Lp[j], L[j]);
+                ly0[j] = fmaf(ey0, tb[ORDER + j], tb[j]);
+                ly1[j] = fmaf(ey1, tb[ORDER + j], tb[j]);
                 lx0[j] = fmaf(ex, M0p[j], M0[j]);
                 lx1[j] = fmaf(ex, M1p[j], M1[j]);
             }
         } else {
-            const float2 xv = lds2(tab + 32);                 // X, d X - iy
-            lagrange<ORDER>(fmaf(a, xv.x, M0[0]), lx0);
-            lagrange<ORDER>(fmaf(a, xv.x, M1[0]), lx1);
-            lagrange<ORDER>(xv.y + ey0, ly0);
-            lagrange<ORDER>(xv.y + ey1, ly1);
+            lagrange<ORDER>(fmaf(a, tb[0], M0[0]), lx0);
+            lagrange<ORDER>(fmaf(a, tb[0], M1[0]), lx1);
+            lagrange<ORDER>(tb[1] + ey0, ly0);
+            lagrange<ORDER>(tb[1] + ey1, ly1);
         }
     }
-    // tensor product for both cells; slot0 = window slot of tap row i = 0
-    template <int PAR, int SLOT0>
-    __device__ __forceinline__ void eval(const float (&lx0)[ORDER], const float (&lx1)[ORDER], const float (&ly0)[ORDER],
-                                         const float (&ly1)[ORDER], float &o0, float &o1) const
+    // inner products of one window row with the weights along p of both cells
+    template <int PAR>
+    __device__ __forceinline__ void inner(int slot, const float (&ly0)[ORDER], const float (&ly1)[ORDER], float &r0,
+                                          float &r1) const
     {
-        float a0 = 0.0f, a1 = 0.0f;
+        const float(&wr)[2 * NPMAX] = win[slot];
+        r0 = ly0[0] * wr[PAR]; r1 = ly1[0] * wr[PAR + 1];
 #pragma unroll
-        for (int i = 0; i < ORDER; ++i) {
-            const float(&wr)[2 * NPMAX] = win[(SLOT0 + i) % ORDER];
-            float r0 = ly0[0] * wr[PAR], r1 = ly1[0] * wr[PAR + 1];
-#pragma unroll
-            for (int j = 1; j < ORDER; ++j) {
-                r0 = fmaf(ly0[j], wr[PAR + j], r0);
-                r1 = fmaf(ly1[j], wr[PAR + 1 + j], r1);
-            }
-            a0 = (i == 0) ? lx0[0] * r0 : fmaf(lx0[i], r0, a0);
-            a1 = (i == 0) ? lx1[0] * r1 : fmaf(lx1[i], r1, a1);
+        for (int j = 1; j < ORDER; ++j) {
+            r0 = fmaf(ly0[j], wr[PAR + j], r0);
+            r1 = fmaf(ly1[j], wr[PAR + 1 + j], r1);
         }
-        o0 = a0; o1 = a1;
     }
-    // one chunk of ORDER target rows, walking in direction DIR.  src = address of window column 0
-    // of tap row i = 0 of the first target row; dst = address of its output pair; tab = its table
-    // row; cont: the window already holds the ORDER - 1 rows shared with the previous chunk.
-    // RS0 = index of the first row sum of this chunk in rs[].
-    template <int PAR, int DIR, int RS0, int SUB = 0>
-    __device__ __forceinline__ void chunk(uint32_t src, uint32_t dst, uint32_t tab, bool cont)
+    // start of a run of chunks: the whole window and the table row of the first target.
+    // src = address of window column 0 of tap row i = 0 of that target, tab = its table row.
+    template <int PAR>
+    __device__ __forceinline__ void start(uint32_t src, uint32_t tab)
     {
-        constexpr int P4 = PITCH * 4;
-        if (SUB == 0 && !cont) {
-            // tap rows i of the first target that later targets reuse: DIR > 0: i = 0..ORDER-2 (slots i),
-            // DIR < 0: i = 1..ORDER-1 (slots i)
 #pragma unroll
-            for (int i = 0; i < ORDER - 1; ++i) {
-                const int ii = (DIR > 0) ? i : i + 1;
-                load_row<PAR>(ii, src + (uint32_t)(ii * P4));
-            }
-        }
-        // target SUB: tap row i lives in slot (SUB + i) % ORDER (DIR > 0) or (i - SUB) mod ORDER (DIR < 0);
-        // the entering tap row is i = ORDER-1 (DIR > 0) or i = 0 (DIR < 0)
+        for (int i = 0; i < ORDER; ++i) load_row<PAR>(i, src + (uint32_t)(i * P4));
+        load_tab(tab);
+    }
+    // target row SUB of a chunk.  Tap row i lives in slot (SUB + i) % ORDER (DIR > 0) or
+    // (i - SUB) mod ORDER (DIR < 0).  The tap row that leaves the window (i = 0 walking down,
+    // i = ORDER - 1 walking up) is consumed first; its slot then receives the entering row of the
+    // next target, and tb the next table row, while the rest of this target is computed.
+    template <int PAR, int DIR, int SUB>
+    __device__ __forceinline__ void row_step(uint32_t src, uint32_t dst, uint32_t tab)
+    {
         constexpr int SLOT0 = (DIR > 0) ? (SUB % ORDER) : ((ORDER - SUB % ORDER) % ORDER);
-        constexpr int IN_I = (DIR > 0) ? ORDER - 1 : 0;
-        load_row<PAR>((SLOT0 + IN_I) % ORDER, src + (uint32_t)((DIR * SUB + IN_I) * P4));
+        constexpr int IL = (DIR > 0) ? 0 : ORDER - 1;
         float lx0[ORDER], lx1[ORDER], ly0[ORDER], ly1[ORDER];
-        weights(tab + (uint32_t)(DIR * SUB * (OC_ROWTAB * 4)), lx0, lx1, ly0, ly1);
-        float o0, o1;
-        eval<PAR, SLOT0>(lx0, lx1, ly0, ly1, o0, o1);
-        sts2(dst + (uint32_t)(DIR * SUB * P4), o0, o1);
-        rs[RS0 + SUB] = o0 + o1;
-        if constexpr (SUB + 1 < ORDER) chunk<PAR, DIR, RS0, SUB + 1>(src, dst, tab, cont);
+        weights(lx0, lx1, ly0, ly1);
+        load_tab(tab + (uint32_t)(DIR * (SUB + 1) * (OC_ROWTAB * 4)));
+        float r0[ORDER], r1[ORDER];
+        inner<PAR>((SLOT0 + IL) % ORDER, ly0, ly1, r0[IL], r1[IL]);
+        load_row<PAR>((SLOT0 + IL) % ORDER, src + (uint32_t)((DIR > 0 ? SUB + ORDER : -(SUB + 1)) * P4));
+#pragma unroll
+        for (int i = 0; i < ORDER; ++i)
+            if (i != IL) inner<PAR>((SLOT0 + i) % ORDER, ly0, ly1, r0[i], r1[i]);
+        float a0 = lx0[0] * r0[0], a1 = lx1[0] * r1[0];
+#pragma unroll
+        for (int i = 1; i < ORDER; ++i) { a0 = fmaf(lx0[i], r0[i], a0); a1 = fmaf(lx1[i], r1[i], a1); }
+        sts2(dst + (uint32_t)(DIR * SUB * P4), a0, a1);
+        rs[SUB] = a0 + a1;
+    }
+    template <int PAR, int DIR, int SUB = 0>
+    __device__ __forceinline__ void chunk(uint32_t src, uint32_t dst, uint32_t tab)
+    {
+        row_step<PAR, DIR, SUB>(src, dst, tab);
+        if constexpr (SUB + 1 < CH) chunk<PAR, DIR, SUB + 1>(src, dst, tab);
     }
 };
 
@@ -424,11 +444,13 @@ k_onchip_step(GridConst G, OnchipArgs A)
     constexpr int P4 = PITCH * 4;
     constexpr int O0 = (ORDER - 1) / 2;
     constexpr int CW = N / 64;
-    constexpr int GW = (N >= 256) ? 8 : 4;                 // cells per lane in the kick pass
-    constexpr int NG = (N / (32 * GW)) > 0 ? (N / (32 * GW)) : 1;   // granules per lane and row
-    constexpr int KL = (32 * GW <= N) ? 32 : N / GW;       // active lanes in the kick pass
+    constexpr int CH = oc_chunk_rows(ORDER);
+    constexpr int NG = (N >= 128) ? N / 128 : 1;           // 4-cell granules per lane and row: columns 4 lane + 128 k
+    constexpr int KL = (N >= 128) ? 32 : N / 4;            // active lanes in the kick pass
+    constexpr bool GREG = (NG <= 2);                       // Fokker-Planck coefficients of the lane's columns stay in registers
     constexpr int NW = N / 128 > 0 ? N / 128 : 1;          // float4 groups of rho per lane in the wake
     constexpr unsigned FULL = 0xffffffffu;
+    using Wk = Walker<ORDER, PITCH, TAB>;
 
     cg::cluster_group cluster = cg::this_cluster();
     const int S = A.S, R = A.R, H = G.H;
@@ -440,7 +462,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
 
     extern __shared__ __align__(16) float smem[];
     float *buf = smem + LY.off_buf;
-    float *rowtab_s = smem + LY.off_rowtab;
+    float *rowtab_s = smem + LY.off_rowtab + OC_ROWTAB;    // entry 0 = first own row (one spare entry before)
     float *gtab = smem + LY.off_gtab;
     float *wf = smem + LY.off_wf;
     float *rhob = smem + LY.off_rho;
@@ -452,7 +474,8 @@ k_onchip_step(GridConst G, OnchipArgs A)
     float *wred = smem + LY.off_wred;
     float *misc = smem + LY.off_misc;                      // [0..7] own partial sums, [8..13] mbarriers, [16] item
     const uint32_t sBuf = smem_u32(buf), sRowtab = smem_u32(rowtab_s), sRho = smem_u32(rhob), sPart = smem_u32(partb);
-    const uint32_t sVtab = smem_u32(vtab), sMisc = smem_u32(misc);
+    const uint32_t sVtab = smem_u32(vtab), sMisc = smem_u32(misc), sRowaddr = smem_u32(rowaddr), sGtab = smem_u32(gtab);
+    const uint32_t sRowpart = smem_u32(rowpart);
     const uint32_t mbRho0 = sMisc + 32, mbHalo = sMisc + 48;        // mbRho[p] = mbRho0 + 8 p
     const int nbrs = (rank > 0 ? 1 : 0) + (rank < S - 1 ? 1 : 0);
     const uint32_t bytesRho = (uint32_t)(N + S * OC_NPART) * 4u, bytesPart = (uint32_t)(S * OC_NPART) * 4u;
@@ -463,7 +486,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
     const bool walker_on = wk < W;
     const int y0 = 64 * cw + 2 * lane;
     const int wb = wk * RPW;                               // first CTA-local row of the walker
-    Walker<ORDER, PITCH, TAB> wkr;
+    Wk wkr;
     int ixc = 0;
     bool cols_ok = false;
     {
@@ -476,23 +499,30 @@ k_onchip_step(GridConst G, OnchipArgs A)
             wkr.M0[i] = ct0[i]; wkr.M0p[i] = ct0[4 + i];
             wkr.M1[i] = ct1[i]; wkr.M1p[i] = ct1[4 + i];
         }
-        // TAB: a (Y - Ymid) in slot 7 of the !TAB layout is unused; both layouts keep e_y in [7]... see host
         wkr.ey0 = TAB ? G.a * ((float)y0 - 0.5f * (float)(N - 1)) : ct0[1];
         wkr.ey1 = TAB ? G.a * ((float)(y0 + 1) - 0.5f * (float)(N - 1)) : ct1[1];
         wkr.a = G.a;
         if (!cols_ok) ixc = 0;
     }
     const uint32_t segA = sBuf + (uint32_t)(wk * SEG) * P4;     // physical row 0 of the walker's segment
+    // lanes 8 k (k < CH) publish the row sum of the chunk's k-th target row
+    const bool rs_writer = ((lane & 7) == 0) && ((lane >> 3) < CH);
 
     // ---- one-time set-up: zero the buffer (pads stay zero for ever), tables, barriers
-    for (int i = tid; i < LY.phys_rows * PITCH; i += OC_THREADS) buf[i] = 0.0f;
-    for (int i = tid; i < R * OC_ROWTAB; i += OC_THREADS) rowtab_s[i] = A.rowtab[(size_t)x0 * OC_ROWTAB + i];
+    for (int i = tid; i < (LY.phys_rows + 1) * PITCH; i += OC_THREADS) buf[i] = 0.0f;
+    for (int i = tid; i < (R + 2) * OC_ROWTAB; i += OC_THREADS) {
+        const int gi = (x0 - 1) * OC_ROWTAB + i;           // entries x0 - 1 .. x0 + R (the outer two are only ever prefetched)
+        rowtab_s[i - OC_ROWTAB] = (gi >= 0 && gi < N * OC_ROWTAB) ? A.rowtab[gi] : 0.0f;
+    }
     {
+        // Fokker-Planck coefficients by column, transposed: gtab[j][y], j = 0..3 <-> G-1, G0, G1, G2
         const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
         for (int y = tid; y < N; y += OC_THREADS) {
             const float c1p = c1 * fmaf((float)y, G.dp, G.p_min);
-            reinterpret_cast<float4 *>(gtab)[y] =
-                make_float4(fmaf(-2.0f, c1p, c2), fmaf(-3.0f, c1p, fmaf(-2.0f, c2, G.fp_b)), fmaf(6.0f, c1p, c2), -c1p);
+            gtab[y] = fmaf(-2.0f, c1p, c2);
+            gtab[N + y] = fmaf(-3.0f, c1p, fmaf(-2.0f, c2, G.fp_b));
+            gtab[2 * N + y] = fmaf(6.0f, c1p, c2);
+            gtab[3 * N + y] = -c1p;
         }
     }
     // per row: parity-0 byte offsets (from sBuf, column 0) of its own slot and of the apron slots it
@@ -520,10 +550,10 @@ k_onchip_step(GridConst G, OnchipArgs A)
     for (int i = tid; i < W * nch; i += OC_THREADS) {
         const int w = i / nch, c = i - w * nch;
         int iy = OC_BAD;
-        if ((c + 1) * ORDER <= RPW) {
-            iy = __float_as_int(rowtab_s[(w * RPW + c * ORDER) * OC_ROWTAB + 10]);
-            for (int k = 1; k < ORDER; ++k)
-                if (__float_as_int(rowtab_s[(w * RPW + c * ORDER + k) * OC_ROWTAB + 10]) != iy) iy = OC_BAD;
+        if ((c + 1) * CH <= RPW) {
+            iy = __float_as_int(rowtab_s[(w * RPW + c * CH) * OC_ROWTAB + 10]);
+            for (int k = 1; k < CH; ++k)
+                if (__float_as_int(rowtab_s[(w * RPW + c * CH + k) * OC_ROWTAB + 10]) != iy) iy = OC_BAD;
         }
         chunkinfo[i] = iy;
     }
@@ -607,74 +637,70 @@ k_onchip_step(GridConst G, OnchipArgs A)
                 const int row0 = p ? H : D + H;
                 const uint32_t rbase = segA + (uint32_t)(row0 * P4);                 // row 0, buffer column -PADC
                 const int dsh = p ? D : -D;                                            // output slot shift (rows)
-                int prev_iy = OC_BAD;
-#pragma unroll
-                for (int k = 0; k < 8; ++k) wkr.rs[k] = 0.0f;
-                int blk_row0 = p ? (RPW - 1) : 0;          // first row (walk order) of the current barrier block
-                for (int ci = 0; ci < nch; ++ci) {
+                const int dir = p ? -1 : 1;
+                int kk = 0;                                // chunks since the last named barrier
+                int ci = 0;                                // chunk index in walk order
+                while (ci < nch) {
                     const int c = p ? nch - 1 - ci : ci;
                     const int iy = chunkinfo[wk * nch + c];
-                    const int kk = ci % KC;                // chunk index inside the barrier block
-                    const int vlo = c * ORDER, nrow = min(ORDER, RPW - vlo);
+                    int nrun = 1;                          // chunks handled in this round
                     if (cols_ok && iy != OC_BAD) {
-                        const bool cont = (prev_iy == iy);
+                        // ---- a run of chunks with the same floors: the window slides through all of them
+                        while (ci + nrun < nch && chunkinfo[wk * nch + (p ? c - nrun : c + nrun)] == iy) ++nrun;
                         const int par = (iy - O0) & 1;
-                        const int v0 = p ? vlo + ORDER - 1 : vlo;                      // first target row in walk order
+                        const int v0 = p ? c * CH + CH - 1 : c * CH;                   // first target row in walk order
                         // window column 0 = grid column y0 + iy - O0 - par
-                        const uint32_t src = rbase + (uint32_t)((v0 + ixc - O0) * P4 + (OC_PADC + y0 + iy - O0 - par) * 4);
-                        const uint32_t dst = rbase + (uint32_t)((v0 + dsh) * P4 + (OC_PADC + y0) * 4);
-                        const uint32_t tab = sRowtab + (uint32_t)((wb + v0) * OC_ROWTAB * 4);
-#define OC_CHUNK(PAR_, DIR_)                                                                       \
-    do {                                                                                            \
-        if constexpr (ORDER == 2) {                                                                 \
-            if (kk == 0) wkr.template chunk<PAR_, DIR_, 0>(src, dst, tab, cont);                    \
-            else if (kk == 1) wkr.template chunk<PAR_, DIR_, 2>(src, dst, tab, cont);               \
-            else if (kk == 2) wkr.template chunk<PAR_, DIR_, 4>(src, dst, tab, cont);               \
-            else wkr.template chunk<PAR_, DIR_, 6>(src, dst, tab, cont);                            \
-        } else {                                                                                    \
-            if (kk == 0) wkr.template chunk<PAR_, DIR_, 0>(src, dst, tab, cont);                    \
-            else wkr.template chunk<PAR_, DIR_, 4>(src, dst, tab, cont);                            \
-        }                                                                                           \
+                        uint32_t src = rbase + (uint32_t)((v0 + ixc - O0) * P4 + (OC_PADC + y0 + iy - O0 - par) * 4);
+                        uint32_t dst = rbase + (uint32_t)((v0 + dsh) * P4 + (OC_PADC + y0) * 4);
+                        uint32_t tab = sRowtab + (uint32_t)((wb + v0) * OC_ROWTAB * 4);
+                        // lane 8 k publishes the sum of the k-th target row of every chunk
+                        uint32_t rp = sRowpart + (uint32_t)(((wb + v0 + dir * (lane >> 3)) * CW + cw) * 4);
+#define OC_RUN(PAR_, DIR_)                                                                                   \
+    do {                                                                                                      \
+        wkr.template start<PAR_>(src, tab);                                                                   \
+        for (int q = 0; q < nrun; ++q) {                                                                      \
+            wkr.template chunk<PAR_, DIR_>(src, dst, tab);                                                    \
+            if (CH < 4) wkr.rs[3] = 0.0f;                                                                     \
+            const float tot = warp_reduce_transposed<4>(wkr.rs, lane);                                        \
+            if (rs_writer) sts(rp, tot);                                                                      \
+            src += (uint32_t)(DIR_ * CH * P4); dst += (uint32_t)(DIR_ * CH * P4);                             \
+            tab += (uint32_t)(DIR_ * CH * OC_ROWTAB * 4); rp += (uint32_t)(DIR_ * CH * CW * 4);               \
+            if (++kk == KC) {                                                                                 \
+                kk = 0;                                                                                       \
+                if (ci + q + 1 < nch) { if (CW > 1) named_barrier(1 + wk, CW * 32); else __syncwarp(); }      \
+            }                                                                                                 \
+        }                                                                                                     \
     } while (0)
-                        if (p == 0) { if (par) OC_CHUNK(1, 1); else OC_CHUNK(0, 1); }
-                        else        { if (par) OC_CHUNK(1, -1); else OC_CHUNK(0, -1); }
-#undef OC_CHUNK
-                        prev_iy = iy;
+                        if (p == 0) { if (par) OC_RUN(1, 1); else OC_RUN(0, 1); }
+                        else        { if (par) OC_RUN(1, -1); else OC_RUN(0, -1); }
+#undef OC_RUN
                     } else {
+                        // ---- cell by cell: a floor changes inside the chunk or the thread's columns, or a ragged last chunk
                         const uint32_t gbase = rbase + (uint32_t)(OC_PADC * 4);
-                        for (int s = 0; s < nrow; ++s) {
+                        const int vlo = c * CH, nrow = min(CH, RPW - vlo);
+                        float rs4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+                        for (int s = 0; s < CH; ++s) {
+                            if (s < nrow) {
+                                const int v = p ? vlo + nrow - 1 - s : vlo + s;
+                                const float o0 = rotate_cell_generic<ORDER, PITCH>(G, gbase, v, x0 + wb + v, y0);
+                                const float o1 = rotate_cell_generic<ORDER, PITCH>(G, gbase, v, x0 + wb + v, y0 + 1);
+                                sts2(rbase + (uint32_t)((v + dsh) * P4 + (OC_PADC + y0) * 4), o0, o1);
+                                rs4[s] = o0 + o1;
+                            }
+                        }
+                        const float tot = warp_reduce_transposed<4>(rs4, lane);
+                        const int s = lane >> 3;
+                        if (rs_writer && s < nrow) {
                             const int v = p ? vlo + nrow - 1 - s : vlo + s;
-                            const float o0 = rotate_cell_generic<ORDER, PITCH>(G, gbase, v, x0 + wb + v, y0);
-                            const float o1 = rotate_cell_generic<ORDER, PITCH>(G, gbase, v, x0 + wb + v, y0 + 1);
-                            sts2(rbase + (uint32_t)((v + dsh) * P4 + (OC_PADC + y0) * 4), o0, o1);
-                            const int ri = kk * ((ORDER == 3) ? 4 : ORDER) + s;
-                            // rs[] is indexed statically: add through a select chain
-#pragma unroll
-                            for (int k = 0; k < 8; ++k) if (k == ri) wkr.rs[k] = o0 + o1;
+                            rowpart[(wb + v) * CW + cw] = tot;
                         }
-                        prev_iy = OC_BAD;
+                        if (++kk == KC) {
+                            kk = 0;
+                            if (ci + 1 < nch) { if (CW > 1) named_barrier(1 + wk, CW * 32); else __syncwarp(); }
+                        }
                     }
-                    if (kk == KC - 1 || ci == nch - 1) {
-                        // row sums of this block: rs[kk' * stride + s] belongs to the row s of chunk kk'
-                        const float tot = warp_reduce_transposed<8>(wkr.rs, lane);
-                        const int idx = lane >> 2;                                     // value index 0..7
-                        constexpr int ST = (ORDER == 3) ? 4 : ORDER;                   // rs slots per chunk
-                        const int kq = idx / ST, s = idx - kq * ST;
-                        const int cq = (ci - kk) + kq;                                 // chunk (walk order) of that value
-                        if ((lane & 3) == 0 && s < ORDER && cq <= ci) {
-                            const int cc = p ? nch - 1 - cq : cq;
-                            const int nr = min(ORDER, RPW - cc * ORDER);
-                            // fast chunks run in walk order; generic rows too (s-th row in walk order)
-                            const int v = p ? cc * ORDER + nr - 1 - s : cc * ORDER + s;
-                            if (s < nr) rowpart[(wb + v) * CW + cw] = tot;
-                        }
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) wkr.rs[k] = 0.0f;
-                        if (ci != nch - 1) {
-                            if (CW > 1) named_barrier(1 + wk, CW * 32); else __syncwarp();
-                        }
-                        (void)blk_row0;
-                    }
+                    ci += nrun;
                 }
             }
             OC_STAMP(1);
@@ -792,89 +818,107 @@ k_onchip_step(GridConst G, OnchipArgs A)
             // ================= 5. kick a4 + Fokker-Planck a5 in place (parity p ^ 1), aprons, moments
             {
                 const int pshift = (p ^ 1) ? D * P4 : 0;       // parity 1 lies D rows above the parity-0 slot
-                float cs[NG][GW];
+                float cs[NG][4];
 #pragma unroll
                 for (int k = 0; k < NG; ++k)
 #pragma unroll
-                    for (int c = 0; c < GW; ++c) cs[k][c] = 0.0f;
+                    for (int c = 0; c < 4; ++c) cs[k][c] = 0.0f;
                 float q1 = 0.0f, q2 = 0.0f, pw = 0.0f;
                 // Fokker-Planck coefficients of the lane's columns: registers for the whole pass when a lane
-                // owns one granule per row, re-read per granule otherwise (N = 512: 64 registers too many)
-                float4 gc[GW];
-                if (NG == 1 && lane < KL) {
+                // owns at most two granules per row, re-read per granule otherwise (N = 512: 64 registers too many)
+                float4 gt[GREG ? NG : 1][4];
+                if (GREG && lane < KL) {
 #pragma unroll
-                    for (int c = 0; c < GW; ++c) gc[c] = reinterpret_cast<const float4 *>(gtab)[GW * lane + c];
+                    for (int k = 0; k < NG; ++k)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) gt[k][j] = lds4(sGtab + (uint32_t)((j * N + 4 * lane + 128 * k) * 4));
                 }
                 const uint32_t mbUp = (rank > 0) ? mapa(mbHalo, rank - 1) : 0u, mbDn = (rank < S - 1) ? mapa(mbHalo, rank + 1) : 0u;
-                for (int r = warp; r < R; r += OC_WARPS) {
+                const uint32_t lane_off = (uint32_t)(16 * lane);
+                float Xf = (float)(x0 + warp) - xc;
+                for (int r = warp; r < R; r += OC_WARPS, Xf += (float)OC_WARPS) {
                     const float4 lw = lds4(sVtab + (uint32_t)r * 32u);
                     const float2 mv = lds2(sVtab + (uint32_t)r * 32u + 16u);
                     const int mm = __float_as_int(mv.x);
-                    const int4 ra = ldsi4(smem_u32(rowaddr) + (uint32_t)r * 16u);
-                    const float lws[4] = {lw.x, lw.y, lw.z, lw.w};
-                    float l[ORDER];
-#pragma unroll
-                    for (int j = 0; j < ORDER; ++j) l[j] = lws[j];
-                    const uint32_t own = sBuf + (uint32_t)(ra.x - pshift);
-                    float o[NG][GW];
+                    const int4 ra = ldsi4(sRowaddr + (uint32_t)r * 16u);
+                    const uint32_t own = sBuf + (uint32_t)(ra.x - pshift) + lane_off;     // cell 4 lane of the row
+                    float o[NG][4];
                     if (lane < KL) {
                         if (mm >= -2 && mm <= 0) {
-                            float b[NG][GW + 8];
+                            const float lws[4] = {lw.x, lw.y, lw.z, lw.w};
+                            float l[ORDER];
 #pragma unroll
-                            for (int k = 0; k < NG; ++k) {
-                                const int g = GW * lane + 32 * GW * k;
+                            for (int j = 0; j < ORDER; ++j) l[j] = lws[j];
+                            float b[NG][12];
 #pragma unroll
-                                for (int i = 0; i < (GW + 8) / 4; ++i) {
-                                    const float4 v = lds4(own + (uint32_t)((g - 4 + 4 * i) * 4));
+                            for (int k = 0; k < NG; ++k)
+#pragma unroll
+                                for (int i = 0; i < 3; ++i) {
+                                    const float4 v = lds4(own + (uint32_t)(512 * k + 16 * i - 16));
                                     b[k][4 * i] = v.x; b[k][4 * i + 1] = v.y; b[k][4 * i + 2] = v.z; b[k][4 * i + 3] = v.w;
                                 }
-                            }
 #pragma unroll
                             for (int k = 0; k < NG; ++k) {
-                                const int g = GW * lane + 32 * GW * k;
-                                if (NG > 1) {
+                                const int g = 4 * lane + 128 * k;
+                                float4 gl[4];
+                                if (!GREG) {
 #pragma unroll
-                                    for (int c = 0; c < GW; ++c) gc[c] = reinterpret_cast<const float4 *>(gtab)[g + c];
+                                    for (int j = 0; j < 4; ++j) gl[j] = lds4(sGtab + (uint32_t)((j * N + g) * 4));
                                 }
-                                if (mm == 0) kick_fp_wide<ORDER, 0, GW>(b[k], l, g, N, gc, o[k]);
-                                else if (mm == -1) kick_fp_wide<ORDER, -1, GW>(b[k], l, g, N, gc, o[k]);
-                                else kick_fp_wide<ORDER, -2, GW>(b[k], l, g, N, gc, o[k]);
+                                const float4(&gk)[4] = GREG ? gt[GREG ? k : 0] : gl;
+                                if (mm == 0) kick_fp4<ORDER, 0>(b[k], l, g, N, gk, o[k]);
+                                else if (mm == -1) kick_fp4<ORDER, -1>(b[k], l, g, N, gk, o[k]);
+                                else kick_fp4<ORDER, -2>(b[k], l, g, N, gk, o[k]);
                             }
                         } else {
                             const float *rowp = buf + ((ra.x - pshift) >> 2);
 #pragma unroll
                             for (int k = 0; k < NG; ++k) {
-                                float tmp[GW];
-                                kick_fp_wide_any<ORDER, GW>(rowp, lw, mm, GW * lane + 32 * GW * k, N,
-                                                            reinterpret_cast<const float4 *>(gtab), tmp);
+                                float tmp[4];
+                                kick_fp4_any<ORDER>(rowp, lw, mm, 4 * lane + 128 * k, N, gtab, tmp);
 #pragma unroll
-                                for (int c = 0; c < GW; ++c) o[k][c] = tmp[c];
+                                for (int c = 0; c < 4; ++c) o[k][c] = tmp[c];
                             }
                         }
                     }
                     __syncwarp();                              // every lane has read the row before anyone overwrites it
                     if (lane < KL) {
-                        const bool up = ra.y != 0, dn = ra.z != 0;
-                        const uint32_t aup = up ? ((ra.w & 1) ? mapa(sBuf + (uint32_t)(ra.y - pshift), rank - 1) : sBuf + (uint32_t)(ra.y - pshift)) : 0u;
-                        const uint32_t adn = dn ? ((ra.w & 2) ? mapa(sBuf + (uint32_t)(ra.z - pshift), rank + 1) : sBuf + (uint32_t)(ra.z - pshift)) : 0u;
+#pragma unroll
+                        for (int k = 0; k < NG; ++k) sts4(own + (uint32_t)(512 * k), make_float4(o[k][0], o[k][1], o[k][2], o[k][3]));
+                        if ((ra.y | ra.z) != 0) {
+                            // boundary row of a walker: copy into the neighbour's apron (local, or in the next CTA)
+                            if (ra.y != 0) {
+                                uint32_t aup = sBuf + (uint32_t)(ra.y - pshift) + lane_off;
+                                if (ra.w & 1) {
+                                    aup = mapa(aup, rank - 1);
+#pragma unroll
+                                    for (int k = 0; k < NG; ++k) st_async4(aup + (uint32_t)(512 * k), make_float4(o[k][0], o[k][1], o[k][2], o[k][3]), mbUp);
+                                } else {
+                                    const float z = (ra.w & 4) ? 0.0f : 1.0f;
+#pragma unroll
+                                    for (int k = 0; k < NG; ++k) sts4(aup + (uint32_t)(512 * k), make_float4(z * o[k][0], z * o[k][1], z * o[k][2], z * o[k][3]));
+                                }
+                            }
+                            if (ra.z != 0) {
+                                uint32_t adn = sBuf + (uint32_t)(ra.z - pshift) + lane_off;
+                                if (ra.w & 2) {
+                                    adn = mapa(adn, rank + 1);
+#pragma unroll
+                                    for (int k = 0; k < NG; ++k) st_async4(adn + (uint32_t)(512 * k), make_float4(o[k][0], o[k][1], o[k][2], o[k][3]), mbDn);
+                                } else {
+                                    const float z = (ra.w & 8) ? 0.0f : 1.0f;
+#pragma unroll
+                                    for (int k = 0; k < NG; ++k) sts4(adn + (uint32_t)(512 * k), make_float4(z * o[k][0], z * o[k][1], z * o[k][2], z * o[k][3]));
+                                }
+                            }
+                        }
                         float q0 = 0.0f;
 #pragma unroll
-                        for (int k = 0; k < NG; ++k) {
-                            const int g = GW * lane + 32 * GW * k;
+                        for (int k = 0; k < NG; ++k)
 #pragma unroll
-                            for (int h4 = 0; h4 < GW / 4; ++h4) {
-                                const float4 ov = make_float4(o[k][4 * h4], o[k][4 * h4 + 1], o[k][4 * h4 + 2], o[k][4 * h4 + 3]);
-                                const float4 z4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-                                const uint32_t off = (uint32_t)((g + 4 * h4) * 4);
-                                sts4(own + off, ov);
-                                if (up) { if (ra.w & 1) st_async4(aup + off, ov, mbUp); else sts4(aup + off, (ra.w & 4) ? z4 : ov); }
-                                if (dn) { if (ra.w & 2) st_async4(adn + off, ov, mbDn); else sts4(adn + off, (ra.w & 8) ? z4 : ov); }
-                            }
-#pragma unroll
-                            for (int c = 0; c < GW; ++c) { cs[k][c] += o[k][c]; q0 += o[k][c]; }
-                        }
-                        const float X = (float)(x0 + r) - xc, tq = q0 * X;
-                        q1 += tq; q2 = fmaf(tq, X, q2);
+                            for (int c = 0; c < 4; ++c) { cs[k][c] += o[k][c]; q0 += o[k][c]; }
+                        const float tq = q0 * Xf;
+                        q1 += tq; q2 = fmaf(tq, Xf, q2);
                         if (lane == 0) pw += mv.y;
                     }
                 }
@@ -885,8 +929,8 @@ k_onchip_step(GridConst G, OnchipArgs A)
 #pragma unroll
                     for (int k = 0; k < NG; ++k)
 #pragma unroll
-                        for (int c = 0; c < GW; ++c) {
-                            const float yy = (float)(GW * lane + 32 * GW * k + c) - yc;
+                        for (int c = 0; c < 4; ++c) {
+                            const float yy = (float)(4 * lane + 128 * k + c) - yc;
                             const float tt = cs[k][c] * yy;
                             v8[0] += cs[k][c]; v8[1] += tt; v8[2] = fmaf(tt, yy, v8[2]);
                         }
