@@ -402,11 +402,12 @@ int onchip_tables(vfps_sim *h, int S)
             const int r = x / R;
             const double Xc = 0.5 * ((double)(r * R) + (double)(r * R + R - 1)) + g.x0c;
             if (tab) {
-                // order 4: L[0..3] L'[0..3] ex;  order 3: L[0..2] ex L'[0..2];  order 2: L[0..1] L'[0..1] ex
+                // order 4: L[0..3] L'[1,2,3,0] ex;  order 3: L[0..2] ex L'[0..2];  order 2: L[0..1] L'[0..1] ex
                 double l[4] = {0, 0, 0, 0}, lp[4] = {0, 0, 0, 0};
                 lagrange_d(order, g.d * X + g.a * Ymid - f0, l, lp);
                 const int olp = (order == 2) ? 2 : 4, oex = (order == 4) ? 8 : (order == 3) ? 3 : 4;
-                for (int j = 0; j < order; ++j) { t[j] = (float)l[j]; t[olp + j] = (float)lp[j]; }
+                // order 4: L' rotated by one (L'1 L'2 L'3 L'0), see Walker::load_tab
+                for (int j = 0; j < order; ++j) { t[j] = (float)l[j]; t[olp + (order == 4 ? (j + 3) % 4 : j)] = (float)lp[j]; }
                 t[oex] = (float)(g.a * (X - Xc));
             } else {
                 t[8] = (float)X;

@@ -312,8 +312,11 @@ struct Walker {
     {
         if (TAB) {
             if (ORDER == 4) {
+                // L0 L1 L2 L3 | L'1 L'2 L'3 L'0: a 128-bit load fills four consecutive registers and the
+                // register file has four banks (register number mod 4, measured: csrc/peaks); L'_j
+                // rotated by one keeps L_j and L'_j, two operands of one FMA, out of the same bank
                 const float4 v = lds4(tab), w = lds4(tab + 16);
-                tb[0] = v.x; tb[1] = v.y; tb[2] = v.z; tb[3] = v.w; tb[4] = w.x; tb[5] = w.y; tb[6] = w.z; tb[7] = w.w;
+                tb[0] = v.x; tb[1] = v.y; tb[2] = v.z; tb[3] = v.w; tb[5] = w.x; tb[6] = w.y; tb[7] = w.z; tb[4] = w.w;
                 tb[2 * ORDER] = lds(tab + 32);
             } else if (ORDER == 3) {
                 const float4 v = lds4(tab), w = lds4(tab + 16);            // L0 L1 L2 ex | L'0 L'1 L'2 -
