@@ -450,7 +450,7 @@ bool onchip_try(vfps_sim *h, int S, int smem_max)
 {
     const int N = h->N, H = h->G.H;
     if (!(N == 64 || N == 128 || N == 256 || N == 512)) return false;
-    if (h->P.flags & (VFPS_FLAG_CLAMP | VFPS_FLAG_ROT_MANHATTAN)) return false;
+    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) return false;
     if (H > OC_MAX_H || N % S) return false;
     const int R = N / S;
     if (R < 4 || (R & 3) || R < H) return false;
@@ -533,7 +533,7 @@ void cluster_configure(vfps_sim *h)
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const int cand_single[5] = {16, 8, 4, 2, 1}, cand_batch[5] = {1, 2, 4, 8, 16};
     const int *cand = (h->members == 1) ? cand_single : cand_batch;
-    // second design (k_onchip_step, kernel id 3): standard rotation, free interpolation; AUTO takes it
+    // in-place design (k_onchip_step, kernel id 3): standard rotation, free or clamped interpolation; AUTO takes it
     if (h->cl_ver_opt == 0 || h->cl_ver_opt == 3) {
         for (int c = 0; c < 5; ++c) {
             const int S = cand[c];

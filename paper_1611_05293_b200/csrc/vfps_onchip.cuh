@@ -217,13 +217,14 @@ __device__ __forceinline__ float warp_reduce_transposed(float (&v)[NV], int lane
     }
 }
 
-// kick (shift by MM + t cells, Lagrange weights l already scaled by 1/C) and Fokker-Planck for the
+// kick (shift by MM + t cells, Lagrange weights l already scaled by 1/C -- un-scaled with CLAMP,
+// where the caller scales the results) and Fokker-Planck for the
 // four cells g..g+3 of one row: b[i] = psi'(g - 4 + i), i = 0..11.  k[i] = kicked value at
 // position g - 1 + i (zero outside the grid, A8).  The Fokker-Planck update (Eq. 15 + 3-point
 // second difference, explicit Euler) is  out = k0 + G[-1] k[-1] + G[0] k0 + G[1] k[1] + G[2] k[2]
 // with the per-column coefficients (G-1, G0, G1, G2): gt[j] holds coefficient j of the columns
 // g..g+3 (all <= 1e-3, so the sum is exact to well below one ulp of k0).
-template <int ORDER, int MM>
+template <int ORDER, int MM, bool CLAMP = false>
 __device__ __forceinline__ void kick_fp4(const float (&b)[12], const float (&l)[ORDER], int g, int N,
                                          const float4 (&gt)[4], float (&out)[4])
 {
@@ -235,6 +236,8 @@ __device__ __forceinline__ void kick_fp4(const float (&b)[12], const float (&l)[
         float acc = l[0] * b[i0];
 #pragma unroll
         for (int j = 1; j < ORDER; ++j) acc = fmaf(l[j], b[i0 + j], acc);
+        // Eq. 14 (reading A9): limit to the interval of the two nodes that bracket the source point
+        if (CLAMP) acc = fminf(fmaxf(acc, fminf(b[i0 + O0], b[i0 + O0 + 1])), fmaxf(b[i0 + O0], b[i0 + O0 + 1]));
         k[i] = acc;
     }
     if (g == 0) k[0] = 0.0f;
@@ -250,7 +253,7 @@ __device__ __forceinline__ void kick_fp4(const float (&b)[12], const float (&l)[
 // any integer shift: reads the row in shared memory with bounds checks (rare: |shift| > 1 cell).
 // Not inlined; weights by value, coefficients from the shared table [4][N], results through local
 // memory, so that the fast path keeps its operands in registers.
-template <int ORDER>
+template <int ORDER, bool CLAMP = false>
 __device__ __noinline__ void kick_fp4_any(const float *row /* index 0 = y 0 */, float4 lw, int mm, int g, int N,
                                           const float *gtab, float *out)
 {
@@ -260,12 +263,15 @@ __device__ __noinline__ void kick_fp4_any(const float *row /* index 0 = y 0 */, 
 #pragma unroll 1
     for (int i = 0; i < 7; ++i) {
         const int y = g - 1 + i;
-        float acc = 0.0f;
+        float acc = 0.0f, lo = 0.0f, hi = 0.0f;
         for (int j = 0; j < ORDER; ++j) {
             const int s = y + mm - O0 + j;
             const float v = (s >= 0 && s < N) ? row[s] : 0.0f;
             acc = fmaf(l[j], v, acc);
+            if (CLAMP && j == O0) lo = v;
+            if (CLAMP && j == O0 + 1) hi = v;
         }
+        if (CLAMP) acc = fminf(fmaxf(acc, fminf(lo, hi)), fmaxf(lo, hi));
         k[i] = (y >= 0 && y < N) ? acc : 0.0f;
     }
 #pragma unroll 1
@@ -282,7 +288,7 @@ __device__ __noinline__ void kick_fp4_any(const float *row /* index 0 = y 0 */, 
 // row per target row.  PAR = (iy - O0) & 1 is the offset of cell y0's first tap inside the window,
 // DIR the walk direction (+1: rows ascending).  At the start of a target row the window and the
 // table row `tb` of that target are complete; its step loads those of the next target.
-template <int ORDER, int PITCH, bool TAB>
+template <int ORDER, int PITCH, bool TAB, bool CLAMP>
 struct Walker {
     static constexpr int O0 = (ORDER - 1) / 2;
     static constexpr int NPMAX = (ORDER + 3) / 2;          // column pairs of the window (PAR = 1)
@@ -385,6 +391,18 @@ struct Walker {
         float lx0[ORDER], lx1[ORDER], ly0[ORDER], ly1[ORDER];
         weights(lx0, lx1, ly0, ly1);
         load_tab(tab + (uint32_t)(DIR * (SUB + 1) * (OC_ROWTAB * 4)));
+        // Eq. 14 (reading A9): interval of the 2 x 2 nodes around each source point -- tap rows O0, O0 + 1
+        // (taken before the window slides), columns O0, O0 + 1 of each cell's stencil
+        float lo0 = 0.0f, hi0 = 0.0f, lo1 = 0.0f, hi1 = 0.0f;
+        if (CLAMP) {
+            const float(&wa)[2 * NPMAX] = win[(SLOT0 + O0) % ORDER];
+            const float(&wb)[2 * NPMAX] = win[(SLOT0 + O0 + 1) % ORDER];
+            float cmn[3], cmx[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { cmn[k] = fminf(wa[PAR + O0 + k], wb[PAR + O0 + k]); cmx[k] = fmaxf(wa[PAR + O0 + k], wb[PAR + O0 + k]); }
+            lo0 = fminf(cmn[0], cmn[1]); hi0 = fmaxf(cmx[0], cmx[1]);
+            lo1 = fminf(cmn[1], cmn[2]); hi1 = fmaxf(cmx[1], cmx[2]);
+        }
         float r0[ORDER], r1[ORDER];
         inner<PAR>((SLOT0 + IL) % ORDER, ly0, ly1, r0[IL], r1[IL]);
         load_row<PAR>((SLOT0 + IL) % ORDER, src + (uint32_t)((DIR > 0 ? SUB + ORDER : -(SUB + 1)) * P4));
@@ -394,6 +412,7 @@ struct Walker {
         float a0 = lx0[0] * r0[0], a1 = lx1[0] * r1[0];
 #pragma unroll
         for (int i = 1; i < ORDER; ++i) { a0 = fmaf(lx0[i], r0[i], a0); a1 = fmaf(lx1[i], r1[i], a1); }
+        if (CLAMP) { a0 = fminf(fmaxf(a0, lo0), hi0); a1 = fminf(fmaxf(a1, lo1), hi1); }
         sts2(dst + (uint32_t)(DIR * SUB * P4), a0, a1);
         rs[SUB] = a0 + a1;
     }
@@ -407,7 +426,7 @@ struct Walker {
 
 // one cell with its own floors and a full window (rows where a floor changes inside the thread's
 // columns or along the chunk)
-template <int ORDER, int PITCH>
+template <int ORDER, int PITCH, bool CLAMP>
 __device__ __forceinline__ float rotate_cell_generic(const GridConst &G, uint32_t rowbase /* segment row 0, column 0 */,
                                                      int v, int x, int y)
 {
@@ -429,6 +448,11 @@ __device__ __forceinline__ float rotate_cell_generic(const GridConst &G, uint32_
         for (int j = 1; j < ORDER; ++j) r = fmaf(ly[j], lds(base + (i * PITCH + j) * 4), r);
         acc = (i == 0) ? lx[0] * r : fmaf(lx[i], r, acc);
     }
+    if (CLAMP) {
+        const float a = lds(base + (O0 * PITCH + O0) * 4), b = lds(base + (O0 * PITCH + O0 + 1) * 4);
+        const float c = lds(base + ((O0 + 1) * PITCH + O0) * 4), d = lds(base + ((O0 + 1) * PITCH + O0 + 1) * 4);
+        acc = fminf(fmaxf(acc, fminf(fminf(a, b), fminf(c, d))), fmaxf(fmaxf(a, b), fmaxf(c, d)));
+    }
     return acc;
 }
 
@@ -438,7 +462,7 @@ __device__ __forceinline__ float rotate_cell_generic(const GridConst &G, uint32_
 // grid = S * (concurrent clusters), cluster = S CTAs, block = 512.  Clusters take work items
 // (chunk j of member m, in the order j * members + m) from a queue in global memory; chunk j of a
 // member starts after its chunk j-1 has been stored (member_done).
-template <int ORDER, int N, bool TAB>
+template <int ORDER, int N, bool TAB, bool CLAMP = false>
 __global__ void __launch_bounds__(OC_THREADS, 1)
 k_onchip_step(GridConst G, OnchipArgs A)
 {
@@ -453,7 +477,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
     constexpr bool GREG = (NG <= 2);                       // Fokker-Planck coefficients of the lane's columns stay in registers
     constexpr int NW = N / 128 > 0 ? N / 128 : 1;          // float4 groups of rho per lane in the wake
     constexpr unsigned FULL = 0xffffffffu;
-    using Wk = Walker<ORDER, PITCH, TAB>;
+    using Wk = Walker<ORDER, PITCH, TAB, CLAMP>;
 
     cg::cluster_group cluster = cg::this_cluster();
     const int S = A.S, R = A.R, H = G.H;
@@ -686,8 +710,8 @@ k_onchip_step(GridConst G, OnchipArgs A)
                         for (int s = 0; s < CH; ++s) {
                             if (s < nrow) {
                                 const int v = p ? vlo + nrow - 1 - s : vlo + s;
-                                const float o0 = rotate_cell_generic<ORDER, PITCH>(G, gbase, v, x0 + wb + v, y0);
-                                const float o1 = rotate_cell_generic<ORDER, PITCH>(G, gbase, v, x0 + wb + v, y0 + 1);
+                                const float o0 = rotate_cell_generic<ORDER, PITCH, CLAMP>(G, gbase, v, x0 + wb + v, y0);
+                                const float o1 = rotate_cell_generic<ORDER, PITCH, CLAMP>(G, gbase, v, x0 + wb + v, y0 + 1);
                                 sts2(rbase + (uint32_t)((v + dsh) * P4 + (OC_PADC + y0) * 4), o0, o1);
                                 rs4[s] = o0 + o1;
                             }
@@ -780,6 +804,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
                     for (int q = warp; q < (R >> 2); q += OC_WARPS) {
                         const int x = x0 + 4 * q;
                         float vq[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+                        float vt[4] = {0.0f, 0.0f, 0.0f, 0.0f};        // CLAMP: transposed wake, sum_x' w[x' - x] rho_x'
                         if (gw != nullptr) {
 #pragma unroll
                             for (int j = 0; j < NW; ++j) {
@@ -794,10 +819,23 @@ k_onchip_step(GridConst G, OnchipArgs A)
                                     for (int k = 0; k < 4; ++k)
 #pragma unroll
                                         for (int c = 0; c < 4; ++c) vq[k] = fmaf(w7[3 + k - c], rc[c], vq[k]);
+                                    if (CLAMP) {
+                                        // w[(x' + c) - (x + k)] at index B + c - k, B = 4 lane + 128 j - x + N - 1 = 3 mod 4
+                                        const int Bq = 4 * lane + 128 * j - x + N - 1;
+                                        const float4 ul = lds4(sWf + (uint32_t)(Bq - 3) * 4u);
+                                        const float4 uh = (Bq + 1 < 2 * N) ? lds4(sWf + (uint32_t)(Bq + 1) * 4u)
+                                                                           : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                                        const float u7[8] = {ul.x, ul.y, ul.z, ul.w, uh.x, uh.y, uh.z, uh.w};
+#pragma unroll
+                                        for (int k = 0; k < 4; ++k)
+#pragma unroll
+                                            for (int c = 0; c < 4; ++c) vt[k] = fmaf(u7[3 + c - k], rc[c], vt[k]);
+                                    }
                                 }
                             }
                         }
                         const float Vr = warp_reduce_transposed<4>(vq, lane);     // lanes 8k .. 8k+7 hold row x + k
+                        const float Vtr = CLAMP ? warp_reduce_transposed<4>(vt, lane) : 0.0f;
                         if ((lane & 7) == 0) {
                             const int k = lane >> 3, r = 4 * q + k;
                             const float V = Vr * sc;
@@ -809,9 +847,19 @@ k_onchip_step(GridConst G, OnchipArgs A)
                             lagrange<ORDER>(t, l);
                             float pl[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll
-                            for (int j = 0; j < ORDER; ++j) pl[j] = l[j] * sc;
+                            for (int j = 0; j < ORDER; ++j) pl[j] = CLAMP ? l[j] : l[j] * sc;   // CLAMP: the kick scales its results
                             sts4(sVtab + (uint32_t)r * 32u, make_float4(pl[0], pl[1], pl[2], pl[3]));
-                            sts2(sVtab + (uint32_t)r * 32u + 16u, __int_as_float(mm), rho_x * V);
+                            if (CLAMP) {
+                                // The clamped kick is not conservative: the profile after it, rho', differs from rho.
+                                // CSR power of the END-of-step density to first order in rho' - rho (the neglected
+                                // term is quadratic, < 1e-6 relative):  sum rho' V' = sum rho V + sum (rho' - rho) U,
+                                // U = V + Vt.  Row term: rho_x V_x - rho_x U_x = -rho_x Vt_x; the kick adds dp U_x
+                                // times its row sums.
+                                const float Vt = Vtr * sc;
+                                sts4(sVtab + (uint32_t)r * 32u + 16u, make_float4(__int_as_float(mm), -rho_x * Vt, G.dp * (V + Vt), 0.0f));
+                            } else {
+                                sts2(sVtab + (uint32_t)r * 32u + 16u, __int_as_float(mm), rho_x * V);
+                            }
                         }
                     }
                 }
@@ -841,7 +889,14 @@ k_onchip_step(GridConst G, OnchipArgs A)
                 float Xf = (float)(x0 + warp) - xc;
                 for (int r = warp; r < R; r += OC_WARPS, Xf += (float)OC_WARPS) {
                     const float4 lw = lds4(sVtab + (uint32_t)r * 32u);
-                    const float2 mv = lds2(sVtab + (uint32_t)r * 32u + 16u);
+                    float2 mv;
+                    float dpU = 0.0f;                          // CLAMP: dp (V + Vt) of the row
+                    if (CLAMP) {
+                        const float4 m4 = lds4(sVtab + (uint32_t)r * 32u + 16u);
+                        mv = make_float2(m4.x, m4.y); dpU = m4.z;
+                    } else {
+                        mv = lds2(sVtab + (uint32_t)r * 32u + 16u);
+                    }
                     const int mm = __float_as_int(mv.x);
                     const int4 ra = ldsi4(sRowaddr + (uint32_t)r * 16u);
                     const uint32_t own = sBuf + (uint32_t)(ra.x - pshift) + lane_off;     // cell 4 lane of the row
@@ -869,19 +924,25 @@ k_onchip_step(GridConst G, OnchipArgs A)
                                     for (int j = 0; j < 4; ++j) gl[j] = lds4(sGtab + (uint32_t)((j * N + g) * 4));
                                 }
                                 const float4(&gk)[4] = GREG ? gt[GREG ? k : 0] : gl;
-                                if (mm == 0) kick_fp4<ORDER, 0>(b[k], l, g, N, gk, o[k]);
-                                else if (mm == -1) kick_fp4<ORDER, -1>(b[k], l, g, N, gk, o[k]);
-                                else kick_fp4<ORDER, -2>(b[k], l, g, N, gk, o[k]);
+                                if (mm == 0) kick_fp4<ORDER, 0, CLAMP>(b[k], l, g, N, gk, o[k]);
+                                else if (mm == -1) kick_fp4<ORDER, -1, CLAMP>(b[k], l, g, N, gk, o[k]);
+                                else kick_fp4<ORDER, -2, CLAMP>(b[k], l, g, N, gk, o[k]);
                             }
                         } else {
                             const float *rowp = buf + ((ra.x - pshift) >> 2);
 #pragma unroll
                             for (int k = 0; k < NG; ++k) {
                                 float tmp[4];
-                                kick_fp4_any<ORDER>(rowp, lw, mm, 4 * lane + 128 * k, N, gtab, tmp);
+                                kick_fp4_any<ORDER, CLAMP>(rowp, lw, mm, 4 * lane + 128 * k, N, gtab, tmp);
 #pragma unroll
                                 for (int c = 0; c < 4; ++c) o[k][c] = tmp[c];
                             }
+                        }
+                        if (CLAMP) {
+#pragma unroll
+                            for (int k = 0; k < NG; ++k)
+#pragma unroll
+                                for (int c = 0; c < 4; ++c) o[k][c] *= sc;
                         }
                     }
                     __syncwarp();                              // every lane has read the row before anyone overwrites it
@@ -922,6 +983,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
                             for (int c = 0; c < 4; ++c) { cs[k][c] += o[k][c]; q0 += o[k][c]; }
                         const float tq = q0 * Xf;
                         q1 += tq; q2 = fmaf(tq, Xf, q2);
+                        if (CLAMP) pw = fmaf(q0, dpU, pw);
                         if (lane == 0) pw += mv.y;
                     }
                 }

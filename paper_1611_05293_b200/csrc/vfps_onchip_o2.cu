@@ -6,7 +6,7 @@ namespace vfps {
 
 const void *onchip_kernel_o2(int N, bool tab, bool clamp)
 {
-    (void)clamp;
+    (void)clamp;          // linear interpolation never leaves the interval of its two nodes: the clamp is the identity
 #define VFPS_OC(NN) (tab ? (const void *)k_onchip_step<2, NN, true> : (const void *)k_onchip_step<2, NN, false>)
     switch (N) {
         case 64: return VFPS_OC(64);

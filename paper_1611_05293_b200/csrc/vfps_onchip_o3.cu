@@ -6,8 +6,9 @@ namespace vfps {
 
 const void *onchip_kernel_o3(int N, bool tab, bool clamp)
 {
-    (void)clamp;
-#define VFPS_OC(NN) (tab ? (const void *)k_onchip_step<3, NN, true> : (const void *)k_onchip_step<3, NN, false>)
+#define VFPS_OC(NN)                                                                                     \
+    (clamp ? (tab ? (const void *)k_onchip_step<3, NN, true, true> : (const void *)k_onchip_step<3, NN, false, true>)  \
+           : (tab ? (const void *)k_onchip_step<3, NN, true, false> : (const void *)k_onchip_step<3, NN, false, false>))
     switch (N) {
         case 64: return VFPS_OC(64);
         case 128: return VFPS_OC(128);

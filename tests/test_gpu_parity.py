@@ -479,9 +479,11 @@ def test_clamped_interpolation(vfps, orc, order, N, manhattan):
     psi0 = (psi0 / (psi0.astype(np.float64).sum() * (12.0 / (N - 1)) ** 2)).astype(np.float32)[None]
     flags = vfps.FLAG_RENORMALISE | vfps.FLAG_CLAMP | (vfps.FLAG_ROT_MANHATTAN if manhattan else 0)
     sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, 1, Z=Z, flags=flags)
-    with pytest.raises(vfps.VfpsError) as e:
-        sim.set_engine(vfps.ENGINE_CLUSTER)
-    assert e.value.code == -5
+    if manhattan or N < 64:
+        # the in-place cluster kernel has the standard rotation on N >= 64; the first design no clamp
+        with pytest.raises(vfps.VfpsError) as e:
+            sim.set_engine(vfps.ENGINE_CLUSTER)
+        assert e.value.code == -5
     sim.set_engine(vfps.ENGINE_STREAM)
     sim.set_psi_host(psi0)
     o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, 300, 2e-3, order, 2, Z[0], manhattan=manhattan, clamp=True)
@@ -518,6 +520,63 @@ def test_clamped_interpolation(vfps, orc, order, N, manhattan):
     assert_psi(psi, o.psi, 1e-4, f"clamp N={N} order={order} manhattan={manhattan} 40 steps, {sim.engine_name} engine")
     assert_diag(d[9, 0], dr[9], tol_p=2e-3)
     # the Fokker-Planck update is the only place left that can produce a (tiny) negative value
+    assert psi.min() > -1e-4 * psi.max() and psi.max() < 1.02 * psi0.max()
+    if not manhattan and N >= 64:
+        # cluster engine (in-place kernel): clamped rotation and kick on chip; its P_csr is that of the
+        # end-of-step density to first order in the profile change of the clamped kick: 1e-4 holds
+        ran = 0
+        for S in (16, 4, 2):
+            try:
+                sim.set_cluster_size(S)
+            except vfps.VfpsError as err:
+                assert err.code == -5
+                continue
+            sim.set_engine(vfps.ENGINE_CLUSTER)
+            assert sim.engine_name == "cluster" and sim.cluster_kernel == 3
+            d = sim.step_host(10)
+            dr = o.step(10)
+            assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"clamp N={N} order={order}, cluster engine S={S}")
+            for i in (0, 9):
+                assert_diag(d[i, 0], dr[i])
+            ran += 1
+        assert ran >= 2
+    sim.close()
+
+
+@pytest.mark.parametrize("order,S", [(4, 16), (4, 2), (3, 8)])
+def test_clamped_interpolation_cluster_c1(vfps, orc, order, S):
+    """VFPS_FLAG_CLAMP on the cluster engine in the regime of the BASELINE configs (256^2, 4000 steps
+    per period: per-launch weight tables): C1 physics on a bunch with a sharp-edged hole, 1 step and
+    100 steps against the oracle's clamped step, every diagnostic (P_csr included) at 1e-4."""
+    wl = get_workload("C1").with_(interp_order=order)
+    N = wl.N
+    psi0 = wl.psi0([0])[0].copy()
+    a, b = N // 2 - N // 8, N // 2 + N // 8
+    psi0[a:b, a:b] = 0.0
+    psi0 = (psi0 / (psi0.astype(np.float64).sum() * wl.dq * wl.dp)).astype(np.float32)[None]
+    Z = wl.impedance([0])
+    sim = vfps.Simulation(N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta, order, wl.pad, 1,
+                          Z=Z, flags=vfps.FLAG_RENORMALISE | vfps.FLAG_CLAMP)
+    sim.set_cluster_size(S)
+    sim.set_engine(vfps.ENGINE_CLUSTER)
+    assert sim.cluster_kernel == 3 and sim.cluster_size == S
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta, order, wl.pad, Z[0], clamp=True)
+    o.set_psi(psi0[0])
+    free = orc.Oracle(N, wl.q_min, wl.q_max, wl.p_min, wl.p_max, wl.steps_per_period, wl.beta, order, wl.pad, Z[0])
+    free.set_psi(psi0[0])
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"clamp C1 order={order} S={S} 1 step")
+    assert_diag(d[0, 0], dr[0])
+    d = sim.step_host(99)
+    dr = o.step(99)
+    free.step(100)
+    psi = sim.get_psi_host()[0]
+    assert_psi(psi, o.psi, 1e-4, f"clamp C1 order={order} S={S} 100 steps")
+    for i in (0, 49, 98):
+        assert_diag(d[i, 0], dr[i])
+    assert np.max(np.abs(o.psi - free.psi)) > 1e-3 * o.psi.max()       # the flag does something
     assert psi.min() > -1e-4 * psi.max() and psi.max() < 1.02 * psi0.max()
     sim.close()
 
