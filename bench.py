@@ -53,7 +53,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4", "T3"])
     ap.add_argument("--inner", type=int, default=0, help="split steps per bench step (0 = one synchrotron period)")
     ap.add_argument("--engine", default="auto", choices=["auto", "stream", "graph", "cluster", "grid"])
     ap.add_argument("--wake", default="auto", choices=["auto", "fft", "direct"])

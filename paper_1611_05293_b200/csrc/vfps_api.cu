@@ -42,7 +42,7 @@ struct vfps_sim {
     float *rho_part = nullptr;                   // [members][N][tiles_y2]
     float *rho = nullptr, *V = nullptr;          // [members][N]
     float *qstat = nullptr;                      // [members][4]
-    float *mom_part = nullptr;                   // [members][kfp2_blocks][5]
+    float *mom_part = nullptr;                   // [members][kfp2_blocks][6]
     float *scale = nullptr;                      // [members]
     unsigned *blkctr = nullptr;                  // [members]
     int *rowctr = nullptr;                       // [members]
@@ -70,6 +70,7 @@ struct vfps_sim {
     // streaming kernels (vfps_stream2.cuh)
     int tiles_x2 = 0, tiles_y2 = 0, kfp2_rows = 0, kfp2_blocks = 0, wd_blocks = 0;
     float *pw_part = nullptr;                    // [members][wd_blocks]
+    float *dpU = nullptr;                        // [members][N], clamped interpolation only (k_wake_direct)
     // persistent cooperative-grid engine (vfps_grid.cuh); gr_blocks = 0: not available
     int gr_blocks = 0, gr_KR = 0;
     size_t gr_smem = 0;
@@ -617,7 +618,7 @@ void grid_configure(vfps_sim *h)
     int blocks = 2 * sms;
     for (int pass = 0; pass < 2; ++pass) {
         const int KR = (N + blocks - 1) / blocks;
-        const size_t smem = grid_smem_floats(N, KR) * sizeof(float);
+        const size_t smem = grid_smem_floats(N, KR, (h->P.flags & VFPS_FLAG_CLAMP) != 0) * sizeof(float);
         int per_sm = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, grid_kernel(h), GR_THREADS, smem);
         if (e != cudaSuccess || per_sm < 1) { cudaGetLastError(); h->gr_why = "grid kernel does not fit an SM"; return; }
@@ -698,13 +699,21 @@ int launch_step_stream2(vfps_sim *h, bool timed)
         h->launches += 1;
     } else if (h->has_wake) {      // without an impedance V stays 0 (set at create) and P = 0
         Bracket br(h, VFPS_KERNEL_WAKE_DIRECT, timed);
-        k_wake_direct<<<dim3(h->wd_blocks, h->members), WD_THREADS, (size_t)(2 * N + WD_ROWS) * sizeof(float), h->stream>>>(
-            N, h->rho, h->wfun, h->V, h->pw_part);
+        const size_t wd_smem = (size_t)((CLAMP ? 3 : 2) * N + 2 * WD_ROWS) * sizeof(float);
+        if (wd_smem > 48 * 1024) {       // N = 4096 with the transposed wake: opt-in, only ever raised
+            static size_t granted = 0;
+            if (wd_smem > granted &&
+                cudaFuncSetAttribute(k_wake_direct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wd_smem) == cudaSuccess)
+                granted = wd_smem;
+        }
+        k_wake_direct<<<dim3(h->wd_blocks, h->members), WD_THREADS, wd_smem, h->stream>>>(
+            N, h->rho, h->wfun, h->V, h->pw_part, CLAMP ? h->dpU : nullptr, h->G.dp);
         h->launches += 1;
     }
     Kfp2Args A;
     A.psi_in = h->psi_tmp; A.psi_out = h->psi; A.V = h->V; A.qstat = h->qstat;
     A.pw_part = direct ? h->pw_part : nullptr; A.npw = h->wd_blocks;
+    A.dpU = (CLAMP && direct && h->has_wake) ? h->dpU : nullptr;
     A.mom_part = h->mom_part; A.scale = h->scale; A.blkctr = h->blkctr; A.rowctr = h->rowctr;
     A.diag = h->diag_cell; A.members = h->members; A.rows_per_cta = h->kfp2_rows;
     {
@@ -833,7 +842,8 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     CUB(dalloc(h, &h->rho, (size_t)M * N));
     CUB(dalloc(h, &h->V, (size_t)M * N));
     CUB(dalloc(h, &h->qstat, (size_t)M * 4));
-    CUB(dalloc(h, &h->mom_part, (size_t)M * h->kfp2_blocks * 5));
+    CUB(dalloc(h, &h->mom_part, (size_t)M * h->kfp2_blocks * 6));
+    if (p->flags & VFPS_FLAG_CLAMP) CUB(dalloc(h, &h->dpU, (size_t)M * N));
     CUB(dalloc(h, &h->scale, (size_t)M));
     CUB(dalloc(h, &h->blkctr, (size_t)M));
     CUB(dalloc(h, &h->rowctr, (size_t)M));
@@ -993,6 +1003,9 @@ int vfps_set_option(vfps_handle h, int option, int value)
     if (option == VFPS_OPT_WAKE) {
         if (!(value == VFPS_WAKE_AUTO || value == VFPS_WAKE_FFT || value == VFPS_WAKE_DIRECT))
             return fail(h, VFPS_ERR_ARG, "unknown wake mode");
+        if (value == VFPS_WAKE_FFT && (h->P.flags & VFPS_FLAG_CLAMP) && h->has_wake)
+            return fail(h, VFPS_ERR_UNSUPPORTED, "clamped interpolation needs the direct-convolution wake (its transposed "
+                                                   "wake gives the CSR power of the end-of-step profile)");
         if (value != h->wake_opt) drop_graph(h);
         h->wake_opt = value;
         return VFPS_OK;

@@ -48,7 +48,12 @@ struct GridArgs {
     long long *dbg;      // nullptr, or [CTA][64 steps][8] clock64 stamps (debug aid)
 };
 
-__host__ __device__ inline size_t grid_smem_floats(int N, int KR) { return (size_t)2 * N + 2 * KR + 8; }
+// profile (N), wake-function window (N + KR), V of the CTA's rows (KR); with clamped interpolation
+// also the window of the transposed wake (N + KR) and dp (V + Vt) of the rows (KR)
+__host__ __device__ inline size_t grid_smem_floats(int N, int KR, bool clamp = false)
+{
+    return (size_t)2 * N + 2 * KR + 8 + (clamp ? (size_t)N + 2 * KR : 0);
+}
 
 template <int ORDER, bool MANH = false, bool CLAMP = false>
 __global__ void __launch_bounds__(GR_THREADS, 2)
@@ -65,6 +70,7 @@ k_grid_step(GridConst G, GridArgs A)
     const int N = G.N, NQ = N >> 2, lgNQ = 31 - __clz(NQ);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     float *srho = gsm, *sw = gsm + N, *sV = gsm + 2 * N + A.KR;       // sw: N + KR - 1 lags
+    float *sw2 = gsm + 2 * N + 2 * A.KR + 8, *sU = sw2 + N + A.KR;     // CLAMP only (grid_smem_floats)
     const int tiles_x = (N + GR_RT - 1) / GR_RT, ntiles = tiles_x * A.tiles_y;
     const int lg_ty = 31 - __clz(A.tiles_y);           // tiles_y is a power of two (N is; 256 columns per tile)
     const float yc = 0.5f * (float)(N - 1);
@@ -188,6 +194,15 @@ k_grid_step(GridConst G, GridArgs A)
             }
             if (A.wfun != nullptr)
                 for (int i = tid; i < N + A.KR - 1; i += GR_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
+            if (CLAMP && A.wfun != nullptr) {
+                // window of the transposed wake: sw2[i] = w at index N - r0 - KR + i, so that
+                // w[x' - x] = sw2[x' + KR - 1 - (x - r0)]
+                const int base2 = N - r0 - A.KR;
+                for (int i = tid; i < N + A.KR - 1; i += GR_THREADS) {
+                    const int k = base2 + i;
+                    sw2[i] = (k >= 0 && k < 2 * N - 1) ? __ldg(A.wfun + k) : 0.0f;
+                }
+            }
             __syncthreads();
             VFPS_STAMP(A.dbg, step, 3);
             // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4), one row per warp at a time
@@ -203,7 +218,25 @@ k_grid_step(GridConst G, GridArgs A)
                     if (xp < N) v0 = fmaf(wx[-xp], srho[xp], v0);
                 }
                 const float v = warp_sum(v0 + v1);
-                if (lane == 0) { sV[r] = v; acc[5] = fmaf(srho[r0 + r], v, acc[5]); }
+                if constexpr (CLAMP) {
+                    // The clamped kick is not conservative: CSR power of the END-of-step profile rho' to first
+                    // order in rho' - rho: sum rho' V' = sum rho V + sum (rho' - rho)(V + Vt), Vt the transposed
+                    // wake.  Row term -rho_x Vt_x here; the kick adds its row sums times dp (V + Vt).
+                    float u0 = 0.0f, u1 = 0.0f;
+                    if (A.wfun != nullptr) {
+                        const float *ux = sw2 + (A.KR - 1 - r);
+                        int xp = lane;
+                        for (; xp + 32 < N; xp += 64) {
+                            u0 = fmaf(ux[xp], srho[xp], u0);
+                            u1 = fmaf(ux[xp + 32], srho[xp + 32], u1);
+                        }
+                        if (xp < N) u0 = fmaf(ux[xp], srho[xp], u0);
+                    }
+                    const float vt = warp_sum(u0 + u1);
+                    if (lane == 0) { sV[r] = v; sU[r] = G.dp * (v + vt); acc[5] = fmaf(-srho[r0 + r], vt, acc[5]); }
+                } else {
+                    if (lane == 0) { sV[r] = v; acc[5] = fmaf(srho[r0 + r], v, acc[5]); }
+                }
             }
             __syncthreads();
             VFPS_STAMP(A.dbg, step, 4);
@@ -252,6 +285,7 @@ k_grid_step(GridConst G, GridArgs A)
                     }
                     const float xx = (float)x - yc, tq = rs * xx;
                     acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+                    if (CLAMP) acc[5] = fmaf(rs, sU[rr], acc[5]);
                 }
             } else {
             // a4 + a5: four cells per thread in registers; four granules per pass, loads first
@@ -302,6 +336,7 @@ k_grid_step(GridConst G, GridArgs A)
                         }
                         const float xx = (float)x - yc, tq = rs * xx;
                         acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+                        if (CLAMP) acc[5] = fmaf(rs, sU[rr], acc[5]);
                     }
                 }
             }

@@ -248,21 +248,32 @@ k_moments_final(GridConst G, const float *__restrict__ rho, const float *__restr
 // wake function this CTA's rows touch are staged with coalesced loads, then warp w evaluates
 // V_x = sum_x' w[x - x'] rho_x' (Eq. 4; w = Re IDFT(Z) from create, lag d at index d + N - 1)
 // for x = r0 + w.  pw_part[m][cta] = sum over the CTA's rows of rho_x V_x.
+// dpU != nullptr (clamped interpolation; N + WD_ROWS more floats of shared memory): the clamped
+// kick is not conservative, so the CSR power of the END-of-step profile rho' is formed to first
+// order in rho' - rho:  sum rho' V' = sum rho V + sum (rho' - rho)(V + Vt),  Vt_x = sum_x' w[x' - x]
+// rho_x' (transposed wake).  Then pw_part = sum -rho_x Vt_x and dpU[m][x] = dp (V_x + Vt_x), which
+// the kick kernel multiplies with its row sums.
 __global__ void __launch_bounds__(WD_THREADS)
 k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wfun, float *__restrict__ V,
-              float *__restrict__ pw_part)
+              float *__restrict__ pw_part, float *__restrict__ dpU, float dp)
 {
     extern __shared__ float wd_smem[];
     __shared__ float wpw[WD_THREADS / 32];
-    float *srho = wd_smem, *sw = wd_smem + N;
+    float *srho = wd_smem, *sw = wd_smem + N, *sw2 = wd_smem + 2 * N + WD_ROWS;
     const int m = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int r0 = blockIdx.x * WD_ROWS;
-    const float *gr = rho + (size_t)m * N, *gw = wfun + (size_t)m * 2 * N + r0;
+    const float *gr = rho + (size_t)m * N, *gw = wfun + (size_t)m * 2 * N;
     for (int i = tid; i < N; i += WD_THREADS) srho[i] = __ldg(gr + i);
-    for (int i = tid; i < N + WD_ROWS - 1; i += WD_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(gw + i) : 0.0f;
+    for (int i = tid; i < N + WD_ROWS - 1; i += WD_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(gw + r0 + i) : 0.0f;
+    const int base2 = N - r0 - WD_ROWS;                // sw2[i] = w at index base2 + i
+    if (dpU != nullptr)
+        for (int i = tid; i < N + WD_ROWS - 1; i += WD_THREADS) {
+            const int k = base2 + i;
+            sw2[i] = (k >= 0 && k < 2 * N - 1) ? __ldg(gw + k) : 0.0f;
+        }
     __syncthreads();
     const int x = r0 + warp;
-    float v0 = 0.0f, v1 = 0.0f;
+    float v0 = 0.0f, v1 = 0.0f, u0 = 0.0f, u1 = 0.0f;
     if (x < N) {
         const float *wx = sw + (warp + N - 1);
         int xp = lane;
@@ -271,13 +282,24 @@ k_wake_direct(int N, const float *__restrict__ rho, const float *__restrict__ wf
             v1 = fmaf(wx[-(xp + 32)], srho[xp + 32], v1);
         }
         if (xp < N) v0 = fmaf(wx[-xp], srho[xp], v0);
+        if (dpU != nullptr) {
+            const float *ux = sw2 + (WD_ROWS - 1 - warp);      // w[x' - x] at ux[x']
+            xp = lane;
+            for (; xp + 32 < N; xp += 64) {
+                u0 = fmaf(ux[xp], srho[xp], u0);
+                u1 = fmaf(ux[xp + 32], srho[xp + 32], u1);
+            }
+            if (xp < N) u0 = fmaf(ux[xp], srho[xp], u0);
+        }
     }
     const float v = warp_sum(v0 + v1);
+    const float vt = (dpU != nullptr) ? warp_sum(u0 + u1) : 0.0f;
     if (lane == 0) {
         float pw = 0.0f;
         if (x < N) {
             V[(size_t)m * N + x] = v;
-            pw = srho[x] * v;
+            if (dpU != nullptr) { dpU[(size_t)m * N + x] = dp * (v + vt); pw = -srho[x] * vt; }
+            else pw = srho[x] * v;
         }
         wpw[warp] = pw;
     }

@@ -414,6 +414,7 @@ struct Kfp2Args {
     const float *qstat;     // [members][4] from k_wake_fft (P_raw in slot 3), used if pw_part == nullptr
     const float *pw_part;   // [members][npw] from k_wake_direct, or nullptr
     int npw;
+    const float *dpU;       // CLAMP: [members][N] dp (V + Vt) from k_wake_direct (see there)
     float *mom_part;        // [members][gridDim.x][5]: sum psi, sum Yc psi, sum Yc^2 psi, sum Xc psi, sum Xc^2 psi
     float *scale;           // [members] out: 1/C
     unsigned *blkctr;       // [members], zero between launches
@@ -489,6 +490,7 @@ k_kick_fp2(GridConst G, Kfp2Args A)
             }
             const float xx = (float)x - yc, tq = rs * xx;
             acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+            if (CLAMP && A.dpU != nullptr) acc[5] = fmaf(rs, __ldg(A.dpU + (size_t)m * N + x), acc[5]);
         }
     } else {
     // four granules per thread and pass: every load of the pass is issued before the first use
@@ -542,6 +544,7 @@ k_kick_fp2(GridConst G, Kfp2Args A)
                 }
                 const float xx = (float)x - yc, tq = rs * xx;
                 acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+                if (CLAMP && A.dpU != nullptr) acc[5] = fmaf(rs, __ldg(A.dpU + (size_t)m * N + x), acc[5]);
             }
         }
     }
@@ -551,11 +554,11 @@ k_kick_fp2(GridConst G, Kfp2Args A)
         if ((lane & 3) == 0) red[((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
     }
     __syncthreads();
-    if (tid < 5) {
+    if (tid < 6) {
         float tsum = 0.0f;
 #pragma unroll
         for (int w = 0; w < K2_THREADS / 32; ++w) tsum += red[tid][w];
-        A.mom_part[((size_t)m * gridDim.x + blockIdx.x) * 5 + tid] = tsum;
+        A.mom_part[((size_t)m * gridDim.x + blockIdx.x) * 6 + tid] = tsum;
         __threadfence();
     }
     // ---- last CTA of this member finalises the step (deterministic: fixed summation order)
@@ -570,11 +573,12 @@ k_kick_fp2(GridConst G, Kfp2Args A)
     if (warp == 0) {
         // (fp32 sums: fp64 adds and shuffles cost ~10 us of serial tail per step on B200)
         float f0 = 0, f1 = 0, f2 = 0, f3 = 0, f4 = 0, fp = 0;
-        const float *mp = A.mom_part + (size_t)m * gridDim.x * 5;
+        const float *mp = A.mom_part + (size_t)m * gridDim.x * 6;
 #pragma unroll 4
         for (int i = lane; i < (int)gridDim.x; i += 32) {
-            f0 += __ldcg(mp + 5 * i); f1 += __ldcg(mp + 5 * i + 1); f2 += __ldcg(mp + 5 * i + 2);
-            f3 += __ldcg(mp + 5 * i + 3); f4 += __ldcg(mp + 5 * i + 4);
+            f0 += __ldcg(mp + 6 * i); f1 += __ldcg(mp + 6 * i + 1); f2 += __ldcg(mp + 6 * i + 2);
+            f3 += __ldcg(mp + 6 * i + 3); f4 += __ldcg(mp + 6 * i + 4);
+            if (CLAMP) fp += __ldcg(mp + 6 * i + 5);          // row sums times dp (V + Vt)
         }
         if (A.pw_part != nullptr)
             for (int i = lane; i < A.npw; i += 32) fp += __ldcg(A.pw_part + (size_t)m * A.npw + i);

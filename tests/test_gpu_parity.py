@@ -23,10 +23,22 @@ def assert_psi(sim_psi, ref_psi, tol, what=""):
     return err
 
 
+def edge_flux_tol(C):
+    """P_csr of a step is formed from the profile the wake acts on, renormalised by the step's
+    charge: P = dq sum rho_x V_x / C^2 (include/vfps.h).  Kick and Fokker-Planck move charge along p
+    only, so the end-of-step profile differs from that one exactly by the charge that crosses the
+    p-edges of the box during the step (C: the step's pre-renormalisation charge of a density that
+    entered it normalised).  P is quadratic in the profile: depending on where the lost charge sat,
+    the end-of-step value lies between P and P / C^2 -- bound 1.5 (1 / C^2 - 1), i.e. 3 |1 - C| for
+    small losses."""
+    C = float(C)
+    return TOL_MOM + 1.5 * abs(1.0 / (C * C) - 1.0)
+
+
 def assert_diag(got, want, has_wake=True, tol_q=TOL_MOM, tol_p=None):
     """tol_q: tolerance of the numbers that may be taken from the post-rotation profile (P_csr; in
     the stream engine also <q>, sigma_q); equal to TOL_MOM unless the bunch overflows the box
-    (edge flux).  tol_p overrides it for P_csr alone."""
+    (edge flux).  tol_p overrides it for P_csr alone (edge_flux_tol)."""
     tol_p = tol_q if tol_p is None else tol_p
     got = np.array(got, dtype=np.float64)
     want = np.array(want, dtype=np.float64)
@@ -139,6 +151,54 @@ def test_c4_one_step_and_1000_steps(vfps, orc):
     for i in (99, 499, 999):
         assert_diag(d[i, 0], dr[0][i])
     sim.close()
+
+
+# ---------------------------------------------------------------- the paper's Table III
+@pytest.mark.parametrize("order", [4, 3])
+def test_t3_table3_one_step_and_1000_steps(vfps, orc, order):
+    """PAPER.md L202-229, Table III: 256^2, 4000 steps per T_s, free-space CSR, xi = 0.516 (read as
+    S_csr, reading A16), damping time 200 T_s; cubic as in the table and quadratic as in the text's
+    second run.  Cluster engine (what AUTO picks), north_star's two bars."""
+    wl = get_workload("T3").with_(interp_order=order)
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1)
+    assert sim.engine_name == "cluster"
+    assert_psi(psi[0], refs[0].psi, TOL_1, f"T3 order {order} 1 step")
+    assert_diag(d[0, 0], dr[0][0])
+    sim.close()
+    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1000, diag_every=100)
+    assert_psi(psi[0], refs[0].psi, TOL_1000, f"T3 order {order} 1000 steps")
+    for i in (99, 499, 999):
+        assert_diag(d[i, 0], dr[0][i])
+    sim.close()
+
+
+def test_t3_quadratic_interpolation_ripples(vfps):
+    """The qualitative statement of L212-229 / Fig. 6-7: with quadratic interpolation the run
+    develops non-physical structures "with a period length of two grid cells" in the bunch profile,
+    with cubic interpolation it does not.  Measure of the two-cell content of a profile: its
+    Nyquist component |sum_x (-1)^x rho_x| relative to its charge.  Over three synchrotron periods
+    (the ripples of Fig. 7 appear around T = 1 T_s) the largest two-cell content seen with
+    quadratic interpolation must exceed that seen with cubic interpolation by two orders of
+    magnitude, and the cubic run must stay calm (sigma_delta within a few per cent of 1: L208-210)."""
+    wl = get_workload("T3")
+    sign = np.where(np.arange(wl.N) % 2 == 0, 1.0, -1.0)
+    content = {}
+    for order in (4, 3):
+        sim = vfps.Simulation.from_workload(wl.with_(interp_order=order))
+        worst = 0.0
+        for _ in range(int(3 * wl.steps_per_period / 250)):
+            d = sim.step_host(250)
+            rho = sim.get_profile_host()[0].astype(np.float64)
+            worst = max(worst, abs(np.dot(sign, rho)) / rho.sum())
+        content[order] = worst
+        if order == 4:
+            # "a relatively calm state with just little oscillation" (L208); the level itself depends on
+            # the xi <-> S_csr reading (A16) and on the Gaussian start, so only calmness is asserted
+            assert 0.85 < d[-1, 0, 4] < 1.15, ("energy spread of the cubic run", d[-1, 0, 4])
+        assert np.all(np.isfinite(d))
+        sim.close()
+    print("two-cell content of the profile: cubic %.2e quadratic %.2e" % (content[4], content[3]))
+    assert content[3] > 100.0 * content[4], content
 
 
 # ---------------------------------------------------------------- full-size runs in bench.py's configuration
@@ -460,7 +520,7 @@ def test_manhattan_c1_and_large_kick(vfps, orc):
     dr = o.step(3)
     # three steps of three successive fp32 interpolations with shifts of up to 8 cells on a 64^2 grid
     assert_psi(sim.get_psi_host()[0], o.psi, 6e-5, "manhattan large kick")
-    assert_diag(d[2, 0], dr[2], tol_p=0.1)
+    assert_diag(d[2, 0], dr[2], tol_p=edge_flux_tol(dr[2][0]))
     sim.close()
 
 
@@ -497,15 +557,15 @@ def test_clamped_interpolation(vfps, orc, order, N, manhattan):
     # differ only where P is within rounding of the bound, and then both results are within
     # rounding of each other: the usual tolerance holds
     assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"clamp N={N} order={order} manhattan={manhattan} 1 step")
-    # P_csr is taken from the wake-stage profile (include/vfps.h); the clamped kick is not
-    # conservative, so on this sharp-edged input it differs from the end-of-step value by ~1e-4
-    assert_diag(d[0, 0], dr[0], tol_p=2e-3)
+    # the clamped kick is not conservative: P_csr is that of the end-of-step profile (to first order
+    # in its change, include/vfps.h), so the 1e-4 bar holds on this sharp-edged input too
+    assert_diag(d[0, 0], dr[0])
     assert np.max(np.abs(o.psi - free.psi)) > 1e-3 * o.psi.max()
     sim.set_engine(vfps.ENGINE_GRAPH)
     d = sim.step_host(29)
     dr = o.step(29)
     assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"clamp N={N} order={order} manhattan={manhattan} 30 steps")
-    assert_diag(d[28, 0], dr[28], tol_p=2e-3)
+    assert_diag(d[28, 0], dr[28])
     if manhattan:
         # the clamped RF kick changes the profile, so the wake needs the profile after it: only the
         # stream / graph engines have that extra pass
@@ -518,7 +578,7 @@ def test_clamped_interpolation(vfps, orc, order, N, manhattan):
     dr = o.step(10)
     psi = sim.get_psi_host()[0]
     assert_psi(psi, o.psi, 1e-4, f"clamp N={N} order={order} manhattan={manhattan} 40 steps, {sim.engine_name} engine")
-    assert_diag(d[9, 0], dr[9], tol_p=2e-3)
+    assert_diag(d[9, 0], dr[9])
     # the Fokker-Planck update is the only place left that can produce a (tiny) negative value
     assert psi.min() > -1e-4 * psi.max() and psi.max() < 1.02 * psi0.max()
     if not manhattan and N >= 64:
@@ -809,17 +869,17 @@ def test_cluster_engine_large_kick_and_switching(vfps, orc, N, kernel):
     # this kick pushes 1.7 % of the charge over the p edge per step: P_csr (taken from the
     # post-rotation profile, include/vfps.h) differs from the end-of-step value by that flux
     assert_psi(sim.get_psi_host()[0], o.psi, 3e-5, "cluster large kick")
-    assert_diag(d[2, 0], dr[2], tol_p=0.1)
+    assert_diag(d[2, 0], dr[2], tol_p=edge_flux_tol(dr[2][0]))
     sim.set_engine(vfps.ENGINE_STREAM)
     d = sim.step_host(3)
     dr = o.step(3)
     assert_psi(sim.get_psi_host()[0], o.psi, 5e-5, "cluster -> stream")
-    assert_diag(d[2, 0], dr[2], tol_p=10.0)      # by now a third of the charge leaves per step
+    assert_diag(d[2, 0], dr[2], tol_p=edge_flux_tol(dr[2][0]))      # by now a third of the charge leaves per step
     sim.set_engine(vfps.ENGINE_CLUSTER)
     d = sim.step_host(2)
     dr = o.step(2)
     assert_psi(sim.get_psi_host()[0], o.psi, 8e-5, "stream -> cluster")
-    assert_diag(d[1, 0], dr[1], tol_p=10.0)
+    assert_diag(d[1, 0], dr[1], tol_p=edge_flux_tol(dr[1][0]))
     sim.close()
 
 
