@@ -61,6 +61,7 @@ def parse_args():
     ap.add_argument("--manhattan", action="store_true", help="Manhattan (symplectic) rotation instead of the standard one")
     ap.add_argument("--clamp", action="store_true", help="clamped interpolation (Eq. 14)")
     ap.add_argument("--cluster-kernel", type=int, default=0, help="cluster engine kernel: 0 auto, 1 first design (k_cluster_step), 3 in-place design (k_onchip_step)")
+    ap.add_argument("--grid-kernel", type=int, default=0, help="grid engine kernel: 0 auto, 1 k_grid_step, 2 k_grid2_step (TMA-staged)")
     ap.add_argument("--members", type=int, default=0, help="batch members (0 = the workload's own count)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -235,6 +236,8 @@ def run_ours(args, wl, rank, local_rank, world):
         sim.set_cluster_kernel(args.cluster_kernel)
     if args.cluster_size:
         sim.set_cluster_size(args.cluster_size)
+    if args.grid_kernel:
+        sim.set_grid_kernel(args.grid_kernel)
     sim.set_engine(ENGINES[args.engine])
     sim.set_wake_mode(WAKES[args.wake])
     sim.set_psi_host(psi0)

@@ -84,6 +84,10 @@ enum {
                               on, vfps_step may synchronise the stream to read finished events)  */
     VFPS_OPT_CLUSTER_SIZE = 4, /* CTAs per cluster of the CLUSTER engine: 0 = auto, 1, 2, 4, 8, 16;
                               vfps_get_option returns the size in use (0 = engine unavailable)  */
+    VFPS_OPT_GRID_KERNEL = 6,    /* kernel of the GRID engine: 0 = auto, 1 = k_grid_step (taps gathered
+                              through L1; also the Manhattan rotation), 2 = k_grid2_step (tiles staged
+                              by TMA, row stripes kicked from shared memory; N a multiple of 256);
+                              get returns the one in use (0 = engine unavailable)                */
     VFPS_OPT_CLUSTER_KERNEL = 5  /* kernel of the CLUSTER engine: 0 = auto, 1 = first design
                               (k_cluster_step: two buffers, weights per cell; also the Manhattan
                               rotation), 3 = in-place design (k_onchip_step: one buffer, per-launch
@@ -97,7 +101,8 @@ enum {
     VFPS_KERNEL_WAKE_DIRECT = 3, /* k_wake_direct: a3 by direct convolution (Eq. 4) on N/8 CTAs   */
     VFPS_KERNEL_KICK_FP2 = 4, /* k_kick_fp2: a4 + a5 + a6 (four cells per thread)                */
     VFPS_KERNEL_GRID = 5,     /* a1..a6 for all n steps of one vfps_step call (grid engine)      */
-    VFPS_NUM_KERNELS = 6
+    VFPS_KERNEL_GRID2 = 6,    /* the same, TMA-staged kernel of the grid engine                  */
+    VFPS_NUM_KERNELS = 7
 };
 enum {
     VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRID (one simulation) or

@@ -8,7 +8,7 @@ from .build import build, build_peaks, lib_path
 from .binding import (
     ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER, ENGINE_GRID,
     WAKE_AUTO, WAKE_FFT, WAKE_DIRECT, OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE,
-    OPT_CLUSTER_KERNEL,
+    OPT_CLUSTER_KERNEL, OPT_GRID_KERNEL,
     FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN,
     VfpsError, VfpsParams, Simulation, load, version, EXPORTS,
 )
@@ -17,7 +17,7 @@ __all__ = [
     "build", "build_peaks", "lib_path", "load", "version", "EXPORTS",
     "ENGINE_AUTO", "ENGINE_STREAM", "ENGINE_GRAPH", "ENGINE_CLUSTER", "ENGINE_GRID",
     "WAKE_AUTO", "WAKE_FFT", "WAKE_DIRECT", "OPT_ENGINE", "OPT_WAKE", "OPT_TIMING", "OPT_CLUSTER_SIZE",
-    "OPT_CLUSTER_KERNEL",
+    "OPT_CLUSTER_KERNEL", "OPT_GRID_KERNEL",
     "FLAG_RENORMALISE", "FLAG_CLAMP", "FLAG_ROT_MANHATTAN",
     "VfpsError", "VfpsParams", "Simulation",
 ]

@@ -15,8 +15,8 @@ from .build import build, lib_path
 
 ENGINE_AUTO, ENGINE_STREAM, ENGINE_GRAPH, ENGINE_CLUSTER, ENGINE_GRID = 0, 1, 2, 3, 4
 WAKE_AUTO, WAKE_FFT, WAKE_DIRECT = 0, 1, 2
-OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL = 1, 2, 3, 4, 5
-NUM_KERNELS = 6
+OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE, OPT_CLUSTER_KERNEL, OPT_GRID_KERNEL = 1, 2, 3, 4, 5, 6
+NUM_KERNELS = 7
 FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN = 1, 2, 4
 
 # every symbol include/vfps.h declares (tests check the library exports each of them)
@@ -190,6 +190,13 @@ class Simulation:
     @property
     def cluster_kernel(self) -> int:
         return self.get_option(OPT_CLUSTER_KERNEL)
+
+    def set_grid_kernel(self, version: int) -> None:
+        self.set_option(OPT_GRID_KERNEL, version)
+
+    @property
+    def grid_kernel(self) -> int:
+        return self.get_option(OPT_GRID_KERNEL)
 
     @property
     def engine_name(self) -> str:

@@ -6,6 +6,7 @@
 #include "vfps_onchip.cuh"
 #include "vfps_stream2.cuh"
 #include "vfps_grid.cuh"
+#include "vfps_grid2.cuh"
 #include "vfps_launch.h"
 
 #include <cmath>
@@ -78,6 +79,15 @@ struct vfps_sim {
     unsigned long long *gr_qacc = nullptr;       // [2] fixed-point charge accumulators
     float *gr_zrow = nullptr;                    // [N] zeros
     std::string gr_why;
+    // TMA-staged grid engine (vfps_grid2.cuh, grid kernel 2); g2_blocks = 0: not available
+    int gr_ver_opt = 0;                          // 0 auto (2 where available), 1 k_grid_step, 2 k_grid2_step
+    int g2_blocks = 0, g2_KRmax = 0, g2_rows_lo = 0, g2_rows_extra = 0;
+    size_t g2_smem = 0;
+    float *g2_coltab = nullptr, *g2_rowtab = nullptr, *g2_rho = nullptr, *g2_mom = nullptr;
+    int *g2_colix = nullptr;
+    unsigned long long *g2_qacc = nullptr;
+    CUtensorMap g2_tmap;
+    std::string g2_why;
     unsigned *tilectr = nullptr;                 // [members][tiles_x2], zero between launches
     size_t fft_smem = 0;
     int fft_threads = 0;
@@ -629,6 +639,155 @@ void grid_configure(vfps_sim *h)
     h->gr_why = "grid kernel occupancy query did not converge";
 }
 
+// ---------------------------------------------------------------- TMA-staged grid engine: host side
+const void *grid2_kernel(const vfps_sim *h)
+{
+    const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0;
+    switch (h->P.interp_order) {
+        case 2: return grid2_kernel_o2(false);      // linear interpolation: the clamp is the identity
+        case 3: return grid2_kernel_o3(clamp);
+        default: return grid2_kernel_o4(clamp);
+    }
+}
+
+// Weight tables of k_grid2_step for `nb` row stripes (as onchip_tables, one stripe per CTA) and the
+// tensor map of psi with a box of 144 columns x (KRmax + 2H) rows.  Leaves g2_blocks = 0 with the
+// reason in g2_why when the engine does not apply.
+int grid2_configure(vfps_sim *h)
+{
+    h->g2_blocks = 0; h->g2_why.clear();
+    const int N = h->N, H = h->G.H, order = h->P.interp_order;
+    if (h->members != 1) { h->g2_why = "one simulation per handle"; return VFPS_OK; }
+    if (h->P.flags & VFPS_FLAG_ROT_MANHATTAN) { h->g2_why = "standard rotation only"; return VFPS_OK; }
+    if (N % 256 != 0) { h->g2_why = "N must be a multiple of 256"; return VFPS_OK; }
+    if (H > G2_MAX_H) { h->g2_why = "rotation halo exceeds 4 rows"; return VFPS_OK; }
+    int dev = 0, coop = 0, sms = 0, smem_max = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (!coop) { h->g2_why = "device does not support cooperative launches"; return VFPS_OK; }
+    const int nb = sms < N ? sms : N;
+    const int rows_lo = N / nb, rows_extra = N % nb, KRmax = rows_lo + (rows_extra ? 1 : 0);
+    const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0 && order > 2;
+    const Grid2Layout L = grid2_layout(N, KRmax, H, order, clamp);
+    const size_t bytes = L.total_floats * sizeof(float);
+    if (bytes + 256 > (size_t)smem_max) { h->g2_why = "tiles and row buffer do not fit shared memory"; return VFPS_OK; }
+    if (L.box_rows > 256) { h->g2_why = "TMA box too tall"; return VFPS_OK; }
+    const RotGeomD g = rot_geom_d(h->P);
+    {   // first-order weight tables must be exact to fp32 rounding over a stripe and over the columns
+        const double ex = std::fabs(g.a) * 0.5 * (double)KRmax, ey = std::fabs(g.a) * 0.5 * (double)N;
+        const double e = ex > ey ? ex : ey;
+        if (e * e > 1.2e-7) { h->g2_why = "rotation angle too large for first-order weight tables"; return VFPS_OK; }
+    }
+    const void *kern = grid2_kernel(h);
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) {
+        cudaGetLastError(); h->g2_why = "shared-memory opt-in refused"; return VFPS_OK;
+    }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, G2_THREADS, bytes) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError(); h->g2_why = "kernel does not fit an SM"; return VFPS_OK;
+    }
+    // ---- tensor map of psi: dim 0 = p (contiguous), dim 1 = q; out-of-range parts of a box read as zero (A8)
+    typedef CUresult (*EncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError(); h->g2_why = "cuTensorMapEncodeTiled not available"; return VFPS_OK;
+    }
+    const cuuint64_t gdim[2] = {(cuuint64_t)N, (cuuint64_t)N};
+    const cuuint64_t gstr[1] = {(cuuint64_t)N * sizeof(float)};
+    const cuuint32_t box[2] = {(cuuint32_t)G2_SUBW, (cuuint32_t)L.box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    if (((EncodeTiled)fn)(&h->g2_tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)h->psi, gdim, gstr, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+        h->g2_why = "cuTensorMapEncodeTiled failed"; return VFPS_OK;
+    }
+    // ---- tables, in double, rounded once
+    std::vector<float> col((size_t)nb * N * OC_COLTAB, 0.0f), row((size_t)N * OC_ROWTAB, 0.0f);
+    std::vector<int> cix((size_t)nb * N, OC_BAD);
+    const double Ymid = 0.5 * (double)(N - 1) + g.y0c;
+    for (int c = 0; c < nb; ++c) {
+        const int nr = rows_lo + (c < rows_extra ? 1 : 0), r0 = c * rows_lo + (c < rows_extra ? c : rows_extra);
+        const double Xlo = (double)r0 + g.x0c, Xhi = (double)(r0 + nr - 1) + g.x0c, Xc = 0.5 * (Xlo + Xhi);
+        for (int y = 0; y < N; ++y) {
+            const double Y = (double)y + g.y0c;
+            const double f0 = std::floor(g.a * Xlo + g.b * Y), f1 = std::floor(g.a * Xhi + g.b * Y);
+            if (f0 != f1) continue;
+            cix[(size_t)c * N + y] = (int)f0;
+            double l[4] = {0, 0, 0, 0}, lp[4] = {0, 0, 0, 0};
+            lagrange_d(order, g.a * Xc + g.b * Y - f0, l, lp);
+            float *t = &col[((size_t)c * N + y) * OC_COLTAB];
+            for (int i = 0; i < 4; ++i) { t[i] = (float)l[i]; t[4 + i] = (float)lp[i]; }
+        }
+        for (int x = r0; x < r0 + nr; ++x) {
+            const double X = (double)x + g.x0c;
+            const double f0 = std::floor(g.d * X + g.a * g.y0c), f1 = std::floor(g.d * X + g.a * ((double)(N - 1) + g.y0c));
+            float *t = &row[(size_t)x * OC_ROWTAB];
+            int iy = OC_BAD;
+            if (f0 == f1) {
+                iy = (int)f0;
+                double l[4] = {0, 0, 0, 0}, lp[4] = {0, 0, 0, 0};
+                lagrange_d(order, g.d * X + g.a * Ymid - f0, l, lp);
+                const int olp = (order == 2) ? 2 : 4, oex = (order == 4) ? 8 : (order == 3) ? 3 : 4;
+                for (int j = 0; j < order; ++j) { t[j] = (float)l[j]; t[olp + (order == 4 ? (j + 3) % 4 : j)] = (float)lp[j]; }
+                t[oex] = (float)(g.a * (X - Xc));
+            }
+            std::memcpy(&t[10], &iy, sizeof(int));
+        }
+    }
+    if (!h->g2_coltab) {
+        CU(dalloc(h, &h->g2_coltab, col.size()));
+        CU(dalloc(h, &h->g2_colix, cix.size()));
+        CU(dalloc(h, &h->g2_rowtab, row.size()));
+        CU(dalloc(h, &h->g2_rho, (size_t)N));
+        CU(dalloc(h, &h->g2_mom, (size_t)nb * G2_NPART));
+        CU(dalloc(h, &h->g2_qacc, (size_t)2));
+    }
+    CU(cudaMemcpyAsync(h->g2_coltab, col.data(), col.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->g2_colix, cix.data(), cix.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->g2_rowtab, row.data(), row.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    h->g2_blocks = nb; h->g2_KRmax = KRmax; h->g2_rows_lo = rows_lo; h->g2_rows_extra = rows_extra; h->g2_smem = bytes;
+    return VFPS_OK;
+}
+
+int launch_grid2_steps(vfps_sim *h, int n, float *diag)
+{
+    Grid2Args A{};
+    A.psi = h->psi; A.psi_tmp = h->psi_tmp; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr;
+    A.rho = h->g2_rho; A.mom_part = h->g2_mom; A.diag = diag; A.nsteps = n;
+    A.coltab = h->g2_coltab; A.colix = h->g2_colix; A.rowtab = h->g2_rowtab; A.qacc = h->g2_qacc;
+    A.rows_lo = h->g2_rows_lo; A.rows_extra = h->g2_rows_extra; A.KRmax = h->g2_KRmax;
+    if (cudaMemsetAsync(h->g2_qacc, 0, 2 * sizeof(unsigned long long), h->stream) != cudaSuccess)
+        return fail(h, VFPS_ERR_CUDA, "cudaMemsetAsync failed");
+    const void *kern = grid2_kernel(h);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->g2_smem);
+    if (e == cudaSuccess) {
+        PhaseDump pd(h, (size_t)h->g2_blocks);
+        A.dbg = pd.dbg;
+        void *args[3] = {(void *)&h->G, (void *)&A, (void *)&h->g2_tmap};
+        Bracket br(h, VFPS_KERNEL_GRID2, h->timing);
+        e = cudaLaunchCooperativeKernel(kern, dim3((unsigned)h->g2_blocks), dim3(G2_THREADS), args, h->g2_smem, h->stream);
+    }
+    if (e != cudaSuccess) return fail(h, VFPS_ERR_CUDA, std::string("cooperative launch (grid2): ") + cudaGetErrorString(e));
+    h->launches += 1;
+    return VFPS_OK;
+}
+
+// which kernel the GRID engine runs: the request, else the TMA-staged one where it applies
+int grid_kernel_in_use(const vfps_sim *h)
+{
+    if (h->gr_ver_opt == 1) return h->gr_blocks > 0 ? 1 : 0;
+    if (h->gr_ver_opt == 2) return h->g2_blocks > 0 ? 2 : 0;
+    if (h->g2_blocks > 0) return 2;
+    return h->gr_blocks > 0 ? 1 : 0;
+}
+
 int launch_grid_steps(vfps_sim *h, int n, float *diag)
 {
     GridArgs A{};
@@ -744,7 +903,7 @@ int resolved_engine(const vfps_sim *h)
     if (h->engine_opt == VFPS_ENGINE_CLUSTER) return VFPS_ENGINE_CLUSTER;
     // AUTO: on-chip grids -> cluster; one large simulation -> cooperative grid; else graph replay
     if (h->cl_S > 0) return VFPS_ENGINE_CLUSTER;
-    return h->gr_blocks > 0 ? VFPS_ENGINE_GRID : VFPS_ENGINE_GRAPH;
+    return (h->gr_blocks > 0 || h->g2_blocks > 0) ? VFPS_ENGINE_GRID : VFPS_ENGINE_GRAPH;
 }
 
 // the captured graph depends on the kernel generation and the wake mode
@@ -884,6 +1043,10 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     }
     cluster_configure(h);
     grid_configure(h);
+    {
+        const int rc2 = grid2_configure(h);
+        if (rc2 != VFPS_OK) return bail(rc2, h->err);
+    }
     if (h->gr_blocks > 0) CUB(dalloc(h, &h->gr_mom, (size_t)h->gr_blocks * GR_NPART));
     if (h->gr_blocks > 0) CUB(dalloc(h, &h->gr_qacc, (size_t)2));
     if (h->gr_blocks > 0) {
@@ -960,7 +1123,8 @@ int vfps_set_option(vfps_handle h, int option, int value)
             return VFPS_OK;
         }
         if (value == VFPS_ENGINE_GRID) {
-            if (h->gr_blocks == 0) return fail(h, VFPS_ERR_UNSUPPORTED, "grid engine unavailable: " + h->gr_why);
+            if (grid_kernel_in_use(h) == 0)
+                return fail(h, VFPS_ERR_UNSUPPORTED, "grid engine unavailable: " + (h->gr_blocks == 0 ? h->gr_why : h->g2_why));
             h->engine_opt = value;
             return VFPS_OK;
         }
@@ -994,6 +1158,14 @@ int vfps_set_option(vfps_handle h, int option, int value)
         }
         return VFPS_OK;
     }
+    if (option == VFPS_OPT_GRID_KERNEL) {
+        if (!(value == 0 || value == 1 || value == 2))
+            return fail(h, VFPS_ERR_ARG, "grid kernel must be 0 (auto), 1 (k_grid_step) or 2 (k_grid2_step)");
+        if (value == 1 && h->gr_blocks == 0) return fail(h, VFPS_ERR_UNSUPPORTED, "k_grid_step unavailable: " + h->gr_why);
+        if (value == 2 && h->g2_blocks == 0) return fail(h, VFPS_ERR_UNSUPPORTED, "k_grid2_step unavailable: " + h->g2_why);
+        h->gr_ver_opt = value;
+        return VFPS_OK;
+    }
     if (option == VFPS_OPT_TIMING) {
         if (value != 0 && value != 1) return fail(h, VFPS_ERR_ARG, "timing must be 0 or 1");
         if (!value) resolve_timing(h);
@@ -1021,6 +1193,7 @@ int vfps_get_option(vfps_handle h, int option, int *value)
     if (option == VFPS_OPT_TIMING) { *value = h->timing ? 1 : 0; return VFPS_OK; }
     if (option == VFPS_OPT_CLUSTER_SIZE) { *value = h->cl_S; return VFPS_OK; }
     if (option == VFPS_OPT_CLUSTER_KERNEL) { *value = h->cl_ver; return VFPS_OK; }
+    if (option == VFPS_OPT_GRID_KERNEL) { *value = grid_kernel_in_use(h); return VFPS_OK; }
     return fail(h, VFPS_ERR_ARG, "unknown option");
 }
 
@@ -1085,7 +1258,7 @@ int vfps_step(vfps_handle h, int n, float *diag)
     if (n == 0) return VFPS_OK;
     if (resolved_engine(h) == VFPS_ENGINE_GRID) {
         if (h->timing) resolve_timing(h);
-        int rc = launch_grid_steps(h, n, diag);
+        int rc = (grid_kernel_in_use(h) == 2) ? launch_grid2_steps(h, n, diag) : launch_grid_steps(h, n, diag);
         if (rc != VFPS_OK) return rc;
         h->steps += n;
         return VFPS_OK;
@@ -1275,6 +1448,7 @@ const char *vfps_kernel_name(int kernel)
         case VFPS_KERNEL_WAKE_DIRECT: return "k_wake_direct";
         case VFPS_KERNEL_KICK_FP2: return "k_kick_fp2";
         case VFPS_KERNEL_GRID: return "k_grid_step";
+        case VFPS_KERNEL_GRID2: return "k_grid2_step";
         default: return nullptr;
     }
 }

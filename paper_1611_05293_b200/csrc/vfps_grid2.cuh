@@ -1,0 +1,523 @@
+// vfps_grid2.cuh -- persistent cooperative engine for one large grid (2048^2), TMA-staged (sm_100a).
+//
+// The first grid engine (vfps_grid.cuh) gathers every rotation tap through L1 with per-thread
+// address arithmetic and three edge paths, and kicks straight from global memory: 147
+// thread-instructions per cell, 29 us per step at 2048^2.  This engine gives the large grid what the
+// in-place cluster kernel (vfps_onchip.cuh) gives the on-chip ones:
+//  * One CTA of 512 threads per SM owns a stripe of N / gridDim rows for the whole launch.
+//  * Rotation a1 + a2: the source region of a tile -- the stripe's rows plus H halo rows, 128
+//    columns plus 8 each side -- comes in through TMA (cp.async.bulk.tensor.2d, completion on an
+//    mbarrier).  psi is zero outside the grid (reading A8), and so is TMA's fill for the part of a
+//    box that lies outside the tensor: no edge path exists.  A group of four warps rotates a tile
+//    of 256 columns (two such boxes) with the cluster kernel's walker: two columns per thread,
+//    ORDER x 6 register window, per-launch weight tables (built in double on the host for the
+//    centre row of every stripe), next row's loads issued mid-row.  Two buffers per group: the
+//    tile after next is in flight while a tile is rotated.  Results go to psi_tmp (64-bit stores),
+//    row sums (transposed warp reduction) to the profile.
+//  -- grid barrier --
+//  * Wake a3 for the stripe's rows (one warp per row, direct convolution, Eq. 4), while the
+//    stripe's rows of psi_tmp stream into shared memory (cp.async, the space of the tile buffers).
+//  * Kick a4 + Fokker-Planck a5 + moments a6 from shared memory: a warp takes a (row, 256-column
+//    block), a lane the 4-cell granules 4 lane + 128 k -- 128-bit loads with a lane stride of 16
+//    bytes -- and writes psi with 128-bit stores.
+//  -- grid barrier -- charge (exact 32.32 fixed-point sum), 1/C, diagnostics as in vfps_grid.cuh.
+// Template CLAMP: clamped interpolation (Eq. 14, reading A9); the CSR power is then that of the
+// end-of-step profile to first order in its change (transposed wake, see k_wake_direct).
+// Standard rotation only; one simulation per handle; N a multiple of 256.
+#pragma once
+#include "vfps_onchip.cuh"
+
+#include <cooperative_groups.h>
+#include <cuda.h>
+
+namespace vfps {
+
+constexpr int G2_THREADS = 512;
+constexpr int G2_WARPS = G2_THREADS / 32;
+constexpr int G2_GROUPS = 4;          // warp groups of four, one tile each at a time
+constexpr int G2_SUBW = 144;          // floats per row of a box: 128 columns + 8 each side
+constexpr int G2_PADC = 8;
+constexpr int G2_NPART = 8;
+constexpr int G2_MAX_H = 4;
+
+struct Grid2Args {
+    float *psi;            // [N][N] in/out, un-normalised (the tensor map of the kernel points at it)
+    float *psi_tmp;        // [N][N] rotated density
+    float *scale;          // [1] in/out: 1/C of the last step
+    const float *wfun;     // [2N] wake function, lag d at index d + N - 1; nullptr = no wake
+    float *rho;            // [N] profile of the step (dp * row sums, un-scaled)
+    float *mom_part;       // [G2_NPART][gridDim.x]
+    float *diag;           // [nsteps][1][6] or nullptr
+    const float *coltab;   // [gridDim.x][N][8]: M[4], M'[4] of column y for the rows of stripe c
+    const int *colix;      // [gridDim.x][N]: floor(dx) of column y over the rows of stripe c, or OC_BAD
+    const float *rowtab;   // [N][12]: as in the cluster kernel (a (X - Xc) relative to the stripe's centre row)
+    unsigned long long *qacc;   // [2] charge of the step in 32.32 fixed point, zero at launch
+    int nsteps;
+    int rows_lo, rows_extra;    // stripe c has rows_lo + (c < rows_extra) rows
+    int KRmax;                  // rows of the largest stripe
+    long long *dbg;
+};
+
+struct Grid2Layout {
+    int box_rows, pitch, nct, nch;
+    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_chunk, off_rho, off_sw, off_sw2, off_red, off_big,
+        total_floats;
+};
+
+__host__ __device__ inline Grid2Layout grid2_layout(int N, int KRmax, int H, int order, bool clamp)
+{
+    Grid2Layout L;
+    const int CH = oc_chunk_rows(order);
+    L.box_rows = (KRmax + 2 * H + 1) & ~1;          // even: a box of 144 floats x rows is then a multiple of 128 bytes (TMA)
+    L.pitch = N + 2 * G2_PADC;
+    L.nct = N / 256;
+    L.nch = (KRmax + CH - 1) / CH;
+    L.tile_floats = (size_t)2 * L.box_rows * G2_SUBW;          // two boxes of 128 columns
+    size_t o = 0;
+    L.off_mbar = o;     o += 32;                                // 2 x G2_GROUPS mbarriers
+    L.off_rowtab = o;   o += (size_t)(KRmax + 2) * OC_ROWTAB;
+    L.off_rowpart = o;  o += (size_t)KRmax * (N / 64);
+    L.off_vtab = o;     o += (size_t)((KRmax * 8 + 3) & ~3);
+    L.off_chunk = o;    o += (size_t)((L.nch + 3) & ~3);
+    L.off_rho = o;      o += (size_t)N;
+    L.off_sw = o;       o += (size_t)((N + KRmax + 3) & ~3);
+    L.off_sw2 = o;      o += clamp ? (size_t)((N + KRmax + 3) & ~3) : 0;
+    L.off_red = o;      o += (size_t)G2_WARPS * 8 + 8;
+    o = (o + 31) & ~(size_t)31;                                 // TMA destinations: 128-byte aligned
+    L.off_big = o;
+    const size_t tiles = (size_t)2 * G2_GROUPS * L.tile_floats + G2_SUBW;   // + one row: the walker prefetches past the end
+    const size_t rows = (size_t)KRmax * L.pitch;
+    o += tiles > rows ? tiles : rows;
+    L.total_floats = o;
+    return L;
+}
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t mbar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                 ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(mbar), "r"(c0), "r"(c1)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+
+// one cell of a tile with its own floors (a floor changes inside the warp's columns or the chunk)
+template <int ORDER, bool CLAMP>
+__device__ __forceinline__ float rotate_cell_tile(const GridConst &G, uint32_t base00 /* tile address of source (row x, column y) */,
+                                                  int x, int y)
+{
+    constexpr int O0 = (ORDER - 1) / 2;
+    constexpr int P = G2_SUBW;
+    const float X = (float)x + G.x0c, Y = (float)y + G.y0c;
+    int ix, iy;
+    float tx, ty;
+    floor_frac(fmaf(G.a, X, G.b * Y), ix, tx);
+    floor_frac(fmaf(G.d, X, G.a * Y), iy, ty);
+    float lx[ORDER], ly[ORDER];
+    lagrange<ORDER>(tx, lx);
+    lagrange<ORDER>(ty, ly);
+    const uint32_t base = base00 + (uint32_t)(((ix - O0) * P + (iy - O0)) * 4);
+    float acc = 0.0f;
+#pragma unroll
+    for (int i = 0; i < ORDER; ++i) {
+        float r = ly[0] * lds(base + (i * P) * 4);
+#pragma unroll
+        for (int j = 1; j < ORDER; ++j) r = fmaf(ly[j], lds(base + (i * P + j) * 4), r);
+        acc = (i == 0) ? lx[0] * r : fmaf(lx[i], r, acc);
+    }
+    if (CLAMP) {
+        const float a = lds(base + (O0 * P + O0) * 4), b = lds(base + (O0 * P + O0 + 1) * 4);
+        const float c = lds(base + ((O0 + 1) * P + O0) * 4), d = lds(base + ((O0 + 1) * P + O0 + 1) * 4);
+        acc = fminf(fmaxf(acc, fminf(fminf(a, b), fminf(c, d))), fmaxf(fmaxf(a, b), fmaxf(c, d)));
+    }
+    return acc;
+}
+
+template <int ORDER, bool CLAMP>
+__global__ void __launch_bounds__(G2_THREADS, 1)
+k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
+{
+    namespace cg = cooperative_groups;
+    constexpr int O0 = (ORDER - 1) / 2;
+    constexpr int CH = oc_chunk_rows(ORDER);
+    constexpr int P4 = G2_SUBW * 4;
+    constexpr unsigned FULL = 0xffffffffu;
+    using Wk = Walker<ORDER, G2_SUBW, true, CLAMP>;
+    cg::grid_group grid = cg::this_grid();
+
+    const int N = G.N, H = G.H, KRmax = A.KRmax;
+    const Grid2Layout LY = grid2_layout(N, KRmax, H, ORDER, CLAMP);
+    const int nct = LY.nct, CWR = N / 64;                  // column tiles; row-sum partials per row
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int grp = warp >> 2, cw = warp & 3;
+    const int c = (int)blockIdx.x;
+    const int rows = A.rows_lo + (c < A.rows_extra ? 1 : 0);
+    const int r0 = c * A.rows_lo + min(c, A.rows_extra);
+    const int nch = (rows + CH - 1) / CH;
+
+    extern __shared__ __align__(128) float g2smem[];
+    float *smem = g2smem;
+    float *rowtab_s = smem + LY.off_rowtab + OC_ROWTAB;
+    float *rowpart = smem + LY.off_rowpart;
+    float *vtab = smem + LY.off_vtab;
+    int *chunkinfo = reinterpret_cast<int *>(smem + LY.off_chunk);
+    float *srho = smem + LY.off_rho, *sw = smem + LY.off_sw, *sw2 = smem + LY.off_sw2;
+    float *red = smem + LY.off_red;
+    float *big = smem + LY.off_big;
+    const uint32_t sBig = smem_u32(big), sRowtab = smem_u32(rowtab_s), sRowpart = smem_u32(rowpart), sVtab = smem_u32(vtab);
+    const uint32_t sMbar = smem_u32(smem + LY.off_mbar);
+    const uint32_t tile_bytes = (uint32_t)LY.tile_floats * 4u, box_bytes = tile_bytes / 2u;
+    const int PITCH = LY.pitch;
+
+    // ---- one-time set-up
+    for (int i = tid; i < (KRmax + 2) * OC_ROWTAB; i += G2_THREADS) {
+        const int gi = (r0 - 1) * OC_ROWTAB + i;
+        rowtab_s[i - OC_ROWTAB] = (gi >= 0 && gi < N * OC_ROWTAB) ? A.rowtab[gi] : 0.0f;
+    }
+    __syncthreads();
+    for (int i = tid; i < LY.nch; i += G2_THREADS) {
+        // floor(dy) of the chunk's rows if they agree (and are good), else OC_BAD
+        int iy = OC_BAD;
+        if (i * CH < rows) {
+            iy = __float_as_int(rowtab_s[(i * CH) * OC_ROWTAB + 10]);
+            for (int k = 1; k < CH && i * CH + k < rows; ++k)
+                if (__float_as_int(rowtab_s[(i * CH + k) * OC_ROWTAB + 10]) != iy) iy = OC_BAD;
+        }
+        chunkinfo[i] = iy;
+    }
+    if (tid == 0) {
+        for (int i = 0; i < 2 * G2_GROUPS; ++i) mbar_init(sMbar + 8u * (uint32_t)i, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const float yc = 0.5f * (float)(N - 1);
+    const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
+    float sc = G.renorm ? A.scale[0] : 1.0f;
+    unsigned use0 = 0u, use1 = 0u;             // how often this group has waited on its buffer 0 / 1
+    const uint32_t mb0 = sMbar + 16u * (uint32_t)grp, mb1 = mb0 + 8u;
+    const uint32_t buf0 = sBig + (uint32_t)(2 * grp) * tile_bytes, buf1 = buf0 + tile_bytes;
+    const bool rs_writer = ((lane & 7) == 0) && ((lane >> 3) < CH);
+    const bool issuer = (cw == 0 && lane == 0);
+    __shared__ float s_tot[6];
+    __shared__ float s_sc;
+
+    for (int step = 0; step < A.nsteps; ++step) {
+        VFPS_STAMP(A.dbg, step, 0);
+        // ================= phase 1: rotation psi -> psi_tmp, row sums.  Group grp: column tiles grp, grp + 4, ...
+        if (rows > 0) {
+            if (issuer) {
+                // psi was written with ordinary stores (by every CTA, before the grid barrier); TMA reads it
+                // through the async proxy
+                asm volatile("fence.proxy.async;" ::: "memory");
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    const int ct = grp + G2_GROUPS * b;
+                    if (ct < nct) {
+                        const uint32_t mb = b ? mb1 : mb0, dst = b ? buf1 : buf0;
+                        mbar_expect_tx(mb, tile_bytes);
+                        tma_load_2d(dst, &tmap, 256 * ct - G2_PADC, r0 - H, mb);
+                        tma_load_2d(dst + box_bytes, &tmap, 256 * ct + 128 - G2_PADC, r0 - H, mb);
+                    }
+                }
+            }
+            int it = 0;
+            for (int ct = grp; ct < nct; ct += G2_GROUPS, ++it) {
+                const int b = it & 1;
+                const uint32_t mb = b ? mb1 : mb0, tile = b ? buf1 : buf0;
+                // this tile's columns: y0, y0 + 1; weights along q from the stripe's table
+                const int y0 = 256 * ct + 64 * cw + 2 * lane;
+                Wk wkr;
+                int ixc;
+                bool cols_ok;
+                {
+                    const int i0 = A.colix[(size_t)c * N + y0], i1 = A.colix[(size_t)c * N + y0 + 1];
+                    ixc = i0;
+                    cols_ok = __all_sync(FULL, i0 != OC_BAD && i0 == i1);
+                    const float4 *ct0 = reinterpret_cast<const float4 *>(A.coltab + ((size_t)c * N + y0) * OC_COLTAB);
+                    const float4 m0 = __ldg(ct0), m0p = __ldg(ct0 + 1), m1 = __ldg(ct0 + 2), m1p = __ldg(ct0 + 3);
+                    const float a0[4] = {m0.x, m0.y, m0.z, m0.w}, a0p[4] = {m0p.x, m0p.y, m0p.z, m0p.w};
+                    const float a1[4] = {m1.x, m1.y, m1.z, m1.w}, a1p[4] = {m1p.x, m1p.y, m1p.z, m1p.w};
+#pragma unroll
+                    for (int i = 0; i < ORDER; ++i) { wkr.M0[i] = a0[i]; wkr.M0p[i] = a0p[i]; wkr.M1[i] = a1[i]; wkr.M1p[i] = a1p[i]; }
+                    wkr.ey0 = G.a * ((float)y0 - yc);
+                    wkr.ey1 = G.a * ((float)(y0 + 1) - yc);
+                    wkr.a = G.a;
+                    if (!cols_ok) ixc = 0;
+                }
+                mbar_wait(mb, (b ? use1 : use0) & 1u);
+                if (b) ++use1; else ++use0;
+                // box of this warp: columns 128 (cw >> 1) ..; local column of y0 inside it
+                const uint32_t box = tile + (uint32_t)(cw >> 1) * box_bytes;
+                const int yl = G2_PADC + 64 * (cw & 1) + 2 * lane;
+                float *gout = A.psi_tmp + (size_t)r0 * N + y0;
+                int ci = 0;
+                while (ci < nch) {
+                    const int iy = chunkinfo[ci];
+                    int nrun = 1;
+                    if (cols_ok && iy != OC_BAD) {
+                        while (ci + nrun < nch && chunkinfo[ci + nrun] == iy) ++nrun;
+                        const int par = (iy - O0) & 1;
+                        const int v0 = ci * CH;
+                        // tile row of source row x is x - (r0 - H); tap row 0 of target v: v + ixc - O0
+                        uint32_t src = box + (uint32_t)((v0 + H + ixc - O0) * P4 + (yl + iy - O0 - par) * 4);
+                        OutGlobal dst{gout + (size_t)v0 * N, N};
+                        uint32_t tab = sRowtab + (uint32_t)(v0 * OC_ROWTAB * 4);
+                        uint32_t rp = sRowpart + (uint32_t)(((v0 + (lane >> 3)) * CWR + 4 * ct + cw) * 4);
+#define G2_RUN(PAR_)                                                                                   \
+    do {                                                                                                \
+        wkr.template start<PAR_>(src, tab);                                                             \
+        for (int q = 0; q < nrun; ++q) {                                                                \
+            const int left = rows - (ci + q) * CH;                                                      \
+            if (left >= CH) wkr.template chunk<PAR_, 1>(src, dst, tab);                                 \
+            else wkr.template chunk_n<PAR_, 1>(src, dst, tab, left);                                    \
+            if (CH < 4) wkr.rs[3] = 0.0f;                                                               \
+            const float tot = warp_reduce_transposed<4>(wkr.rs, lane);                                  \
+            if (rs_writer && (lane >> 3) < left) sts(rp, tot);                                          \
+            src += (uint32_t)(CH * P4); dst.p += (size_t)CH * N;                                        \
+            tab += (uint32_t)(CH * OC_ROWTAB * 4); rp += (uint32_t)(CH * CWR * 4);                      \
+        }                                                                                               \
+    } while (0)
+                        if (par) G2_RUN(1); else G2_RUN(0);
+#undef G2_RUN
+                    } else {
+                        const int vlo = ci * CH, nrow = min(CH, rows - vlo);
+                        float rs4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+                        for (int s = 0; s < CH; ++s) {
+                            if (s < nrow) {
+                                const int v = vlo + s;
+                                const uint32_t b00 = box + (uint32_t)(((v + H) * G2_SUBW + yl) * 4);
+                                const float o0 = rotate_cell_tile<ORDER, CLAMP>(G, b00, r0 + v, y0);
+                                const float o1 = rotate_cell_tile<ORDER, CLAMP>(G, b00 + 4u, r0 + v, y0 + 1);
+                                *reinterpret_cast<float2 *>(gout + (size_t)v * N) = make_float2(o0, o1);
+                                rs4[s] = o0 + o1;
+                            }
+                        }
+                        const float tot = warp_reduce_transposed<4>(rs4, lane);
+                        const int s = lane >> 3;
+                        if (rs_writer && s < nrow) rowpart[(vlo + s) * CWR + 4 * ct + cw] = tot;
+                    }
+                    ci += nrun;
+                }
+                // the whole group has finished reading this buffer: refill it with the tile after next
+                named_barrier(1 + grp, 128);
+                const int ct2 = ct + 2 * G2_GROUPS;
+                if (issuer && ct2 < nct) {
+                    mbar_expect_tx(mb, tile_bytes);
+                    tma_load_2d(tile, &tmap, 256 * ct2 - G2_PADC, r0 - H, mb);
+                    tma_load_2d(tile + box_bytes, &tmap, 256 * ct2 + 128 - G2_PADC, r0 - H, mb);
+                }
+            }
+        }
+        VFPS_STAMP(A.dbg, step, 1);
+        __syncthreads();
+        if (tid < rows) {
+            float s = 0.0f;
+            for (int k = 0; k < CWR; ++k) s += rowpart[tid * CWR + k];
+            A.rho[r0 + tid] = s * G.dp;
+        }
+        __threadfence();
+        grid.sync();
+        VFPS_STAMP(A.dbg, step, 2);
+        // ================= phase 2: wake of the stripe's rows while its rotated rows stream into shared memory
+        float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 pw - -
+        if (rows > 0) {
+            const int NQ = N >> 2;
+            for (int i = tid; i < rows * NQ; i += G2_THREADS) {
+                const int r = i / NQ, q = i - r * NQ;
+                cp_async16(sBig + (uint32_t)((r * PITCH + G2_PADC + 4 * q) * 4), A.psi_tmp + (size_t)(r0 + r) * N + 4 * q);
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            for (int i = tid; i < rows * 2 * G2_PADC; i += G2_THREADS) {      // zero pads left and right of every row
+                const int r = i / (2 * G2_PADC), k = i - r * (2 * G2_PADC);
+                big[r * PITCH + (k < G2_PADC ? k : N + k)] = 0.0f;
+            }
+            for (int i = tid; i < N; i += G2_THREADS) srho[i] = __ldcg(A.rho + i);
+            if (A.wfun != nullptr) {
+                for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
+                if (CLAMP) {
+                    const int base2 = N - r0 - KRmax;          // sw2[i] = w at index base2 + i: w[x' - x] = sw2[x' + KRmax - 1 - (x - r0)]
+                    for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) {
+                        const int k = base2 + i;
+                        sw2[i] = (k >= 0 && k < 2 * N - 1) ? __ldg(A.wfun + k) : 0.0f;
+                    }
+                }
+            }
+            __syncthreads();
+            VFPS_STAMP(A.dbg, step, 3);
+            // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4), one row per warp
+            for (int r = warp; r < rows; r += G2_WARPS) {
+                float v0 = 0.0f, v1 = 0.0f, u0 = 0.0f, u1 = 0.0f;
+                if (A.wfun != nullptr) {
+                    const float *wx = sw + (r + N - 1);
+                    for (int xp = lane; xp < N; xp += 64) {
+                        v0 = fmaf(wx[-xp], srho[xp], v0);
+                        v1 = fmaf(wx[-(xp + 32)], srho[xp + 32], v1);
+                    }
+                    if (CLAMP) {
+                        const float *ux = sw2 + (KRmax - 1 - r);
+                        for (int xp = lane; xp < N; xp += 64) {
+                            u0 = fmaf(ux[xp], srho[xp], u0);
+                            u1 = fmaf(ux[xp + 32], srho[xp + 32], u1);
+                        }
+                    }
+                }
+                const float Vr = warp_sum(v0 + v1);
+                const float Vtr = CLAMP ? warp_sum(u0 + u1) : 0.0f;
+                if (lane == 0) {
+                    const float V = Vr * sc, rho_x = srho[r0 + r] * sc;
+                    int mm;
+                    float t;
+                    floor_frac(G.kick_c * V, mm, t);
+                    float l[ORDER];
+                    lagrange<ORDER>(t, l);
+                    float pl[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+                    for (int j = 0; j < ORDER; ++j) pl[j] = CLAMP ? l[j] : l[j] * sc;
+                    sts4(sVtab + (uint32_t)r * 32u, make_float4(pl[0], pl[1], pl[2], pl[3]));
+                    if (CLAMP) {
+                        const float Vt = Vtr * sc;
+                        sts4(sVtab + (uint32_t)r * 32u + 16u, make_float4(__int_as_float(mm), -rho_x * Vt, G.dp * (V + Vt), 0.0f));
+                    } else {
+                        sts2(sVtab + (uint32_t)r * 32u + 16u, __int_as_float(mm), rho_x * V);
+                    }
+                }
+            }
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();
+            VFPS_STAMP(A.dbg, step, 4);
+            // a4 + a5 + a6: unit = (row, 256-column block); lane owns the granules 4 lane and 4 lane + 128 of the block
+            const int nunits = rows * nct;
+            for (int u = warp; u < nunits; u += G2_WARPS) {
+                const int r = u / nct, blk = u - r * nct;
+                const float4 lw = lds4(sVtab + (uint32_t)r * 32u);
+                float2 mv;
+                float dpU = 0.0f;
+                if (CLAMP) {
+                    const float4 m4 = lds4(sVtab + (uint32_t)r * 32u + 16u);
+                    mv = make_float2(m4.x, m4.y); dpU = m4.z;
+                } else {
+                    mv = lds2(sVtab + (uint32_t)r * 32u + 16u);
+                }
+                const int mm = __float_as_int(mv.x);
+                const int g0 = 256 * blk + 4 * lane;
+                const uint32_t own = sBig + (uint32_t)((r * PITCH + G2_PADC + g0) * 4);
+                const float lws[4] = {lw.x, lw.y, lw.z, lw.w};
+                float l[ORDER];
+#pragma unroll
+                for (int j = 0; j < ORDER; ++j) l[j] = lws[j];
+                float o[2][4];
+                if (mm >= -2 && mm <= 0) {
+                    float b[2][12];
+#pragma unroll
+                    for (int k = 0; k < 2; ++k)
+#pragma unroll
+                        for (int i = 0; i < 3; ++i) {
+                            const float4 v = lds4(own + (uint32_t)(512 * k + 16 * i - 16));
+                            b[k][4 * i] = v.x; b[k][4 * i + 1] = v.y; b[k][4 * i + 2] = v.z; b[k][4 * i + 3] = v.w;
+                        }
+#pragma unroll
+                    for (int k = 0; k < 2; ++k) {
+                        const int g = g0 + 128 * k;
+                        float c1p[4];
+#pragma unroll
+                        for (int cc = 0; cc < 4; ++cc) c1p[cc] = c1 * fmaf((float)(g + cc), G.dp, G.p_min);
+                        if (mm == 0) kick_fp_granule<ORDER, 0, CLAMP>(b[k], l, g, N, G.fp_b, c2, c1p, o[k]);
+                        else if (mm == -1) kick_fp_granule<ORDER, -1, CLAMP>(b[k], l, g, N, G.fp_b, c2, c1p, o[k]);
+                        else kick_fp_granule<ORDER, -2, CLAMP>(b[k], l, g, N, G.fp_b, c2, c1p, o[k]);
+                    }
+                } else {
+                    const float *rowp = big + r * PITCH + G2_PADC;
+#pragma unroll
+                    for (int k = 0; k < 2; ++k) {
+                        const int g = g0 + 128 * k;
+                        float c1p[4];
+#pragma unroll
+                        for (int cc = 0; cc < 4; ++cc) c1p[cc] = c1 * fmaf((float)(g + cc), G.dp, G.p_min);
+                        kick_fp_granule_any<ORDER, CLAMP>(rowp, l, mm, g, N, G.fp_b, c2, c1p, o[k]);
+                    }
+                }
+                if (CLAMP) {
+#pragma unroll
+                    for (int k = 0; k < 2; ++k)
+#pragma unroll
+                        for (int cc = 0; cc < 4; ++cc) o[k][cc] *= sc;
+                }
+                float *orow = A.psi + (size_t)(r0 + r) * N + g0;
+                float rs = 0.0f;
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    *reinterpret_cast<float4 *>(orow + 128 * k) = make_float4(o[k][0], o[k][1], o[k][2], o[k][3]);
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc) {
+                        const float yy = (float)(g0 + 128 * k + cc) - yc, tt = o[k][cc] * yy;
+                        rs += o[k][cc]; acc[1] += tt; acc[2] = fmaf(tt, yy, acc[2]);
+                    }
+                }
+                const float xx = (float)(r0 + r) - yc, tq = rs * xx;
+                acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+                if (CLAMP) acc[5] = fmaf(rs, dpU, acc[5]);
+                if (lane == 0 && blk == 0) acc[5] += mv.y;
+            }
+        }
+        {
+            const float tot = warp_reduce_transposed<8>(acc, lane);       // lanes 4 j .. 4 j + 3 hold sum j
+            if ((lane & 3) == 0) red[warp * 8 + (lane >> 2)] = tot;
+        }
+        __syncthreads();
+        if (tid < G2_NPART) {
+            float s = 0.0f;
+#pragma unroll
+            for (int w = 0; w < G2_WARPS; ++w) s += red[w * 8 + tid];
+            A.mom_part[(size_t)tid * gridDim.x + blockIdx.x] = s;
+            // charge: one 64-bit fixed-point accumulator (integer atomics: exact, order-independent)
+            if (tid == 0) atomicAdd(A.qacc + (step & 1), (unsigned long long)__float2ll_rn(s * 4294967296.0f));
+        }
+        // psi of this step is read by the next rotation through TMA (async proxy)
+        asm volatile("fence.proxy.async;" ::: "memory");
+        __threadfence();
+        VFPS_STAMP(A.dbg, step, 5);
+        grid.sync();
+        VFPS_STAMP(A.dbg, step, 6);
+        // ================= phase 3: a6 -- every CTA forms C and 1/C from the same accumulator
+        if (tid == 0) {
+            const long long q = (long long)__ldcg(A.qacc + (step & 1));
+            const float f = (float)((double)q * (1.0 / 4294967296.0));
+            s_tot[0] = f;
+            s_sc = G.renorm ? 1.0f / ((G.dq * G.dp) * f) : 1.0f;
+            if (blockIdx.x == 0) A.qacc[(step + 1) & 1] = 0ull;      // nobody touches it before the next barrier
+        }
+        if (blockIdx.x == 0 && warp >= 1 && warp < 6) {              // the other sums, for the diagnostics row
+            const float *mp = A.mom_part + (size_t)warp * gridDim.x;
+            float f = 0.0f;
+#pragma unroll 8
+            for (int i = lane; i < (int)gridDim.x; i += 32) f += __ldcg(mp + i);
+            f = warp_sum(f);
+            if (lane == 0) s_tot[warp] = f;
+        }
+        __syncthreads();
+        if (blockIdx.x == 0 && tid == 0 && A.diag != nullptr) {
+            const float t0 = s_tot[0], i0 = 1.0f / t0;
+            const float C = (G.dq * G.dp) * t0;
+            const float mp_c = s_tot[1] * i0, vp = fmaf(-mp_c, mp_c, s_tot[2] * i0);
+            const float mq_c = s_tot[3] * i0, vq = fmaf(-mq_c, mq_c, s_tot[4] * i0);
+            const float cc = G.renorm ? C : 1.0f;
+            float *o = A.diag + (size_t)step * 6;
+            o[0] = C;
+            o[1] = fmaf(mq_c + yc, G.dq, G.q_min);
+            o[2] = fmaf(mp_c + yc, G.dp, G.p_min);
+            o[3] = sqrtf(fmaxf(vq, 0.0f)) * G.dq;
+            o[4] = sqrtf(fmaxf(vp, 0.0f)) * G.dp;
+            o[5] = s_tot[5] * G.dq / (cc * cc);
+        }
+        sc = s_sc;
+        __syncthreads();
+        VFPS_STAMP(A.dbg, step, 7);
+    }
+    if (blockIdx.x == 0 && tid == 0) A.scale[0] = sc;
+}
+
+}  // namespace vfps

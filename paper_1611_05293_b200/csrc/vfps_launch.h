@@ -23,4 +23,9 @@ const void *grid_kernel_o2(bool manh, bool clamp);
 const void *grid_kernel_o3(bool manh, bool clamp);
 const void *grid_kernel_o4(bool manh, bool clamp);
 
+// k_grid2_step<ORDER, CLAMP> (vfps_grid2.cuh); arguments (GridConst, Grid2Args, CUtensorMap)
+const void *grid2_kernel_o2(bool clamp);
+const void *grid2_kernel_o3(bool clamp);
+const void *grid2_kernel_o4(bool clamp);
+
 }  // namespace vfps

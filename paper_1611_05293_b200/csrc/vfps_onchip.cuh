@@ -383,8 +383,8 @@ struct Walker {
     // (i - SUB) mod ORDER (DIR < 0).  The tap row that leaves the window (i = 0 walking down,
     // i = ORDER - 1 walking up) is consumed first; its slot then receives the entering row of the
     // next target, and tb the next table row, while the rest of this target is computed.
-    template <int PAR, int DIR, int SUB>
-    __device__ __forceinline__ void row_step(uint32_t src, uint32_t dst, uint32_t tab)
+    template <int PAR, int DIR, int SUB, class OUT>
+    __device__ __forceinline__ void row_step(uint32_t src, const OUT &dst, uint32_t tab)
     {
         constexpr int SLOT0 = (DIR > 0) ? (SUB % ORDER) : ((ORDER - SUB % ORDER) % ORDER);
         constexpr int IL = (DIR > 0) ? 0 : ORDER - 1;
@@ -413,14 +413,38 @@ struct Walker {
 #pragma unroll
         for (int i = 1; i < ORDER; ++i) { a0 = fmaf(lx0[i], r0[i], a0); a1 = fmaf(lx1[i], r1[i], a1); }
         if (CLAMP) { a0 = fminf(fmaxf(a0, lo0), hi0); a1 = fminf(fmaxf(a1, lo1), hi1); }
-        sts2(dst + (uint32_t)(DIR * SUB * P4), a0, a1);
+        dst.template put<DIR * SUB>(a0, a1);
         rs[SUB] = a0 + a1;
     }
-    template <int PAR, int DIR, int SUB = 0>
-    __device__ __forceinline__ void chunk(uint32_t src, uint32_t dst, uint32_t tab)
+    template <int PAR, int DIR, class OUT, int SUB = 0>
+    __device__ __forceinline__ void chunk(uint32_t src, const OUT &dst, uint32_t tab)
     {
         row_step<PAR, DIR, SUB>(src, dst, tab);
-        if constexpr (SUB + 1 < CH) chunk<PAR, DIR, SUB + 1>(src, dst, tab);
+        if constexpr (SUB + 1 < CH) chunk<PAR, DIR, OUT, SUB + 1>(src, dst, tab);
+    }
+    // a ragged last chunk: only the first nrows (< CH) target rows exist (warp-uniform)
+    template <int PAR, int DIR, class OUT, int SUB = 0>
+    __device__ __forceinline__ void chunk_n(uint32_t src, const OUT &dst, uint32_t tab, int nrows)
+    {
+        if (SUB < nrows) row_step<PAR, DIR, SUB>(src, dst, tab); else rs[SUB] = 0.0f;
+        if constexpr (SUB + 1 < CH) chunk_n<PAR, DIR, OUT, SUB + 1>(src, dst, tab, nrows);
+    }
+};
+
+// where a walker puts the two rotated cells of target row R (relative to the chunk's first target)
+template <int P4>
+struct OutShared {                     // shared memory, row pitch P4 bytes
+    uint32_t a;
+    template <int R>
+    __device__ __forceinline__ void put(float x, float y) const { sts2(a + (uint32_t)(R * P4), x, y); }
+};
+struct OutGlobal {                     // global memory, row pitch n floats
+    float *p;
+    int n;
+    template <int R>
+    __device__ __forceinline__ void put(float x, float y) const
+    {
+        *reinterpret_cast<float2 *>(p + (ptrdiff_t)R * n) = make_float2(x, y);
     }
 };
 
@@ -686,7 +710,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
     do {                                                                                                      \
         wkr.template start<PAR_>(src, tab);                                                                   \
         for (int q = 0; q < nrun; ++q) {                                                                      \
-            wkr.template chunk<PAR_, DIR_>(src, dst, tab);                                                    \
+            wkr.template chunk<PAR_, DIR_>(src, OutShared<P4>{dst}, tab);                                     \
             if (CH < 4) wkr.rs[3] = 0.0f;                                                                     \
             const float tot = warp_reduce_transposed<4>(wkr.rs, lane);                                        \
             if (rs_writer) sts(rp, tot);                                                                      \

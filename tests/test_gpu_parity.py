@@ -143,6 +143,7 @@ def test_c3_batched_members(vfps, orc):
 def test_c4_one_step_and_1000_steps(vfps, orc):
     wl = get_workload("C4")
     sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 1)
+    assert sim.engine_name == "grid" and sim.grid_kernel == 2         # what AUTO picks, what bench.py times
     assert_psi(psi[0], refs[0].psi, TOL_1, "C4 1 step")
     assert_diag(d[0, 0], dr[0][0])
     sim.close()
@@ -707,6 +708,75 @@ def test_grid_engine(vfps, orc, order, N):
     assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"grid -> stream -> grid N={N}")
     assert_diag(d[1, 0], dr[3], tol_q=tol_q)
     assert sim.step_count() == 64
+    sim.close()
+
+
+@pytest.mark.parametrize("clamp", [False, True])
+@pytest.mark.parametrize("order", [2, 3, 4])
+@pytest.mark.parametrize("N,spp", [(256, 4000), (512, 4000), (1024, 8000)])
+def test_grid2_engine(vfps, orc, N, spp, order, clamp):
+    """TMA-staged kernel of the grid engine (k_grid2_step): asymmetric box (the grid edges cut through
+    tiles on all four sides: TMA's zero fill is reading A8), off-centre mismatched bunch, free-space
+    wake; stripes of 1-2 (N = 256), 3-4 (512) and 6-7 (1024) rows per CTA, so ragged chunks and
+    stripes shorter than the halo all occur.  1 step and 60 steps with every diagnostics row, then
+    hand-over to the first grid kernel and back."""
+    if clamp and order == 2:
+        pytest.skip("the clamp is the identity for linear interpolation: same kernel as without the flag")
+    Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
+    psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)
+    if clamp:
+        a, b = N // 2 - N // 8, N // 2 + N // 8
+        psi0[a:b, a:b] = 0.0
+        psi0 = (psi0 / (psi0.astype(np.float64).sum() * (12.0 / (N - 1)) ** 2)).astype(np.float32)
+    psi0 = psi0[None]
+    flags = vfps.FLAG_RENORMALISE | (vfps.FLAG_CLAMP if clamp else 0)
+    sim = vfps.Simulation(N, -5.0, 7.0, -6.5, 5.5, spp, 2e-3, order, 2, 1, Z=Z, flags=flags)
+    sim.set_grid_kernel(2)
+    sim.set_engine(vfps.ENGINE_GRID)
+    assert sim.engine_name == "grid" and sim.grid_kernel == 2 and sim.wake_name == "direct"
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, -5.0, 7.0, -6.5, 5.5, spp, 2e-3, order, 2, Z[0], clamp=clamp)
+    o.set_psi(psi0[0])
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, f"grid2 N={N} order={order} 1 step")
+    assert_diag(d[0, 0], dr[0])
+    d = sim.step_host(59)
+    dr = o.step(59)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"grid2 N={N} order={order} 60 steps")
+    for i in (0, 30, 58):
+        assert_diag(d[i, 0], dr[i])
+    sim.set_grid_kernel(1)
+    assert sim.grid_kernel == 1
+    sim.step_host(2)
+    sim.set_grid_kernel(2)
+    d = sim.step_host(2)
+    dr = o.step(4)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"grid2 -> grid -> grid2 N={N}")
+    assert_diag(d[1, 0], dr[3])
+    assert sim.step_count() == 64
+    sim.close()
+
+
+def test_grid2_engine_refusals(vfps):
+    """k_grid2_step needs N % 256 == 0, the standard rotation and a rotation angle small enough for
+    first-order weight tables; the request is refused otherwise (AUTO then keeps k_grid_step)."""
+    sim = vfps.Simulation(128, -6, 6, -6, 6, 4000, 1e-3, 4)
+    with pytest.raises(vfps.VfpsError) as e:
+        sim.set_grid_kernel(2)
+    assert e.value.code == -5
+    sim.set_engine(vfps.ENGINE_GRID)
+    assert sim.grid_kernel == 1
+    sim.close()
+    sim = vfps.Simulation(256, -6, 6, -6, 6, 300, 1e-3, 4)            # 1.2 degrees per step
+    with pytest.raises(vfps.VfpsError) as e:
+        sim.set_grid_kernel(2)
+    assert e.value.code == -5
+    sim.close()
+    sim = vfps.Simulation(256, -6, 6, -6, 6, 4000, 1e-3, 4, flags=vfps.FLAG_RENORMALISE | vfps.FLAG_ROT_MANHATTAN)
+    with pytest.raises(vfps.VfpsError) as e:
+        sim.set_grid_kernel(2)
+    assert e.value.code == -5
     sim.close()
 
 
