@@ -59,26 +59,23 @@ struct Grid2Args {
 };
 
 struct Grid2Layout {
-    int box_rows, pitch, nct, nch;
-    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_chunk, off_rho, off_sw, off_sw2, off_red, off_big,
+    int box_rows, pitch, nct;
+    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_rho, off_sw, off_sw2, off_red, off_big,
         total_floats;
 };
 
 __host__ __device__ inline Grid2Layout grid2_layout(int N, int KRmax, int H, int order, bool clamp)
 {
     Grid2Layout L;
-    const int CH = oc_chunk_rows(order);
     L.box_rows = (KRmax + 2 * H + 1) & ~1;          // even: a box of 144 floats x rows is then a multiple of 128 bytes (TMA)
     L.pitch = N + 2 * G2_PADC;
     L.nct = N / 256;
-    L.nch = (KRmax + CH - 1) / CH;
     L.tile_floats = (size_t)2 * L.box_rows * G2_SUBW;          // two boxes of 128 columns
     size_t o = 0;
     L.off_mbar = o;     o += 32;                                // 2 x G2_GROUPS mbarriers
     L.off_rowtab = o;   o += (size_t)(KRmax + 2) * OC_ROWTAB;
     L.off_rowpart = o;  o += (size_t)KRmax * (N / 64);
     L.off_vtab = o;     o += (size_t)((KRmax * 8 + 3) & ~3);
-    L.off_chunk = o;    o += (size_t)((L.nch + 3) & ~3);
     L.off_rho = o;      o += (size_t)N;
     L.off_sw = o;       o += (size_t)((N + KRmax + 3) & ~3);
     L.off_sw2 = o;      o += clamp ? (size_t)((N + KRmax + 3) & ~3) : 0;
@@ -155,14 +152,12 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     const int c = (int)blockIdx.x;
     const int rows = A.rows_lo + (c < A.rows_extra ? 1 : 0);
     const int r0 = c * A.rows_lo + min(c, A.rows_extra);
-    const int nch = (rows + CH - 1) / CH;
 
     extern __shared__ __align__(128) float g2smem[];
     float *smem = g2smem;
     float *rowtab_s = smem + LY.off_rowtab + OC_ROWTAB;
     float *rowpart = smem + LY.off_rowpart;
     float *vtab = smem + LY.off_vtab;
-    int *chunkinfo = reinterpret_cast<int *>(smem + LY.off_chunk);
     float *srho = smem + LY.off_rho, *sw = smem + LY.off_sw, *sw2 = smem + LY.off_sw2;
     float *red = smem + LY.off_red;
     float *big = smem + LY.off_big;
@@ -177,15 +172,17 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         rowtab_s[i - OC_ROWTAB] = (gi >= 0 && gi < N * OC_ROWTAB) ? A.rowtab[gi] : 0.0f;
     }
     __syncthreads();
-    for (int i = tid; i < LY.nch; i += G2_THREADS) {
-        // floor(dy) of the chunk's rows if they agree (and are good), else OC_BAD
-        int iy = OC_BAD;
-        if (i * CH < rows) {
-            iy = __float_as_int(rowtab_s[(i * CH) * OC_ROWTAB + 10]);
-            for (int k = 1; k < CH && i * CH + k < rows; ++k)
-                if (__float_as_int(rowtab_s[(i * CH + k) * OC_ROWTAB + 10]) != iy) iy = OC_BAD;
+    if (A.wfun != nullptr) {
+        // the lags this stripe's rows touch: sw[i] = w at index r0 + i (V_x = sum_x' sw[x - r0 + N - 1 - x'] rho_x');
+        // CLAMP: sw2[i] = w at index N - r0 - KRmax + i (transposed wake: w[x' - x] = sw2[x' + KRmax - 1 - (x - r0)])
+        for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
+        if (CLAMP) {
+            const int base2 = N - r0 - KRmax;
+            for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) {
+                const int k = base2 + i;
+                sw2[i] = (k >= 0 && k < 2 * N - 1) ? __ldg(A.wfun + k) : 0.0f;
+            }
         }
-        chunkinfo[i] = iy;
     }
     if (tid == 0) {
         for (int i = 0; i < 2 * G2_GROUPS; ++i) mbar_init(sMbar + 8u * (uint32_t)i, 1);
@@ -204,25 +201,29 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     __shared__ float s_tot[6];
     __shared__ float s_sc;
 
+    // the first two tiles of a group's rotation.  psi was written with ordinary stores (by every CTA,
+    // before a grid barrier) and TMA reads it through the async proxy: proxy fence first.
+#define G2_ISSUE_FIRST()                                                                                \
+    do {                                                                                                \
+        if (issuer) {                                                                                   \
+            asm volatile("fence.proxy.async;" ::: "memory");                                            \
+            for (int b_ = 0; b_ < 2; ++b_) {                                                            \
+                const int ct_ = grp + G2_GROUPS * b_;                                                   \
+                if (ct_ < nct) {                                                                        \
+                    const uint32_t mb_ = b_ ? mb1 : mb0, dst_ = b_ ? buf1 : buf0;                       \
+                    mbar_expect_tx(mb_, tile_bytes);                                                    \
+                    tma_load_2d(dst_, &tmap, 256 * ct_ - G2_PADC, r0 - H, mb_);                         \
+                    tma_load_2d(dst_ + box_bytes, &tmap, 256 * ct_ + 128 - G2_PADC, r0 - H, mb_);       \
+                }                                                                                       \
+            }                                                                                           \
+        }                                                                                               \
+    } while (0)
+
     for (int step = 0; step < A.nsteps; ++step) {
         VFPS_STAMP(A.dbg, step, 0);
         // ================= phase 1: rotation psi -> psi_tmp, row sums.  Group grp: column tiles grp, grp + 4, ...
         if (rows > 0) {
-            if (issuer) {
-                // psi was written with ordinary stores (by every CTA, before the grid barrier); TMA reads it
-                // through the async proxy
-                asm volatile("fence.proxy.async;" ::: "memory");
-#pragma unroll
-                for (int b = 0; b < 2; ++b) {
-                    const int ct = grp + G2_GROUPS * b;
-                    if (ct < nct) {
-                        const uint32_t mb = b ? mb1 : mb0, dst = b ? buf1 : buf0;
-                        mbar_expect_tx(mb, tile_bytes);
-                        tma_load_2d(dst, &tmap, 256 * ct - G2_PADC, r0 - H, mb);
-                        tma_load_2d(dst + box_bytes, &tmap, 256 * ct + 128 - G2_PADC, r0 - H, mb);
-                    }
-                }
-            }
+            if (step == 0) G2_ISSUE_FIRST();
             int it = 0;
             for (int ct = grp; ct < nct; ct += G2_GROUPS, ++it) {
                 const int b = it & 1;
@@ -253,24 +254,25 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                 const uint32_t box = tile + (uint32_t)(cw >> 1) * box_bytes;
                 const int yl = G2_PADC + 64 * (cw & 1) + 2 * lane;
                 float *gout = A.psi_tmp + (size_t)r0 * N + y0;
-                int ci = 0;
-                while (ci < nch) {
-                    const int iy = chunkinfo[ci];
-                    int nrun = 1;
+                // runs of consecutive rows with the same floor(dy): the window slides through a run; a floor
+                // changes at most once in a stripe (at the row through the rotation centre)
+                int v = 0;
+                while (v < rows) {
+                    const int iy = __float_as_int(rowtab_s[v * OC_ROWTAB + 10]);
                     if (cols_ok && iy != OC_BAD) {
-                        while (ci + nrun < nch && chunkinfo[ci + nrun] == iy) ++nrun;
+                        int ve = v + 1;
+                        while (ve < rows && __float_as_int(rowtab_s[ve * OC_ROWTAB + 10]) == iy) ++ve;
                         const int par = (iy - O0) & 1;
-                        const int v0 = ci * CH;
                         // tile row of source row x is x - (r0 - H); tap row 0 of target v: v + ixc - O0
-                        uint32_t src = box + (uint32_t)((v0 + H + ixc - O0) * P4 + (yl + iy - O0 - par) * 4);
-                        OutGlobal dst{gout + (size_t)v0 * N, N};
-                        uint32_t tab = sRowtab + (uint32_t)(v0 * OC_ROWTAB * 4);
-                        uint32_t rp = sRowpart + (uint32_t)(((v0 + (lane >> 3)) * CWR + 4 * ct + cw) * 4);
+                        uint32_t src = box + (uint32_t)((v + H + ixc - O0) * P4 + (yl + iy - O0 - par) * 4);
+                        OutGlobal dst{gout + (size_t)v * N, N};
+                        uint32_t tab = sRowtab + (uint32_t)(v * OC_ROWTAB * 4);
+                        uint32_t rp = sRowpart + (uint32_t)(((v + (lane >> 3)) * CWR + 4 * ct + cw) * 4);
 #define G2_RUN(PAR_)                                                                                   \
     do {                                                                                                \
         wkr.template start<PAR_>(src, tab);                                                             \
-        for (int q = 0; q < nrun; ++q) {                                                                \
-            const int left = rows - (ci + q) * CH;                                                      \
+        for (int vv = v; vv < ve; vv += CH) {                                                           \
+            const int left = ve - vv;                                                                   \
             if (left >= CH) wkr.template chunk<PAR_, 1>(src, dst, tab);                                 \
             else wkr.template chunk_n<PAR_, 1>(src, dst, tab, left);                                    \
             if (CH < 4) wkr.rs[3] = 0.0f;                                                               \
@@ -282,25 +284,17 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     } while (0)
                         if (par) G2_RUN(1); else G2_RUN(0);
 #undef G2_RUN
+                        v = ve;
                     } else {
-                        const int vlo = ci * CH, nrow = min(CH, rows - vlo);
-                        float rs4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-#pragma unroll
-                        for (int s = 0; s < CH; ++s) {
-                            if (s < nrow) {
-                                const int v = vlo + s;
-                                const uint32_t b00 = box + (uint32_t)(((v + H) * G2_SUBW + yl) * 4);
-                                const float o0 = rotate_cell_tile<ORDER, CLAMP>(G, b00, r0 + v, y0);
-                                const float o1 = rotate_cell_tile<ORDER, CLAMP>(G, b00 + 4u, r0 + v, y0 + 1);
-                                *reinterpret_cast<float2 *>(gout + (size_t)v * N) = make_float2(o0, o1);
-                                rs4[s] = o0 + o1;
-                            }
-                        }
-                        const float tot = warp_reduce_transposed<4>(rs4, lane);
-                        const int s = lane >> 3;
-                        if (rs_writer && s < nrow) rowpart[(vlo + s) * CWR + 4 * ct + cw] = tot;
+                        // one row, cell by cell: floor(dx) changes inside the warp's columns, or floor(dy) along the row
+                        const uint32_t b00 = box + (uint32_t)(((v + H) * G2_SUBW + yl) * 4);
+                        const float o0 = rotate_cell_tile<ORDER, CLAMP>(G, b00, r0 + v, y0);
+                        const float o1 = rotate_cell_tile<ORDER, CLAMP>(G, b00 + 4u, r0 + v, y0 + 1);
+                        *reinterpret_cast<float2 *>(gout + (size_t)v * N) = make_float2(o0, o1);
+                        const float tot = warp_sum(o0 + o1);
+                        if (lane == 0) rowpart[v * CWR + 4 * ct + cw] = tot;
+                        ++v;
                     }
-                    ci += nrun;
                 }
                 // the whole group has finished reading this buffer: refill it with the tile after next
                 named_barrier(1 + grp, 128);
@@ -319,33 +313,24 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             for (int k = 0; k < CWR; ++k) s += rowpart[tid * CWR + k];
             A.rho[r0 + tid] = s * G.dp;
         }
+        // the stripe's rows of psi_tmp (this CTA wrote them) stream into the space of the tile buffers
+        // while the grid meets at the barrier
+        for (int i = tid; i < rows * (N >> 2); i += G2_THREADS) {
+            const int r = i / (N >> 2), q = i - r * (N >> 2);
+            cp_async16(sBig + (uint32_t)((r * PITCH + G2_PADC + 4 * q) * 4), A.psi_tmp + (size_t)(r0 + r) * N + 4 * q);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        for (int i = tid; i < rows * 2 * G2_PADC; i += G2_THREADS) {      // zero pads left and right of every row
+            const int r = i / (2 * G2_PADC), k = i - r * (2 * G2_PADC);
+            big[r * PITCH + (k < G2_PADC ? k : N + k)] = 0.0f;
+        }
         __threadfence();
         grid.sync();
         VFPS_STAMP(A.dbg, step, 2);
         // ================= phase 2: wake of the stripe's rows while its rotated rows stream into shared memory
         float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 pw - -
         if (rows > 0) {
-            const int NQ = N >> 2;
-            for (int i = tid; i < rows * NQ; i += G2_THREADS) {
-                const int r = i / NQ, q = i - r * NQ;
-                cp_async16(sBig + (uint32_t)((r * PITCH + G2_PADC + 4 * q) * 4), A.psi_tmp + (size_t)(r0 + r) * N + 4 * q);
-            }
-            asm volatile("cp.async.commit_group;" ::: "memory");
-            for (int i = tid; i < rows * 2 * G2_PADC; i += G2_THREADS) {      // zero pads left and right of every row
-                const int r = i / (2 * G2_PADC), k = i - r * (2 * G2_PADC);
-                big[r * PITCH + (k < G2_PADC ? k : N + k)] = 0.0f;
-            }
             for (int i = tid; i < N; i += G2_THREADS) srho[i] = __ldcg(A.rho + i);
-            if (A.wfun != nullptr) {
-                for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
-                if (CLAMP) {
-                    const int base2 = N - r0 - KRmax;          // sw2[i] = w at index base2 + i: w[x' - x] = sw2[x' + KRmax - 1 - (x - r0)]
-                    for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) {
-                        const int k = base2 + i;
-                        sw2[i] = (k >= 0 && k < 2 * N - 1) ? __ldg(A.wfun + k) : 0.0f;
-                    }
-                }
-            }
             __syncthreads();
             VFPS_STAMP(A.dbg, step, 3);
             // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4), one row per warp
@@ -389,10 +374,11 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncthreads();
             VFPS_STAMP(A.dbg, step, 4);
-            // a4 + a5 + a6: unit = (row, 256-column block); lane owns the granules 4 lane and 4 lane + 128 of the block
-            const int nunits = rows * nct;
-            for (int u = warp; u < nunits; u += G2_WARPS) {
-                const int r = u / nct, blk = u - r * nct;
+            // a4 + a5 + a6: a warp takes (row, 256-column block); a lane owns the granules 4 lane and 4 lane + 128 of the block
+            // a warp keeps its column block: column sums serve the p-moments
+            const int blk = warp % nct, rstride = G2_WARPS / nct;
+            float cs[2][4] = {{0.0f, 0.0f, 0.0f, 0.0f}, {0.0f, 0.0f, 0.0f, 0.0f}};
+            for (int r = warp / nct; r < rows; r += rstride) {
                 const float4 lw = lds4(sVtab + (uint32_t)r * 32u);
                 float2 mv;
                 float dpU = 0.0f;
@@ -452,16 +438,20 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                 for (int k = 0; k < 2; ++k) {
                     *reinterpret_cast<float4 *>(orow + 128 * k) = make_float4(o[k][0], o[k][1], o[k][2], o[k][3]);
 #pragma unroll
-                    for (int cc = 0; cc < 4; ++cc) {
-                        const float yy = (float)(g0 + 128 * k + cc) - yc, tt = o[k][cc] * yy;
-                        rs += o[k][cc]; acc[1] += tt; acc[2] = fmaf(tt, yy, acc[2]);
-                    }
+                    for (int cc = 0; cc < 4; ++cc) { cs[k][cc] += o[k][cc]; rs += o[k][cc]; }
                 }
                 const float xx = (float)(r0 + r) - yc, tq = rs * xx;
-                acc[0] += rs; acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
+                acc[3] += tq; acc[4] = fmaf(tq, xx, acc[4]);
                 if (CLAMP) acc[5] = fmaf(rs, dpU, acc[5]);
                 if (lane == 0 && blk == 0) acc[5] += mv.y;
             }
+#pragma unroll
+            for (int k = 0; k < 2; ++k)
+#pragma unroll
+                for (int cc = 0; cc < 4; ++cc) {
+                    const float yy = (float)(256 * blk + 4 * lane + 128 * k + cc) - yc, tt = cs[k][cc] * yy;
+                    acc[0] += cs[k][cc]; acc[1] += tt; acc[2] = fmaf(tt, yy, acc[2]);
+                }
         }
         {
             const float tot = warp_reduce_transposed<8>(acc, lane);       // lanes 4 j .. 4 j + 3 hold sum j
@@ -482,6 +472,9 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         VFPS_STAMP(A.dbg, step, 5);
         grid.sync();
         VFPS_STAMP(A.dbg, step, 6);
+        // the next rotation's first tiles are on their way while C and the diagnostics are formed
+        // (the tile buffers are free: every thread has finished its kick)
+        if (rows > 0 && step + 1 < A.nsteps) G2_ISSUE_FIRST();
         // ================= phase 3: a6 -- every CTA forms C and 1/C from the same accumulator
         if (tid == 0) {
             const long long q = (long long)__ldcg(A.qacc + (step & 1));
@@ -517,6 +510,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         __syncthreads();
         VFPS_STAMP(A.dbg, step, 7);
     }
+#undef G2_ISSUE_FIRST
     if (blockIdx.x == 0 && tid == 0) A.scale[0] = sc;
 }
 
