@@ -81,7 +81,7 @@ struct vfps_sim {
     std::string gr_why;
     // TMA-staged grid engine (vfps_grid2.cuh, grid kernel 2); g2_blocks = 0: not available
     int gr_ver_opt = 0;                          // 0 auto (2 where available), 1 k_grid_step, 2 k_grid2_step
-    int g2_blocks = 0, g2_KRmax = 0, g2_rows_lo = 0, g2_rows_extra = 0;
+    int g2_blocks = 0, g2_KRmax = 0, g2_rows_lo = 0, g2_rows_extra = 0, g2_nbuf = 0;
     size_t g2_smem = 0;
     float *g2_coltab = nullptr, *g2_rowtab = nullptr, *g2_rho = nullptr, *g2_mom = nullptr;
     int *g2_colix = nullptr;
@@ -670,7 +670,10 @@ int grid2_configure(vfps_sim *h)
     const int nb = sms < N ? sms : N;
     const int rows_lo = N / nb, rows_extra = N % nb, KRmax = rows_lo + (rows_extra ? 1 : 0);
     const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0 && order > 2;
-    const Grid2Layout L = grid2_layout(N, KRmax, H, order, clamp);
+    // two tile buffers per warp group where they fit beside the stripe's rows, else one
+    int nbuf = 2;
+    Grid2Layout L = grid2_layout(N, KRmax, H, nbuf, clamp);
+    if (L.total_floats * sizeof(float) + 256 > (size_t)smem_max) { nbuf = 1; L = grid2_layout(N, KRmax, H, nbuf, clamp); }
     const size_t bytes = L.total_floats * sizeof(float);
     if (bytes + 256 > (size_t)smem_max) { h->g2_why = "tiles and row buffer do not fit shared memory"; return VFPS_OK; }
     if (L.box_rows > 256) { h->g2_why = "TMA box too tall"; return VFPS_OK; }
@@ -698,11 +701,12 @@ int grid2_configure(vfps_sim *h)
         qres != cudaDriverEntryPointSuccess) {
         cudaGetLastError(); h->g2_why = "cuTensorMapEncodeTiled not available"; return VFPS_OK;
     }
-    const cuuint64_t gdim[2] = {(cuuint64_t)N, (cuuint64_t)N};
+    // (8-byte elements = pairs of floats: a box dimension is limited to 256 elements, a tile row has 272 floats)
+    const cuuint64_t gdim[2] = {(cuuint64_t)N / 2, (cuuint64_t)N};
     const cuuint64_t gstr[1] = {(cuuint64_t)N * sizeof(float)};
-    const cuuint32_t box[2] = {(cuuint32_t)G2_SUBW, (cuuint32_t)L.box_rows};
+    const cuuint32_t box[2] = {(cuuint32_t)G2_SUBW / 2, (cuuint32_t)L.box_rows};
     const cuuint32_t estr[2] = {1, 1};
-    if (((EncodeTiled)fn)(&h->g2_tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)h->psi, gdim, gstr, box, estr,
+    if (((EncodeTiled)fn)(&h->g2_tmap, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, (void *)h->psi, gdim, gstr, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
         h->g2_why = "cuTensorMapEncodeTiled failed"; return VFPS_OK;
@@ -752,6 +756,7 @@ int grid2_configure(vfps_sim *h)
     CU(cudaMemcpyAsync(h->g2_colix, cix.data(), cix.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(h->g2_rowtab, row.data(), row.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
     CU(cudaStreamSynchronize(h->stream));
+    h->g2_nbuf = nbuf;
     h->g2_blocks = nb; h->g2_KRmax = KRmax; h->g2_rows_lo = rows_lo; h->g2_rows_extra = rows_extra; h->g2_smem = bytes;
     return VFPS_OK;
 }
@@ -759,10 +764,10 @@ int grid2_configure(vfps_sim *h)
 int launch_grid2_steps(vfps_sim *h, int n, float *diag)
 {
     Grid2Args A{};
-    A.psi = h->psi; A.psi_tmp = h->psi_tmp; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr;
+    A.psi = h->psi; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr;
     A.rho = h->g2_rho; A.mom_part = h->g2_mom; A.diag = diag; A.nsteps = n;
     A.coltab = h->g2_coltab; A.colix = h->g2_colix; A.rowtab = h->g2_rowtab; A.qacc = h->g2_qacc;
-    A.rows_lo = h->g2_rows_lo; A.rows_extra = h->g2_rows_extra; A.KRmax = h->g2_KRmax;
+    A.rows_lo = h->g2_rows_lo; A.rows_extra = h->g2_rows_extra; A.KRmax = h->g2_KRmax; A.nbuf = h->g2_nbuf;
     if (cudaMemsetAsync(h->g2_qacc, 0, 2 * sizeof(unsigned long long), h->stream) != cudaSuccess)
         return fail(h, VFPS_ERR_CUDA, "cudaMemsetAsync failed");
     const void *kern = grid2_kernel(h);

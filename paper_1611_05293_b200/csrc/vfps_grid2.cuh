@@ -5,18 +5,19 @@
 // thread-instructions per cell, 29 us per step at 2048^2.  This engine gives the large grid what the
 // in-place cluster kernel (vfps_onchip.cuh) gives the on-chip ones:
 //  * One CTA of 512 threads per SM owns a stripe of N / gridDim rows for the whole launch.
-//  * Rotation a1 + a2: the source region of a tile -- the stripe's rows plus H halo rows, 128
-//    columns plus 8 each side -- comes in through TMA (cp.async.bulk.tensor.2d, completion on an
-//    mbarrier).  psi is zero outside the grid (reading A8), and so is TMA's fill for the part of a
+//  * Rotation a1 + a2: the source region of a tile -- the stripe's rows plus H halo rows, 256
+//    columns plus 8 each side -- comes in through TMA (cp.async.bulk.tensor.2d over a tensor map of
+//    8-byte elements, so that one box holds the 272 floats of a tile row; completion on an mbarrier).  psi is zero outside the grid (reading A8), and so is TMA's fill for the part of a
 //    box that lies outside the tensor: no edge path exists.  A group of four warps rotates a tile
-//    of 256 columns (two such boxes) with the cluster kernel's walker: two columns per thread,
+//    with the cluster kernel's walker: two columns per thread,
 //    ORDER x 6 register window, per-launch weight tables (built in double on the host for the
-//    centre row of every stripe), next row's loads issued mid-row.  Two buffers per group: the
-//    tile after next is in flight while a tile is rotated.  Results go to psi_tmp (64-bit stores),
-//    row sums (transposed warp reduction) to the profile.
+//    centre row of every stripe), next row's loads issued mid-row.  Two tile buffers per group where
+//    they fit (the tile after next is in flight while a tile is rotated), else one; the first tiles
+//    of a step are issued right after the previous step's last barrier.  The rotated cells stay in
+//    shared memory (the stripe's rows: no psi_tmp round trip through L2), row sums (transposed warp
+//    reduction) go to the profile.
 //  -- grid barrier --
-//  * Wake a3 for the stripe's rows (one warp per row, direct convolution, Eq. 4), while the
-//    stripe's rows of psi_tmp stream into shared memory (cp.async, the space of the tile buffers).
+//  * Wake a3 for the stripe's rows (one warp per row, direct convolution, Eq. 4).
 //  * Kick a4 + Fokker-Planck a5 + moments a6 from shared memory: a warp takes a (row, 256-column
 //    block), a lane the 4-cell granules 4 lane + 128 k -- 128-bit loads with a lane stride of 16
 //    bytes -- and writes psi with 128-bit stores.
@@ -35,14 +36,13 @@ namespace vfps {
 constexpr int G2_THREADS = 512;
 constexpr int G2_WARPS = G2_THREADS / 32;
 constexpr int G2_GROUPS = 4;          // warp groups of four, one tile each at a time
-constexpr int G2_SUBW = 144;          // floats per row of a box: 128 columns + 8 each side
+constexpr int G2_SUBW = 272;          // floats per row of a tile: 256 columns + 8 each side (one TMA box of 136 8-byte elements)
 constexpr int G2_PADC = 8;
 constexpr int G2_NPART = 8;
 constexpr int G2_MAX_H = 4;
 
 struct Grid2Args {
     float *psi;            // [N][N] in/out, un-normalised (the tensor map of the kernel points at it)
-    float *psi_tmp;        // [N][N] rotated density
     float *scale;          // [1] in/out: 1/C of the last step
     const float *wfun;     // [2N] wake function, lag d at index d + N - 1; nullptr = no wake
     float *rho;            // [N] profile of the step (dp * row sums, un-scaled)
@@ -55,22 +55,23 @@ struct Grid2Args {
     int nsteps;
     int rows_lo, rows_extra;    // stripe c has rows_lo + (c < rows_extra) rows
     int KRmax;                  // rows of the largest stripe
+    int nbuf;                   // tile buffers per warp group: 2, or 1 where two do not fit beside the stripe's rows
     long long *dbg;
 };
 
 struct Grid2Layout {
     int box_rows, pitch, nct;
-    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_rho, off_sw, off_sw2, off_red, off_big,
+    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_rho, off_sw, off_sw2, off_red, off_rows, off_big,
         total_floats;
 };
 
-__host__ __device__ inline Grid2Layout grid2_layout(int N, int KRmax, int H, int order, bool clamp)
+__host__ __device__ inline Grid2Layout grid2_layout(int N, int KRmax, int H, int nbuf, bool clamp)
 {
     Grid2Layout L;
-    L.box_rows = (KRmax + 2 * H + 1) & ~1;          // even: a box of 144 floats x rows is then a multiple of 128 bytes (TMA)
+    L.box_rows = (KRmax + 2 * H + 1) & ~1;          // even: a tile of 272 floats x rows is then a multiple of 128 bytes (TMA)
     L.pitch = N + 2 * G2_PADC;
     L.nct = N / 256;
-    L.tile_floats = (size_t)2 * L.box_rows * G2_SUBW;          // two boxes of 128 columns
+    L.tile_floats = (size_t)L.box_rows * G2_SUBW;
     size_t o = 0;
     L.off_mbar = o;     o += 32;                                // 2 x G2_GROUPS mbarriers
     L.off_rowtab = o;   o += (size_t)(KRmax + 2) * OC_ROWTAB;
@@ -80,11 +81,9 @@ __host__ __device__ inline Grid2Layout grid2_layout(int N, int KRmax, int H, int
     L.off_sw = o;       o += (size_t)((N + KRmax + 3) & ~3);
     L.off_sw2 = o;      o += clamp ? (size_t)((N + KRmax + 3) & ~3) : 0;
     L.off_red = o;      o += (size_t)G2_WARPS * 8 + 8;
+    L.off_rows = o;     o += (size_t)KRmax * L.pitch;           // the stripe's rotated rows
     o = (o + 31) & ~(size_t)31;                                 // TMA destinations: 128-byte aligned
-    L.off_big = o;
-    const size_t tiles = (size_t)2 * G2_GROUPS * L.tile_floats + G2_SUBW;   // + one row: the walker prefetches past the end
-    const size_t rows = (size_t)KRmax * L.pitch;
-    o += tiles > rows ? tiles : rows;
+    L.off_big = o;      o += (size_t)nbuf * G2_GROUPS * L.tile_floats + G2_SUBW;   // + one row: the walker prefetches past the end
     L.total_floats = o;
     return L;
 }
@@ -145,7 +144,8 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     cg::grid_group grid = cg::this_grid();
 
     const int N = G.N, H = G.H, KRmax = A.KRmax;
-    const Grid2Layout LY = grid2_layout(N, KRmax, H, ORDER, CLAMP);
+    const int nbuf = A.nbuf;
+    const Grid2Layout LY = grid2_layout(N, KRmax, H, nbuf, CLAMP);
     const int nct = LY.nct, CWR = N / 64;                  // column tiles; row-sum partials per row
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int grp = warp >> 2, cw = warp & 3;
@@ -161,9 +161,10 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     float *srho = smem + LY.off_rho, *sw = smem + LY.off_sw, *sw2 = smem + LY.off_sw2;
     float *red = smem + LY.off_red;
     float *big = smem + LY.off_big;
-    const uint32_t sBig = smem_u32(big), sRowtab = smem_u32(rowtab_s), sRowpart = smem_u32(rowpart), sVtab = smem_u32(vtab);
+    float *rowsb = smem + LY.off_rows;               // [KRmax][PITCH]: the stripe's rotated rows, 8 zero floats each side
+    const uint32_t sBig = smem_u32(big), sRows = smem_u32(rowsb), sRowtab = smem_u32(rowtab_s), sRowpart = smem_u32(rowpart), sVtab = smem_u32(vtab);
     const uint32_t sMbar = smem_u32(smem + LY.off_mbar);
-    const uint32_t tile_bytes = (uint32_t)LY.tile_floats * 4u, box_bytes = tile_bytes / 2u;
+    const uint32_t tile_bytes = (uint32_t)LY.tile_floats * 4u;
     const int PITCH = LY.pitch;
 
     // ---- one-time set-up
@@ -184,6 +185,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             }
         }
     }
+    for (int i = tid; i < KRmax * PITCH; i += G2_THREADS) rowsb[i] = 0.0f;       // the pads stay zero for ever
     if (tid == 0) {
         for (int i = 0; i < 2 * G2_GROUPS; ++i) mbar_init(sMbar + 8u * (uint32_t)i, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -195,7 +197,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     float sc = G.renorm ? A.scale[0] : 1.0f;
     unsigned use0 = 0u, use1 = 0u;             // how often this group has waited on its buffer 0 / 1
     const uint32_t mb0 = sMbar + 16u * (uint32_t)grp, mb1 = mb0 + 8u;
-    const uint32_t buf0 = sBig + (uint32_t)(2 * grp) * tile_bytes, buf1 = buf0 + tile_bytes;
+    const uint32_t buf0 = sBig + (uint32_t)(nbuf * grp) * tile_bytes, buf1 = buf0 + tile_bytes;     // buf1 only if nbuf == 2
     const bool rs_writer = ((lane & 7) == 0) && ((lane >> 3) < CH);
     const bool issuer = (cw == 0 && lane == 0);
     __shared__ float s_tot[6];
@@ -207,13 +209,12 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     do {                                                                                                \
         if (issuer) {                                                                                   \
             asm volatile("fence.proxy.async;" ::: "memory");                                            \
-            for (int b_ = 0; b_ < 2; ++b_) {                                                            \
+            for (int b_ = 0; b_ < nbuf; ++b_) {                                                         \
                 const int ct_ = grp + G2_GROUPS * b_;                                                   \
                 if (ct_ < nct) {                                                                        \
                     const uint32_t mb_ = b_ ? mb1 : mb0, dst_ = b_ ? buf1 : buf0;                       \
                     mbar_expect_tx(mb_, tile_bytes);                                                    \
-                    tma_load_2d(dst_, &tmap, 256 * ct_ - G2_PADC, r0 - H, mb_);                         \
-                    tma_load_2d(dst_ + box_bytes, &tmap, 256 * ct_ + 128 - G2_PADC, r0 - H, mb_);       \
+                    tma_load_2d(dst_, &tmap, (256 * ct_ - G2_PADC) / 2, r0 - H, mb_);                   \
                 }                                                                                       \
             }                                                                                           \
         }                                                                                               \
@@ -221,12 +222,12 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
 
     for (int step = 0; step < A.nsteps; ++step) {
         VFPS_STAMP(A.dbg, step, 0);
-        // ================= phase 1: rotation psi -> psi_tmp, row sums.  Group grp: column tiles grp, grp + 4, ...
+        // ================= phase 1: rotation psi -> the stripe's rows in shared memory, row sums.  Group grp: column tiles grp, grp + 4, ...
         if (rows > 0) {
             if (step == 0) G2_ISSUE_FIRST();
             int it = 0;
             for (int ct = grp; ct < nct; ct += G2_GROUPS, ++it) {
-                const int b = it & 1;
+                const int b = (nbuf == 2) ? (it & 1) : 0;
                 const uint32_t mb = b ? mb1 : mb0, tile = b ? buf1 : buf0;
                 // this tile's columns: y0, y0 + 1; weights along q from the stripe's table
                 const int y0 = 256 * ct + 64 * cw + 2 * lane;
@@ -250,10 +251,10 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                 }
                 mbar_wait(mb, (b ? use1 : use0) & 1u);
                 if (b) ++use1; else ++use0;
-                // box of this warp: columns 128 (cw >> 1) ..; local column of y0 inside it
-                const uint32_t box = tile + (uint32_t)(cw >> 1) * box_bytes;
-                const int yl = G2_PADC + 64 * (cw & 1) + 2 * lane;
-                float *gout = A.psi_tmp + (size_t)r0 * N + y0;
+                // local column of y0 inside the tile; the rotated cells go to the stripe's rows in shared memory
+                const uint32_t box = tile;
+                const int yl = G2_PADC + 64 * cw + 2 * lane;
+                const uint32_t sout = sRows + (uint32_t)((G2_PADC + y0) * 4), RP4 = (uint32_t)PITCH * 4u;
                 // runs of consecutive rows with the same floor(dy): the window slides through a run; a floor
                 // changes at most once in a stripe (at the row through the rotation centre)
                 int v = 0;
@@ -265,7 +266,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                         const int par = (iy - O0) & 1;
                         // tile row of source row x is x - (r0 - H); tap row 0 of target v: v + ixc - O0
                         uint32_t src = box + (uint32_t)((v + H + ixc - O0) * P4 + (yl + iy - O0 - par) * 4);
-                        OutGlobal dst{gout + (size_t)v * N, N};
+                        OutSharedRt dst{sout + (uint32_t)v * RP4, RP4};
                         uint32_t tab = sRowtab + (uint32_t)(v * OC_ROWTAB * 4);
                         uint32_t rp = sRowpart + (uint32_t)(((v + (lane >> 3)) * CWR + 4 * ct + cw) * 4);
 #define G2_RUN(PAR_)                                                                                   \
@@ -278,7 +279,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             if (CH < 4) wkr.rs[3] = 0.0f;                                                               \
             const float tot = warp_reduce_transposed<4>(wkr.rs, lane);                                  \
             if (rs_writer && (lane >> 3) < left) sts(rp, tot);                                          \
-            src += (uint32_t)(CH * P4); dst.p += (size_t)CH * N;                                        \
+            src += (uint32_t)(CH * P4); dst.a += (uint32_t)CH * RP4;                                    \
             tab += (uint32_t)(CH * OC_ROWTAB * 4); rp += (uint32_t)(CH * CWR * 4);                      \
         }                                                                                               \
     } while (0)
@@ -290,7 +291,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                         const uint32_t b00 = box + (uint32_t)(((v + H) * G2_SUBW + yl) * 4);
                         const float o0 = rotate_cell_tile<ORDER, CLAMP>(G, b00, r0 + v, y0);
                         const float o1 = rotate_cell_tile<ORDER, CLAMP>(G, b00 + 4u, r0 + v, y0 + 1);
-                        *reinterpret_cast<float2 *>(gout + (size_t)v * N) = make_float2(o0, o1);
+                        sts2(sout + (uint32_t)v * RP4, o0, o1);
                         const float tot = warp_sum(o0 + o1);
                         if (lane == 0) rowpart[v * CWR + 4 * ct + cw] = tot;
                         ++v;
@@ -298,11 +299,10 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                 }
                 // the whole group has finished reading this buffer: refill it with the tile after next
                 named_barrier(1 + grp, 128);
-                const int ct2 = ct + 2 * G2_GROUPS;
+                const int ct2 = ct + nbuf * G2_GROUPS;
                 if (issuer && ct2 < nct) {
                     mbar_expect_tx(mb, tile_bytes);
-                    tma_load_2d(tile, &tmap, 256 * ct2 - G2_PADC, r0 - H, mb);
-                    tma_load_2d(tile + box_bytes, &tmap, 256 * ct2 + 128 - G2_PADC, r0 - H, mb);
+                    tma_load_2d(tile, &tmap, (256 * ct2 - G2_PADC) / 2, r0 - H, mb);
                 }
             }
         }
@@ -312,17 +312,6 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             float s = 0.0f;
             for (int k = 0; k < CWR; ++k) s += rowpart[tid * CWR + k];
             A.rho[r0 + tid] = s * G.dp;
-        }
-        // the stripe's rows of psi_tmp (this CTA wrote them) stream into the space of the tile buffers
-        // while the grid meets at the barrier
-        for (int i = tid; i < rows * (N >> 2); i += G2_THREADS) {
-            const int r = i / (N >> 2), q = i - r * (N >> 2);
-            cp_async16(sBig + (uint32_t)((r * PITCH + G2_PADC + 4 * q) * 4), A.psi_tmp + (size_t)(r0 + r) * N + 4 * q);
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        for (int i = tid; i < rows * 2 * G2_PADC; i += G2_THREADS) {      // zero pads left and right of every row
-            const int r = i / (2 * G2_PADC), k = i - r * (2 * G2_PADC);
-            big[r * PITCH + (k < G2_PADC ? k : N + k)] = 0.0f;
         }
         __threadfence();
         grid.sync();
@@ -371,7 +360,6 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                     }
                 }
             }
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncthreads();
             VFPS_STAMP(A.dbg, step, 4);
             // a4 + a5 + a6: a warp takes (row, 256-column block); a lane owns the granules 4 lane and 4 lane + 128 of the block
@@ -390,7 +378,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                 }
                 const int mm = __float_as_int(mv.x);
                 const int g0 = 256 * blk + 4 * lane;
-                const uint32_t own = sBig + (uint32_t)((r * PITCH + G2_PADC + g0) * 4);
+                const uint32_t own = sRows + (uint32_t)((r * PITCH + G2_PADC + g0) * 4);
                 const float lws[4] = {lw.x, lw.y, lw.z, lw.w};
                 float l[ORDER];
 #pragma unroll
@@ -416,7 +404,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                         else kick_fp_granule<ORDER, -2, CLAMP>(b[k], l, g, N, G.fp_b, c2, c1p, o[k]);
                     }
                 } else {
-                    const float *rowp = big + r * PITCH + G2_PADC;
+                    const float *rowp = rowsb + r * PITCH + G2_PADC;
 #pragma unroll
                     for (int k = 0; k < 2; ++k) {
                         const int g = g0 + 128 * k;
@@ -473,7 +461,6 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         grid.sync();
         VFPS_STAMP(A.dbg, step, 6);
         // the next rotation's first tiles are on their way while C and the diagnostics are formed
-        // (the tile buffers are free: every thread has finished its kick)
         if (rows > 0 && step + 1 < A.nsteps) G2_ISSUE_FIRST();
         // ================= phase 3: a6 -- every CTA forms C and 1/C from the same accumulator
         if (tid == 0) {

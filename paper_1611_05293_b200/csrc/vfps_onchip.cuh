@@ -438,6 +438,11 @@ struct OutShared {                     // shared memory, row pitch P4 bytes
     template <int R>
     __device__ __forceinline__ void put(float x, float y) const { sts2(a + (uint32_t)(R * P4), x, y); }
 };
+struct OutSharedRt {                   // shared memory, row pitch p4 bytes known at run time
+    uint32_t a, p4;
+    template <int R>
+    __device__ __forceinline__ void put(float x, float y) const { sts2(a + (uint32_t)R * p4, x, y); }
+};
 struct OutGlobal {                     // global memory, row pitch n floats
     float *p;
     int n;
