@@ -749,8 +749,8 @@ int grid2_configure(vfps_sim *h)
         CU(dalloc(h, &h->g2_colix, cix.size()));
         CU(dalloc(h, &h->g2_rowtab, row.size()));
         CU(dalloc(h, &h->g2_rho, (size_t)N));
-        CU(dalloc(h, &h->g2_mom, (size_t)nb * G2_NPART));
-        CU(dalloc(h, &h->g2_qacc, (size_t)2));
+        CU(dalloc(h, &h->g2_mom, (size_t)2 * nb * G2_NPART));
+        CU(dalloc(h, &h->g2_qacc, (size_t)16 + (size_t)16 * nb));   // three charge accumulators, barrier counter, one 128-byte flag line per CTA
     }
     CU(cudaMemcpyAsync(h->g2_coltab, col.data(), col.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(h->g2_colix, cix.data(), cix.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
@@ -768,7 +768,9 @@ int launch_grid2_steps(vfps_sim *h, int n, float *diag)
     A.rho = h->g2_rho; A.mom_part = h->g2_mom; A.diag = diag; A.nsteps = n;
     A.coltab = h->g2_coltab; A.colix = h->g2_colix; A.rowtab = h->g2_rowtab; A.qacc = h->g2_qacc;
     A.rows_lo = h->g2_rows_lo; A.rows_extra = h->g2_rows_extra; A.KRmax = h->g2_KRmax; A.nbuf = h->g2_nbuf;
-    if (cudaMemsetAsync(h->g2_qacc, 0, 2 * sizeof(unsigned long long), h->stream) != cudaSuccess)
+    A.bar = reinterpret_cast<unsigned int *>(h->g2_qacc + 3);
+    A.flags = reinterpret_cast<unsigned int *>(h->g2_qacc + 16);
+    if (cudaMemsetAsync(h->g2_qacc, 0, (16 + (size_t)16 * h->g2_blocks) * sizeof(unsigned long long), h->stream) != cudaSuccess)
         return fail(h, VFPS_ERR_CUDA, "cudaMemsetAsync failed");
     const void *kern = grid2_kernel(h);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->g2_smem);

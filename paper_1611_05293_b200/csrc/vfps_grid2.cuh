@@ -21,7 +21,10 @@
 //  * Kick a4 + Fokker-Planck a5 + moments a6 from shared memory: a warp takes a (row, 256-column
 //    block), a lane the 4-cell granules 4 lane + 128 k -- 128-bit loads with a lane stride of 16
 //    bytes -- and writes psi with 128-bit stores.
-//  -- grid barrier -- charge (exact 32.32 fixed-point sum), 1/C, diagnostics as in vfps_grid.cuh.
+//  ONE grid barrier per step: between a kick and the next rotation a CTA only needs the stripes above
+//  and below (their halo rows), so it waits for those two CTAs' flags; the charge of a step (exact
+//  32.32 fixed-point sum) and the partial sums for its diagnostics row are complete at the next
+//  step's barrier, which is where 1/C is needed next.
 // Template CLAMP: clamped interpolation (Eq. 14, reading A9); the CSR power is then that of the
 // end-of-step profile to first order in its change (transposed wake, see k_wake_direct).
 // Standard rotation only; one simulation per handle; N a multiple of 256.
@@ -46,12 +49,14 @@ struct Grid2Args {
     float *scale;          // [1] in/out: 1/C of the last step
     const float *wfun;     // [2N] wake function, lag d at index d + N - 1; nullptr = no wake
     float *rho;            // [N] profile of the step (dp * row sums, un-scaled)
-    float *mom_part;       // [G2_NPART][gridDim.x]
+    float *mom_part;       // [2][G2_NPART][gridDim.x], by step parity
     float *diag;           // [nsteps][1][6] or nullptr
     const float *coltab;   // [gridDim.x][N][8]: M[4], M'[4] of column y for the rows of stripe c
     const int *colix;      // [gridDim.x][N]: floor(dx) of column y over the rows of stripe c, or OC_BAD
     const float *rowtab;   // [N][12]: as in the cluster kernel (a (X - Xc) relative to the stripe's centre row)
-    unsigned long long *qacc;   // [2] charge of the step in 32.32 fixed point, zero at launch
+    unsigned long long *qacc;   // [3] charge of step t in slot t % 3, 32.32 fixed point, zero at launch
+    unsigned int *bar;          // grid barrier counter, zero at launch
+    unsigned int *flags;        // [gridDim.x][32] (one 128-byte line each): kicks finished by the CTA in this launch, zero at launch
     int nsteps;
     int rows_lo, rows_extra;    // stripe c has rows_lo + (c < rows_extra) rows
     int KRmax;                  // rows of the largest stripe
@@ -99,6 +104,26 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 
+// Grid barrier on one monotonic counter (zero at launch; the launch is cooperative, so every CTA is
+// resident): arrival = one atomic, release = the counter reaching gen * gridDim.x.  About half the cost
+// of cooperative_groups' grid.sync() here.
+__device__ __forceinline__ void grid_barrier(unsigned int *ctr, unsigned int &gen)
+{
+    __syncthreads();
+    ++gen;
+    if (threadIdx.x == 0) {
+        const unsigned int target = gen * gridDim.x;
+        __threadfence();
+        atomicAdd(ctr, 1u);
+        unsigned int seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
+        } while ((int)(seen - target) < 0);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
 // one cell of a tile with its own floors (a floor changes inside the warp's columns or the chunk)
 template <int ORDER, bool CLAMP>
 __device__ __forceinline__ float rotate_cell_tile(const GridConst &G, uint32_t base00 /* tile address of source (row x, column y) */,
@@ -141,7 +166,6 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     constexpr int P4 = G2_SUBW * 4;
     constexpr unsigned FULL = 0xffffffffu;
     using Wk = Walker<ORDER, G2_SUBW, true, CLAMP>;
-    cg::grid_group grid = cg::this_grid();
 
     const int N = G.N, H = G.H, KRmax = A.KRmax;
     const int nbuf = A.nbuf;
@@ -195,6 +219,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     const float yc = 0.5f * (float)(N - 1);
     const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
     float sc = G.renorm ? A.scale[0] : 1.0f;
+    unsigned int bar_gen = 0u;
     unsigned use0 = 0u, use1 = 0u;             // how often this group has waited on its buffer 0 / 1
     const uint32_t mb0 = sMbar + 16u * (uint32_t)grp, mb1 = mb0 + 8u;
     const uint32_t buf0 = sBig + (uint32_t)(nbuf * grp) * tile_bytes, buf1 = buf0 + tile_bytes;     // buf1 only if nbuf == 2
@@ -203,8 +228,8 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     __shared__ float s_tot[6];
     __shared__ float s_sc;
 
-    // the first two tiles of a group's rotation.  psi was written with ordinary stores (by every CTA,
-    // before a grid barrier) and TMA reads it through the async proxy: proxy fence first.
+    // The first tiles of a group's rotation.  psi was written with ordinary stores and TMA reads it
+    // through the async proxy: proxy fence first.
 #define G2_ISSUE_FIRST()                                                                                \
     do {                                                                                                \
         if (issuer) {                                                                                   \
@@ -220,11 +245,58 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         }                                                                                               \
     } while (0)
 
+    // diagnostics row of step T from the CTA partial sums (fp32, fixed order), by the last CTA
+#define G2_DIAG(T)                                                                                      \
+    do {                                                                                                \
+        if (blockIdx.x == gridDim.x - 1 && A.diag != nullptr) {                                         \
+            if (warp < 6) {                                                                             \
+                const float *mp_ = A.mom_part + ((size_t)((T) & 1) * G2_NPART + warp) * gridDim.x;      \
+                float f_ = 0.0f;                                                                        \
+                for (int i_ = lane; i_ < (int)gridDim.x; i_ += 32) f_ += __ldcg(mp_ + i_);              \
+                f_ = warp_sum(f_);                                                                      \
+                if (lane == 0) s_tot[warp] = f_;                                                        \
+            }                                                                                           \
+            __syncthreads();                                                                            \
+            if (tid == 0) {                                                                             \
+                const float t0_ = s_tot[0], i0_ = 1.0f / t0_;                                           \
+                const float C_ = (G.dq * G.dp) * t0_;                                                   \
+                const float mp_c_ = s_tot[1] * i0_, vp_ = fmaf(-mp_c_, mp_c_, s_tot[2] * i0_);          \
+                const float mq_c_ = s_tot[3] * i0_, vq_ = fmaf(-mq_c_, mq_c_, s_tot[4] * i0_);          \
+                const float cc_ = G.renorm ? C_ : 1.0f;                                                 \
+                float *o_ = A.diag + (size_t)(T) * 6;                                                   \
+                o_[0] = C_;                                                                             \
+                o_[1] = fmaf(mq_c_ + yc, G.dq, G.q_min);                                                \
+                o_[2] = fmaf(mp_c_ + yc, G.dp, G.p_min);                                                \
+                o_[3] = sqrtf(fmaxf(vq_, 0.0f)) * G.dq;                                                 \
+                o_[4] = sqrtf(fmaxf(vp_, 0.0f)) * G.dp;                                                 \
+                o_[5] = s_tot[5] * G.dq / (cc_ * cc_);                                                  \
+            }                                                                                           \
+            __syncthreads();                                                                            \
+        }                                                                                               \
+    } while (0)
+
     for (int step = 0; step < A.nsteps; ++step) {
         VFPS_STAMP(A.dbg, step, 0);
         // ================= phase 1: rotation psi -> the stripe's rows in shared memory, row sums.  Group grp: column tiles grp, grp + 4, ...
+        if (step > 0) {
+            // The halo rows of this step's tiles belong to the stripes above and below: those two CTAs must
+            // have finished the kick of step - 1 (no grid barrier between a kick and the next rotation).  One
+            // poller per CTA, one 128-byte line per flag: hundreds of pollers on a few lines starve the writers.
+            if (tid == 0) {
+                for (int nb = c - 1; nb <= c + 1; nb += 2) {
+                    if (nb < 0 || nb >= (int)gridDim.x) continue;
+                    unsigned int seen;
+                    for (;;) {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(A.flags + 32 * nb) : "memory");
+                        if ((int)(seen - (unsigned int)step) >= 0) break;
+                        __nanosleep(64);
+                    }
+                }
+            }
+            __syncthreads();
+        }
         if (rows > 0) {
-            if (step == 0) G2_ISSUE_FIRST();
+            G2_ISSUE_FIRST();
             int it = 0;
             for (int ct = grp; ct < nct; ct += G2_GROUPS, ++it) {
                 const int b = (nbuf == 2) ? (it & 1) : 0;
@@ -308,19 +380,27 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         }
         VFPS_STAMP(A.dbg, step, 1);
         __syncthreads();
-        if (tid < rows) {
-            float s = 0.0f;
-            for (int k = 0; k < CWR; ++k) s += rowpart[tid * CWR + k];
-            A.rho[r0 + tid] = s * G.dp;
+        for (int r = warp; r < rows; r += G2_WARPS) {          // CWR <= 64 partials per row
+            float s = (lane < CWR) ? rowpart[r * CWR + lane] : 0.0f;
+            if (lane + 32 < CWR) s += rowpart[r * CWR + lane + 32];
+            s = warp_sum(s);
+            if (lane == 0) A.rho[r0 + r] = s * G.dp;
         }
-        __threadfence();
-        grid.sync();
+        grid_barrier(A.bar, bar_gen);
         VFPS_STAMP(A.dbg, step, 2);
         // ================= phase 2: wake of the stripe's rows while its rotated rows stream into shared memory
         float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 pw - -
         if (rows > 0) {
             for (int i = tid; i < N; i += G2_THREADS) srho[i] = __ldcg(A.rho + i);
+            if (tid == 0 && step > 0) {
+                // charge of the previous step: every CTA has added its share before it arrived at this step's barrier
+                const long long q = (long long)__ldcg(A.qacc + (step - 1) % 3);
+                const float f = (float)((double)q * (1.0 / 4294967296.0));
+                s_sc = G.renorm ? 1.0f / ((G.dq * G.dp) * f) : 1.0f;
+                if (blockIdx.x == 0) A.qacc[(step + 1) % 3] = 0ull;      // slot of step - 2: read by everybody before this barrier
+            }
             __syncthreads();
+            if (step > 0) sc = s_sc;
             VFPS_STAMP(A.dbg, step, 3);
             // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4), one row per warp
             for (int r = warp; r < rows; r += G2_WARPS) {
@@ -450,55 +530,33 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             float s = 0.0f;
 #pragma unroll
             for (int w = 0; w < G2_WARPS; ++w) s += red[w * 8 + tid];
-            A.mom_part[(size_t)tid * gridDim.x + blockIdx.x] = s;
+            A.mom_part[((size_t)(step & 1) * G2_NPART + tid) * gridDim.x + blockIdx.x] = s;
             // charge: one 64-bit fixed-point accumulator (integer atomics: exact, order-independent)
-            if (tid == 0) atomicAdd(A.qacc + (step & 1), (unsigned long long)__float2ll_rn(s * 4294967296.0f));
+            if (tid == 0) atomicAdd(A.qacc + step % 3, (unsigned long long)__float2ll_rn(s * 4294967296.0f));
         }
-        // psi of this step is read by the next rotation through TMA (async proxy)
+        // psi of this step is read by the neighbours' next rotation through TMA (async proxy)
         asm volatile("fence.proxy.async;" ::: "memory");
-        __threadfence();
         VFPS_STAMP(A.dbg, step, 5);
-        grid.sync();
-        VFPS_STAMP(A.dbg, step, 6);
-        // the next rotation's first tiles are on their way while C and the diagnostics are formed
-        if (rows > 0 && step + 1 < A.nsteps) G2_ISSUE_FIRST();
-        // ================= phase 3: a6 -- every CTA forms C and 1/C from the same accumulator
+        __syncthreads();
         if (tid == 0) {
-            const long long q = (long long)__ldcg(A.qacc + (step & 1));
-            const float f = (float)((double)q * (1.0 / 4294967296.0));
-            s_tot[0] = f;
-            s_sc = G.renorm ? 1.0f / ((G.dq * G.dp) * f) : 1.0f;
-            if (blockIdx.x == 0) A.qacc[(step + 1) & 1] = 0ull;      // nobody touches it before the next barrier
+            __threadfence();
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(A.flags + 32 * c), "r"((unsigned int)(step + 1)) : "memory");
         }
-        if (blockIdx.x == 0 && warp >= 1 && warp < 6) {              // the other sums, for the diagnostics row
-            const float *mp = A.mom_part + (size_t)warp * gridDim.x;
-            float f = 0.0f;
-#pragma unroll 8
-            for (int i = lane; i < (int)gridDim.x; i += 32) f += __ldcg(mp + i);
-            f = warp_sum(f);
-            if (lane == 0) s_tot[warp] = f;
-        }
-        __syncthreads();
-        if (blockIdx.x == 0 && tid == 0 && A.diag != nullptr) {
-            const float t0 = s_tot[0], i0 = 1.0f / t0;
-            const float C = (G.dq * G.dp) * t0;
-            const float mp_c = s_tot[1] * i0, vp = fmaf(-mp_c, mp_c, s_tot[2] * i0);
-            const float mq_c = s_tot[3] * i0, vq = fmaf(-mq_c, mq_c, s_tot[4] * i0);
-            const float cc = G.renorm ? C : 1.0f;
-            float *o = A.diag + (size_t)step * 6;
-            o[0] = C;
-            o[1] = fmaf(mq_c + yc, G.dq, G.q_min);
-            o[2] = fmaf(mp_c + yc, G.dp, G.p_min);
-            o[3] = sqrtf(fmaxf(vq, 0.0f)) * G.dq;
-            o[4] = sqrtf(fmaxf(vp, 0.0f)) * G.dp;
-            o[5] = s_tot[5] * G.dq / (cc * cc);
-        }
-        sc = s_sc;
-        __syncthreads();
+        // a6 of the previous step: the last CTA (the shortest stripe) writes its diagnostics row; the partial
+        // sums of every CTA were complete at this step's barrier
+        if (step > 0) G2_DIAG(step - 1);
         VFPS_STAMP(A.dbg, step, 7);
     }
+    // ---- the last step's charge and diagnostics
+    grid_barrier(A.bar, bar_gen);
+    if (tid == 0) {
+        const long long q = (long long)__ldcg(A.qacc + (A.nsteps - 1) % 3);
+        const float f = (float)((double)q * (1.0 / 4294967296.0));
+        if (blockIdx.x == 0) A.scale[0] = G.renorm ? 1.0f / ((G.dq * G.dp) * f) : 1.0f;
+    }
+    G2_DIAG(A.nsteps - 1);
+#undef G2_DIAG
 #undef G2_ISSUE_FIRST
-    if (blockIdx.x == 0 && tid == 0) A.scale[0] = sc;
 }
 
 }  // namespace vfps
