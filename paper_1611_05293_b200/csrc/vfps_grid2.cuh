@@ -446,6 +446,24 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             // a warp keeps its column block: column sums serve the p-moments
             const int blk = warp % nct, rstride = G2_WARPS / nct;
             float cs[2][4] = {{0.0f, 0.0f, 0.0f, 0.0f}, {0.0f, 0.0f, 0.0f, 0.0f}};
+            // ... and its Fokker-Planck coefficients (G-1, G0, G1, G2 of kick_fp4) stay in registers for the pass
+            float4 gt[2][4];
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                float cm[4], c0[4], cp[4], c2p[4];
+#pragma unroll
+                for (int cc = 0; cc < 4; ++cc) {
+                    const float c1p = c1 * fmaf((float)(256 * blk + 4 * lane + 128 * k + cc), G.dp, G.p_min);
+                    cm[cc] = fmaf(-2.0f, c1p, c2);
+                    c0[cc] = fmaf(-3.0f, c1p, fmaf(-2.0f, c2, G.fp_b));
+                    cp[cc] = fmaf(6.0f, c1p, c2);
+                    c2p[cc] = -c1p;
+                }
+                gt[k][0] = make_float4(cm[0], cm[1], cm[2], cm[3]);
+                gt[k][1] = make_float4(c0[0], c0[1], c0[2], c0[3]);
+                gt[k][2] = make_float4(cp[0], cp[1], cp[2], cp[3]);
+                gt[k][3] = make_float4(c2p[0], c2p[1], c2p[2], c2p[3]);
+            }
             for (int r = warp / nct; r < rows; r += rstride) {
                 const float4 lw = lds4(sVtab + (uint32_t)r * 32u);
                 float2 mv;
@@ -476,12 +494,9 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll
                     for (int k = 0; k < 2; ++k) {
                         const int g = g0 + 128 * k;
-                        float c1p[4];
-#pragma unroll
-                        for (int cc = 0; cc < 4; ++cc) c1p[cc] = c1 * fmaf((float)(g + cc), G.dp, G.p_min);
-                        if (mm == 0) kick_fp_granule<ORDER, 0, CLAMP>(b[k], l, g, N, G.fp_b, c2, c1p, o[k]);
-                        else if (mm == -1) kick_fp_granule<ORDER, -1, CLAMP>(b[k], l, g, N, G.fp_b, c2, c1p, o[k]);
-                        else kick_fp_granule<ORDER, -2, CLAMP>(b[k], l, g, N, G.fp_b, c2, c1p, o[k]);
+                        if (mm == 0) kick_fp4<ORDER, 0, CLAMP>(b[k], l, g, N, gt[k], o[k]);
+                        else if (mm == -1) kick_fp4<ORDER, -1, CLAMP>(b[k], l, g, N, gt[k], o[k]);
+                        else kick_fp4<ORDER, -2, CLAMP>(b[k], l, g, N, gt[k], o[k]);
                     }
                 } else {
                     const float *rowp = rowsb + r * PITCH + G2_PADC;
