@@ -66,7 +66,7 @@ struct Grid2Args {
 
 struct Grid2Layout {
     int box_rows, pitch, nct;
-    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_rho, off_sw, off_sw2, off_red, off_rows, off_big,
+    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_rho, off_sw, off_sw2, off_vpart, off_red, off_rows, off_big,
         total_floats;
 };
 
@@ -83,8 +83,10 @@ __host__ __device__ inline Grid2Layout grid2_layout(int N, int KRmax, int H, int
     L.off_rowpart = o;  o += (size_t)KRmax * (N / 64);
     L.off_vtab = o;     o += (size_t)((KRmax * 8 + 3) & ~3);
     L.off_rho = o;      o += (size_t)N;
-    L.off_sw = o;       o += (size_t)((N + KRmax + 3) & ~3);
-    L.off_sw2 = o;      o += clamp ? (size_t)((N + KRmax + 3) & ~3) : 0;
+    const int KP = (KRmax + 3) & ~3;
+    L.off_sw = o;       o += (size_t)(N + KP + 4);                // lags of the wake function the stripe's rows touch
+    L.off_sw2 = o;      o += clamp ? (size_t)(N + KP + 4) : 0;    // ... and of the transposed wake
+    L.off_vpart = o;    o += (size_t)8 * KP;                      // wake partial sums [4 quarters (+ 4 transposed)][KP rows]
     L.off_red = o;      o += (size_t)G2_WARPS * 8 + 8;
     L.off_rows = o;     o += (size_t)KRmax * L.pitch;           // the stripe's rotated rows
     o = (o + 31) & ~(size_t)31;                                 // TMA destinations: 128-byte aligned
@@ -183,7 +185,9 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     float *rowpart = smem + LY.off_rowpart;
     float *vtab = smem + LY.off_vtab;
     float *srho = smem + LY.off_rho, *sw = smem + LY.off_sw, *sw2 = smem + LY.off_sw2;
-    float *red = smem + LY.off_red;
+    float *red = smem + LY.off_red, *vpart = smem + LY.off_vpart;
+    const int KP = (KRmax + 3) & ~3;
+    const uint32_t sRho = smem_u32(srho), sSw = smem_u32(sw), sSw2 = smem_u32(sw2);
     float *big = smem + LY.off_big;
     float *rowsb = smem + LY.off_rows;               // [KRmax][PITCH]: the stripe's rotated rows, 8 zero floats each side
     const uint32_t sBig = smem_u32(big), sRows = smem_u32(rowsb), sRowtab = smem_u32(rowtab_s), sRowpart = smem_u32(rowpart), sVtab = smem_u32(vtab);
@@ -199,11 +203,11 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     __syncthreads();
     if (A.wfun != nullptr) {
         // the lags this stripe's rows touch: sw[i] = w at index r0 + i (V_x = sum_x' sw[x - r0 + N - 1 - x'] rho_x');
-        // CLAMP: sw2[i] = w at index N - r0 - KRmax + i (transposed wake: w[x' - x] = sw2[x' + KRmax - 1 - (x - r0)])
-        for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
+        // CLAMP: sw2[i] = w at index N - r0 - KP + i (transposed wake: w[x' - x] = sw2[x' + KP - 1 - (x - r0)])
+        for (int i = tid; i < N + KP + 4; i += G2_THREADS) sw[i] = (r0 + i < 2 * N - 1) ? __ldg(A.wfun + r0 + i) : 0.0f;
         if (CLAMP) {
-            const int base2 = N - r0 - KRmax;
-            for (int i = tid; i < N + KRmax - 1; i += G2_THREADS) {
+            const int base2 = N - r0 - KP;
+            for (int i = tid; i < N + KP + 4; i += G2_THREADS) {
                 const int k = base2 + i;
                 sw2[i] = (k >= 0 && k < 2 * N - 1) ? __ldg(A.wfun + k) : 0.0f;
             }
@@ -402,42 +406,65 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             __syncthreads();
             if (step > 0) sc = s_sc;
             VFPS_STAMP(A.dbg, step, 3);
-            // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4), one row per warp
-            for (int r = warp; r < rows; r += G2_WARPS) {
-                float v0 = 0.0f, v1 = 0.0f, u0 = 0.0f, u1 = 0.0f;
-                if (A.wfun != nullptr) {
-                    const float *wx = sw + (r + N - 1);
-                    for (int xp = lane; xp < N; xp += 64) {
-                        v0 = fmaf(wx[-xp], srho[xp], v0);
-                        v1 = fmaf(wx[-(xp + 32)], srho[xp + 32], v1);
-                    }
-                    if (CLAMP) {
-                        const float *ux = sw2 + (KRmax - 1 - r);
-                        for (int xp = lane; xp < N; xp += 64) {
-                            u0 = fmaf(ux[xp], srho[xp], u0);
-                            u1 = fmaf(ux[xp + 32], srho[xp + 32], u1);
+            // a3: V_x = sum_x' w[x - x'] rho_x' (Eq. 4).  Warp (q, s) = (warp & 3, warp >> 2): the four rows
+            // 4q .. 4q + 3 of the stripe against the quarter s of the profile, 128-bit loads of the wake
+            // function as in the cluster kernel (index A + k - c, A = 3 mod 4); partial sums -> vpart
+            {
+                const int SL = N >> 2, xs = SL * (warp >> 2);
+                for (int q = warp & 3; 4 * q < rows; q += 4) {
+                    float vq[4] = {0.0f, 0.0f, 0.0f, 0.0f}, vt[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+                    if (A.wfun != nullptr) {
+                        for (int xl = 4 * lane; xl < SL; xl += 128) {
+                            const int xp = xs + xl;
+                            const float4 r4 = lds4(sRho + (uint32_t)xp * 4u);
+                            const float rc[4] = {r4.x, r4.y, r4.z, r4.w};
+                            {
+                                const int Aq = 4 * q - xp + N - 1;             // sw[i] = w at index r0 + i
+                                const float4 wl = lds4(sSw + (uint32_t)(Aq - 3) * 4u), wh = lds4(sSw + (uint32_t)(Aq + 1) * 4u);
+                                const float w7[8] = {wl.x, wl.y, wl.z, wl.w, wh.x, wh.y, wh.z, wh.w};
+#pragma unroll
+                                for (int k = 0; k < 4; ++k)
+#pragma unroll
+                                    for (int cc = 0; cc < 4; ++cc) vq[k] = fmaf(w7[3 + k - cc], rc[cc], vq[k]);
+                            }
+                            if (CLAMP) {
+                                const int Bq = xp + KP - 1 - 4 * q;            // sw2[i] = w at index N - r0 - KP + i
+                                const float4 ul = lds4(sSw2 + (uint32_t)(Bq - 3) * 4u), uh = lds4(sSw2 + (uint32_t)(Bq + 1) * 4u);
+                                const float u7[8] = {ul.x, ul.y, ul.z, ul.w, uh.x, uh.y, uh.z, uh.w};
+#pragma unroll
+                                for (int k = 0; k < 4; ++k)
+#pragma unroll
+                                    for (int cc = 0; cc < 4; ++cc) vt[k] = fmaf(u7[3 + cc - k], rc[cc], vt[k]);
+                            }
                         }
                     }
-                }
-                const float Vr = warp_sum(v0 + v1);
-                const float Vtr = CLAMP ? warp_sum(u0 + u1) : 0.0f;
-                if (lane == 0) {
-                    const float V = Vr * sc, rho_x = srho[r0 + r] * sc;
-                    int mm;
-                    float t;
-                    floor_frac(G.kick_c * V, mm, t);
-                    float l[ORDER];
-                    lagrange<ORDER>(t, l);
-                    float pl[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-#pragma unroll
-                    for (int j = 0; j < ORDER; ++j) pl[j] = CLAMP ? l[j] : l[j] * sc;
-                    sts4(sVtab + (uint32_t)r * 32u, make_float4(pl[0], pl[1], pl[2], pl[3]));
-                    if (CLAMP) {
-                        const float Vt = Vtr * sc;
-                        sts4(sVtab + (uint32_t)r * 32u + 16u, make_float4(__int_as_float(mm), -rho_x * Vt, G.dp * (V + Vt), 0.0f));
-                    } else {
-                        sts2(sVtab + (uint32_t)r * 32u + 16u, __int_as_float(mm), rho_x * V);
+                    const float Vr = warp_reduce_transposed<4>(vq, lane);     // lanes 8k .. 8k + 7 hold row 4q + k
+                    const float Vtr = CLAMP ? warp_reduce_transposed<4>(vt, lane) : 0.0f;
+                    if ((lane & 7) == 0) {
+                        vpart[(warp >> 2) * KP + 4 * q + (lane >> 3)] = Vr;
+                        if (CLAMP) vpart[(4 + (warp >> 2)) * KP + 4 * q + (lane >> 3)] = Vtr;
                     }
+                }
+            }
+            __syncthreads();
+            if (tid < rows) {
+                const int r = tid;
+                const float Vr = (vpart[r] + vpart[KP + r]) + (vpart[2 * KP + r] + vpart[3 * KP + r]);
+                const float V = Vr * sc, rho_x = srho[r0 + r] * sc;
+                int mm;
+                float t;
+                floor_frac(G.kick_c * V, mm, t);
+                float l[ORDER];
+                lagrange<ORDER>(t, l);
+                float pl[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+                for (int j = 0; j < ORDER; ++j) pl[j] = CLAMP ? l[j] : l[j] * sc;
+                sts4(sVtab + (uint32_t)r * 32u, make_float4(pl[0], pl[1], pl[2], pl[3]));
+                if (CLAMP) {
+                    const float Vt = ((vpart[4 * KP + r] + vpart[5 * KP + r]) + (vpart[6 * KP + r] + vpart[7 * KP + r])) * sc;
+                    sts4(sVtab + (uint32_t)r * 32u + 16u, make_float4(__int_as_float(mm), -rho_x * Vt, G.dp * (V + Vt), 0.0f));
+                } else {
+                    sts2(sVtab + (uint32_t)r * 32u + 16u, __int_as_float(mm), rho_x * V);
                 }
             }
             __syncthreads();
