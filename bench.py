@@ -36,16 +36,7 @@ if ROOT not in sys.path:
 METRIC = "phase-space cell-updates/s"
 UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_STEP = 8.0     # one fp32 read + one fp32 write per cell per split step
-FMA_OPS_PER_CELL_STEP = 60.0      # FMA-pipe operations per cell per split step
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the ncu
-# --set full captures under profiles/ (psi is loaded once per launch and stays on chip / in L2, so
-# the figure does not depend on the number of steps in the launch)
-NCU_TRAFFIC = {
-    ("C1", "k_cluster_step"): (0.322e6, "profiles/r01_c1_cluster.md"),
-    ("C3", "k_cluster_step"): (77.7e6, "profiles/r01_c1_cluster.md"),
-    ("C4", "k_grid_step"): (18.6e6, "profiles/r01_c4_grid_and_stream.md"),
-}
-
+FMA_OPS_PER_CELL_STEP = 46.0      # FMA-pipe operations per cell per split step where no ncu count is on file
 
 def parse_args():
     ap = argparse.ArgumentParser()
@@ -65,6 +56,7 @@ def parse_args():
     ap.add_argument("--members", type=int, default=0, help="batch members (0 = the workload's own count)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="default C1 line only: skip the C3 and C4 measurements that ride along")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU-oracle sample budget")
     ap.add_argument("--peaks", action="store_true",
                     help="only run the on-chip / L2 / FMA micro-benchmarks (libvfps_peaks.so) and print them")
@@ -206,23 +198,93 @@ def run_reference(args, wl, rank, world):
 # ------------------------------------------------------------------------------------ our arm
 ENGINES = {"auto": 0, "stream": 1, "graph": 2, "cluster": 3, "grid": 4}
 WAKES = {"auto": 0, "fft": 1, "direct": 2}
+NOMINAL_FMA_LANES = 128            # fp32 FMA lanes per SM and clock (4 sub-partitions x 32), B200 guide
 
 
-def run_ours(args, wl, rank, local_rank, world):
+def ncu_counters():
+    """Per (workload, kernel) counters of the committed ncu captures (profiles/r02_ncu_counters.csv,
+    written from the .ncu-rep files named there): DRAM bytes per launch, FMA-pipe operations and
+    thread instructions per cell and step, shared-memory wavefronts per cell and step."""
+    import csv
+    out = {}
+    path = os.path.join(ROOT, "profiles", "r02_ncu_counters.csv")
+    try:
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                out[(row["workload"], row["kernel"])] = row
+    except OSError:
+        pass
+    return out
+
+
+def roofline_block(wl_name, kname, kt_ms, kc, cells, steps_per_launch, sm_max_mhz, sms_used, measured):
+    """Roofline of the dominant kernel.  The persistent kernels keep psi on chip (or in L2): DRAM
+    traffic is a fraction of a per cent of the algorithmic bytes, no memory level is saturated, the
+    FMA pipe and instruction issue are what bound them -- so the primary figure is
+    the ALU one; the 8 B per cell HBM figure and the shared-memory figure ride along."""
+    hbm_peak, peak_src = peaks()
+    cnt = ncu_counters().get((wl_name, kname), {})
+    fma_ops = float(cnt.get("fma_pipe_ops_per_cell_step", 0) or 0) or FMA_OPS_PER_CELL_STEP
+    launch_s = kt_ms / kc * 1e-3
+    cell_steps = cells * steps_per_launch
+    alu_ach = fma_ops * cell_steps / launch_s / 1e9
+    alu_peak = 148 * NOMINAL_FMA_LANES * sm_max_mhz * 1e6 / 1e9
+    rl = {"bound": "alu", "kernel": kname, "achieved": alu_ach, "peak": alu_peak, "unit": "G FMA-pipe op/s",
+          "frac": alu_ach / alu_peak,
+          "peak_source": "148 SMs x 128 fp32 FMA lanes x max SM clock (B200 guide unit counts; DESIGN.md section 8)",
+          "ops_per_cell_step": fma_ops,
+          "ops_source": cnt.get("source", "DESIGN.md section 8 (no ncu capture for this workload / kernel)"),
+          "traffic": float(cnt["dram_bytes_per_launch"]) if cnt.get("dram_bytes_per_launch") else None,
+          "traffic_source": cnt.get("source"),
+          "sms_used": sms_used, "frac_of_sms_used": alu_ach / (alu_peak * sms_used / 148.0),
+          "avg_launch_us": 1e6 * launch_s, "algorithmic_bytes_per_launch": ALG_BYTES_PER_CELL_STEP * cell_steps}
+    hbm_ach = ALG_BYTES_PER_CELL_STEP * cell_steps / launch_s / 1e9
+    rl["hbm"] = {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
+                 "peak_source": peak_src, "bytes_per_cell_step": ALG_BYTES_PER_CELL_STEP}
+    if measured:
+        lanes = measured.get("ffma_shared_operands_lanes_per_clk_sm") or 0.0
+        lanes3 = measured.get("ffma_lanes_per_clk_sm") or 0.0
+        mhz = measured.get("sm_mhz_during_ffma") or sm_max_mhz
+        if lanes > 0:
+            mp = 148 * lanes * mhz * 1e6 / 1e9
+            rl["alu_measured"] = {"peak": mp, "frac": alu_ach / mp, "lanes_per_clk_sm": lanes,
+                                  "peak_three_register_operands": 148 * lanes3 * mhz * 1e6 / 1e9,
+                                  "frac_three_register_operands": alu_ach / (148 * lanes3 * mhz * 1e6 / 1e9) if lanes3 > 0 else None,
+                                  "peak_source": "measured: bench.py --peaks (csrc/peaks/vfps_peaks.cu), FFMA with two operands "
+                                                 "shared by all accumulators / with three distinct register operands"}
+        smem = measured.get("smem_rw_GBs") or 0.0
+        if smem > 0:
+            wf = float(cnt.get("smem_wavefront_bytes_per_cell_step", 0) or 0)
+            oc = {"peak": smem, "unit": "GB/s", "peak_source": "measured: bench.py --peaks, shared-memory read+write stream on every SM",
+                  "algorithmic": {"bytes_per_cell_step": 16.0, "achieved": 16.0 * cell_steps / launch_s / 1e9,
+                                  "frac": 16.0 * cell_steps / launch_s / 1e9 / smem}}
+            if wf > 0:
+                oc["wavefronts"] = {"bytes_per_cell_step": wf, "achieved": wf * cell_steps / launch_s / 1e9,
+                                    "frac": wf * cell_steps / launch_s / 1e9 / smem, "source": cnt.get("source")}
+            rl["onchip"] = oc
+    return rl
+
+
+def time_workload(args, wl, rank, local_rank, world, steps, warmup, do_e2e, measured, strong_members=False):
+    """Device-resident timing (and optionally the end-to-end leg) of one workload; returns the fields
+    of a bench line."""
     import torch
     import paper_1611_05293_b200 as pkg
     from paper_1611_05293_b200 import dist
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the vfps library has no CPU fallback")
-    torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:                                   # replicas: independent simulations per rank
-        wl = wl.with_(seeds=dist.replica_seeds(wl.seeds, rank))
-    members = args.members if args.members > 0 else wl.members
-    idx = list(range(members))
-    if members > wl.members:
+    total_members = args.members if args.members > 0 else wl.members
+    if total_members > wl.members:
         raise SystemExit("--members exceeds the workload's member count")
+    if strong_members and world > 1:
+        idx = dist.shard_members(total_members, rank, world)          # the scan's members dealt out to the ranks
+        if not idx:
+            raise SystemExit("more ranks than batch members")
+    else:
+        if world > 1:                                                 # replicas: independent simulations per rank
+            wl = wl.with_(seeds=dist.replica_seeds(wl.seeds, rank))
+        idx = list(range(total_members))
+    members = len(idx)
     n_inner = args.inner if args.inner > 0 else wl.steps_per_period
     cells = wl.N * wl.N * members
 
@@ -245,7 +307,7 @@ def run_ours(args, wl, rank, local_rank, world):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
     # ---- device-resident timing: W warm-up + K timed bench steps, L2 flushed between them
-    for _ in range(max(args.warmup, 0)):
+    for _ in range(max(warmup, 0)):
         sim.step(n_inner, diag)
     torch.cuda.synchronize()
     dist.barrier()
@@ -254,8 +316,8 @@ def run_ours(args, wl, rank, local_rank, world):
     l0 = sim.launch_count()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for k in range(args.steps):
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for k in range(steps):
         flush.fill_(k & 0xFF)
         ev[k][0].record()
         sim.step(n_inner, diag)
@@ -271,11 +333,12 @@ def run_ours(args, wl, rank, local_rank, world):
     engine, wake = sim.engine_name, sim.wake_name
     cluster_size = sim.cluster_size if engine == "cluster" else None
     cluster_kernel = {1: "k_cluster_step", 3: "k_onchip_step"}.get(sim.cluster_kernel) if engine == "cluster" else None
+    grid_kernel = {1: "k_grid_step", 2: "k_grid2_step"}.get(sim.grid_kernel) if engine == "grid" else None
     diag_last = diag[-1].cpu().numpy().astype(float)
-    value = cells * n_inner * args.steps * world / (ms * 1e-3)
+    all_cells = dist.reduce_sum(float(cells), dev) if world > 1 else float(cells)
+    value = all_cells * n_inner * steps / (ms * 1e-3)
 
     # ---- roofline of the dominant kernel (device events bracketing each launch of that kernel)
-    hbm_peak, peak_src = peaks()
     if not any(c for _, (_, c) in ktimes.items()):
         # engines that replay a graph cannot bracket single kernels: same kernels, stream engine
         sim.set_engine(ENGINES["stream"])
@@ -288,27 +351,24 @@ def run_ours(args, wl, rank, local_rank, world):
         sim.set_engine(ENGINES[args.engine])
     tot = sum(t for _, (t, c) in ktimes.items())
     kname, (kt, kc) = max(ktimes.items(), key=lambda kv: kv[1][0])
-    steps_per_launch = n_inner if (kname.startswith("k_cluster") or kname.startswith("k_grid")) else 1
-    alg_bytes = ALG_BYTES_PER_CELL_STEP * cells * steps_per_launch
-    achieved = alg_bytes / (kt / kc * 1e-3) / 1e9
-    traffic, traffic_src = NCU_TRAFFIC.get((wl.name, kname), (None, None)) if members == wl.members else (None, None)
+    persistent = kname.startswith("k_cluster") or kname.startswith("k_grid")
+    if engine == "cluster":
+        kname = cluster_kernel
+    steps_per_launch = n_inner if persistent else 1
     sm_mhz = clocks.get("sm_max_mhz") or 1965
-    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e9                     # G FMA-pipe lane-operations per second
-    alu_ach = FMA_OPS_PER_CELL_STEP * cells * steps_per_launch / (kt / kc * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                "frac": achieved / hbm_peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
-                "alu": {"achieved": alu_ach, "peak": alu_peak, "unit": "G FMA-pipe op/s", "frac": alu_ach / alu_peak,
-                        "ops_per_cell_step": FMA_OPS_PER_CELL_STEP,
-                        "note": "the path sits at the ridge: 8 B and ~60 fp32 pipe operations per cell per step (DESIGN.md section 8)"},
-                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": 1e3 * kt / kc,
-                "share_of_step": kt / tot if tot > 0 else None,
-                "kernels_ms": {k: {"ms": t, "launches": c} for k, (t, c) in ktimes.items()}}
+    if engine == "cluster":
+        sms_used = min(148, cluster_size * min(members, max(1, 148 // cluster_size)))
+    else:
+        sms_used = 148
+    roofline = roofline_block(wl.name, kname, kt, kc, cells, steps_per_launch, sm_mhz, sms_used, measured)
+    roofline["share_of_step"] = kt / tot if tot > 0 else None
+    roofline["kernels_ms"] = {k: {"ms": t, "launches": c} for k, (t, c) in ktimes.items() if c}
 
     # ---- end to end through the host-pointer entry points (pinned host buffers)
     e2e = None
-    if not args.no_e2e:
+    if do_e2e:
         pin_in = torch.from_numpy(psi0).pin_memory()
-        k_e2e = max(1, min(args.steps, 5))
+        k_e2e = max(1, min(steps, 5))
         sim.set_psi_host(pin_in.numpy()); sim.step_host(n_inner); sim.get_psi_host()     # warm-up
         torch.cuda.synchronize()
         dist.barrier()
@@ -319,10 +379,61 @@ def run_ours(args, wl, rank, local_rank, world):
             psi_host = sim.get_psi_host()
         torch.cuda.synchronize()
         el = dist.reduce_max(time.perf_counter() - t0, dev)
-        e2e = {"value": cells * n_inner * k_e2e * world / el, "unit": UNIT,
+        e2e = {"value": all_cells * n_inner * k_e2e / el, "unit": UNIT,
                "h2d_bytes_per_step": int(psi0.nbytes), "d2h_bytes_per_step": int(psi_host.nbytes + d_host.nbytes),
                "bench_steps": k_e2e, "ms_per_step": 1e3 * el / k_e2e}
     sim.close()
+    del flush, diag
+    torch.cuda.empty_cache()
+    return {
+        "value": value, "ms_per_step": ms / steps, "steps": steps, "warmup": warmup,
+        "steps_per_s": n_inner * steps / (ms * 1e-3), "us_per_split_step": 1e3 * ms / (n_inner * steps),
+        "config": {"workload": wl.name, "N": wl.N, "members": int(round(all_cells / (wl.N * wl.N))),
+                   "members_per_gpu": members, "split_steps_per_bench_step": n_inner,
+                   "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
+                   "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size,
+                   "rotation": "manhattan" if args.manhattan else "standard", "clamp": bool(args.clamp),
+                   "cluster_kernel": cluster_kernel, "grid_kernel": grid_kernel,
+                   "parallelism": "single GPU" if world == 1 else
+                   (f"{world} GPUs, the scan's members dealt out, no collective" if strong_members
+                    else f"{world} independent replicas"),
+                   "l2": "256 MB buffer written between timed bench steps (L2 flush)"},
+        "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "diag_last": {"C": diag_last[0, 0], "sigma_q": diag_last[0, 3], "sigma_p": diag_last[0, 4],
+                      "P_csr": diag_last[0, 5]},
+    }
+
+
+def run_ours(args, wl, rank, local_rank, world):
+    import torch
+    from paper_1611_05293_b200 import dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the vfps library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    torch.zeros(1, device="cuda")
+    measured = None
+    try:
+        measured = measure_peaks()                  # a second or two: on-chip / FMA denominators of this device
+    except Exception as exc:                        # the harness is optional evidence, never the product path
+        measured = None
+        if rank == 0:
+            print(f"bench.py: peaks harness unavailable ({exc})", file=sys.stderr)
+    strong = (wl.members > 1)                       # a batched scan shards its members across GPUs
+    main = time_workload(args, wl, rank, local_rank, world, args.steps, args.warmup, not args.no_e2e, measured, strong)
+
+    # the batched scan (C3) and the large grid (C4) ride along on the default line, so that their
+    # numbers are driver-run too (a few seconds)
+    also = None
+    default_line = (wl.name == "C1" and args.engine == "auto" and not args.manhattan and not args.clamp
+                    and args.members == 0 and args.inner == 0 and not args.cluster_kernel and not args.cluster_size)
+    if default_line and world == 1 and not args.no_also:
+        from workloads import get_workload
+        also = {}
+        for name, k, w in (("C3", 2, 1), ("C4", 3, 1)):
+            r = time_workload(args, get_workload(name), rank, local_rank, world, k, w, False, measured, False)
+            also[name] = {key: r[key] for key in ("value", "ms_per_step", "steps", "warmup", "steps_per_s",
+                                                  "us_per_split_step", "config", "roofline", "gpu_launches", "clocks")}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -333,24 +444,13 @@ def run_ours(args, wl, rank, local_rank, world):
                "sample": f"member 0 of {wl.name}, {n} split steps in {el:.1f} s (double precision, OpenMP)"}
 
     if rank == 0:
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "steps_per_s": n_inner * args.steps / (ms * 1e-3),
-            "us_per_split_step": 1e3 * ms / (n_inner * args.steps),
-            "config": {"workload": wl.name, "N": wl.N, "members": members, "split_steps_per_bench_step": n_inner,
-                       "steps_per_period": wl.steps_per_period, "interp_order": wl.interp_order,
-                       "wake_fft_length": wl.Nf, "engine": engine, "wake": wake, "cluster_size": cluster_size,
-                       "rotation": "manhattan" if args.manhattan else "standard", "clamp": bool(args.clamp),
-                       "cluster_kernel": cluster_kernel,
-                       "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
-                       "l2": "256 MB buffer written between timed bench steps (L2 flush)"},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
-            "clocks": clocks,
-            "diag_last": {"C": diag_last[0, 0], "sigma_q": diag_last[0, 3], "sigma_p": diag_last[0, 4],
-                          "P_csr": diag_last[0, 5]},
-        }
+        line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True,
+                "scaling": "strong" if (strong and world > 1) else "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic", "steps_per_s": main["steps_per_s"], "us_per_split_step": main["us_per_split_step"],
+                "config": main["config"], "roofline": main["roofline"], "cpu_baseline": cpu, "e2e": main["e2e"],
+                "gpu_launches": main["gpu_launches"], "clocks": main["clocks"], "diag_last": main["diag_last"],
+                "measured_peaks": measured, "also": also}
         print(json.dumps(line), flush=True)
 
 

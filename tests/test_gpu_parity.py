@@ -711,17 +711,15 @@ def test_grid_engine(vfps, orc, order, N):
     sim.close()
 
 
-@pytest.mark.parametrize("clamp", [False, True])
-@pytest.mark.parametrize("order", [2, 3, 4])
+@pytest.mark.parametrize("order,clamp", [(2, False), (3, False), (4, False), (3, True), (4, True)])
 @pytest.mark.parametrize("N,spp", [(256, 4000), (512, 4000), (1024, 8000)])
 def test_grid2_engine(vfps, orc, N, spp, order, clamp):
     """TMA-staged kernel of the grid engine (k_grid2_step): asymmetric box (the grid edges cut through
     tiles on all four sides: TMA's zero fill is reading A8), off-centre mismatched bunch, free-space
     wake; stripes of 1-2 (N = 256), 3-4 (512) and 6-7 (1024) rows per CTA, so ragged chunks and
-    stripes shorter than the halo all occur.  1 step and 60 steps with every diagnostics row, then
+    stripes shorter than the halo all occur (the clamp is the identity for linear interpolation, so
+    order 2 runs without the flag only).  1 step and 60 steps with every diagnostics row, then
     hand-over to the first grid kernel and back."""
-    if clamp and order == 2:
-        pytest.skip("the clamp is the identity for linear interpolation: same kernel as without the flag")
     Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
     psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 1e-5, 9, q0=0.5, p0=-0.4)
     if clamp:
