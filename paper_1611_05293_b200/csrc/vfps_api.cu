@@ -544,38 +544,54 @@ void cluster_configure(vfps_sim *h)
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const int cand_single[5] = {16, 8, 4, 2, 1}, cand_batch[5] = {1, 2, 4, 8, 16};
     const int *cand = (h->members == 1) ? cand_single : cand_batch;
-    // in-place design (k_onchip_step, kernel id 3): standard rotation, free or clamped interpolation; AUTO takes it
-    if (h->cl_ver_opt == 0 || h->cl_ver_opt == 3) {
+    // in-place design (k_onchip_step, kernel id 3): standard rotation, free or clamped interpolation
+    auto try_inplace = [&]() -> bool {
         for (int c = 0; c < 5; ++c) {
             const int S = cand[c];
             if (h->cl_S_opt && S != h->cl_S_opt) continue;
             if (!onchip_try(h, S, smem_max)) continue;
             h->cl_S = S; h->cl_ver = 3;
-            return;
+            return true;
         }
-        if (h->cl_ver_opt == 3) { h->cl_why = "second cluster design not feasible for this grid / flags / cluster size"; return; }
-    }
-    // first design (k_cluster_step, kernel id 1): also the Manhattan rotation
-    if (h->P.flags & VFPS_FLAG_CLAMP) { h->cl_why = "the cluster engine implements free (un-clamped) interpolation only"; return; }
-    if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return; }
-    if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return; }
-    for (int c = 0; c < 5; ++c) {
-        const int S = cand[c];
-        if (h->cl_S_opt && S != h->cl_S_opt) continue;
-        if (N / S < (H > 1 ? H : 1) || N % S) continue;
-        const int R = N / S;
-        const size_t bytes = cluster_smem_floats(N, S, H) * sizeof(float);
-        if (bytes > (size_t)smem_max) continue;
-        h->cl_smem = bytes;
-        h->cl_ver = 1;
-        ClusterArgs A{};
-        A.S = S; A.R = R;
-        int mc = 0;
-        cudaError_t e = cluster_launch(h, A, 1, true, &mc);
-        if (e != cudaSuccess || mc < 1) { cudaGetLastError(); continue; }
-        h->cl_S = S; h->cl_max_clusters = mc;
+        return false;
+    };
+    // first design (k_cluster_step, kernel id 1): free interpolation; also the Manhattan rotation
+    auto try_first = [&]() -> bool {
+        if (h->P.flags & VFPS_FLAG_CLAMP) { h->cl_why = "k_cluster_step implements free (un-clamped) interpolation only"; return false; }
+        if (!(N == 32 || N == 64 || N == 128 || N == 256 || N == 512)) { h->cl_why = "cluster engine supports N = 32, 64, 128, 256, 512"; return false; }
+        if (H > CL_PAD) { h->cl_why = "rotation halo exceeds the cluster engine's row padding"; return false; }
+        for (int c = 0; c < 5; ++c) {
+            const int S = cand[c];
+            if (h->cl_S_opt && S != h->cl_S_opt) continue;
+            if (N / S < (H > 1 ? H : 1) || N % S) continue;
+            const int R = N / S;
+            const size_t bytes = cluster_smem_floats(N, S, H) * sizeof(float);
+            if (bytes > (size_t)smem_max) continue;
+            h->cl_smem = bytes;
+            h->cl_ver = 1;
+            ClusterArgs A{};
+            A.S = S; A.R = R;
+            int mc = 0;
+            cudaError_t e = cluster_launch(h, A, 1, true, &mc);
+            if (e != cudaSuccess || mc < 1) { cudaGetLastError(); continue; }
+            h->cl_S = S; h->cl_max_clusters = mc;
+            return true;
+        }
+        h->cl_why = "no feasible cluster size (shared memory or cluster scheduling)";
+        return false;
+    };
+    if (h->cl_ver_opt == 3) {
+        if (!try_inplace()) h->cl_why = "in-place cluster kernel not feasible for this grid / flags / cluster size";
         return;
     }
+    if (h->cl_ver_opt == 1) { try_first(); return; }
+    // AUTO.  A batch: the in-place kernel (a 256^2 member on two CTAs: every SM busy).  One simulation of up to
+    // 256^2 on 16 CTAs is a chain of short phases, where the first design's lighter per-step set-up wins
+    // (measured: C0 1.79 against 2.99 us per step, C1 3.56 against 3.79; 512^2: 9.40 against 9.20).
+    const bool first_preferred = (h->members == 1 && N <= 256);
+    if (first_preferred) { if (try_first()) return; h->cl_ver = 0; if (try_inplace()) { h->cl_why.clear(); return; } return; }
+    if (try_inplace()) return;
+    if (try_first()) return;
     h->cl_ver = 0;
     h->cl_why = "no feasible cluster size (shared memory or cluster scheduling)";
 }

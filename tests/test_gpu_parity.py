@@ -389,23 +389,34 @@ def test_error_paths_on_gpu(vfps):
 # ---------------------------------------------------------------- engines
 def _engine_id(vfps, name):
     return {"stream": vfps.ENGINE_STREAM, "graph": vfps.ENGINE_GRAPH, "cluster": vfps.ENGINE_CLUSTER,
-            "cluster1": vfps.ENGINE_CLUSTER, "grid": vfps.ENGINE_GRID}[name]
+            "cluster3": vfps.ENGINE_CLUSTER, "grid": vfps.ENGINE_GRID, "grid2": vfps.ENGINE_GRID}[name]
 
 
-@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster1", "grid"])
+@pytest.mark.parametrize("engine", ["stream", "graph", "cluster", "cluster3", "grid", "grid2"])
 def test_c1_every_engine_100_steps(vfps, orc, engine):
     """The same 100 steps of C1 through each engine (graph: two replays of 50 captured steps;
-    cluster: the in-place kernel k_onchip_step, which AUTO picks; cluster1: the first design
-    k_cluster_step; grid: the persistent cooperative kernel)."""
+    cluster: what AUTO picks for one 256^2 simulation, the first design k_cluster_step; cluster3:
+    the in-place kernel k_onchip_step; grid / grid2: the two persistent cooperative kernels)."""
     wl = get_workload("C1")
-    sim, psi, d, refs, dr = run_pair(vfps, orc, wl, 100, engine=_engine_id(vfps, engine), diag_every=1,
-                                     cluster_kernel=1 if engine == "cluster1" else None)
-    assert sim.engine_name == engine.rstrip("1")
+    idx = [0]
+    sim = vfps.Simulation.from_workload(wl, idx)
+    if engine == "cluster3":
+        sim.set_cluster_kernel(3)
+    if engine.startswith("grid"):
+        sim.set_grid_kernel(2 if engine == "grid2" else 1)
+    sim.set_engine(_engine_id(vfps, engine))
+    assert sim.engine_name == engine.rstrip("23")
     if engine.startswith("cluster"):
-        assert sim.cluster_kernel == (1 if engine == "cluster1" else 3)
-    assert_psi(psi[0], refs[0].psi, 1e-4, f"C1 100 steps, {engine}")
+        assert sim.cluster_kernel == (3 if engine == "cluster3" else 1)
+    if engine.startswith("grid"):
+        assert sim.grid_kernel == (2 if engine == "grid2" else 1)
+    d = sim.step_host(100)
+    psi = sim.get_psi_host()
+    o = orc.Oracle.from_workload(wl, 0)
+    dr = o.step(100)
+    assert_psi(psi[0], o.psi, 1e-4, f"C1 100 steps, {engine}")
     for i in (0, 1, 49, 50, 99):
-        assert_diag(d[i, 0], dr[0][i])
+        assert_diag(d[i, 0], dr[i])
     sim.close()
 
 
