@@ -59,9 +59,11 @@ enum {
     VFPS_FLAG_RENORMALISE = 1,   /* psi <- psi / C after every step (BASELINE north_star (6)) */
     VFPS_FLAG_CLAMP = 2,         /* clamped interpolation (Eq. 14, read as: limit every
                                     interpolated value to the interval of its bracketing nodes);
-                                    STREAM / GRAPH / GRID engines                                 */
+                                    every engine (with ROT_MANHATTAN: STREAM / GRAPH only); the
+                                    wake must be evaluated by direct convolution                 */
     VFPS_FLAG_ROT_MANHATTAN = 4  /* a1 is the symplectic "Manhattan" rotation (L136): drift along q then
-                                    RF kick along p, two 1-D interpolations; every engine            */
+                                    RF kick along p, two 1-D interpolations; every engine (CLUSTER:
+                                    k_cluster_step, GRID: k_grid_step)                              */
 };
 
 typedef struct vfps_params {
@@ -72,7 +74,7 @@ typedef struct vfps_params {
     double beta;           /* 1/(f_s tau_d): damping per synchrotron period (Eq. 1)          */
     int interp_order;      /* Lagrange points per axis: 2 linear, 3 quadratic, 4 cubic (Eq. 10)  */
     int pad;               /* zero-padding factor of the wake FFT, power of two >= 2             */
-    int members;           /* independent simulations advanced per call, >= 1                    */
+    int members;           /* independent simulations advanced per call, 1 .. 65535              */
     int flags;             /* VFPS_FLAG_*                                                        */
 } vfps_params;
 
@@ -151,9 +153,13 @@ int vfps_set_psi_host(vfps_handle h, const float *psi_host);
 
 /* Advance n >= 0 steps a1..a6.  diag: NULL or [n][members][6] floats; row (i, m) =
  * { C (charge before renormalisation), <q>, <p>, sigma_q, sigma_p, P_csr } after step i.
- * All moments are those of the end-of-step psi.  P_csr is taken from the post-rotation profile of
- * the same step, scaled by 1/C^2 (kick and Fokker-Planck act along p only and leave rho unchanged
- * up to the flux over the p edges of the box).
+ * All moments are those of the end-of-step psi (the STREAM / GRAPH engines take <q>, sigma_q from the
+ * post-rotation profile).  P_csr (Eq. 16-17, normalised as the energy loss per radian) is formed from
+ * the profile the wake acts on in the same step, scaled by 1/C^2: kick and Fokker-Planck act along p
+ * only and leave the profile unchanged up to the charge that crosses the p edges of the box during the
+ * step (< 1e-6 relative for densities that fit their box).  With VFPS_FLAG_CLAMP, where the kick is not
+ * conservative, it is the CSR power of the END-of-step profile rho' to first order in rho' - rho
+ * (transposed wake; the neglected term is quadratic in the change of the profile).
  * Asynchronous on the handle's stream.  vfps_step_host copies diag to host memory and returns
  * when the n steps have completed. */
 int vfps_step(vfps_handle h, int n, float *diag);

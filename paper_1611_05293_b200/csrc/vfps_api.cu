@@ -150,6 +150,7 @@ int validate(const vfps_params *p, std::string &why)
     if (p->pad < 2 || !is_pow2(p->pad)) { why = "pad must be a power of two >= 2"; return VFPS_ERR_ARG; }
     if (!is_pow2((long long)p->N * p->pad)) { why = "N*pad must be a power of two"; return VFPS_ERR_ARG; }
     if (p->members < 1) { why = "members must be >= 1"; return VFPS_ERR_ARG; }
+    if (p->members > 65535) { why = "at most 65535 members per handle (batched launches use gridDim.y = members)"; return VFPS_ERR_UNSUPPORTED; }
     if (p->flags & ~(VFPS_FLAG_RENORMALISE | VFPS_FLAG_CLAMP | VFPS_FLAG_ROT_MANHATTAN)) { why = "unknown flag"; return VFPS_ERR_ARG; }
     if (p->N % 4 != 0) { why = "N must be a multiple of 4 (float4 rows)"; return VFPS_ERR_UNSUPPORTED; }
     if ((long long)p->N * p->pad > 8192) { why = "N*pad > 8192: wake FFT does not fit one CTA's shared memory"; return VFPS_ERR_UNSUPPORTED; }
