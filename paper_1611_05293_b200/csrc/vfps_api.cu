@@ -1004,7 +1004,7 @@ int create_impl(const vfps_params *p, const vfps_complex *Z, bool z_on_host, voi
     h->kfp2_blocks = (N + h->kfp2_rows - 1) / h->kfp2_rows;
     h->wd_blocks = (N + WD_ROWS - 1) / WD_ROWS;
     h->fft_threads = h->Nf / 2 < 1024 ? (h->Nf / 2 < 32 ? 32 : h->Nf / 2) : 1024;
-    h->fft_smem = (size_t)(2 * h->Nf) * sizeof(float2);              // points + per-stage twiddle tables
+    h->fft_smem = (size_t)h->Nf * sizeof(float2);                    // Nf/2 packed points + per-stage twiddle tables
 
 #define CUB(call)                                                                             \
     do {                                                                                      \

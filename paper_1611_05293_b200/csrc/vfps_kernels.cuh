@@ -42,13 +42,19 @@ k_project(GridConst G, const float *__restrict__ psi, const float *__restrict__ 
 }
 
 // ---------------------------------------------------------------- a3: wake by FFT (Eq. 5)
-// One CTA per member, blockDim = min(1024, Nf/2).  Complex radix-2 FFT of length Nf in shared
-// memory (two radix-2 stages per pass in registers): forward decimation-in-frequency (natural in,
-// bit-reversed out), multiply by the
-// Hermitian-extended impedance at the bit-reversed positions, inverse decimation-in-time
-// (bit-reversed in, natural out) -- no permutation pass.  tw[j] = exp(-2 pi i j/Nf), j < Nf/2.
+// One CTA per member, blockDim = min(1024, Nf/4).  The zero-padded profile is real and the impedance
+// Hermitian, so only wave numbers k >= 0 are needed (L149: "a factor of two"): the Nf real samples are
+// packed as M = Nf/2 complex points z[n] = rho[2n] + i rho[2n+1], ONE complex FFT of length M runs in
+// shared memory (two radix-2 stages per pass in registers; forward decimation in frequency, natural
+// in, bit-reversed out), the spectrum R_k, k = 0..M, of the real sequence is split off pairwise
+//     R_k = (A + conj B)/2 - (i/2) w_k (A - conj B),   A = Z_k, B = Z_{M-k},  w_k = exp(-2 pi i k/Nf),
+// multiplied by the impedance, Y_k = Z_k^imp R_k, and packed again for the inverse transform of the
+// real result,  E_k = (Y_k + conj Y_{M-k}) + i conj(w_k) (Y_k - conj Y_{M-k}),  which an inverse
+// decimation-in-time FFT of length M (bit-reversed in, natural out: no permutation pass) turns into
+// V[2n] + i V[2n+1].  tw[j] = exp(-2 pi i j/Nf), j < Nf/2.
 // Outputs: rho[m][x] (summed partials), V[m][x], qstat[m] = { sum rho, sum Xc rho, sum Xc^2 rho,
-// P_raw } with Xc the centred q index and P_raw = (dq/Nf) sum_k Re Z_k |R_k|^2 (Eq. 16-17).
+// P_raw } with Xc the centred q index and P_raw = (dq/Nf) sum_k Re Z_k |R_k|^2 over all Nf wave
+// numbers (Eq. 16-17; k and Nf - k contribute equally).
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 {
     return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
@@ -59,41 +65,47 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *rho_part, int npart
            const float2 *__restrict__ Z, const float2 *__restrict__ tw, float *rho_out /* may be rho_part (nparts = 1) */,
            float *__restrict__ V, float *__restrict__ qstat)
 {
-    extern __shared__ float2 s[];          // Nf points, then Nf - 1 twiddles, one contiguous table per stage
+    extern __shared__ float2 s[];          // M points, then M - 1 twiddles, one contiguous table per stage
     __shared__ float red[4][32];
-    float2 *stw = s + Nf;
+    const int M = Nf >> 1, logM = log2Nf - 1;
+    float2 *stw = s + M;
     const int m = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
     const float xc = 0.5f * (float)(N - 1);
     float s0 = 0, s1 = 0, s2 = 0, pw = 0;
-    for (int x = tid; x < Nf; x += nt) {
-        float r = 0.0f;
-        if (x < N) {
-            const float *pp = rho_part + ((size_t)m * N + x) * nparts;
+    for (int n = tid; n < M; n += nt) {
+        float r[2] = {0.0f, 0.0f};
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int x = 2 * n + h;
+            if (x < N) {
+                const float *pp = rho_part + ((size_t)m * N + x) * nparts;
+                float acc = 0.0f;
 #pragma unroll 8
-            for (int k = 0; k < nparts; ++k) r += pp[k];
-            rho_out[(size_t)m * N + x] = r;
-            const float c = (float)x - xc, t = c * r;
-            s0 += r; s1 += t; s2 = fmaf(t, c, s2);
+                for (int k = 0; k < nparts; ++k) acc += pp[k];
+                rho_out[(size_t)m * N + x] = acc;
+                const float c = (float)x - xc, t = c * acc;
+                s0 += acc; s1 += t; s2 = fmaf(t, c, s2);
+                r[h] = acc;
+            }
         }
-        s[x] = make_float2(r, 0.0f);
+        s[n] = make_float2(r[0], r[1]);
     }
     if (Z != nullptr) {
         const float2 *Zm = Z + (size_t)m * (Nf / 2 + 1);
-        // The twiddles are read 2 log2(Nf) times: stage them once, as one contiguous table per
-        // butterfly span (entry half - 1 + pos = tw[pos * (Nf/2) / half]): reading the single
-        // table with stride (Nf/2)/half put up to 32 lanes on one bank in most stages.
-        for (int j = tid; j < Nf - 1; j += nt) {
+        // The twiddles are read 2 log2(M) times: stage them once, as one contiguous table per
+        // butterfly span (entry half - 1 + pos = exp(-2 pi i pos / (2 half)) = tw[pos * (Nf/2) / half]):
+        // reading the single table with a stride put up to 32 lanes on one bank in most stages.
+        for (int j = tid; j < M - 1; j += nt) {
             const int half = 1 << (31 - __clz(j + 1)), pos = j + 1 - half;
             stw[j] = __ldg(tw + pos * ((Nf >> 1) / half));
         }
         __syncthreads();
-        // forward, decimation in frequency; two radix-2 stages (spans 2q and q) per pass in registers:
-        // half as many passes over shared memory and half as many barriers
-        int half = Nf >> 1;
+        // forward, decimation in frequency; two radix-2 stages (spans 2q and q) per pass in registers
+        int half = M >> 1;
         for (; half >= 2; half >>= 2) {
             const int q = half >> 1;
             const float2 *w2 = stw + (half - 1), *w1 = stw + (q - 1);
-            for (int j = tid; j < (Nf >> 2); j += nt) {
+            for (int j = tid; j < (M >> 2); j += nt) {
                 const int pos = j & (q - 1), i0 = ((j - pos) << 2) + pos, i1 = i0 + q, i2 = i1 + q, i3 = i2 + q;
                 const float2 x0 = s[i0], x1 = s[i1], x2 = s[i2], x3 = s[i3];
                 const float2 u0 = make_float2(x0.x + x2.x, x0.y + x2.y), u1 = make_float2(x1.x + x3.x, x1.y + x3.y);
@@ -107,34 +119,59 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *rho_part, int npart
             }
             __syncthreads();
         }
-        if (half == 1) {                                          // odd log2(Nf): one radix-2 stage left (w = 1)
-            for (int j = tid; j < (Nf >> 1); j += nt) {
+        if (half == 1) {                                          // odd log2(M): one radix-2 stage left (w = 1)
+            for (int j = tid; j < (M >> 1); j += nt) {
                 const float2 u = s[2 * j], v = s[2 * j + 1];
                 s[2 * j] = make_float2(u.x + v.x, u.y + v.y);
                 s[2 * j + 1] = make_float2(u.x - v.x, u.y - v.y);
             }
             __syncthreads();
         }
-        for (int i = tid; i < Nf; i += nt) {                      // x Z, power spectrum
-            const int k = (int)(__brev((unsigned)i) >> (32 - log2Nf));
-            float2 z;
-            if (k <= (Nf >> 1)) {
-                z = __ldg(Zm + k);
-                if (k == 0 || k == (Nf >> 1)) z.y = 0.0f;
-            } else {
-                z = __ldg(Zm + (Nf - k));
-                z.y = -z.y;
+        // split off the spectrum of the real sequence, x Z, power spectrum, pack for the inverse transform;
+        // thread k handles the pair (k, M - k); Z_k of the packed sequence sits at the bit-reversed position
+        for (int k = tid; k <= (M >> 1); k += nt) {
+            const int ia = (int)(__brev((unsigned)k) >> (32 - logM));
+            if (k == 0) {
+                const float2 A = s[ia];
+                const float R0 = A.x + A.y, RM = A.x - A.y;                 // k = 0 and the Nyquist wave number M: real
+                const float z0 = __ldg(Zm).x, zM = __ldg(Zm + M).x;           // their imaginary parts are ignored
+                pw = fmaf(z0, R0 * R0, fmaf(zM, RM * RM, pw));
+                const float Y0 = z0 * R0, YM = zM * RM;
+                s[ia] = make_float2(Y0 + YM, Y0 - YM);                        // E_0 = (Y_0 + Y_M) + i (Y_0 - Y_M)
+                continue;
             }
-            const float2 R = s[i];
-            pw = fmaf(z.x, fmaf(R.x, R.x, R.y * R.y), pw);
-            s[i] = cmul(R, z);
+            const int ib = (int)(__brev((unsigned)(M - k)) >> (32 - logM));
+            const float2 A = s[ia], B = s[ib], w = __ldg(tw + k);
+            // R_k = (A + conj B)/2 - (i/2) w (A - conj B);  R_{M-k} = (B + conj A)/2 + (i/2) conj(w) (B - conj A)
+            const float2 sm = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));      // (A + conj B)/2
+            const float2 df = make_float2(0.5f * (A.x - B.x), 0.5f * (A.y + B.y));      // (A - conj B)/2
+            const float2 t = cmul(w, df);                                                // w (A - conj B)/2
+            const float2 Rk = make_float2(sm.x + t.y, sm.y - t.x);                       // sm - i t
+            // R_{M-k} = conj(sm) + (i/2) conj(w) (B - conj A), and B - conj A = -conj(A - conj B):  = conj(sm) - i conj(t)
+            const float2 Rm = make_float2(sm.x - t.y, -sm.y - t.x);
+            const float2 zk = __ldg(Zm + k), zm = __ldg(Zm + (M - k));
+            pw = fmaf(2.0f * zk.x, fmaf(Rk.x, Rk.x, Rk.y * Rk.y), pw);     // every 0 < k < M stands for k and Nf - k
+            const float2 Yk = cmul(Rk, zk);
+            if (2 * k == M) {
+                // E = (Y + conj Y) + i conj(w) (Y - conj Y), conj(w) = i:  2 Re Y - 2 i ... = (2 Re Y, -2 Im Y)
+                s[ia] = make_float2(2.0f * Yk.x, -2.0f * Yk.y);
+                continue;
+            }
+            pw = fmaf(2.0f * zm.x, fmaf(Rm.x, Rm.x, Rm.y * Rm.y), pw);
+            const float2 Ym = cmul(Rm, zm);
+            // E_k = (Y_k + conj Y_m) + i conj(w) (Y_k - conj Y_m);  E_{M-k} = (Y_m + conj Y_k) - i w (Y_m - conj Y_k)
+            const float2 sp = make_float2(Yk.x + Ym.x, Yk.y - Ym.y), dm = make_float2(Yk.x - Ym.x, Yk.y + Ym.y);
+            const float2 u = cmul(make_float2(w.x, -w.y), dm);                           // conj(w) (Y_k - conj Y_m)
+            s[ia] = make_float2(sp.x - u.y, sp.y + u.x);                                 // sp + i u
+            // Y_m - conj Y_k = -conj(dm):  -i w (-conj dm) = i w conj(dm) = i conj(conj(w) dm) = i conj(u)
+            s[ib] = make_float2(sp.x + u.y, -sp.y + u.x);                                // conj(sp) + i conj(u)
         }
         __syncthreads();
-        // inverse, decimation in time, mirrored: the single radix-2 stage first if log2(Nf) is odd,
+        // inverse, decimation in time, mirrored: the single radix-2 stage first if log2(M) is odd,
         // then spans q and 2q per pass
         int hq = 1;
-        if (log2Nf & 1) {
-            for (int j = tid; j < (Nf >> 1); j += nt) {
+        if (logM & 1) {
+            for (int j = tid; j < (M >> 1); j += nt) {
                 const float2 u = s[2 * j], v = s[2 * j + 1];
                 s[2 * j] = make_float2(u.x + v.x, u.y + v.y);
                 s[2 * j + 1] = make_float2(u.x - v.x, u.y - v.y);
@@ -142,9 +179,9 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *rho_part, int npart
             __syncthreads();
             hq = 2;
         }
-        for (int q = hq; q <= (Nf >> 2); q <<= 2) {
+        for (int q = hq; q <= (M >> 2); q <<= 2) {
             const float2 *w1 = stw + (q - 1), *w2 = stw + (2 * q - 1);
-            for (int j = tid; j < (Nf >> 2); j += nt) {
+            for (int j = tid; j < (M >> 2); j += nt) {
                 const int pos = j & (q - 1), i0 = ((j - pos) << 2) + pos, i1 = i0 + q, i2 = i1 + q, i3 = i2 + q;
                 float2 wq = w1[pos], wa = w2[pos], wb = w2[pos + q];
                 wq.y = -wq.y; wa.y = -wa.y; wb.y = -wb.y;
@@ -161,7 +198,11 @@ k_wake_fft(int N, int Nf, int log2Nf, float dq, const float *rho_part, int npart
             __syncthreads();
         }
         const float inv = 1.0f / (float)Nf;
-        for (int x = tid; x < N; x += nt) V[(size_t)m * N + x] = s[x].x * inv;
+        for (int n = tid; 2 * n < N; n += nt) {
+            const float2 v = s[n];
+            V[(size_t)m * N + 2 * n] = v.x * inv;
+            if (2 * n + 1 < N) V[(size_t)m * N + 2 * n + 1] = v.y * inv;
+        }
     } else {
         for (int x = tid; x < N; x += nt) V[(size_t)m * N + x] = 0.0f;
     }
