@@ -501,9 +501,12 @@ k_onchip_step(GridConst G, OnchipArgs A)
     constexpr int O0 = (ORDER - 1) / 2;
     constexpr int CW = N / 64;
     constexpr int CH = oc_chunk_rows(ORDER);
-    constexpr int NG = (N >= 128) ? N / 128 : 1;           // 4-cell granules per lane and row: columns 4 lane + 128 k
+    // kick pass: a warp takes a block of up to 256 columns of a row; a lane owns the 4-cell granules 4 lane + 128 k
+    // of the block.  N = 512: two warps per row, each keeps its half for the whole pass, so the Fokker-Planck
+    // coefficients of a lane's columns (2 x 4 float4) stay in registers for every N.
+    constexpr int NBLK = (N > 256) ? N / 256 : 1;          // column blocks (= warps) per row
+    constexpr int NG = (N >= 256) ? 2 : 1;                 // granules per lane and block
     constexpr int KL = (N >= 128) ? 32 : N / 4;            // active lanes in the kick pass
-    constexpr bool GREG = (NG <= 2);                       // Fokker-Planck coefficients of the lane's columns stay in registers
     constexpr int NW = N / 128 > 0 ? N / 128 : 1;          // float4 groups of rho per lane in the wake
     constexpr unsigned FULL = 0xffffffffu;
     using Wk = Walker<ORDER, PITCH, TAB, CLAMP>;
@@ -904,19 +907,19 @@ k_onchip_step(GridConst G, OnchipArgs A)
 #pragma unroll
                     for (int c = 0; c < 4; ++c) cs[k][c] = 0.0f;
                 float q1 = 0.0f, q2 = 0.0f, pw = 0.0f;
-                // Fokker-Planck coefficients of the lane's columns: registers for the whole pass when a lane
-                // owns at most two granules per row, re-read per granule otherwise (N = 512: 64 registers too many)
-                float4 gt[GREG ? NG : 1][4];
-                if (GREG && lane < KL) {
+                const int blk = warp % NBLK;                  // this warp's column block
+                // Fokker-Planck coefficients of the lane's columns: registers for the whole pass
+                float4 gt[NG][4];
+                if (lane < KL) {
 #pragma unroll
                     for (int k = 0; k < NG; ++k)
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) gt[k][j] = lds4(sGtab + (uint32_t)((j * N + 4 * lane + 128 * k) * 4));
+                        for (int j = 0; j < 4; ++j) gt[k][j] = lds4(sGtab + (uint32_t)((j * N + 256 * blk + 4 * lane + 128 * k) * 4));
                 }
                 const uint32_t mbUp = (rank > 0) ? mapa(mbHalo, rank - 1) : 0u, mbDn = (rank < S - 1) ? mapa(mbHalo, rank + 1) : 0u;
-                const uint32_t lane_off = (uint32_t)(16 * lane);
-                float Xf = (float)(x0 + warp) - xc;
-                for (int r = warp; r < R; r += OC_WARPS, Xf += (float)OC_WARPS) {
+                const uint32_t lane_off = (uint32_t)(1024 * blk + 16 * lane);
+                float Xf = (float)(x0 + warp / NBLK) - xc;
+                for (int r = warp / NBLK; r < R; r += OC_WARPS / NBLK, Xf += (float)(OC_WARPS / NBLK)) {
                     const float4 lw = lds4(sVtab + (uint32_t)r * 32u);
                     float2 mv;
                     float dpU = 0.0f;                          // CLAMP: dp (V + Vt) of the row
@@ -946,23 +949,17 @@ k_onchip_step(GridConst G, OnchipArgs A)
                                 }
 #pragma unroll
                             for (int k = 0; k < NG; ++k) {
-                                const int g = 4 * lane + 128 * k;
-                                float4 gl[4];
-                                if (!GREG) {
-#pragma unroll
-                                    for (int j = 0; j < 4; ++j) gl[j] = lds4(sGtab + (uint32_t)((j * N + g) * 4));
-                                }
-                                const float4(&gk)[4] = GREG ? gt[GREG ? k : 0] : gl;
-                                if (mm == 0) kick_fp4<ORDER, 0, CLAMP>(b[k], l, g, N, gk, o[k]);
-                                else if (mm == -1) kick_fp4<ORDER, -1, CLAMP>(b[k], l, g, N, gk, o[k]);
-                                else kick_fp4<ORDER, -2, CLAMP>(b[k], l, g, N, gk, o[k]);
+                                const int g = 256 * blk + 4 * lane + 128 * k;
+                                if (mm == 0) kick_fp4<ORDER, 0, CLAMP>(b[k], l, g, N, gt[k], o[k]);
+                                else if (mm == -1) kick_fp4<ORDER, -1, CLAMP>(b[k], l, g, N, gt[k], o[k]);
+                                else kick_fp4<ORDER, -2, CLAMP>(b[k], l, g, N, gt[k], o[k]);
                             }
                         } else {
                             const float *rowp = buf + ((ra.x - pshift) >> 2);
 #pragma unroll
                             for (int k = 0; k < NG; ++k) {
                                 float tmp[4];
-                                kick_fp4_any<ORDER, CLAMP>(rowp, lw, mm, 4 * lane + 128 * k, N, gtab, tmp);
+                                kick_fp4_any<ORDER, CLAMP>(rowp, lw, mm, 256 * blk + 4 * lane + 128 * k, N, gtab, tmp);
 #pragma unroll
                                 for (int c = 0; c < 4; ++c) o[k][c] = tmp[c];
                             }
@@ -974,7 +971,8 @@ k_onchip_step(GridConst G, OnchipArgs A)
                                 for (int c = 0; c < 4; ++c) o[k][c] *= sc;
                         }
                     }
-                    __syncwarp();                              // every lane has read the row before anyone overwrites it
+                    // every lane has read the row before anyone overwrites it (N = 512: both warps of the row)
+                    if (NBLK > 1) named_barrier(8 + warp / NBLK, 32 * NBLK); else __syncwarp();
                     if (lane < KL) {
 #pragma unroll
                         for (int k = 0; k < NG; ++k) sts4(own + (uint32_t)(512 * k), make_float4(o[k][0], o[k][1], o[k][2], o[k][3]));
@@ -1013,7 +1011,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
                         const float tq = q0 * Xf;
                         q1 += tq; q2 = fmaf(tq, Xf, q2);
                         if (CLAMP) pw = fmaf(q0, dpU, pw);
-                        if (lane == 0) pw += mv.y;
+                        if (lane == 0 && blk == 0) pw += mv.y;
                     }
                 }
                 OC_STAMP(6);
@@ -1024,7 +1022,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
                     for (int k = 0; k < NG; ++k)
 #pragma unroll
                         for (int c = 0; c < 4; ++c) {
-                            const float yy = (float)(4 * lane + 128 * k + c) - yc;
+                            const float yy = (float)(256 * blk + 4 * lane + 128 * k + c) - yc;
                             const float tt = cs[k][c] * yy;
                             v8[0] += cs[k][c]; v8[1] += tt; v8[2] = fmaf(tt, yy, v8[2]);
                         }
