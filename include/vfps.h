@@ -107,8 +107,9 @@ enum {
     VFPS_NUM_KERNELS = 7
 };
 enum {
-    VFPS_ENGINE_AUTO = 0,     /* CLUSTER if the grid fits on chip, else GRID (one simulation) or
-                                 GRAPH (a batch)                                                 */
+    VFPS_ENGINE_AUTO = 0,     /* one simulation with N >= 512: GRID where its TMA kernel is
+                                 feasible; else CLUSTER if the grid fits on chip, else GRID (one
+                                 simulation) or GRAPH (a batch)                                  */
     VFPS_ENGINE_STREAM = 1,   /* one launch per kernel per step on the stream                    */
     VFPS_ENGINE_GRAPH = 2,    /* the same kernels replayed from a CUDA graph of many steps       */
     VFPS_ENGINE_CLUSTER = 3,  /* persistent thread-block-cluster kernel, psi resident in

@@ -925,7 +925,9 @@ int resolved_engine(const vfps_sim *h)
     if (h->engine_opt == VFPS_ENGINE_GRAPH) return VFPS_ENGINE_GRAPH;
     if (h->engine_opt == VFPS_ENGINE_GRID) return VFPS_ENGINE_GRID;
     if (h->engine_opt == VFPS_ENGINE_CLUSTER) return VFPS_ENGINE_CLUSTER;
-    // AUTO: on-chip grids -> cluster; one large simulation -> cooperative grid; else graph replay
+    // AUTO: on-chip grids -> cluster; one large simulation -> cooperative grid; else graph replay.
+    // One 512^2 simulation: the TMA-staged grid kernel on 148 SMs beats the cluster of 16 (8.3 against 8.85 us per step)
+    if (h->members == 1 && h->N >= 512 && h->g2_blocks > 0 && h->gr_ver_opt != 1) return VFPS_ENGINE_GRID;
     if (h->cl_S > 0) return VFPS_ENGINE_CLUSTER;
     return (h->gr_blocks > 0 || h->g2_blocks > 0) ? VFPS_ENGINE_GRID : VFPS_ENGINE_GRAPH;
 }
