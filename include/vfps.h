@@ -59,7 +59,7 @@ enum {
     VFPS_FLAG_RENORMALISE = 1,   /* psi <- psi / C after every step (BASELINE north_star (6)) */
     VFPS_FLAG_CLAMP = 2,         /* clamped interpolation (Eq. 14, read as: limit every
                                     interpolated value to the interval of its bracketing nodes);
-                                    every engine (with ROT_MANHATTAN: STREAM / GRAPH only); the
+                                    every engine (with ROT_MANHATTAN: STREAM / GRAPH / GRID); the
                                     wake must be evaluated by direct convolution                 */
     VFPS_FLAG_ROT_MANHATTAN = 4  /* a1 is the symplectic "Manhattan" rotation (L136): drift along q then
                                     RF kick along p, two 1-D interpolations; every engine (CLUSTER:

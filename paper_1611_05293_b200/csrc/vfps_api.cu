@@ -631,10 +631,6 @@ const void *grid_kernel(const vfps_sim *h)
 void grid_configure(vfps_sim *h)
 {
     h->gr_blocks = 0; h->gr_why.clear();
-    if ((h->P.flags & VFPS_FLAG_ROT_MANHATTAN) && (h->P.flags & VFPS_FLAG_CLAMP)) {
-        h->gr_why = "Manhattan rotation with clamped interpolation needs the profile after the RF kick (stream / graph engines)";
-        return;
-    }
     if (h->members != 1) { h->gr_why = "grid engine advances one simulation per handle"; return; }
     int dev = 0, coop = 0, sms = 0;
     cudaGetDevice(&dev);

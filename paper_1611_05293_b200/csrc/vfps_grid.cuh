@@ -16,7 +16,8 @@
 //            CTAs fed with integer atomics in phase 2 (exact, order-independent) -> C, 1/C;
 //            CTA 0 sums the other partial sums in a fixed order and writes the diagnostics row.
 // With VFPS_FLAG_ROT_MANHATTAN (template MANH) phase 1 is the drift (1-D shift along q) and phase 2
-// applies the RF kick before the wake kick (vfps_stream2.cuh: k_drift2, rf_stage).
+// applies the RF kick before the wake kick (vfps_stream2.cuh: k_drift2, rf_stage); with CLAMP as well the
+// profile is that of the RF-kicked rows, formed by their owners behind a third grid barrier.
 // Template CLAMP: clamped interpolation (Eq. 14, reading A9) in every interpolation of the step.
 // One simulation per handle (members == 1); batches of on-chip grids use the cluster engine.
 #pragma once
@@ -163,7 +164,7 @@ k_grid_step(GridConst G, GridArgs A)
             const float tot = warp_reduce8(out, lane);
             if ((lane & 3) == 0) redt[k & 1][((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)][warp] = tot;
             __syncthreads();
-            if (tid < GR_RT && xg + tid < N) {
+            if (!(MANH && CLAMP) && tid < GR_RT && xg + tid < N) {
                 float s = 0.0f;
 #pragma unroll
                 for (int w = 0; w < GR_WARPS; ++w) s += redt[k & 1][tid][w];
@@ -173,8 +174,27 @@ k_grid_step(GridConst G, GridArgs A)
         VFPS_STAMP(A.dbg, step, 1);
         grid.sync();
         VFPS_STAMP(A.dbg, step, 2);
-        // ================= phase 2: profile, wake, kick + Fokker-Planck of the rows r0 .. r1-1
         const int r0 = blockIdx.x * A.KR, r1 = min(N, r0 + A.KR);
+        if constexpr (MANH && CLAMP) {
+            // The clamped RF kick does not conserve the row sums, and the wake acts on the profile AFTER
+            // it (L136 order drift, RF kick, wake kick): row sums of the RF-kicked rows r0 .. r1-1 (as
+            // k_rf_profile), then one more grid barrier before anybody reads the profile.
+            for (int r = warp; r < r1 - r0; r += GR_WARPS) {
+                const int x = r0 + r;
+                const float *row = A.psi_tmp + (size_t)x * N;
+                int mm1;
+                float t1;
+                floor_frac(G.mh_p * ((float)x + G.x0c), mm1, t1);
+                float l1[ORDER];
+                lagrange<ORDER>(t1, l1);
+                float s = 0.0f;
+                for (int y = lane; y < N; y += 32) s += rf_value<ORDER, true>(row, N, y, mm1, l1);
+                s = warp_sum(s);
+                if (lane == 0) A.rho_part[x] = G.dp * s;
+            }
+            grid.sync();
+        }
+        // ================= phase 2: profile, wake, kick + Fokker-Planck of the rows r0 .. r1-1
         float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};   // s0 s1 s2 q1 q2 pw - -
         if (r0 < N) {
             for (int x4 = tid; x4 < NQ; x4 += 2 * GR_THREADS) {   // two columns of float4 per pass: up to
@@ -182,7 +202,7 @@ k_grid_step(GridConst G, GridArgs A)
                 const bool two = (x4b < NQ);
                 float4 r = make_float4(0.0f, 0.0f, 0.0f, 0.0f), q = r;
 #pragma unroll 8
-                for (int k = 0; k < A.tiles_y; ++k) {
+                for (int k = 0; k < ((MANH && CLAMP) ? 1 : A.tiles_y); ++k) {
                     const float4 *pk = reinterpret_cast<const float4 *>(A.rho_part + (size_t)k * N);
                     const float4 v = __ldcg(pk + x4);
                     const float4 u = two ? __ldcg(pk + x4b) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);

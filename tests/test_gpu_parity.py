@@ -542,7 +542,7 @@ def test_clamped_interpolation(vfps, orc, order, N, manhattan):
     """VFPS_FLAG_CLAMP (Eq. 14, reading A9) against the oracle's clamped step, standard
     and Manhattan rotation.  The input is a bunch with a sharp-edged hole, where the free cubic /
     quadratic interpolant overshoots and the clamp is active in thousands of cells; stream engine
-    for 1 step, graph for 29 more, grid engine (standard rotation) for 10 more.  The clamped and the free run must
+    for 1 step, graph for 29 more, grid engine for 10 more.  The clamped and the free run must
     differ (the flag does something) and the clamped density never leaves [0, max psi_0]."""
     Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, None)[None, :]
     psi0 = make_psi0(N, -5.0, 7.0, -6.5, 5.5, 1.2, 0.8, 0.0, 9, q0=0.5, p0=-0.4)
@@ -578,14 +578,10 @@ def test_clamped_interpolation(vfps, orc, order, N, manhattan):
     dr = o.step(29)
     assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, f"clamp N={N} order={order} manhattan={manhattan} 30 steps")
     assert_diag(d[28, 0], dr[28])
-    if manhattan:
-        # the clamped RF kick changes the profile, so the wake needs the profile after it: only the
-        # stream / graph engines have that extra pass
-        with pytest.raises(vfps.VfpsError) as e:
-            sim.set_engine(vfps.ENGINE_GRID)
-        assert e.value.code == -5
-    else:
-        sim.set_engine(vfps.ENGINE_GRID)
+    # (Manhattan: the clamped RF kick changes the profile, so the wake needs the profile after it --
+    # an extra pass in the stream / graph engines, a third grid barrier in k_grid_step)
+    sim.set_engine(vfps.ENGINE_GRID)
+    assert sim.engine_name == "grid" and (sim.grid_kernel == 1 if manhattan else sim.grid_kernel in (1, 2))
     d = sim.step_host(10)
     dr = o.step(10)
     psi = sim.get_psi_host()[0]
