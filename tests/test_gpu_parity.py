@@ -23,6 +23,81 @@ def assert_psi(sim_psi, ref_psi, tol, what=""):
     return err
 
 
+def test_maximum_grid_4096(vfps, orc):
+    """The largest grid the library accepts (N * pad = 8192 is the limit of the wake FFT's shared
+    memory): 4096^2, asymmetric box, cubic interpolation, parallel-plates wake.  AUTO (the grid engine)
+    for 1 and 4 more steps, then the stream engine with the FFT wake at its maximum
+    length for 2 more, every cell against the oracle."""
+    N, spp = 4096, 16000
+    box = (-5.0, 7.0, -6.5, 5.5)
+    Z = make_impedance(N, 2, 12.0 / (N - 1), 0.4, 0.8)[None, :]
+    psi0 = make_psi0(N, *box, 1.1, 0.9, 0.0, 5, q0=0.4, p0=-0.3)[None]
+    sim = vfps.Simulation(N, *box, spp, 2e-3, 4, 2, 1, Z=Z)
+    sim.set_psi_host(psi0)
+    o = orc.Oracle(N, *box, spp, 2e-3, 4, 2, Z[0])
+    o.set_psi(psi0[0])
+    # a stripe of 4096 / 148 = 28 rows of 4096 cells does not fit the shared memory of an SM: the TMA-staged
+    # kernel is refused and AUTO takes the first grid kernel (psi through L2)
+    assert sim.engine_name == "grid" and sim.grid_kernel == 1
+    with pytest.raises(vfps.VfpsError) as e:
+        sim.set_grid_kernel(2)
+    assert e.value.code == -5
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, "4096^2, 1 step")
+    assert_diag(d[0, 0], dr[0])
+    d = sim.step_host(4)
+    dr = o.step(4)
+    assert_psi(sim.get_psi_host()[0], o.psi, 2e-5, "4096^2, 5 steps")
+    assert_diag(d[3, 0], dr[3])
+    sim.set_engine(vfps.ENGINE_STREAM)
+    sim.set_wake_mode(vfps.WAKE_FFT)
+    d = sim.step_host(2)
+    dr = o.step(2)
+    assert sim.wake_name == "fft"
+    assert_psi(sim.get_psi_host()[0], o.psi, 3e-5, "4096^2, 7 steps, FFT wake of length 8192")
+    assert_diag(d[1, 0], dr[1])
+    sim.close()
+    with pytest.raises(vfps.VfpsError) as e:
+        vfps.Simulation(8192, *box, spp, 2e-3, 4, 2, 1)
+    assert e.value.code == -5
+
+
+@pytest.mark.parametrize("engine", ["stream", "cluster", "cluster3", "grid", "grid2"])
+@pytest.mark.parametrize("order", [3, 4])
+def test_single_cell_density_and_zero_steps(vfps, orc, engine, order):
+    """Degenerate inputs: all of the charge in ONE cell (after a step the density is the 4 x 4 / 3 x 3
+    stencil of Lagrange weights around the image of that cell, positive and negative lobes included, then
+    the kick of a one-row profile) and a vfps_step of zero steps (no change, nothing written)."""
+    N, spp = 256, 4000
+    Z = make_impedance(N, 2, 12.0 / (N - 1), 0.05, 0.8)[None, :]
+    psi0 = np.zeros((1, N, N), dtype=np.float32)
+    psi0[0, 171, 90] = 1.0 / (12.0 / (N - 1)) ** 2
+    sim = vfps.Simulation(N, -6, 6, -6, 6, spp, 1e-3, order, 2, 1, Z=Z)
+    if engine in ("cluster", "cluster3"):
+        sim.set_cluster_kernel(1 if engine == "cluster" else 3)
+    if engine in ("grid", "grid2"):
+        sim.set_grid_kernel(1 if engine == "grid" else 2)
+    sim.set_engine(_engine_id(vfps, engine))
+    sim.set_psi_host(psi0)
+    d0 = sim.step_host(0)
+    assert d0.shape[0] == 0
+    np.testing.assert_array_equal(sim.get_psi_host(), psi0)
+    o = orc.Oracle(N, -6, 6, -6, 6, spp, 1e-3, order, 2, Z[0])
+    o.set_psi(psi0[0])
+    d = sim.step_host(1)
+    dr = o.step(1)
+    psi = sim.get_psi_host()[0]
+    assert_psi(psi, o.psi, TOL_1, f"single cell, {engine}, order {order}, 1 step")
+    assert (psi != 0).sum() <= 6 * (order + 3) and psi.min() < 0          # the stencil and nothing else
+    d = sim.step_host(20)
+    dr = o.step(20)
+    assert_psi(sim.get_psi_host()[0], o.psi, 5e-5, f"single cell, {engine}, order {order}, 21 steps")
+    # sigma of a few-cell density is a difference of nearly equal sums: absolute tolerance in cells
+    assert abs(d[19, 0, 0] - dr[19][0]) < 1e-4 and abs(d[19, 0, 1] - dr[19][1]) < 1e-3 * 12.0 / (N - 1)
+    sim.close()
+
+
 def edge_flux_tol(C):
     """P_csr of a step is formed from the profile the wake acts on, renormalised by the step's
     charge: P = dq sum rho_x V_x / C^2 (include/vfps.h).  Kick and Fokker-Planck move charge along p
