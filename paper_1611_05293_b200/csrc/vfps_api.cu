@@ -725,7 +725,7 @@ int grid2_configure(vfps_sim *h)
         h->g2_why = "cuTensorMapEncodeTiled failed"; return VFPS_OK;
     }
     // ---- tables, in double, rounded once
-    std::vector<float> col((size_t)nb * N * OC_COLTAB, 0.0f), row((size_t)N * OC_ROWTAB, 0.0f);
+    std::vector<float> col((size_t)nb * N, 0.0f), row((size_t)N * OC_ROWTAB, 0.0f);
     std::vector<int> cix((size_t)nb * N, OC_BAD);
     const double Ymid = 0.5 * (double)(N - 1) + g.y0c;
     for (int c = 0; c < nb; ++c) {
@@ -736,10 +736,7 @@ int grid2_configure(vfps_sim *h)
             const double f0 = std::floor(g.a * Xlo + g.b * Y), f1 = std::floor(g.a * Xhi + g.b * Y);
             if (f0 != f1) continue;
             cix[(size_t)c * N + y] = (int)f0;
-            double l[4] = {0, 0, 0, 0}, lp[4] = {0, 0, 0, 0};
-            lagrange_d(order, g.a * Xc + g.b * Y - f0, l, lp);
-            float *t = &col[((size_t)c * N + y) * OC_COLTAB];
-            for (int i = 0; i < 4; ++i) { t[i] = (float)l[i]; t[4 + i] = (float)lp[i]; }
+            col[(size_t)c * N + y] = (float)(g.a * Xc + g.b * Y - f0);     // the kernel forms M, M' from it (Eq. 13)
         }
         for (int x = r0; x < r0 + nr; ++x) {
             const double X = (double)x + g.x0c;

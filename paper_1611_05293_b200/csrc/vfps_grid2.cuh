@@ -51,7 +51,7 @@ struct Grid2Args {
     float *rho;            // [N] profile of the step (dp * row sums, un-scaled)
     float *mom_part;       // [2][G2_NPART][gridDim.x], by step parity
     float *diag;           // [nsteps][1][6] or nullptr
-    const float *coltab;   // [gridDim.x][N][8]: M[4], M'[4] of column y for the rows of stripe c
+    const float *coltab;   // [gridDim.x][N]: fractional source position along q of column y at the centre row of stripe c
     const int *colix;      // [gridDim.x][N]: floor(dx) of column y over the rows of stripe c, or OC_BAD
     const float *rowtab;   // [N][12]: as in the cluster kernel (a (X - Xc) relative to the stripe's centre row)
     unsigned long long *qacc;   // [3] charge of step t in slot t % 3, 32.32 fixed point, zero at launch
@@ -124,6 +124,23 @@ __device__ __forceinline__ void grid_barrier(unsigned int *ctr, unsigned int &ge
         __threadfence();
     }
     __syncthreads();
+}
+
+// d l_k / dt of the Lagrange weights (Eq. 13); multiplies a (X - Xc) ~ 1e-6 in the row-wise first-order correction
+template <int ORDER>
+__device__ __forceinline__ void lagrange_deriv(float t, float (&lp)[ORDER])
+{
+    if (ORDER == 2) {
+        lp[0] = -1.0f; lp[1] = 1.0f;
+    } else if (ORDER == 3) {
+        lp[0] = t - 0.5f; lp[1] = -2.0f * t; lp[ORDER - 1] = t + 0.5f;
+    } else {
+        const float t2 = 3.0f * t * t;
+        lp[0] = -(t2 - 6.0f * t + 2.0f) * (1.0f / 6.0f);
+        lp[1] = (t2 - 4.0f * t - 1.0f) * 0.5f;
+        lp[ORDER - 2] = -(t2 - 2.0f * t - 2.0f) * 0.5f;
+        lp[ORDER - 1] = (t2 - 1.0f) * (1.0f / 6.0f);
+    }
 }
 
 // one cell of a tile with its own floors (a floor changes inside the warp's columns or the chunk)
@@ -223,6 +240,17 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     const float yc = 0.5f * (float)(N - 1);
     const float c1 = G.fp_b / (6.0f * G.dp), c2 = G.fp_b / (G.dp * G.dp);
     float sc = G.renorm ? A.scale[0] : 1.0f;
+    // column data of the group's NEXT tile (cyclic: after the last tile of a step comes the first of the next):
+    // two 64-bit loads, issued a whole tile ahead of their use (L2 latency off the tile-to-tile path)
+    float2 tnx = make_float2(0.0f, 0.0f);
+    int2 inx = make_int2(OC_BAD, OC_BAD);
+#define G2_COL_FETCH(ct_)                                                                              \
+    do {                                                                                                \
+        const size_t o_ = (size_t)c * N + 256 * (ct_) + 64 * cw + 2 * lane;                             \
+        tnx = __ldg(reinterpret_cast<const float2 *>(A.coltab + o_));                                   \
+        inx = __ldg(reinterpret_cast<const int2 *>(A.colix + o_));                                      \
+    } while (0)
+    if (grp < nct) G2_COL_FETCH(grp);
     unsigned int bar_gen = 0u;
     unsigned use0 = 0u, use1 = 0u;             // how often this group has waited on its buffer 0 / 1
     const uint32_t mb0 = sMbar + 16u * (uint32_t)grp, mb1 = mb0 + 8u;
@@ -311,15 +339,15 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                 int ixc;
                 bool cols_ok;
                 {
-                    const int i0 = A.colix[(size_t)c * N + y0], i1 = A.colix[(size_t)c * N + y0 + 1];
+                    // weights along q at the stripe's centre row and their t-derivatives (Eq. 13) from the
+                    // fractional positions the host rounded once from double
+                    const int i0 = inx.x, i1 = inx.y;
+                    const float t0 = tnx.x, t1 = tnx.y;
+                    G2_COL_FETCH(ct + G2_GROUPS < nct ? ct + G2_GROUPS : grp);
                     ixc = i0;
                     cols_ok = __all_sync(FULL, i0 != OC_BAD && i0 == i1);
-                    const float4 *ct0 = reinterpret_cast<const float4 *>(A.coltab + ((size_t)c * N + y0) * OC_COLTAB);
-                    const float4 m0 = __ldg(ct0), m0p = __ldg(ct0 + 1), m1 = __ldg(ct0 + 2), m1p = __ldg(ct0 + 3);
-                    const float a0[4] = {m0.x, m0.y, m0.z, m0.w}, a0p[4] = {m0p.x, m0p.y, m0p.z, m0p.w};
-                    const float a1[4] = {m1.x, m1.y, m1.z, m1.w}, a1p[4] = {m1p.x, m1p.y, m1p.z, m1p.w};
-#pragma unroll
-                    for (int i = 0; i < ORDER; ++i) { wkr.M0[i] = a0[i]; wkr.M0p[i] = a0p[i]; wkr.M1[i] = a1[i]; wkr.M1p[i] = a1p[i]; }
+                    lagrange<ORDER>(t0, wkr.M0); lagrange_deriv<ORDER>(t0, wkr.M0p);
+                    lagrange<ORDER>(t1, wkr.M1); lagrange_deriv<ORDER>(t1, wkr.M1p);
                     wkr.ey0 = G.a * ((float)y0 - yc);
                     wkr.ey1 = G.a * ((float)(y0 + 1) - yc);
                     wkr.a = G.a;
@@ -599,6 +627,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     G2_DIAG(A.nsteps - 1);
 #undef G2_DIAG
 #undef G2_ISSUE_FIRST
+#undef G2_COL_FETCH
 }
 
 }  // namespace vfps
