@@ -482,3 +482,130 @@ def test_p15_clamp_is_identity_on_smooth_data_and_bounds_the_rotation(orc):
     for f in (orc.drift, orc.rf_kick):
         c = f(box, -L, L, -L, L, 25 * dphi, 4, clamp=True)
         assert c.max() <= 1.0 and c.min() >= 0.0
+
+
+# ---------------------------------------------------------------- the whole step, written out from the paper
+def _lagrange_bf(order, t):
+    """Eq. 13 (L107) literally: l_k(t) = prod_{m != k} (t - o_m) / (o_k - o_m), nodes o_k = k - floor((order-1)/2)."""
+    o = [k - (order - 1) // 2 for k in range(order)]
+    w = []
+    for k in range(order):
+        v = 1.0
+        for m in range(order):
+            if m != k:
+                v *= (t - o[m]) / (o[k] - o[m])
+        w.append(v)
+    return o, w
+
+
+def _step_bruteforce(psi, box, spp, beta, order, pad, Z, manhattan=False, clamp=False):
+    """One Warnock-Ellison split step (L29-40) with explicit Python loops over cells and taps, straight from the
+    paper's formulas and the readings A1-A14 of DESIGN.md -- no call into oracle/: rotation about the origin by
+    the angle 2 pi / spp (Eq. 1: q_s = c q - s p, p_s = s q + c p, tensor-product Lagrange interpolation, psi = 0
+    outside the grid), profile, wake through numpy's FFT (Eq. 5), kick by -dphi V, Fokker-Planck (Eq. 15 and the
+    three-point second difference), charge, renormalisation, moments and CSR power (Eq. 16-17) of the end-of-step
+    density.  manhattan: the rotation is the drift psi_A(q, p) = psi(q - dphi p, p) followed by the RF kick
+    psi_B(q, p) = psi_A(q, p + dphi q), two 1-D interpolations (L136, reading A15).  clamp: every interpolated value
+    is limited to the interval of the nodes that bracket its source point (Eq. 14, reading A9)."""
+    N = psi.shape[0]
+    qmin, qmax, pmin, pmax = box
+    dq, dp = (qmax - qmin) / (N - 1), (pmax - pmin) / (N - 1)
+    dphi = TWO_PI / spp
+    c, s = math.cos(dphi), math.sin(dphi)
+
+    def at(a, x, y):
+        return a[x, y] if 0 <= x < N and 0 <= y < N else 0.0
+
+    def interp1(a, x, ysrc, along_q):
+        """1-D Lagrange interpolation of row / column through (x, .) at the fractional index ysrc"""
+        m = math.floor(ysrc)
+        o, w = _lagrange_bf(order, ysrc - m)
+        get = (lambda k: at(a, m + k, x)) if along_q else (lambda k: at(a, x, m + k))
+        v = sum(w[j] * get(o[j]) for j in range(order))
+        if clamp:
+            v = min(max(v, min(get(0), get(1))), max(get(0), get(1)))
+        return v
+
+    rot = np.zeros((N, N))
+    if manhattan:
+        dr = np.zeros((N, N))
+        for x in range(N):
+            for y in range(N):
+                dr[x, y] = interp1(psi, y, x - dphi * (pmin + y * dp) / dq, True)
+        for x in range(N):
+            for y in range(N):
+                rot[x, y] = interp1(dr, x, y + dphi * (qmin + x * dq) / dp, False)
+    else:
+        for x in range(N):
+            for y in range(N):
+                q, p = qmin + x * dq, pmin + y * dp
+                xs, ys = (c * q - s * p - qmin) / dq, (s * q + c * p - pmin) / dp
+                mx, my = math.floor(xs), math.floor(ys)
+                ox, wx = _lagrange_bf(order, xs - mx)
+                oy, wy = _lagrange_bf(order, ys - my)
+                v = sum(wx[i] * wy[j] * at(psi, mx + ox[i], my + oy[j]) for i in range(order) for j in range(order))
+                if clamp:
+                    nb = [at(psi, mx + i, my + j) for i in (0, 1) for j in (0, 1)]
+                    v = min(max(v, min(nb)), max(nb))
+                rot[x, y] = v
+    rho = dp * rot.sum(axis=1)
+    Nf = pad * N
+    V = np.fft.irfft(Z * np.fft.rfft(rho, Nf), Nf)[:N] if Z is not None else np.zeros(N)
+    kick = np.zeros((N, N))
+    for x in range(N):
+        for y in range(N):
+            kick[x, y] = interp1(rot, x, y + dphi * V[x] / dp, False)      # delta p = -dphi V: source = y + dphi V / dp
+    b = beta / spp
+    fp = np.zeros((N, N))
+    for x in range(N):
+        for y in range(N):
+            f = [at(kick, x, y + k) for k in (-1, 0, 1, 2)]
+            d1 = (-2 * f[0] - 3 * f[1] + 6 * f[2] - f[3]) / (6 * dp)
+            d2 = (f[0] - 2 * f[1] + f[2]) / dp ** 2
+            fp[x, y] = f[1] + b * (f[1] + (pmin + y * dp) * d1 + d2)
+    C = fp.sum() * dq * dp
+    out = fp / C
+    qa, pa = qmin + dq * np.arange(N), pmin + dp * np.arange(N)
+    tot = out.sum()
+    mq, mp = (out.sum(axis=1) * qa).sum() / tot, (out.sum(axis=0) * pa).sum() / tot
+    sq = math.sqrt((out.sum(axis=1) * qa ** 2).sum() / tot - mq ** 2)
+    sp = math.sqrt((out.sum(axis=0) * pa ** 2).sum() / tot - mp ** 2)
+    P = 0.0
+    if Z is not None:
+        R = np.fft.rfft(dp * out.sum(axis=1), Nf)
+        wgt = np.full(Nf // 2 + 1, 2.0)
+        wgt[0] = wgt[-1] = 1.0
+        P = dq / Nf * float((wgt * Z.real * np.abs(R) ** 2).sum())
+    return out, np.array([C, mq, mp, sq, sp, P])
+
+
+@pytest.mark.parametrize("manhattan,clamp", [(False, False), (True, False), (False, True), (True, True)])
+@pytest.mark.parametrize("order", [2, 3, 4])
+def test_whole_step_against_loops_written_from_the_paper(orc, order, manhattan, clamp):
+    """Pins the composition of vfpo_step -- sub-step order a1..a6 (A14), kick sign (A6), which density the
+    diagnostics refer to (A10), renormalisation -- and every sub-step once more, against an implementation that
+    shares nothing with oracle/: 16 x 16 cells, asymmetric box, off-centre bunch, a step large enough that the
+    stencil floors change across the grid, an impedance strong enough that the kick moves rows by more than a cell;
+    three consecutive steps; standard and Manhattan rotation (A15), free and clamped interpolation (A9)."""
+    N, spp, beta, pad = 16, 40, 0.3, 2
+    box = (-4.0, 5.0, -4.5, 3.5)
+    rng = np.random.default_rng(7)
+    psi = make_psi0(N, *box, 1.1, 0.8, 0.0, 0, q0=0.4, p0=-0.3).astype(np.float64)
+    psi += 1e-3 * psi.max() * rng.random((N, N))
+    dq, dp = 9.0 / (N - 1), 8.0 / (N - 1)
+    psi /= psi.sum() * dq * dp
+    k = np.arange(pad * N // 2 + 1)
+    Z = (18.0 + 8.0j * np.sin(0.37 * k)) * np.exp(-0.02 * k)
+    Z[0] = 0.0
+    Z[-1] = Z[-1].real
+    o = orc.Oracle(N, *box, spp, beta, order, pad, Z.astype(np.complex128), manhattan=manhattan, clamp=clamp)
+    o.set_psi(psi)
+    ref = psi.copy()
+    moved = 0.0
+    for step in range(3):
+        d = o.step(1)
+        ref, dref = _step_bruteforce(ref, box, spp, beta, order, pad, Z, manhattan, clamp)
+        np.testing.assert_allclose(o.psi, ref, rtol=0, atol=1e-12 * ref.max(), err_msg=f"order {order}, step {step}")
+        np.testing.assert_allclose(d[0], dref, rtol=1e-10, atol=1e-12)
+        moved = max(moved, np.abs(o.wake()).max() * TWO_PI / spp / dp)
+    assert moved > 1.0            # the kick did move some row by more than a cell
