@@ -1048,3 +1048,71 @@ def test_cluster_engine_no_wake_no_renormalise(vfps, orc, kernel):
     assert_psi(sim.get_psi_host()[0], o.psi, 5e-4, "cluster C0 no renormalise")
     assert_diag(d[499, 0], dr[499], has_wake=False)
     sim.close()
+
+
+# ---------------------------------------------------------------- seeded random configurations
+def _random_case(seed):
+    """A seeded draw of grid size, box, step, damping, current, interpolation order, flags and bunch: the boxes are
+    asymmetric and of unequal aspect, the steps range from a few hundred to several thousand per period, the bunch
+    sits off centre -- the combinations no hand-written case happens to pick."""
+    rng = np.random.default_rng(1000 + seed)
+    N = int(rng.choice([64, 128, 256, 512]))
+    order = int(rng.choice([4, 3, 4, 2]))
+    qmin, qmax = -float(rng.uniform(4.5, 7.0)), float(rng.uniform(4.5, 7.0))
+    pmin, pmax = -float(rng.uniform(4.5, 7.0)), float(rng.uniform(4.5, 7.0))
+    spp = int(np.exp(rng.uniform(np.log(12.0 * N), np.log(16000.0))))      # |displacement| stays within the 4-row halo
+    beta = float(np.exp(rng.uniform(np.log(1e-4), np.log(2e-2))))
+    S = float(rng.uniform(0.05, 0.8))
+    plates = None if rng.random() < 0.3 else float(rng.uniform(0.3, 2.0))
+    clamp = bool(rng.random() < 0.3)
+    manhattan = bool(rng.random() < 0.25)
+    bunch = dict(sigma_q=float(rng.uniform(0.7, 1.3)), sigma_p=float(rng.uniform(0.7, 1.3)), noise=1e-6, seed=seed,
+                 q0=float(rng.uniform(-0.5, 0.5)), p0=float(rng.uniform(-0.5, 0.5)))
+    return dict(N=N, order=order, box=(qmin, qmax, pmin, pmax), spp=spp, beta=beta, S=S, plates=plates, clamp=clamp,
+                manhattan=manhattan, bunch=bunch)
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_configurations(vfps, orc, seed):
+    """24 seeded random configurations, each on the engine AUTO picks and then on every other engine that accepts
+    it: 1 step at 1e-5, 25 steps at 1e-4, all six diagnostics at 1e-4 (P_csr with the edge-flux allowance)."""
+    cs = _random_case(seed)
+    N, order, box = cs["N"], cs["order"], cs["box"]
+    dq = (box[1] - box[0]) / (N - 1)
+    Z = make_impedance(N, 2, dq, cs["S"], cs["plates"])[None, :]
+    b = cs["bunch"]
+    psi0 = make_psi0(N, *box, b["sigma_q"], b["sigma_p"], b["noise"], b["seed"], q0=b["q0"], p0=b["p0"])[None]
+    flags = vfps.FLAG_RENORMALISE | (vfps.FLAG_CLAMP if cs["clamp"] else 0) | (vfps.FLAG_ROT_MANHATTAN if cs["manhattan"] else 0)
+    sim = vfps.Simulation(N, *box, cs["spp"], cs["beta"], order, 2, 1, Z=Z, flags=flags)
+    o = orc.Oracle(N, *box, cs["spp"], cs["beta"], order, 2, Z[0], manhattan=cs["manhattan"], clamp=cs["clamp"])
+    sim.set_psi_host(psi0)
+    o.set_psi(psi0[0])
+    what = f"seed {seed}: {cs}"
+    d = sim.step_host(1)
+    dr = o.step(1)
+    assert_psi(sim.get_psi_host()[0], o.psi, TOL_1, what + f" 1 step, {sim.engine_name}")
+    assert_diag(d[0, 0], dr[0], tol_p=edge_flux_tol(dr[0][0]))
+    d = sim.step_host(24)
+    dr = o.step(24)
+    assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, what + f" 25 steps, {sim.engine_name}")
+    assert_diag(d[23, 0], dr[23], tol_p=edge_flux_tol(dr[23][0]))
+    auto = sim.engine_name
+    ran = [auto]
+    for name, eng in (("stream", vfps.ENGINE_STREAM), ("graph", vfps.ENGINE_GRAPH), ("cluster", vfps.ENGINE_CLUSTER),
+                      ("grid", vfps.ENGINE_GRID)):
+        if name == auto:
+            continue
+        try:
+            sim.set_engine(eng)
+        except vfps.VfpsError as e:
+            assert e.code == -5                           # refused with a reason, never a wrong answer
+            continue
+        sim.set_psi_host(psi0)
+        o.set_psi(psi0[0])
+        d = sim.step_host(25)
+        dr = o.step(25)
+        assert_psi(sim.get_psi_host()[0], o.psi, 1e-4, what + f" 25 steps, {name}")
+        assert_diag(d[24, 0], dr[24], tol_p=edge_flux_tol(dr[24][0]))
+        ran.append(name)
+    assert len(ran) >= 3, ran
+    sim.close()
