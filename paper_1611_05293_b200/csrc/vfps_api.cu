@@ -15,6 +15,8 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <algorithm>
+#include <utility>
 #include <vector>
 
 using namespace vfps;
@@ -81,7 +83,8 @@ struct vfps_sim {
     std::string gr_why;
     // TMA-staged grid engine (vfps_grid2.cuh, grid kernel 2); g2_blocks = 0: not available
     int gr_ver_opt = 0;                          // 0 auto (2 where available), 1 k_grid_step, 2 k_grid2_step
-    int g2_blocks = 0, g2_KRmax = 0, g2_rows_lo = 0, g2_rows_extra = 0, g2_nbuf = 0;
+    int g2_blocks = 0, g2_KRmax = 0, g2_nbuf = 0;
+    int *g2_row0 = nullptr;
     size_t g2_smem = 0;
     float *g2_coltab = nullptr, *g2_rowtab = nullptr, *g2_rho = nullptr, *g2_mom = nullptr;
     int *g2_colix = nullptr;
@@ -681,7 +684,56 @@ int grid2_configure(vfps_sim *h)
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     if (!coop) { h->g2_why = "device does not support cooperative launches"; return VFPS_OK; }
     const int nb = sms < N ? sms : N;
-    const int rows_lo = N / nb, rows_extra = N % nb, KRmax = rows_lo + (rows_extra ? 1 : 0);
+    const RotGeomD g = rot_geom_d(h->P);
+    // Row stripes.  floor(dy) is constant along a row and changes between two rows at most a few times over the grid
+    // (once, through the rotation centre, for the usual boxes); a stripe that contains such a change splits its rotation
+    // into two runs and is the last to arrive at every barrier.  So the stripes are dealt out per segment of constant
+    // floor(dy), CTAs in proportion to the rows, as evenly as possible inside a segment -- unless that makes the
+    // tallest stripe taller than the even split of all rows does.
+    std::vector<int> row0(nb + 1, 0);
+    int KRmax = (N + nb - 1) / nb;
+    {
+        auto row_floor = [&](int x) {
+            const double X = (double)x + g.x0c;
+            const double f0 = std::floor(g.d * X + g.a * g.y0c), f1 = std::floor(g.d * X + g.a * ((double)(N - 1) + g.y0c));
+            return f0 == f1 ? (int)f0 : OC_BAD;
+        };
+        std::vector<int> seg(1, 0);                          // first rows of the segments
+        for (int x = 1, last = row_floor(0); x < N; ++x) {
+            const int f = row_floor(x);
+            if (f == OC_BAD) continue;                       // a row that changes along itself stays with its predecessor
+            if (last != OC_BAD && f != last) seg.push_back(x);
+            last = f;
+        }
+        seg.push_back(N);
+        const int ns = (int)seg.size() - 1;
+        std::vector<int> cnt(ns, 0);
+        bool ok = ns >= 2 && ns <= nb;
+        if (ok) {
+            int used = 0;
+            std::vector<std::pair<double, int>> frac;
+            for (int i = 0; i < ns; ++i) {
+                const double share = (double)nb * (seg[i + 1] - seg[i]) / N;
+                cnt[i] = (int)share < 1 ? 1 : (int)share;
+                used += cnt[i];
+                frac.push_back({share - std::floor(share), i});
+            }
+            std::sort(frac.begin(), frac.end(), [](const std::pair<double, int> &a, const std::pair<double, int> &b) { return a.first > b.first; });
+            for (int k = 0; used < nb && k < ns; ++k, ++used) ++cnt[frac[k].second];
+            ok = used == nb;
+            for (int i = 0; ok && i < ns; ++i) ok = (seg[i + 1] - seg[i] + cnt[i] - 1) / cnt[i] <= KRmax && cnt[i] <= seg[i + 1] - seg[i];
+        }
+        if (ok) {
+            int c = 0;
+            for (int i = 0; i < ns; ++i) {
+                const int len = seg[i + 1] - seg[i], lo = len / cnt[i], extra = len % cnt[i];
+                for (int k = 0; k < cnt[i]; ++k, ++c) row0[c + 1] = row0[c] + lo + (k < extra ? 1 : 0);
+            }
+        } else {
+            const int lo = N / nb, extra = N % nb;
+            for (int c = 0; c < nb; ++c) row0[c + 1] = row0[c] + lo + (c < extra ? 1 : 0);
+        }
+    }
     const bool clamp = (h->P.flags & VFPS_FLAG_CLAMP) != 0 && order > 2;
     // two tile buffers per warp group where they fit beside the stripe's rows, else one
     int nbuf = 2;
@@ -690,7 +742,6 @@ int grid2_configure(vfps_sim *h)
     const size_t bytes = L.total_floats * sizeof(float);
     if (bytes + 256 > (size_t)smem_max) { h->g2_why = "tiles and row buffer do not fit shared memory"; return VFPS_OK; }
     if (L.box_rows > 256) { h->g2_why = "TMA box too tall"; return VFPS_OK; }
-    const RotGeomD g = rot_geom_d(h->P);
     {   // first-order weight tables must be exact to fp32 rounding over a stripe and over the columns
         const double ex = std::fabs(g.a) * 0.5 * (double)KRmax, ey = std::fabs(g.a) * 0.5 * (double)N;
         const double e = ex > ey ? ex : ey;
@@ -729,7 +780,7 @@ int grid2_configure(vfps_sim *h)
     std::vector<int> cix((size_t)nb * N, OC_BAD);
     const double Ymid = 0.5 * (double)(N - 1) + g.y0c;
     for (int c = 0; c < nb; ++c) {
-        const int nr = rows_lo + (c < rows_extra ? 1 : 0), r0 = c * rows_lo + (c < rows_extra ? c : rows_extra);
+        const int r0 = row0[c], nr = row0[c + 1] - r0;
         const double Xlo = (double)r0 + g.x0c, Xhi = (double)(r0 + nr - 1) + g.x0c, Xc = 0.5 * (Xlo + Xhi);
         for (int y = 0; y < N; ++y) {
             const double Y = (double)y + g.y0c;
@@ -758,6 +809,7 @@ int grid2_configure(vfps_sim *h)
         CU(dalloc(h, &h->g2_coltab, col.size()));
         CU(dalloc(h, &h->g2_colix, cix.size()));
         CU(dalloc(h, &h->g2_rowtab, row.size()));
+        CU(dalloc(h, &h->g2_row0, row0.size()));
         CU(dalloc(h, &h->g2_rho, (size_t)N));
         CU(dalloc(h, &h->g2_mom, (size_t)2 * nb * G2_NPART));
         CU(dalloc(h, &h->g2_qacc, (size_t)16 + (size_t)16 * nb));   // three charge accumulators, barrier counter, one 128-byte flag line per CTA
@@ -765,9 +817,10 @@ int grid2_configure(vfps_sim *h)
     CU(cudaMemcpyAsync(h->g2_coltab, col.data(), col.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(h->g2_colix, cix.data(), cix.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(h->g2_rowtab, row.data(), row.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->g2_row0, row0.data(), row0.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     h->g2_nbuf = nbuf;
-    h->g2_blocks = nb; h->g2_KRmax = KRmax; h->g2_rows_lo = rows_lo; h->g2_rows_extra = rows_extra; h->g2_smem = bytes;
+    h->g2_blocks = nb; h->g2_KRmax = KRmax; h->g2_smem = bytes;
     return VFPS_OK;
 }
 
@@ -777,7 +830,7 @@ int launch_grid2_steps(vfps_sim *h, int n, float *diag)
     A.psi = h->psi; A.scale = h->scale; A.wfun = h->has_wake ? h->wfun : nullptr;
     A.rho = h->g2_rho; A.mom_part = h->g2_mom; A.diag = diag; A.nsteps = n;
     A.coltab = h->g2_coltab; A.colix = h->g2_colix; A.rowtab = h->g2_rowtab; A.qacc = h->g2_qacc;
-    A.rows_lo = h->g2_rows_lo; A.rows_extra = h->g2_rows_extra; A.KRmax = h->g2_KRmax; A.nbuf = h->g2_nbuf;
+    A.row0 = h->g2_row0; A.KRmax = h->g2_KRmax; A.nbuf = h->g2_nbuf;
     A.bar = reinterpret_cast<unsigned int *>(h->g2_qacc + 3);
     A.flags = reinterpret_cast<unsigned int *>(h->g2_qacc + 16);
     if (cudaMemsetAsync(h->g2_qacc, 0, (16 + (size_t)16 * h->g2_blocks) * sizeof(unsigned long long), h->stream) != cudaSuccess)

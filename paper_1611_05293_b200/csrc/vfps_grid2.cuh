@@ -58,7 +58,7 @@ struct Grid2Args {
     unsigned int *bar;          // grid barrier counter, zero at launch
     unsigned int *flags;        // [gridDim.x][32] (one 128-byte line each): kicks finished by the CTA in this launch, zero at launch
     int nsteps;
-    int rows_lo, rows_extra;    // stripe c has rows_lo + (c < rows_extra) rows
+    const int *row0;            // [gridDim.x + 1] first row of every stripe (stripe c: rows row0[c] .. row0[c + 1] - 1)
     int KRmax;                  // rows of the largest stripe
     int nbuf;                   // tile buffers per warp group: 2, or 1 where two do not fit beside the stripe's rows
     long long *dbg;
@@ -193,8 +193,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int grp = warp >> 2, cw = warp & 3;
     const int c = (int)blockIdx.x;
-    const int rows = A.rows_lo + (c < A.rows_extra ? 1 : 0);
-    const int r0 = c * A.rows_lo + min(c, A.rows_extra);
+    const int r0 = A.row0[c], rows = A.row0[c + 1] - r0;
 
     extern __shared__ __align__(128) float g2smem[];
     float *smem = g2smem;
