@@ -4,16 +4,18 @@
 // address arithmetic and three edge paths, and kicks straight from global memory: 147
 // thread-instructions per cell, 29 us per step at 2048^2.  This engine gives the large grid what the
 // in-place cluster kernel (vfps_onchip.cuh) gives the on-chip ones:
-//  * One CTA of 512 threads per SM owns a stripe of N / gridDim rows for the whole launch.
+//  * One CTA of 512 threads per SM owns a stripe of about N / gridDim rows for the whole launch (stripe
+//    boundaries where floor(dy) changes from one row to the next: a stripe's rotation is one run).
 //  * Rotation a1 + a2: the source region of a tile -- the stripe's rows plus H halo rows, 256
 //    columns plus 8 each side -- comes in through TMA (cp.async.bulk.tensor.2d over a tensor map of
-//    8-byte elements, so that one box holds the 272 floats of a tile row; completion on an mbarrier).  psi is zero outside the grid (reading A8), and so is TMA's fill for the part of a
+//    8-byte elements, so that one box holds the 272 floats of a tile row; completion on an
+//    mbarrier).  psi is zero outside the grid (reading A8), and so is TMA's fill for the part of a
 //    box that lies outside the tensor: no edge path exists.  A group of four warps rotates a tile
-//    with the cluster kernel's walker: two columns per thread,
-//    ORDER x 6 register window, per-launch weight tables (built in double on the host for the
-//    centre row of every stripe), next row's loads issued mid-row.  Two tile buffers per group where
-//    they fit (the tile after next is in flight while a tile is rotated), else one; the first tiles
-//    of a step are issued right after the previous step's last barrier.  The rotated cells stay in
+//    with the cluster kernel's walker: two columns per thread, ORDER x 6 register window,
+//    per-launch weight tables (rows: L, L' in shared memory; columns: the fractional source
+//    position at the stripe's centre row, rounded once from double, fetched a tile ahead), next
+//    row's loads issued mid-row.  Two tile buffers per group where they fit (the tile after next is
+//    in flight while a tile is rotated), else one.  The rotated cells stay in
 //    shared memory (the stripe's rows: no psi_tmp round trip through L2), row sums (transposed warp
 //    reduction) go to the profile.
 //  -- grid barrier --
