@@ -117,13 +117,14 @@ __device__ __forceinline__ void grid_barrier(unsigned int *ctr, unsigned int &ge
     ++gen;
     if (threadIdx.x == 0) {
         const unsigned int target = gen * gridDim.x;
-        __threadfence();
-        atomicAdd(ctr, 1u);
+        // release: the CTA's global stores before the __syncthreads above are ordered before the arrival;
+        // acquire: the poll that sees the last arrival orders every CTA's stores before what follows the
+        // __syncthreads below (no further fence needed: the readers use L1-bypassing loads)
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
         unsigned int seen;
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
         } while ((int)(seen - target) < 0);
-        __threadfence();
     }
     __syncthreads();
 }
@@ -609,10 +610,8 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         asm volatile("fence.proxy.async;" ::: "memory");
         VFPS_STAMP(A.dbg, step, 5);
         __syncthreads();
-        if (tid == 0) {
-            __threadfence();
+        if (tid == 0)       // release: orders the CTA's psi stores (before the __syncthreads) before the flag
             asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(A.flags + 32 * c), "r"((unsigned int)(step + 1)) : "memory");
-        }
         // a6 of the previous step: the last CTA (the shortest stripe) writes its diagnostics row; the partial
         // sums of every CTA were complete at this step's barrier
         if (step > 0) G2_DIAG(step - 1);
