@@ -606,8 +606,8 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
             // charge: one 64-bit fixed-point accumulator (integer atomics: exact, order-independent)
             if (tid == 0) atomicAdd(A.qacc + step % 3, (unsigned long long)__float2ll_rn(s * 4294967296.0f));
         }
-        // psi of this step is read by the neighbours' next rotation through TMA (async proxy)
-        asm volatile("fence.proxy.async;" ::: "memory");
+        // (psi of this step is read by the next rotations through TMA, i.e. the async proxy: the proxy fence sits on
+        // the reader's side, in G2_ISSUE_FIRST, after the flags have been acquired)
         VFPS_STAMP(A.dbg, step, 5);
         __syncthreads();
         if (tid == 0)       // release: orders the CTA's psi stores (before the __syncthreads) before the flag
