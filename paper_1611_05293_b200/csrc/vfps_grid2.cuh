@@ -315,10 +315,10 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         if (step > 0) {
             // The halo rows of this step's tiles belong to the stripes above and below: those two CTAs must
             // have finished the kick of step - 1 (no grid barrier between a kick and the next rotation).  One
-            // poller per CTA, one 128-byte line per flag: hundreds of pollers on a few lines starve the writers.
-            if (tid == 0) {
-                for (int nb = c - 1; nb <= c + 1; nb += 2) {
-                    if (nb < 0 || nb >= (int)gridDim.x) continue;
+            // poller per flag, one 128-byte line per flag: hundreds of pollers on a few lines starve the writers.
+            if (tid < 2) {                                  // the two flags in flight together: one L2 round trip, not two
+                const int nb = c - 1 + 2 * tid;
+                if (nb >= 0 && nb < (int)gridDim.x) {
                     unsigned int seen;
                     for (;;) {
                         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(A.flags + 32 * nb) : "memory");
