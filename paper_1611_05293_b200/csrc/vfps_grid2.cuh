@@ -68,7 +68,7 @@ struct Grid2Args {
 
 struct Grid2Layout {
     int box_rows, pitch, nct;
-    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_rho, off_sw, off_sw2, off_vpart, off_red, off_rows, off_big,
+    size_t tile_floats, off_mbar, off_rowtab, off_rowpart, off_vtab, off_rho, off_sw, off_sw2, off_vpart, off_red, off_runend, off_rows, off_big,
         total_floats;
 };
 
@@ -90,6 +90,7 @@ __host__ __device__ inline Grid2Layout grid2_layout(int N, int KRmax, int H, int
     L.off_sw2 = o;      o += clamp ? (size_t)(N + KP + 4) : 0;    // ... and of the transposed wake
     L.off_vpart = o;    o += (size_t)8 * KP;                      // wake partial sums [4 quarters (+ 4 transposed)][KP rows]
     L.off_red = o;      o += (size_t)G2_WARPS * 8 + 8;
+    L.off_runend = o;   o += (size_t)((KRmax + 3) & ~3);         // per row: end of its run of constant floor(dy)
     L.off_rows = o;     o += (size_t)KRmax * L.pitch;           // the stripe's rotated rows
     o = (o + 31) & ~(size_t)31;                                 // TMA destinations: 128-byte aligned
     L.off_big = o;      o += (size_t)nbuf * G2_GROUPS * L.tile_floats + G2_SUBW;   // + one row: the walker prefetches past the end
@@ -220,6 +221,14 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
         rowtab_s[i - OC_ROWTAB] = (gi >= 0 && gi < N * OC_ROWTAB) ? A.rowtab[gi] : 0.0f;
     }
     __syncthreads();
+    // runs of consecutive rows with the same floor(dy) (the window slides through a run): end of the run of every row
+    int *runend = reinterpret_cast<int *>(smem + LY.off_runend);
+    if (tid < rows) {
+        const int iy = __float_as_int(rowtab_s[tid * OC_ROWTAB + 10]);
+        int ve = tid + 1;
+        while (iy != OC_BAD && ve < rows && __float_as_int(rowtab_s[ve * OC_ROWTAB + 10]) == iy) ++ve;
+        runend[tid] = ve;
+    }
     if (A.wfun != nullptr) {
         // the lags this stripe's rows touch: sw[i] = w at index r0 + i (V_x = sum_x' sw[x - r0 + N - 1 - x'] rho_x');
         // CLAMP: sw2[i] = w at index N - r0 - KP + i (transposed wake: w[x' - x] = sw2[x' + KP - 1 - (x - r0)])
@@ -367,8 +376,7 @@ k_grid2_step(GridConst G, Grid2Args A, const __grid_constant__ CUtensorMap tmap)
                 while (v < rows) {
                     const int iy = __float_as_int(rowtab_s[v * OC_ROWTAB + 10]);
                     if (cols_ok && iy != OC_BAD) {
-                        int ve = v + 1;
-                        while (ve < rows && __float_as_int(rowtab_s[ve * OC_ROWTAB + 10]) == iy) ++ve;
+                        const int ve = runend[v];
                         const int par = (iy - O0) & 1;
                         // tile row of source row x is x - (r0 - H); tap row 0 of target v: v + ixc - O0
                         uint32_t src = box + (uint32_t)((v + H + ixc - O0) * P4 + (yl + iy - O0 - par) * 4);
