@@ -138,7 +138,7 @@ __host__ __device__ inline OnchipLayout onchip_layout(int N, int S, int H, int o
     L.off_rowpart = o;  o += (size_t)((R * L.CW + 3) & ~3);
     L.off_vtab = o;     o += (size_t)R * 8;
     L.off_rowaddr = o;  o += (size_t)R * 4;
-    L.off_chunk = o;    o += (size_t)((L.W * L.nch + 3) & ~3);
+    L.off_chunk = o;    o += (size_t)((3 * L.W * L.nch + 3) & ~3);   // per (walker, chunk): iy, run length walking down, walking up
     L.off_wred = o;     o += (size_t)OC_WARPS * 8;
     L.off_rowtab = o;   o += (size_t)(R + 2) * OC_ROWTAB;      // one spare entry before and after (prefetch)
     L.off_buf = o;      o += (size_t)(L.phys_rows + 1) * L.pitch;
@@ -616,6 +616,19 @@ k_onchip_step(GridConst G, OnchipArgs A)
         }
         chunkinfo[i] = iy;
     }
+    __syncthreads();
+    // ... and how many chunks with the same floors follow it in either walk direction (the window slides through the
+    // whole run): found once here, not by a chain of dependent loads in front of every step's rotation
+    for (int i = tid; i < W * nch; i += OC_THREADS) {
+        const int w = i / nch, c = i - w * nch, iy = chunkinfo[i];
+        int nd = 1, nu = 1;
+        if (iy != OC_BAD) {
+            while (c + nd < nch && chunkinfo[w * nch + c + nd] == iy) ++nd;
+            while (c - nu >= 0 && chunkinfo[w * nch + c - nu] == iy) ++nu;
+        }
+        chunkinfo[W * nch + 2 * i] = nd;
+        chunkinfo[W * nch + 2 * i + 1] = nu;
+    }
     if (tid == 0) {
         mbar_init(mbRho0, 1); mbar_init(mbRho0 + 8, 1); mbar_init(mbHalo, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -705,7 +718,7 @@ k_onchip_step(GridConst G, OnchipArgs A)
                     int nrun = 1;                          // chunks handled in this round
                     if (cols_ok && iy != OC_BAD) {
                         // ---- a run of chunks with the same floors: the window slides through all of them
-                        while (ci + nrun < nch && chunkinfo[wk * nch + (p ? c - nrun : c + nrun)] == iy) ++nrun;
+                        nrun = chunkinfo[W * nch + 2 * (wk * nch + c) + p];
                         const int par = (iy - O0) & 1;
                         const int v0 = p ? c * CH + CH - 1 : c * CH;                   // first target row in walk order
                         // window column 0 = grid column y0 + iy - O0 - par
