@@ -783,18 +783,35 @@ k_onchip_step(GridConst G, OnchipArgs A)
                 const uint32_t rb = sRho + (uint32_t)(p * N) * 4u, pb = sPart + (uint32_t)(p * OC_MAX_S * OC_NPART) * 4u;
                 const uint32_t mb = mbRho0 + 8u * (uint32_t)p;
                 if (!last) {
-                    const int nq = R >> 2;
-                    for (int i = tid; i < S * nq; i += OC_THREADS) {
-                        const int dd = i / nq, q = i - dd * nq;
-                        float pv[4];
+                    // thread t < R: the sum of row t's CW partials (one vector load, lane stride CW floats: no bank
+                    // conflicts); the four lanes of a row quad gather its four sums and share the destinations
+                    float pv = 0.0f;
+                    if (tid < R) {
+                        float pc[CW];
+                        const uint32_t a = sRowpart + (uint32_t)(tid * CW) * 4u;
+                        if (CW >= 4) {
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {
-                            float s = 0.0f;
-#pragma unroll
-                            for (int c = 0; c < CW; ++c) s += rowpart[(4 * q + k) * CW + c];
-                            pv[k] = s * G.dp;
+                            for (int c = 0; c < CW; c += 4) {
+                                const float4 v = lds4(a + 4u * (uint32_t)c);
+                                pc[c] = v.x; pc[(c + 1) % CW] = v.y; pc[(c + 2) % CW] = v.z; pc[(c + 3) % CW] = v.w;
+                            }
+                        } else if (CW == 2) {
+                            const float2 v = lds2(a);
+                            pc[0] = v.x; pc[CW - 1] = v.y;
+                        } else {
+                            pc[0] = lds(a);
                         }
-                        st_async4(mapa(rb + (uint32_t)(x0 + 4 * q) * 4u, dd), make_float4(pv[0], pv[1], pv[2], pv[3]), mapa(mb, dd));
+                        float sum = 0.0f;
+#pragma unroll
+                        for (int c = 0; c < CW; ++c) sum += pc[c];
+                        pv = sum * G.dp;
+                    }
+                    const int l4 = lane & ~3;
+                    const float4 quad = make_float4(__shfl_sync(FULL, pv, l4), __shfl_sync(FULL, pv, l4 + 1),
+                                                    __shfl_sync(FULL, pv, l4 + 2), __shfl_sync(FULL, pv, l4 + 3));
+                    if (tid < R) {
+                        const uint32_t dsta = rb + (uint32_t)(x0 + (tid & ~3)) * 4u;
+                        for (int dd = lane & 3; dd < S; dd += 4) st_async4(mapa(dsta, dd), quad, mapa(mb, dd));
                     }
                 }
                 if (tid >= OC_THREADS - 2 * S) {
