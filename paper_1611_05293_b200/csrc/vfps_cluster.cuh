@@ -54,9 +54,9 @@ __host__ __device__ inline size_t cluster_smem_floats(int N, int S, int H)
     return (size_t)(R + 2 * H) * pitch      // bufA
            + (size_t)R * pitch              // bufB
            + 2 * (size_t)N                  // wake function
-           + (size_t)N                      // rho (all rows)
+           + 2 * (size_t)N                  // rho (all rows), two parities
            + 2 * CL_MAX_S * CL_NPART        // partial sums of all CTAs, two parities
-           + CL_WARPS * 8 + 8;              // block reduction scratch, mbarriers
+           + CL_WARPS * 8 + 16;             // block reduction scratch, five mbarriers
 }
 
 // floor for |v| < 2^22 on the FMA pipe: v + 1.5*2^23 rounded toward -inf has floor(v) in its low
@@ -401,13 +401,16 @@ struct Rotator {
 // Synchronisation between the CTAs of a cluster is pure data flow: every remote store is an
 // st.async that counts its bytes on an mbarrier of the receiving CTA, and a consumer waits for the
 // expected byte count of the current phase (one phase per step and barrier):
-//   MB_RHO   N floats            rho_x of step t from every CTA (all-gather)
+//   MB_RHO[t & 1]  N floats      un-normalised rho_x of step t from every CTA (all-gather), buffer t & 1
 //   MB_HALO  nbrs * H * N floats  the neighbours' boundary rows of psi_t
-//   MB_PART  S * CL_NPART floats  the partial sums of step t from every CTA
-// Write-after-read safety needs no extra barrier: a CTA sends rho(t+1) only after it has part(t)
-// from every CTA, which each CTA sends after it has consumed rho(t); halo(t+1) and part(t+1) are
-// sent after rho(t+1) has arrived from every CTA, which each CTA sends after it has consumed
-// halo(t) and part(t).
+//   MB_PART[t & 1]  S * CL_NPART floats  the partial sums of step t from every CTA
+// The charge of step t-1 (-> 1/C) is formed from part(t-1) AFTER rho(t) has been sent, inside the latency of
+// the all-gather; rho travels un-normalised and V and rho are scaled where they are used.
+// Write-after-read safety needs no extra barrier: rho is double-buffered with a barrier per parity, and a
+// CTA can send rho(t+2) only after it has rho(t+1) from every CTA, which each CTA sends after its kick of
+// step t, i.e. after it has consumed rho(t); halo(t+1) and part(t+1) are sent after rho(t+1) has arrived
+// from every CTA, which each CTA sends after it has consumed halo(t); part(t) (buffer and barrier t & 1) is
+// consumed before the wait for rho(t+1), and part(t+2) is sent after rho(t+2) has arrived from every CTA.
 template <int ORDER, int N, bool MANH = false>
 __global__ void __launch_bounds__(CL_THREADS, 1)
 k_cluster_step(GridConst G, ClusterArgs A)
@@ -431,12 +434,12 @@ k_cluster_step(GridConst G, ClusterArgs A)
     float *bufA = smem;                                   // (R + 2H) rows
     float *bufB = bufA + (size_t)(R + 2 * H) * PITCH;     // R rows
     float *wf = bufB + (size_t)R * PITCH;                 // 2N
-    float *rho = wf + 2 * N;                              // N
-    float *part = rho + N;                                // 2 * CL_MAX_S * CL_NPART
+    float *rho2 = wf + 2 * N;                             // 2 x N (step parity)
+    float *part = rho2 + 2 * N;                           // 2 * CL_MAX_S * CL_NPART
     float *wred = part + 2 * CL_MAX_S * CL_NPART;         // CL_WARPS * 8
-    float *scal = wred + CL_WARPS * 8;                    // [2..7] = three mbarriers
-    const uint32_t sA = smem_u32(bufA), sB = smem_u32(bufB), sRho = smem_u32(rho), sPart = smem_u32(part);
-    const uint32_t mbRho = smem_u32(scal + 2), mbHalo = mbRho + 8, mbPart = mbRho + 16;
+    float *scal = wred + CL_WARPS * 8;                    // [2..11] = five mbarriers
+    const uint32_t sA = smem_u32(bufA), sB = smem_u32(bufB), sRho2 = smem_u32(rho2), sPart = smem_u32(part);
+    const uint32_t mbRho0 = smem_u32(scal + 2), mbHalo = mbRho0 + 16, mbPart0 = mbRho0 + 24;    // mbRho[p] = mbRho0 + 8 p, mbPart[p] = mbPart0 + 8 p
     const int nbrs = (rank > 0 ? 1 : 0) + (rank < S - 1 ? 1 : 0);
     const uint32_t bytesRho = ((R & 3) == 0 ? (uint32_t)(N - R) : (uint32_t)N) * 4u, bytesHalo = (uint32_t)(nbrs * H * N) * 4u, bytesPart = (uint32_t)(S - 1) * CL_NPART * 4u;
 
@@ -473,10 +476,12 @@ k_cluster_step(GridConst G, ClusterArgs A)
         for (int c = 0; c < 4; ++c) c1p[k][c] = c1 * fmaf((float)(4 * lane + 128 * k + c), G.dp, G.p_min);
 
     if (tid == 0) {
-        mbar_init(mbRho, 1); mbar_init(mbHalo, 1); mbar_init(mbPart, 1);
+        mbar_init(mbRho0, 1); mbar_init(mbRho0 + 8, 1); mbar_init(mbHalo, 1); mbar_init(mbPart0, 1); mbar_init(mbPart0 + 8, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    unsigned phase = 0;      // parity of the current phase of all three barriers
+    unsigned phase = 0;      // parity of the current phase of the halo barrier
+    unsigned rho_use0 = 0u, rho_use1 = 0u;      // how often mbRho[p] has been waited on
+    unsigned part_use0 = 0u, part_use1 = 0u;    // ... and mbPart[p]
 
     for (int m = cid; m < A.members; m += nclusters) {
         float *gpsi = A.psi + (size_t)m * N * N;
@@ -496,9 +501,11 @@ k_cluster_step(GridConst G, ClusterArgs A)
         // waited on: arming it would complete its phase at once, and a warp that has not yet reached
         // its wait would see the parity flip twice and hang
         if (tid == 0) {
-            if (bytesRho) mbar_expect_tx(mbRho, bytesRho);
+            if (bytesRho) mbar_expect_tx(mbRho0, bytesRho);
+            if (bytesRho && A.nsteps > 1) mbar_expect_tx(mbRho0 + 8, bytesRho);
             if (bytesHalo) mbar_expect_tx(mbHalo, bytesHalo);
-            if (bytesPart) mbar_expect_tx(mbPart, bytesPart);
+            if (bytesPart) mbar_expect_tx(mbPart0, bytesPart);
+            if (bytesPart && A.nsteps > 1) mbar_expect_tx(mbPart0 + 8, bytesPart);
         }
         // nobody may store into this CTA before it has finished initialising
         cluster.sync();
@@ -534,10 +541,47 @@ k_cluster_step(GridConst G, ClusterArgs A)
             VFPS_STAMP(A.dbg, step, 1);
             __syncthreads();
             VFPS_STAMP(A.dbg, step, 2);
+            const int p = step & 1;
+            float *rho = rho2 + p * N;
+            const uint32_t sRho = sRho2 + (uint32_t)(p * N) * 4u, mbRho = mbRho0 + 8u * (uint32_t)p;
+            VFPS_STAMP(A.dbg, step, 3);
+            if (!last) {
+                // ================= 2. projection: rho_x = dp * sum_y bufB(x, y) (un-normalised), all-gathered into buffer p
+                for (int r = warp; r < R; r += CL_WARPS) {
+                    const uint32_t row = sB + (uint32_t)((r * PITCH + CL_PAD) * 4);
+                    float s = 0.0f;
+#pragma unroll
+                    for (int k = 0; k < NG; ++k) {
+                        const int g = 4 * lane + 128 * k;
+                        if (g < N) {
+                            const float4 v = lds4(row + g * 4);
+                            s += (v.x + v.y) + (v.z + v.w);
+                        }
+                    }
+                    s = warp_sum(s) * G.dp;
+                    if ((R & 3) != 0) {
+                        if (lane < S) st_async(mapa(sRho + (uint32_t)(x0 + r) * 4u, lane), s, mapa(mbRho, lane));
+                    } else if (lane == 0) {
+                        rho[x0 + r] = s;          // own slot of the local rho array doubles as staging
+                    }
+                }
+                if ((R & 3) == 0) {
+                    // one 16-byte message per four rows and destination (few large DSMEM transactions)
+                    __syncthreads();
+                    const int nq = R >> 2;
+                    for (int i = tid; i < (S - 1) * nq; i += CL_THREADS) {
+                        const int dd0 = i / nq, q = i - dd0 * nq, dd = dd0 + (dd0 >= rank ? 1 : 0);
+                        const uint32_t a = sRho + (uint32_t)(x0 + 4 * q) * 4u;
+                        st_async4(mapa(a, dd), lds4(a), mapa(mbRho, dd));
+                    }
+                }
+            }
             if (step > 0) {
-                // ================= 6. a6 of step t-1: charge, scale, diagnostics
-                if (bytesPart) mbar_wait(mbPart, phase ^ 1u);
-                if (tid == 0 && !last && bytesPart) mbar_expect_tx(mbPart, bytesPart);
+                // ================= 6. a6 of step t-1: charge, scale, diagnostics -- inside the latency of the all-gather
+                const int pq = (step - 1) & 1;             // part(t) travels on barrier t & 1; part(t + 2) re-uses it
+                if (bytesPart) mbar_wait(mbPart0 + 8u * (uint32_t)pq, (pq ? part_use1 : part_use0) & 1u);
+                if (pq) ++part_use1; else ++part_use0;
+                if (tid == 0 && step + 1 < A.nsteps && bytesPart) mbar_expect_tx(mbPart0 + 8u * (uint32_t)pq, bytesPart);
                 // lane = (g4, j): partial j summed over the CTAs g4, g4 + 4, ..., then over the four
                 // lane groups -- the same order in every warp of every CTA
                 const float *pp = part + ((step - 1) & 1) * (CL_MAX_S * CL_NPART);
@@ -568,40 +612,11 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 }
             }
             if (last) break;
-            VFPS_STAMP(A.dbg, step, 3);
-            // ================= 2. projection: rho_x = dp * sc * sum_y bufB(x, y), all-gathered
-            for (int r = warp; r < R; r += CL_WARPS) {
-                const uint32_t row = sB + (uint32_t)((r * PITCH + CL_PAD) * 4);
-                float s = 0.0f;
-#pragma unroll
-                for (int k = 0; k < NG; ++k) {
-                    const int g = 4 * lane + 128 * k;
-                    if (g < N) {
-                        const float4 v = lds4(row + g * 4);
-                        s += (v.x + v.y) + (v.z + v.w);
-                    }
-                }
-                s = warp_sum(s) * (G.dp * sc);
-                if ((R & 3) != 0) {
-                    if (lane < S) st_async(mapa(sRho + (uint32_t)(x0 + r) * 4u, lane), s, mapa(mbRho, lane));
-                } else if (lane == 0) {
-                    rho[x0 + r] = s;          // own slot of the local rho array doubles as staging
-                }
-            }
-            if ((R & 3) == 0) {
-                // one 16-byte message per four rows and destination (few large DSMEM transactions)
-                __syncthreads();
-                const int nq = R >> 2;
-                for (int i = tid; i < (S - 1) * nq; i += CL_THREADS) {
-                    const int dd0 = i / nq, q = i - dd0 * nq, dd = dd0 + (dd0 >= rank ? 1 : 0);
-                    const uint32_t a = sRho + (uint32_t)(x0 + 4 * q) * 4u;
-                    st_async4(mapa(a, dd), lds4(a), mapa(mbRho, dd));
-                }
-            }
             VFPS_STAMP(A.dbg, step, 4);
-            if (bytesRho) mbar_wait(mbRho, phase);
+            if (bytesRho) mbar_wait(mbRho, (p ? rho_use1 : rho_use0) & 1u);
+            if (p) ++rho_use1; else ++rho_use0;
             VFPS_STAMP(A.dbg, step, 5);
-            if (tid == 0 && step + 1 < A.nsteps && bytesRho) mbar_expect_tx(mbRho, bytesRho);
+            if (tid == 0 && step + 2 < A.nsteps && bytesRho) mbar_expect_tx(mbRho, bytesRho);
             // ================= 3.+4. wake (own rows), kick + Fokker-Planck: bufB -> bufA
             // per-warp sums: s0 sum psi, s1/s2 p moments (per lane), q1/q2 q moments, pw = sum rho V
             float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, q1 = 0.0f, q2 = 0.0f, pw = 0.0f;
@@ -615,9 +630,9 @@ k_cluster_step(GridConst G, ClusterArgs A)
                         const int xp = lane + 32 * k;
                         V = fmaf(wf[x - xp + N - 1], rho[xp], V);
                     }
-                    V = warp_sum(V);
+                    V = warp_sum(V) * sc;
                 }
-                pw = fmaf(rho[x], V, pw);
+                pw = fmaf(rho[x] * sc, V, pw);
                 int mm;
                 float t;
                 floor_frac(G.kick_c * V, mm, t);
@@ -719,7 +734,7 @@ k_cluster_step(GridConst G, ClusterArgs A)
                 __syncwarp();
                 for (int i = lane; i < 2 * (S - 1); i += 32) {
                     const int dd0 = i >> 1, hh = i & 1, dd = dd0 + (dd0 >= rank ? 1 : 0);
-                    st_async4(mapa(slot + hh * 16, dd), lds4(slot + hh * 16), mapa(mbPart, dd));
+                    st_async4(mapa(slot + hh * 16, dd), lds4(slot + hh * 16), mapa(mbPart0 + 8u * (uint32_t)(step & 1), dd));
                 }
             }
             VFPS_STAMP(A.dbg, step, 7);
