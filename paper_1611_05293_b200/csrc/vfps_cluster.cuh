@@ -707,17 +707,18 @@ k_cluster_step(GridConst G, ClusterArgs A)
                         rs += q0;
                     }
                 }
-                // q moments of the END-of-step psi from the row sum (the same value in every lane)
-                rs = warp_sum(rs);
+                // q moments of the END-of-step psi from the lane's share of the row sum (reduced over the lanes
+                // once, at the end of the pass, together with the other sums)
                 const float X = (float)x - xc, tq = rs * X;
                 s0 += rs; q1 += tq; q2 = fmaf(tq, X, q2);
             }
             VFPS_STAMP(A.dbg, step, 6);
             // ================= 5. partial sums of this CTA -> every CTA
-            s1 = warp_sum(s1); s2 = warp_sum(s2);
-            if (lane == 0) {
-                *reinterpret_cast<float4 *>(wred + warp * 8) = make_float4(s0, s1, s2, q1);
-                *reinterpret_cast<float4 *>(wred + warp * 8 + 4) = make_float4(q2, pw, 0.0f, 0.0f);
+            {
+                // one transposed reduction of all six sums (pw is the same in every lane: lane 0's counts)
+                float v8[8] = {s0, s1, s2, q1, q2, lane == 0 ? pw : 0.0f, 0.0f, 0.0f};
+                const float tot = warp_reduce_transposed<8>(v8, lane);       // lanes 4 j .. 4 j + 3 hold sum j
+                if ((lane & 3) == 0) wred[warp * 8 + (lane >> 2)] = tot;
             }
             __syncthreads();
             if (warp == 0) {

@@ -167,56 +167,6 @@ __device__ __forceinline__ void named_barrier(int id, int nthreads)
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// Transposed warp reduction of NV (power of two <= 8) per-lane values: afterwards every lane holds
-// the warp total of value index  idx = lane >> (5 - log2 NV)  (the top bits of the lane number).
-// NV/2 + NV/4 + ... + 1 + (5 - log2 NV) shuffles instead of 5 NV.
-template <int NV>
-__device__ __forceinline__ float warp_reduce_transposed(float (&v)[NV], int lane)
-{
-    constexpr unsigned FULL = 0xffffffffu;
-    if constexpr (NV == 1) {
-        return warp_sum(v[0]);
-    } else {
-        // level with xor offset 16, 8, 4: keep the half of the values selected by that lane bit
-        float u[NV / 2];
-        const bool hi = (lane & 16) != 0;
-#pragma unroll
-        for (int i = 0; i < NV / 2; ++i) {
-            const float keep = hi ? v[NV / 2 + i] : v[i];
-            const float send = hi ? v[i] : v[NV / 2 + i];
-            u[i] = keep + __shfl_xor_sync(FULL, send, 16);
-        }
-        if constexpr (NV == 2) {
-            float r = u[0];
-#pragma unroll
-            for (int o = 8; o > 0; o >>= 1) r += __shfl_xor_sync(FULL, r, o);
-            return r;
-        } else {
-            float w[NV / 4];
-            const bool hi2 = (lane & 8) != 0;
-#pragma unroll
-            for (int i = 0; i < NV / 4; ++i) {
-                const float keep = hi2 ? u[NV / 4 + i] : u[i];
-                const float send = hi2 ? u[i] : u[NV / 4 + i];
-                w[i] = keep + __shfl_xor_sync(FULL, send, 8);
-            }
-            float r;
-            if constexpr (NV == 4) {
-                r = w[0];
-                r += __shfl_xor_sync(FULL, r, 4);
-            } else {
-                const bool hi3 = (lane & 4) != 0;
-                const float keep = hi3 ? w[1] : w[0];
-                const float send = hi3 ? w[0] : w[1];
-                r = keep + __shfl_xor_sync(FULL, send, 4);
-            }
-            r += __shfl_xor_sync(FULL, r, 2);
-            r += __shfl_xor_sync(FULL, r, 1);
-            return r;
-        }
-    }
-}
-
 // kick (shift by MM + t cells, Lagrange weights l already scaled by 1/C -- un-scaled with CLAMP,
 // where the caller scales the results) and Fokker-Planck for the
 // four cells g..g+3 of one row: b[i] = psi'(g - 4 + i), i = 0..11.  k[i] = kicked value at
