@@ -203,6 +203,31 @@ const char *vfps_kernel_name(int kernel);
 const char *vfps_engine_name(vfps_handle h);
 const char *vfps_wake_name(vfps_handle h);
 
+/* ---- a3 without a handle and without any allocation ------------------------------------------
+ * Wake potential of a caller-held profile (Eq. 4-5):
+ *     V_x = sum_x' w[x - x'] rho_x',  w = Re IDFT(Z) of the Hermitian spectrum Z_k, k = 0..N*pad/2
+ * -- what vfps_get_wake returns for the profile of its handle (identical up to rounding: direct
+ * convolution here, FFT there).  For callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): the call makes no cudaMalloc / cudaFree
+ * and uses no allocating library routine.  Its scratch, the wake function w (2N floats), lives in a
+ * built-in device array of 2 * VFPS_NOALLOC_MAX_N floats (32 KB) that every GPU that loads the
+ * library holds until the process exits.
+ *   N, pad   grid points and zero-padding factor: pad >= 2 and N*pad powers of two, N >= 8;
+ *            N > VFPS_NOALLOC_MAX_N or N*pad > 8192 -> VFPS_ERR_UNSUPPORTED
+ *   Z        DEVICE, N*pad/2 + 1 values (as vfps_create's, one member), read only
+ *   rho      DEVICE, N floats, read only;  V_out  DEVICE, N floats, written (must not alias rho)
+ *   cuda_stream  a cudaStream_t (NULL = the legacy default stream); two kernels are launched on it,
+ *            the call does not synchronise.  The first call on each device looks up the address
+ *            of the scratch array (cudaGetSymbolAddress): make it outside a graph capture.
+ * All calls on a device share the scratch array, which keeps the last call's wake function until
+ * the next call overwrites it (nothing in it accumulates, so nothing needs clearing): calls that
+ * overlap on the GPU -- different streams, concurrently replayed graphs -- race on it; serialise them.
+ * Returns VFPS_OK or a negative vfps_status; vfps_noalloc_last_error() gives the text (per thread,
+ * valid until the thread's next vfps_wake_noalloc call). */
+#define VFPS_NOALLOC_MAX_N 4096
+int vfps_wake_noalloc(int N, int pad, const vfps_complex *Z, const float *rho, float *V_out, void *cuda_stream);
+const char *vfps_noalloc_last_error(void);
+
 /* Text of the last error on this handle (or of the last failed vfps_create when h is NULL).
  * Valid until the next call on the same handle. */
 const char *vfps_last_error(vfps_handle h);

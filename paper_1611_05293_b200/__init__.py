@@ -10,7 +10,7 @@ from .binding import (
     WAKE_AUTO, WAKE_FFT, WAKE_DIRECT, OPT_ENGINE, OPT_WAKE, OPT_TIMING, OPT_CLUSTER_SIZE,
     OPT_CLUSTER_KERNEL, OPT_GRID_KERNEL,
     FLAG_RENORMALISE, FLAG_CLAMP, FLAG_ROT_MANHATTAN,
-    VfpsError, VfpsParams, Simulation, load, version, EXPORTS,
+    VfpsError, VfpsParams, Simulation, load, version, EXPORTS, wake_noalloc, NOALLOC_MAX_N,
 )
 
 __all__ = [
@@ -19,5 +19,5 @@ __all__ = [
     "WAKE_AUTO", "WAKE_FFT", "WAKE_DIRECT", "OPT_ENGINE", "OPT_WAKE", "OPT_TIMING", "OPT_CLUSTER_SIZE",
     "OPT_CLUSTER_KERNEL", "OPT_GRID_KERNEL",
     "FLAG_RENORMALISE", "FLAG_CLAMP", "FLAG_ROT_MANHATTAN",
-    "VfpsError", "VfpsParams", "Simulation",
+    "VfpsError", "VfpsParams", "Simulation", "wake_noalloc", "NOALLOC_MAX_N",
 ]

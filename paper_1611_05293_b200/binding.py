@@ -29,7 +29,9 @@ EXPORTS = [
     "vfps_step_count", "vfps_launch_count", "vfps_engine_name", "vfps_wake_name",
     "vfps_kernel_time", "vfps_reset_kernel_times", "vfps_kernel_name",
     "vfps_last_error", "vfps_version",
+    "vfps_wake_noalloc", "vfps_noalloc_last_error",
 ]
+NOALLOC_MAX_N = 4096      # VFPS_NOALLOC_MAX_N of include/vfps.h
 
 
 class VfpsError(RuntimeError):
@@ -73,7 +75,10 @@ def load():
     L.vfps_kernel_time.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.vfps_reset_kernel_times.argtypes = [vp]
     L.vfps_kernel_name.argtypes = [ip]
-    strings = ("vfps_engine_name", "vfps_wake_name", "vfps_last_error", "vfps_version", "vfps_kernel_name")
+    L.vfps_wake_noalloc.argtypes = [ip, ip, vp, vp, vp, vp]
+    L.vfps_noalloc_last_error.argtypes = []
+    strings = ("vfps_engine_name", "vfps_wake_name", "vfps_last_error", "vfps_version", "vfps_kernel_name",
+               "vfps_noalloc_last_error")
     for name in EXPORTS:
         getattr(L, name).restype = C.c_char_p if name in strings else C.c_int
     for name in strings[:3]:
@@ -94,6 +99,23 @@ def _dev_ptr(t, dtype_name: str, numel: int, what: str) -> int:
     if t.numel() != numel:
         raise ValueError(f"{what}: expected {numel} elements, got {t.numel()}")
     return t.data_ptr()
+
+
+def wake_noalloc(N: int, pad: int, Z, rho, V_out, stream=None) -> None:
+    """vfps_wake_noalloc (include/vfps.h): V_out[x] = sum_x' w[x - x'] rho[x'], w = Re IDFT(Z), with no device
+    allocation -- the wake function lives in a 32 KB array built into the library (N <= NOALLOC_MAX_N).
+    Z: complex64 CUDA tensor of N*pad/2 + 1 values; rho, V_out: float32 CUDA tensors of N values (V_out is written).
+    stream: a torch.cuda.Stream, default the current one.  Calls that overlap on the GPU race on the built-in array."""
+    import torch
+    L = load()
+    nz = (N * pad) // 2 + 1 if N > 0 and pad > 0 else 0
+    zp = None if Z is None else _dev_ptr(Z, "complex64", nz, "Z")
+    rp = None if rho is None else _dev_ptr(rho, "float32", N, "rho")
+    vo = None if V_out is None else _dev_ptr(V_out, "float32", N, "V_out")
+    st = (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+    rc = L.vfps_wake_noalloc(int(N), int(pad), zp, rp, vo, st)
+    if rc != 0:
+        raise VfpsError(rc, L.vfps_noalloc_last_error().decode())
 
 
 def _host_arr(a, dtype, numel: int, what: str) -> np.ndarray:
