@@ -165,6 +165,10 @@ def run_reference(args, wl, rank, world):
     """--impl reference: the oracle on the host cores, rank 0 only (the other ranks exit 0)."""
     if rank != 0:
         return
+    if world > 1 and os.environ.get("OMP_NUM_THREADS") == "1":
+        # torchrun sets OMP_NUM_THREADS=1 for its workers; the other ranks do no work here, so rank 0 runs
+        # the oracle on the host cores it may use, as at N = 1 (set before the oracle's OpenMP runtime loads)
+        os.environ["OMP_NUM_THREADS"] = str(len(os.sched_getaffinity(0)))
     import oracle
     oracle.build()
     n_inner = args.inner if args.inner > 0 else 25
